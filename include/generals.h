@@ -1,0 +1,188 @@
+/*
+ * generals.h -- C ABI of the B200-native batched Generals.io environment step.
+ *
+ * The hot path of arXiv 2606.23348 ("P:Lnn" = line nn of PAPER.md; "Rn" = reading n of DESIGN.md):
+ * for N independent games at once, apply every player's move with combat / capture / land transfer
+ * (section IV-D/E), army growth (IV-C), termination, reward and auto-reset
+ * (P:L61), and emit each player's fog-of-war observation planes (IV-B, IV-G).
+ *
+ * Conventions for every call below
+ *   - All `gen_buffers` members are DEVICE pointers owned by the caller (e.g. torch tensors), 16-byte
+ *     aligned, sized as `gen_query_sizes` reports.  The library owns only the `gen_env` handle; it
+ *     never allocates board memory, never synchronises and never copies to the host (except
+ *     `gen_step_host`, which says so).  A call enqueues kernels on `cuda_stream` (a cudaStream_t
+ *     passed as void*, NULL = the legacy default stream) and returns; buffers must stay alive until
+ *     that work has completed.
+ *   - Return value: 0 = GEN_OK, negative = error (see gen_error_string).  Invalid GAME actions are
+ *     not errors: they are passes (R5, R10).
+ *   - Layout: plane stride S = round_up(H*W, 16) cells; cell index c = row*W + col.  Encodings (R18):
+ *     terrain int8 {0 plain, 1 mountain, 2 city(castle), 3 general}; owner int8 {-1 neutral, 0..P-1};
+ *     army int16 >= 0 (saturating at 32767, R21).  Fogged cells read army 0, owner -2, terrain 4.
+ *   - Determinism: outputs are a pure function of (config, policy, seed, global game id =
+ *     game_id_base + g, actions); independent of N, of launch geometry, and of whether K steps were
+ *     made by K gen_step calls or one gen_rollout(K).
+ *   - sm_100a only.  There is no CPU fallback and no other architecture.
+ */
+#ifndef GENERALS_H_
+#define GENERALS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    GEN_OK = 0,
+    GEN_ERR_NULL = -1,    /* a required pointer is NULL */
+    GEN_ERR_CONFIG = -2,  /* H/W/P/team_size out of range, lo > hi, infeasible counts */
+    GEN_ERR_ALIGN = -3,   /* a device pointer is not 16-byte aligned */
+    GEN_ERR_ARG = -4,     /* K <= 0, unknown flag, missing buffer for the requested mode */
+    GEN_ERR_CUDA = -5     /* launch / runtime error (cudaGetLastError captured; see gen_last_cuda_error) */
+};
+
+/* rule_flags: alternative readings of the paper, honoured by both sides (R2, R11, R6) */
+enum {
+    GEN_RULE_TICK_PLAIN_ONLY = 1,    /* 50-turn tick skips cities and generals */
+    GEN_RULE_CAPTURE_HALF_FLOOR = 2, /* transferred armies are floor(a/2) instead of ceil(a/2) */
+    GEN_RULE_ROTATE_PRIORITY = 4     /* first mover is turn % P instead of player 0 */
+};
+
+/* gen_rollout flags */
+enum {
+    GEN_OBS_DIGEST = 0,     /* chain a 64-bit digest of every step's observation (R28); write final-step planes */
+    GEN_OBS_EVERY_STEP = 1, /* write every step's planes / reward / done / winner to slot k of [K]-strided buffers */
+    GEN_OBS_NONE = 2        /* state only (reported separately, never the headline) */
+};
+
+/* gen_reset flags */
+enum { GEN_KEEP_EPISODE = 1 /* regenerate with the episode counters found in the buffer */ };
+
+typedef struct gen_config {
+    int32_t n_games;       /* N >= 0 */
+    int32_t height, width; /* 1..32 each, H*W >= 2 */
+    int32_t n_players;     /* P, 2..8 */
+    int32_t team_size;     /* 1 = 1v1 / free-for-all; teams are p / team_size (R19) */
+    int32_t n_cities;      /* neutral castles placed at reset (R14) */
+    int32_t city_army_lo, city_army_hi; /* castle garrison uniform in [lo, hi] */
+    int32_t spawn_dmin;    /* min Manhattan distance between generals (R29) */
+    int32_t spawn_dmax;    /* 0 = unbounded; 1v1 window [dmin, dmax] */
+    int32_t spawn_exact;   /* 1: per game draw d ~ U{dmin..dmax} and spawn at exactly d (P:L169 curriculum) */
+    int32_t max_turns;     /* 0 = none; truncation (R16) */
+    int32_t auto_reset;    /* 1: a finished game is regenerated inside the same call (R17) */
+    uint32_t rule_flags;
+    uint32_t game_id_base; /* global game id = game_id_base + g keys every random draw */
+    uint32_t mountain_thr; /* P(mountain) = mountain_thr / 2^32 per non-general cell */
+    uint64_t seed;         /* Philox4x32-10 key */
+} gen_config;
+
+/* probabilities as uint32 thresholds floor(p * 2^32): no float enters the hot path (R24, R25) */
+typedef struct gen_policy {
+    uint32_t pass_thr; /* P(pass) */
+    uint32_t half_thr; /* P(half split | move) */
+    uint32_t bias_thr; /* P(restrict to the largest owned stack) */
+} gen_policy;
+
+/* Device buffers.  [N] etc. are element counts; S = plane stride; K = slots of an EVERY_STEP rollout
+ * (1 otherwise).  "state" members are read and written; "out" members are written only. */
+typedef struct gen_buffers {
+    int16_t *army;           /* state [N][S] */
+    int8_t *owner;           /* state [N][S] */
+    int8_t *terrain;         /* state [N][S] */
+    int32_t *turn;           /* state [N] */
+    uint32_t *episode;       /* state [N] */
+    uint8_t *alive;          /* state [N]   bit p = player p's general lives */
+    int16_t *general_cell;   /* state [N][P]  -1 once captured */
+    int32_t *land;           /* state [N][P]  public scoreboard (R23) */
+    int32_t *army_total;     /* state [N][P] */
+    int8_t *reward;          /* out   [K][N][P]  +1 / -1 on the terminal step, else 0 (R20) */
+    uint8_t *done;           /* state [K][N]  bit0 terminated, bit1 truncated */
+    int8_t *winner;          /* state [K][N]  winning team or -1 */
+    int16_t *obs_army;       /* out   [K][N][P][S] */
+    int8_t *obs_owner;       /* out   [K][N][P][S] */
+    int8_t *obs_terrain;     /* out   [K][N][P][S] */
+    uint8_t *obs_vis;        /* out   [K][N][P][S] */
+    uint32_t *episodes_done; /* state [N]   accumulators */
+    uint32_t *wins;          /* state [N][P] */
+    uint32_t *truncations;   /* state [N] */
+    uint32_t *sat_events;    /* state [N]   int16 saturations (R21) */
+    uint64_t *obs_digest;    /* state [N]   may be NULL for gen_reset / gen_step (no digest then) */
+    int32_t *actions_out;    /* out   [K][N][P]  the actions actually applied; may be NULL */
+} gen_buffers;
+
+/* byte sizes of the buffers above for K slots */
+typedef struct gen_sizes {
+    int32_t plane_stride;    /* S in cells */
+    int32_t alignment;       /* 16 */
+    size_t army, owner, terrain, turn, episode, alive, general_cell, land, army_total;
+    size_t reward, done, winner, obs_army, obs_owner, obs_terrain, obs_vis;
+    size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out;
+} gen_sizes;
+
+typedef struct gen_env gen_env;
+
+/* Sizes of every device buffer for `cfg` with `k_slots` >= 1 output slots.  Host-only. */
+int gen_query_sizes(const gen_config *cfg, int32_t k_slots, gen_sizes *out);
+
+/* Validate `cfg`, build the host-side handle.  Allocates no device memory.  Policy defaults to
+ * pass 0, half 1/2, bias 0.  GEN_ERR_CONFIG on a bad config. */
+int gen_init(const gen_config *cfg, gen_env **out);
+
+/* Set the built-in sampler's thresholds (a12; R24, R25). */
+int gen_set_policy(gen_env *env, const gen_policy *policy);
+
+/* Count of steps since gen_reset: the Philox counter word of the action stream. */
+uint32_t gen_global_step(const gen_env *env);
+int gen_set_global_step(gen_env *env, uint32_t step);
+
+/* a1: generate all N boards (Philox keyed by seed, global game id, episode; R13-R15, R29, R30),
+ * zero the accumulators, write scoreboard + initial observation (+ digest if obs_digest != NULL),
+ * global_step <- 0.  flags: 0 or GEN_KEEP_EPISODE. */
+int gen_reset(gen_env *env, const gen_buffers *bufs, uint32_t flags, void *cuda_stream);
+
+/* a2-a12: one turn for all games.  d_actions: device int32 [N][P] flat action indices
+ * a = cell*9 + k, k = 0 pass, else 1 + 2*dir + half, dir 0 up 1 down 2 left 3 right (R22);
+ * NULL = draw them with the built-in valid-action sampler.  Writes state, scoreboard, reward, done,
+ * winner, the four observation planes per player, actions_out / obs_digest if given.
+ * global_step += 1. */
+int gen_step(gen_env *env, const gen_buffers *bufs, const int32_t *d_actions, void *cuda_stream);
+
+/* a13: K sampled turns in ONE launch, the board resident in shared memory throughout (R28).
+ * flags: one of GEN_OBS_DIGEST / GEN_OBS_EVERY_STEP / GEN_OBS_NONE.  EVERY_STEP needs buffers sized
+ * for K slots.  Otherwise reward / done / winner / planes of the last step land in slot 0.
+ * global_step += K. */
+int gen_rollout(gen_env *env, const gen_buffers *bufs, int32_t K, uint32_t flags, void *cuda_stream);
+
+/* Recount the scoreboard of a state written by the caller and emit its observation (no turn is
+ * played).  For hand-built boards. */
+int gen_observe(gen_env *env, const gen_buffers *bufs, void *cuda_stream);
+
+/* The sampler alone (a12): d_actions_out int32 [N][P] drawn on the boards as they stand with the
+ * current global_step; no state change. */
+int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, void *cuda_stream);
+
+/* End-to-end convenience: HOST actions in (int32 [N][P], may be NULL = sampler), HOST results out
+ * (reward int8 [N][P], done uint8 [N]; either may be NULL).  Copies host->device into
+ * bufs->actions_out (must be non-NULL when h_actions is given), runs gen_step, copies device->host,
+ * all on cuda_stream, and synchronises that stream before returning.  Use pinned host memory. */
+int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
+                  uint8_t *h_done, void *cuda_stream);
+
+/* Launch geometry override for tuning: warps (games) per CTA in {1,2,4,8,16}; 0 restores the default. */
+int gen_set_launch(gen_env *env, int32_t warps_per_cta);
+
+/* Number of kernels this handle has launched (bench.py's gpu_launches). */
+uint64_t gen_launch_count(const gen_env *env);
+
+/* cudaError_t of the last failing runtime call made through this handle (0 if none). */
+int gen_last_cuda_error(const gen_env *env);
+
+void gen_destroy(gen_env *env);
+const char *gen_error_string(int code);
+const char *gen_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GENERALS_H_ */

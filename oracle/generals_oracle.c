@@ -376,7 +376,7 @@ static void step_game(const orc_config *cfg, const orc_buffers *b, int g, const 
         } else if (m > d) {                                                              /* P:L93 */
             army[dst] = (int16_t)(m - d);
             owner[dst] = (int8_t)p;
-            if (terrain[dst] == T_GENERAL) capture(cfg, b, g, p, t, dst);               /* R11, R12 */
+            if (terrain[dst] == T_GENERAL && t >= 0) capture(cfg, b, g, p, t, dst);     /* R11, R12 */
         } else {
             army[dst] = (int16_t)(d - m);                 /* tie -> 0, previous owner keeps the cell */
         }
@@ -488,7 +488,10 @@ int32_t orc_rollout(const orc_config *cfg, const orc_buffers *b, int32_t K, uint
         v.obs_army += (size_t)k * N * P * S; v.obs_owner += (size_t)k * N * P * S;
         v.obs_terrain += (size_t)k * N * P * S; v.obs_vis += (size_t)k * N * P * S;
         v.reward += (size_t)k * N * P; v.done += (size_t)k * N; v.winner += (size_t)k * N;
-        if (k > 0) memcpy(v.done, v.done - N, (size_t)N);      /* carry the frozen flag forward */
+        if (k > 0) {                                           /* carry the frozen game's flags forward */
+            memcpy(v.done, v.done - N, (size_t)N);
+            memcpy(v.winner, v.winner - N, (size_t)N);
+        }
         orc_step(cfg, &v, NULL, global_step0 + (uint32_t)k, NULL);
     }
     return 0;

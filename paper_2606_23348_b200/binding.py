@@ -1,0 +1,264 @@
+"""ctypes binding of include/generals.h.  Argument marshalling only.
+
+The product path fails loudly when the CUDA library is missing: there is no CPU fallback and this
+module never imports anything from oracle/.
+"""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libgenerals.so")
+
+OBS_DIGEST, OBS_EVERY_STEP, OBS_NONE = 0, 1, 2
+GEN_KEEP_EPISODE = 1
+RULE_TICK_PLAIN_ONLY, RULE_CAPTURE_HALF_FLOOR, RULE_ROTATE_PRIORITY = 1, 2, 4
+
+EXPORTS = ["gen_query_sizes", "gen_init", "gen_set_policy", "gen_global_step", "gen_set_global_step",
+           "gen_reset", "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host",
+           "gen_set_launch", "gen_launch_count", "gen_last_cuda_error", "gen_destroy",
+           "gen_error_string", "gen_version"]
+
+
+class GenError(RuntimeError):
+    pass
+
+
+class GenConfig(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in (
+        "n_games", "height", "width", "n_players", "team_size", "n_cities", "city_army_lo",
+        "city_army_hi", "spawn_dmin", "spawn_dmax", "spawn_exact", "max_turns", "auto_reset")] + [
+        (n, C.c_uint32) for n in ("rule_flags", "game_id_base", "mountain_thr")] + [("seed", C.c_uint64)]
+
+
+class GenPolicy(C.Structure):
+    _fields_ = [(n, C.c_uint32) for n in ("pass_thr", "half_thr", "bias_thr")]
+
+
+# name -> (torch dtype name, shape builder(N, P, S, K))
+BUFFERS = [
+    ("army", "int16", lambda N, P, S, K: (N, S)),
+    ("owner", "int8", lambda N, P, S, K: (N, S)),
+    ("terrain", "int8", lambda N, P, S, K: (N, S)),
+    ("turn", "int32", lambda N, P, S, K: (N,)),
+    ("episode", "int32", lambda N, P, S, K: (N,)),            # bits of uint32
+    ("alive", "uint8", lambda N, P, S, K: (N,)),
+    ("general_cell", "int16", lambda N, P, S, K: (N, P)),
+    ("land", "int32", lambda N, P, S, K: (N, P)),
+    ("army_total", "int32", lambda N, P, S, K: (N, P)),
+    ("reward", "int8", lambda N, P, S, K: (K, N, P)),
+    ("done", "uint8", lambda N, P, S, K: (K, N)),
+    ("winner", "int8", lambda N, P, S, K: (K, N)),
+    ("obs_army", "int16", lambda N, P, S, K: (K, N, P, S)),
+    ("obs_owner", "int8", lambda N, P, S, K: (K, N, P, S)),
+    ("obs_terrain", "int8", lambda N, P, S, K: (K, N, P, S)),
+    ("obs_vis", "uint8", lambda N, P, S, K: (K, N, P, S)),
+    ("episodes_done", "int32", lambda N, P, S, K: (N,)),      # bits of uint32
+    ("wins", "int32", lambda N, P, S, K: (N, P)),
+    ("truncations", "int32", lambda N, P, S, K: (N,)),
+    ("sat_events", "int32", lambda N, P, S, K: (N,)),
+    ("obs_digest", "int64", lambda N, P, S, K: (N,)),         # bits of uint64
+    ("actions_out", "int32", lambda N, P, S, K: (K, N, P)),
+]
+
+
+class GenBuffers(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n, _, _ in BUFFERS]
+
+
+class GenSizes(C.Structure):
+    _fields_ = [("plane_stride", C.c_int32), ("alignment", C.c_int32)] + [(n, C.c_size_t) for n, _, _ in BUFFERS]
+
+
+_lib = None
+
+
+def load_library(path=None):
+    """dlopen libgenerals.so and declare the signatures.  Raises if it has not been built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or LIB_PATH
+    if not os.path.exists(path):
+        raise GenError(f"{path} is missing: build it with `python -m paper_2606_23348_b200.build` "
+                       "(hand-written sm_100a kernels; there is no CPU fallback)")
+    lib = C.CDLL(path)
+    env_p = C.c_void_p
+    lib.gen_query_sizes.argtypes = [C.POINTER(GenConfig), C.c_int32, C.POINTER(GenSizes)]
+    lib.gen_init.argtypes = [C.POINTER(GenConfig), C.POINTER(env_p)]
+    lib.gen_set_policy.argtypes = [env_p, C.POINTER(GenPolicy)]
+    lib.gen_global_step.argtypes = [env_p]
+    lib.gen_global_step.restype = C.c_uint32
+    lib.gen_set_global_step.argtypes = [env_p, C.c_uint32]
+    lib.gen_reset.argtypes = [env_p, C.POINTER(GenBuffers), C.c_uint32, C.c_void_p]
+    lib.gen_step.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
+    lib.gen_rollout.argtypes = [env_p, C.POINTER(GenBuffers), C.c_int32, C.c_uint32, C.c_void_p]
+    lib.gen_observe.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p]
+    lib.gen_sample.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
+    lib.gen_step_host.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.gen_set_launch.argtypes = [env_p, C.c_int32]
+    lib.gen_launch_count.argtypes = [env_p]
+    lib.gen_launch_count.restype = C.c_uint64
+    lib.gen_last_cuda_error.argtypes = [env_p]
+    lib.gen_destroy.argtypes = [env_p]
+    lib.gen_destroy.restype = None
+    lib.gen_error_string.argtypes = [C.c_int]
+    lib.gen_error_string.restype = C.c_char_p
+    lib.gen_version.restype = C.c_char_p
+    for name in ("gen_query_sizes", "gen_init", "gen_set_policy", "gen_set_global_step", "gen_reset",
+                 "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host", "gen_set_launch",
+                 "gen_last_cuda_error"):
+        getattr(lib, name).restype = C.c_int
+    if path == LIB_PATH:
+        _lib = lib
+    return lib
+
+
+_CFG_KEYS = [n for n, _ in GenConfig._fields_]
+_POLICY_KEYS = ("pass_thr", "half_thr", "bias_thr")
+
+
+def make_config(cfg):
+    """dict -> GenConfig; the policy thresholds (pass_thr / half_thr / bias_thr) are split off."""
+    c = GenConfig()
+    c.team_size = 1
+    pol = {}
+    for k, v in cfg.items():
+        if k in _POLICY_KEYS:
+            pol[k] = int(v)
+        elif k in _CFG_KEYS:
+            setattr(c, k, int(v))
+        else:
+            raise KeyError(f"unknown config key {k!r}")
+    return c, pol
+
+
+class GeneralsEnv:
+    """N games on one GPU.  Owns the torch tensors the library works on.
+
+    cfg: dict with the gen_config keys plus optional pass_thr / half_thr / bias_thr.
+    k_slots > 1 sizes the output buffers for rollout(K, OBS_EVERY_STEP).
+    """
+
+    def __init__(self, cfg, device="cuda:0", k_slots=1, digest=True, actions_out=True):
+        import torch
+        self.torch = torch
+        self.lib = load_library()
+        if not torch.cuda.is_available():
+            raise GenError("no CUDA device: the Generals.io step runs only on the GPU (no CPU fallback)")
+        self.cfg, pol = make_config(cfg)
+        self.device = torch.device(device)
+        self.N, self.P, self.H, self.W = self.cfg.n_games, self.cfg.n_players, self.cfg.height, self.cfg.width
+        self.HW = self.H * self.W
+        self.K = int(k_slots)
+        sizes = GenSizes()
+        self._check(self.lib.gen_query_sizes(C.byref(self.cfg), self.K, C.byref(sizes)))
+        self.S = sizes.plane_stride
+        self._env = C.c_void_p()
+        self._check(self.lib.gen_init(C.byref(self.cfg), C.byref(self._env)))
+        self.bufs = GenBuffers()
+        self.tensors = {}
+        for name, dt, shape in BUFFERS:
+            if (name == "obs_digest" and not digest) or (name == "actions_out" and not actions_out):
+                setattr(self.bufs, name, None)
+                continue
+            t = torch.zeros(shape(self.N, self.P, self.S, self.K), dtype=getattr(torch, dt), device=self.device)
+            assert t.numel() * t.element_size() == getattr(sizes, name), name
+            self.tensors[name] = t
+            setattr(self, name, t)
+            setattr(self.bufs, name, t.data_ptr() if t.numel() else None)
+        if self.N == 0:
+            for name, _, _ in BUFFERS:                     # any aligned non-NULL value passes validation
+                if name in self.tensors:
+                    setattr(self.bufs, name, 16)
+        self.set_policy(**pol)
+
+    # ------------------------------------------------------------------ plumbing
+    def _check(self, code):
+        if code != 0:
+            msg = self.lib.gen_error_string(code).decode()
+            cuda = self.lib.gen_last_cuda_error(self._env) if getattr(self, "_env", None) else 0
+            raise GenError(f"generals: {msg} (code {code}, cuda error {cuda})")
+
+    def _stream(self, stream=None):
+        s = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        return C.c_void_p(s.cuda_stream)
+
+    def close(self):
+        if getattr(self, "_env", None):
+            self.lib.gen_destroy(self._env)
+            self._env = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ------------------------------------------------------------------ the C ABI, same names
+    def set_policy(self, pass_thr=0, half_thr=1 << 31, bias_thr=0):
+        p = GenPolicy(int(pass_thr), int(half_thr), int(bias_thr))
+        self._check(self.lib.gen_set_policy(self._env, C.byref(p)))
+
+    @property
+    def global_step(self):
+        return int(self.lib.gen_global_step(self._env))
+
+    @global_step.setter
+    def global_step(self, v):
+        self._check(self.lib.gen_set_global_step(self._env, int(v)))
+
+    def set_launch(self, warps_per_cta):
+        self._check(self.lib.gen_set_launch(self._env, int(warps_per_cta)))
+
+    @property
+    def launch_count(self):
+        return int(self.lib.gen_launch_count(self._env))
+
+    def reset(self, keep_episode=False, stream=None):
+        self._check(self.lib.gen_reset(self._env, C.byref(self.bufs), GEN_KEEP_EPISODE if keep_episode else 0,
+                                       self._stream(stream)))
+
+    def step(self, actions=None, stream=None):
+        """actions: int32 CUDA tensor [N][P] of flat action indices, or None for the built-in sampler."""
+        ptr = None
+        if actions is not None:
+            assert actions.is_cuda and actions.dtype == self.torch.int32 and actions.is_contiguous()
+            assert actions.numel() == self.N * self.P
+            ptr = C.c_void_p(actions.data_ptr())
+        self._check(self.lib.gen_step(self._env, C.byref(self.bufs), ptr, self._stream(stream)))
+
+    def rollout(self, K, obs_mode=OBS_DIGEST, stream=None):
+        if obs_mode == OBS_EVERY_STEP and K > self.K:
+            raise GenError(f"rollout(K={K}, OBS_EVERY_STEP) needs k_slots >= {K}, have {self.K}")
+        self._check(self.lib.gen_rollout(self._env, C.byref(self.bufs), int(K), int(obs_mode), self._stream(stream)))
+
+    def observe(self, stream=None):
+        self._check(self.lib.gen_observe(self._env, C.byref(self.bufs), self._stream(stream)))
+
+    def sample(self, out=None, stream=None):
+        if out is None:
+            out = self.torch.zeros((self.N, self.P), dtype=self.torch.int32, device=self.device)
+        self._check(self.lib.gen_sample(self._env, C.byref(self.bufs), C.c_void_p(out.data_ptr()), self._stream(stream)))
+        return out
+
+    def step_host(self, h_actions=None, h_reward=None, h_done=None, stream=None):
+        """End to end through host buffers (pinned CPU tensors); synchronises the stream."""
+        ptr = lambda t: None if t is None else C.c_void_p(t.data_ptr())   # noqa: E731
+        for t in (h_actions, h_reward, h_done):
+            assert t is None or (not t.is_cuda and t.is_contiguous())
+        self._check(self.lib.gen_step_host(self._env, C.byref(self.bufs), ptr(h_actions), ptr(h_reward),
+                                           ptr(h_done), self._stream(stream)))
+
+    # ------------------------------------------------------------------ helpers
+    def field(self, name, slot=0):
+        """numpy view of a buffer (unsigned where the C type is unsigned); slot 0 of [K]-strided ones."""
+        import numpy as np
+        t = self.tensors[name]
+        if name in ("reward", "done", "winner", "obs_army", "obs_owner", "obs_terrain", "obs_vis", "actions_out"):
+            t = t[slot]
+        a = t.cpu().numpy()
+        if name in ("episode", "episodes_done", "wins", "truncations", "sat_events"):
+            a = a.view(np.uint32)
+        elif name == "obs_digest":
+            a = a.view(np.uint64)
+        return a

@@ -1,0 +1,294 @@
+// generals_api.cu -- the C ABI of include/generals.h: host-side validation, launch geometry, launches.
+// No torch types, no allocation of board memory, no synchronisation (except gen_step_host).
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "generals_kernels.cuh"
+
+struct gen_env {
+    gen_config cfg;
+    gen_policy policy;
+    gen::KParams base;       // config-derived fields, filled once
+    uint32_t global_step;
+    int32_t warps_per_cta;   // 0 = default
+    uint64_t launches;
+    int last_cuda_error;
+    bool attr_set[3][5];     // cudaFuncSetAttribute done for <NP idx, WPC idx>
+};
+
+namespace {
+
+inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+int validate(const gen_config *c) {
+    if (c->n_games < 0) return GEN_ERR_CONFIG;
+    if (c->height < 1 || c->height > 32 || c->width < 1 || c->width > 32) return GEN_ERR_CONFIG;
+    if (c->n_players < 2 || c->n_players > 8) return GEN_ERR_CONFIG;
+    if (c->height * c->width < c->n_players) return GEN_ERR_CONFIG;
+    if (c->team_size < 1 || c->team_size > c->n_players) return GEN_ERR_CONFIG;
+    if (c->n_cities < 0 || c->n_cities > c->height * c->width) return GEN_ERR_CONFIG;
+    if (c->city_army_lo < 0 || c->city_army_hi < c->city_army_lo || c->city_army_hi > 32767) return GEN_ERR_CONFIG;
+    if (c->spawn_dmin < 0 || c->spawn_dmax < 0) return GEN_ERR_CONFIG;
+    if (c->spawn_dmax > 0 && c->spawn_dmax < c->spawn_dmin) return GEN_ERR_CONFIG;
+    if (c->spawn_exact && c->spawn_dmax <= 0) return GEN_ERR_CONFIG;
+    if (c->max_turns < 0) return GEN_ERR_CONFIG;
+    if (c->rule_flags & ~7u) return GEN_ERR_CONFIG;
+    if ((uint64_t)c->game_id_base + (uint64_t)c->n_games > 0x100000000ull) return GEN_ERR_CONFIG;
+    return GEN_OK;
+}
+
+void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
+    const size_t N = (size_t)c->n_games, P = (size_t)c->n_players, k = (size_t)K;
+    const size_t S = (size_t)round_up(c->height * c->width, 16);
+    std::memset(s, 0, sizeof(*s));
+    s->plane_stride = (int32_t)S;
+    s->alignment = 16;
+    s->army = N * S * 2; s->owner = N * S; s->terrain = N * S;
+    s->turn = N * 4; s->episode = N * 4; s->alive = N; s->general_cell = N * P * 2;
+    s->land = N * P * 4; s->army_total = N * P * 4;
+    s->reward = k * N * P; s->done = k * N; s->winner = k * N;
+    s->obs_army = k * N * P * S * 2; s->obs_owner = k * N * P * S; s->obs_terrain = k * N * P * S;
+    s->obs_vis = k * N * P * S;
+    s->episodes_done = N * 4; s->wins = N * P * 4; s->truncations = N * 4; s->sat_events = N * 4;
+    s->obs_digest = N * 8; s->actions_out = k * N * P * 4;
+}
+
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+int check_buffers(const gen_buffers *b, bool need_obs) {
+    const void *req[] = {b->army, b->owner, b->terrain, b->turn, b->episode, b->alive, b->general_cell,
+                         b->land, b->army_total, b->reward, b->done, b->winner, b->episodes_done, b->wins,
+                         b->truncations, b->sat_events};
+    for (const void *p : req) {
+        if (!p) return GEN_ERR_NULL;
+        if (!aligned16(p)) return GEN_ERR_ALIGN;
+    }
+    const void *obs[] = {b->obs_army, b->obs_owner, b->obs_terrain, b->obs_vis};
+    for (const void *p : obs) {
+        if (need_obs && !p) return GEN_ERR_NULL;
+        if (p && !aligned16(p)) return GEN_ERR_ALIGN;
+    }
+    if (b->obs_digest && !aligned16(b->obs_digest)) return GEN_ERR_ALIGN;
+    if (b->actions_out && !aligned16(b->actions_out)) return GEN_ERR_ALIGN;
+    return GEN_OK;
+}
+
+template <int NP, int WPC>
+int launch_one(gen_env *env, const gen::KParams &kp, int np_idx, int wpc_idx, cudaStream_t stream) {
+    const size_t smem = (size_t)kp.key_bytes + (size_t)WPC * kp.per_warp_bytes;
+    auto kernel = gen::k_generals<NP, WPC>;
+    if (!env->attr_set[np_idx][wpc_idx]) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
+        env->attr_set[np_idx][wpc_idx] = true;
+    }
+    const int grid = (kp.N + WPC - 1) / WPC;
+    kernel<<<grid, WPC * 32, smem, stream>>>(kp);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
+    env->launches += 1;
+    return GEN_OK;
+}
+
+template <int NP>
+int launch_np(gen_env *env, const gen::KParams &kp, int np_idx, int wpc, cudaStream_t stream) {
+    switch (wpc) {
+        case 1: return launch_one<NP, 1>(env, kp, np_idx, 0, stream);
+        case 2: return launch_one<NP, 2>(env, kp, np_idx, 1, stream);
+        case 4: return launch_one<NP, 4>(env, kp, np_idx, 2, stream);
+        case 16: return launch_one<NP, 16>(env, kp, np_idx, 4, stream);
+        default: return launch_one<NP, 8>(env, kp, np_idx, 3, stream);
+    }
+}
+
+int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, const int32_t *actions,
+           int32_t *sample_out, void *stream) {
+    if (env->cfg.n_games == 0) return GEN_OK;
+    gen::KParams kp = env->base;
+    kp.pass_thr = env->policy.pass_thr;
+    kp.half_thr = env->policy.half_thr;
+    kp.bias_thr = env->policy.bias_thr;
+    kp.global_step0 = env->global_step;
+    kp.flags = flags;
+    kp.K = K;
+    kp.b = *bufs;
+    kp.actions = actions;
+    kp.sample_out = sample_out;
+    kp.key_bytes = (flags & gen::F_DIGEST) ? (uint32_t)(8 * kp.S) : 0u;
+    const int np = kp.P <= 2 ? 2 : (kp.P <= 4 ? 4 : 8);
+    kp.per_warp_bytes = (uint32_t)(4 * kp.S + (np + 3) * gen::MASK_STRIDE);
+    int wpc = env->warps_per_cta ? env->warps_per_cta : 8;
+    while (wpc > 1 && kp.key_bytes + (size_t)wpc * kp.per_warp_bytes > 200u * 1024u) wpc >>= 1;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (np == 2) return launch_np<2>(env, kp, 0, wpc, s);
+    if (np == 4) return launch_np<4>(env, kp, 1, wpc, s);
+    return launch_np<8>(env, kp, 2, wpc, s);
+}
+
+}  // namespace
+
+extern "C" {
+
+int gen_query_sizes(const gen_config *cfg, int32_t k_slots, gen_sizes *out) {
+    if (!cfg || !out) return GEN_ERR_NULL;
+    if (int e = validate(cfg)) return e;
+    if (k_slots < 1) return GEN_ERR_ARG;
+    fill_sizes(cfg, k_slots, out);
+    return GEN_OK;
+}
+
+int gen_init(const gen_config *cfg, gen_env **out) {
+    if (!cfg || !out) return GEN_ERR_NULL;
+    *out = nullptr;
+    if (int e = validate(cfg)) return e;
+    gen_env *env = new (std::nothrow) gen_env();
+    if (!env) return GEN_ERR_ARG;
+    std::memset(env, 0, sizeof(*env));
+    env->cfg = *cfg;
+    env->policy.pass_thr = 0;
+    env->policy.half_thr = 0x80000000u;
+    env->policy.bias_thr = 0;
+    gen::KParams &k = env->base;
+    k.N = cfg->n_games; k.H = cfg->height; k.W = cfg->width; k.P = cfg->n_players;
+    k.HW = k.H * k.W; k.S = round_up(k.HW, 16); k.NW = (k.HW + 31) / 32; k.NC8 = k.S / 8;
+    k.team_size = cfg->team_size;
+    k.n_teams = (cfg->n_players + cfg->team_size - 1) / cfg->team_size;
+    k.n_cities = cfg->n_cities; k.city_lo = cfg->city_army_lo;
+    k.city_span = cfg->city_army_hi - cfg->city_army_lo + 1;
+    k.dmin = cfg->spawn_dmin; k.dmax = cfg->spawn_dmax; k.spawn_exact = cfg->spawn_exact;
+    k.max_turns = cfg->max_turns; k.auto_reset = cfg->auto_reset;
+    k.rule_flags = cfg->rule_flags; k.gid_base = cfg->game_id_base; k.mountain_thr = cfg->mountain_thr;
+    k.key0 = (uint32_t)(cfg->seed & 0xffffffffu); k.key1 = (uint32_t)(cfg->seed >> 32);
+    // row = (cell * recipW) >> 16 must equal cell / W for every cell of the largest board
+    k.recipW = 65536u / (uint32_t)k.W + 1u;
+    for (uint32_t c = 0; c < 1024u; ++c)
+        if (((c * k.recipW) >> 16) != c / (uint32_t)k.W) { delete env; return GEN_ERR_CONFIG; }
+    for (int j = 0; j < 32; ++j) {
+        uint32_t n0 = 0, nl = 0, in = 0;
+        for (int b = 0; b < 32; ++b) {
+            const int c = 32 * j + b;
+            if (c >= k.HW) continue;
+            in |= 1u << b;
+            if (c % k.W != 0) n0 |= 1u << b;
+            if (c % k.W != k.W - 1) nl |= 1u << b;
+        }
+        k.notcol0[j] = n0; k.notcolL[j] = nl; k.inb[j] = in;
+    }
+    *out = env;
+    return GEN_OK;
+}
+
+int gen_set_policy(gen_env *env, const gen_policy *policy) {
+    if (!env || !policy) return GEN_ERR_NULL;
+    env->policy = *policy;
+    return GEN_OK;
+}
+
+uint32_t gen_global_step(const gen_env *env) { return env ? env->global_step : 0u; }
+
+int gen_set_global_step(gen_env *env, uint32_t step) {
+    if (!env) return GEN_ERR_NULL;
+    env->global_step = step;
+    return GEN_OK;
+}
+
+int gen_reset(gen_env *env, const gen_buffers *bufs, uint32_t flags, void *cuda_stream) {
+    if (!env || !bufs) return GEN_ERR_NULL;
+    if (flags & ~(uint32_t)GEN_KEEP_EPISODE) return GEN_ERR_ARG;
+    if (int e = check_buffers(bufs, true)) return e;
+    env->global_step = 0;
+    uint32_t f = gen::F_RESET | gen::F_OBS_PLANES;
+    if (flags & GEN_KEEP_EPISODE) f |= gen::F_KEEP_EPISODE;
+    if (bufs->obs_digest) f |= gen::F_DIGEST;
+    return launch(env, bufs, f, 0, nullptr, nullptr, cuda_stream);
+}
+
+int gen_step(gen_env *env, const gen_buffers *bufs, const int32_t *d_actions, void *cuda_stream) {
+    if (!env || !bufs) return GEN_ERR_NULL;
+    if (int e = check_buffers(bufs, true)) return e;
+    if (d_actions && !aligned16(d_actions)) return GEN_ERR_ALIGN;
+    uint32_t f = gen::F_OBS_PLANES;
+    if (!d_actions) f |= gen::F_SAMPLER;
+    if (bufs->obs_digest) f |= gen::F_DIGEST;
+    const int e = launch(env, bufs, f, 1, d_actions, nullptr, cuda_stream);
+    if (e == GEN_OK) env->global_step += 1;
+    return e;
+}
+
+int gen_rollout(gen_env *env, const gen_buffers *bufs, int32_t K, uint32_t flags, void *cuda_stream) {
+    if (!env || !bufs) return GEN_ERR_NULL;
+    if (K <= 0) return GEN_ERR_ARG;
+    if (flags != GEN_OBS_DIGEST && flags != GEN_OBS_EVERY_STEP && flags != GEN_OBS_NONE) return GEN_ERR_ARG;
+    if (int e = check_buffers(bufs, flags != GEN_OBS_NONE)) return e;
+    if (flags == GEN_OBS_DIGEST && !bufs->obs_digest) return GEN_ERR_NULL;
+    uint32_t f = gen::F_SAMPLER;
+    if (flags == GEN_OBS_DIGEST) f |= gen::F_DIGEST | gen::F_OBS_PLANES;
+    if (flags == GEN_OBS_EVERY_STEP) {
+        f |= gen::F_OBS_PLANES | gen::F_OBS_EVERY;
+        if (bufs->obs_digest) f |= gen::F_DIGEST;
+    }
+    const int e = launch(env, bufs, f, K, nullptr, nullptr, cuda_stream);
+    if (e == GEN_OK) env->global_step += (uint32_t)K;
+    return e;
+}
+
+int gen_observe(gen_env *env, const gen_buffers *bufs, void *cuda_stream) {
+    if (!env || !bufs) return GEN_ERR_NULL;
+    if (int e = check_buffers(bufs, true)) return e;
+    return launch(env, bufs, gen::F_OBSERVE_ONLY | gen::F_OBS_PLANES, 0, nullptr, nullptr, cuda_stream);
+}
+
+int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, void *cuda_stream) {
+    if (!env || !bufs || !d_actions_out) return GEN_ERR_NULL;
+    if (int e = check_buffers(bufs, false)) return e;
+    return launch(env, bufs, gen::F_SAMPLE_ONLY | gen::F_SAMPLER, 0, nullptr, d_actions_out, cuda_stream);
+}
+
+int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
+                  uint8_t *h_done, void *cuda_stream) {
+    if (!env || !bufs) return GEN_ERR_NULL;
+    if (h_actions && !bufs->actions_out) return GEN_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    const size_t N = (size_t)env->cfg.n_games, P = (size_t)env->cfg.n_players;
+    cudaError_t ce = cudaSuccess;
+    if (h_actions) ce = cudaMemcpyAsync(bufs->actions_out, h_actions, N * P * 4, cudaMemcpyHostToDevice, s);
+    if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
+    const int e = gen_step(env, bufs, h_actions ? bufs->actions_out : nullptr, cuda_stream);
+    if (e != GEN_OK) return e;
+    if (h_reward) ce = cudaMemcpyAsync(h_reward, bufs->reward, N * P, cudaMemcpyDeviceToHost, s);
+    if (ce == cudaSuccess && h_done) ce = cudaMemcpyAsync(h_done, bufs->done, N, cudaMemcpyDeviceToHost, s);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
+    if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
+    return GEN_OK;
+}
+
+int gen_set_launch(gen_env *env, int32_t warps_per_cta) {
+    if (!env) return GEN_ERR_NULL;
+    if (warps_per_cta != 0 && warps_per_cta != 1 && warps_per_cta != 2 && warps_per_cta != 4 &&
+        warps_per_cta != 8 && warps_per_cta != 16)
+        return GEN_ERR_ARG;
+    env->warps_per_cta = warps_per_cta;
+    return GEN_OK;
+}
+
+uint64_t gen_launch_count(const gen_env *env) { return env ? env->launches : 0; }
+int gen_last_cuda_error(const gen_env *env) { return env ? env->last_cuda_error : 0; }
+
+void gen_destroy(gen_env *env) { delete env; }
+
+const char *gen_error_string(int code) {
+    switch (code) {
+        case GEN_OK: return "ok";
+        case GEN_ERR_NULL: return "a required pointer is NULL";
+        case GEN_ERR_CONFIG: return "invalid configuration";
+        case GEN_ERR_ALIGN: return "device pointer not 16-byte aligned";
+        case GEN_ERR_ARG: return "invalid argument";
+        case GEN_ERR_CUDA: return "CUDA runtime error (see gen_last_cuda_error)";
+        default: return "unknown error code";
+    }
+}
+
+const char *gen_version(void) { return "generals-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,91 @@
+"""Host-only checks of the C-ABI library: it loads, exports every symbol include/generals.h declares,
+validates configurations and reports sizes.  No kernel is launched (no GPU needed)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2606_23348_b200 import binding, build, workloads
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load_library()
+
+
+def test_exports_every_declared_symbol(lib):
+    header = open(os.path.join(ROOT, "include", "generals.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(gen_[a-z_]+)\s*\(", header))
+    assert declared == set(binding.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert b"sm_100a" in lib.gen_version()
+
+
+def test_struct_layouts_match_header():
+    assert C.sizeof(binding.GenConfig) == 13 * 4 + 3 * 4 + 8
+    assert C.sizeof(binding.GenBuffers) == 22 * 8
+    assert C.sizeof(binding.GenSizes) == 8 + 22 * C.sizeof(C.c_size_t)
+
+
+def test_query_sizes(lib):
+    cfg, _ = binding.make_config(workloads.config("c2_24x24")[0])
+    s = binding.GenSizes()
+    assert lib.gen_query_sizes(C.byref(cfg), 1, C.byref(s)) == 0
+    N, P, S = 16384, 2, 576
+    assert s.plane_stride == S and s.alignment == 16
+    assert s.army == N * S * 2 and s.owner == N * S and s.terrain == N * S
+    assert s.obs_army == N * P * S * 2 and s.obs_vis == N * P * S
+    assert s.reward == N * P and s.done == N and s.obs_digest == 8 * N
+    assert lib.gen_query_sizes(C.byref(cfg), 32, C.byref(s)) == 0
+    assert s.obs_owner == 32 * N * P * S and s.army == N * S * 2
+    cfg5, _ = binding.make_config(workloads.config("c1_8x8", height=5, width=7)[0])
+    assert lib.gen_query_sizes(C.byref(cfg5), 1, C.byref(s)) == 0
+    assert s.plane_stride == 48          # round_up(35, 16)
+
+
+@pytest.mark.parametrize("bad", [dict(height=0), dict(height=33), dict(width=40), dict(n_players=1),
+                                 dict(n_players=9), dict(team_size=0), dict(team_size=3),
+                                 dict(city_army_lo=60), dict(n_cities=-1), dict(spawn_exact=1, spawn_dmax=0),
+                                 dict(spawn_dmax=2), dict(rule_flags=64), dict(max_turns=-5),
+                                 dict(n_games=-1), dict(city_army_hi=40000)])
+def test_bad_config_is_rejected(lib, bad):
+    cfg, _ = binding.make_config(workloads.config("c1_8x8", **bad)[0])
+    env = C.c_void_p()
+    assert lib.gen_init(C.byref(cfg), C.byref(env)) == -2            # GEN_ERR_CONFIG
+    assert not env.value
+    s = binding.GenSizes()
+    assert lib.gen_query_sizes(C.byref(cfg), 1, C.byref(s)) == -2
+
+
+def test_init_argument_errors_without_gpu(lib):
+    cfg, _ = binding.make_config(workloads.config("c1_8x8")[0])
+    env = C.c_void_p()
+    assert lib.gen_init(None, C.byref(env)) == -1
+    assert lib.gen_init(C.byref(cfg), C.byref(env)) == 0 and env.value
+    bufs = binding.GenBuffers()                                       # all NULL
+    assert lib.gen_step(env, C.byref(bufs), None, None) == -1         # GEN_ERR_NULL, nothing launched
+    assert lib.gen_reset(env, C.byref(bufs), 0, None) == -1
+    assert lib.gen_reset(env, C.byref(bufs), 8, None) == -4           # unknown flag
+    assert lib.gen_rollout(env, C.byref(bufs), 0, 0, None) == -4      # K <= 0
+    assert lib.gen_rollout(env, C.byref(bufs), 4, 7, None) == -4      # unknown obs mode
+    for name, _, _ in binding.BUFFERS:
+        setattr(bufs, name, 0x1000)
+    bufs.owner = 0x1008                                               # misaligned
+    assert lib.gen_step(env, C.byref(bufs), None, None) == -3         # GEN_ERR_ALIGN
+    assert lib.gen_set_launch(env, 3) == -4 and lib.gen_set_launch(env, 4) == 0
+    assert lib.gen_launch_count(env) == 0
+    assert lib.gen_set_global_step(env, 41) == 0 and lib.gen_global_step(env) == 41
+    for code in (0, -1, -2, -3, -4, -5, -99):
+        assert lib.gen_error_string(code)
+    lib.gen_destroy(env)
+
+
+def test_missing_library_fails_loudly(tmp_path):
+    with pytest.raises(binding.GenError):
+        binding.load_library(str(tmp_path / "nope.so"))

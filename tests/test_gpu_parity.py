@@ -1,0 +1,400 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle: bit-exact on every state plane,
+observation plane, scoreboard, reward, done flag, accumulator and digest, on the same seeded inputs.
+All of this is integer work, so the bar is equality (BASELINE.json north_star)."""
+import numpy as np
+import pytest
+
+from helpers import DOWN, LEFT, OUT_FIELDS, PASS, RIGHT, STATE_FIELDS, UP, act
+from paper_2606_23348_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+PL, MT, CT, GN = 0, 1, 2, 3
+ALL_FIELDS = STATE_FIELDS + OUT_FIELDS
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    import paper_2606_23348_b200 as g
+    g.load_library()
+    return g
+
+
+def compare(env, o, fields=ALL_FIELDS, digest=True, slot=0, oslot=0, where=""):
+    env.torch.cuda.synchronize()
+    for f in fields:
+        got = env.field(f, slot)
+        want = np.asarray(getattr(o, f))
+        if f in OUT_FIELDS:
+            want = want[oslot]
+        if not np.array_equal(got, want.reshape(got.shape)):
+            bad = np.argwhere(got != want.reshape(got.shape))
+            raise AssertionError(f"{where}: field {f} differs at {bad[:5].tolist()} "
+                                 f"got {got[tuple(bad[0])]} want {want.reshape(got.shape)[tuple(bad[0])]}")
+    if digest:
+        assert np.array_equal(env.field("obs_digest"), o.obs_digest), f"{where}: digest"
+
+
+def make_pair(gpu, oracle_mod, cfg, k_slots=1):
+    env = gpu.GeneralsEnv(cfg, k_slots=k_slots)
+    o = oracle_mod.Oracle(cfg, every_step_K=k_slots if k_slots > 1 else 0)
+    return env, o
+
+
+# ------------------------------------------------------------------------------- config 1 in full
+def test_config1_sampler_every_step(gpu, oracle_mod):
+    """BASELINE config 1: 1v1 8x8, 64 games, 300 steps, built-in sampler; every tensor every step."""
+    cfg, T = workloads.config("c1_8x8")
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    compare(env, o, where="reset")
+    for t in range(T):
+        env.step()
+        acts = o.step(want_actions=True)
+        compare(env, o, where=f"step {t}")
+        assert np.array_equal(env.field("actions_out"), acts)
+    assert env.global_step == T
+    assert int(o.done[0].astype(bool).sum()) > 0          # some games end inside 300 steps
+
+
+def test_config1_explicit_actions(gpu, oracle_mod):
+    """Explicit action path with uniformly random (mostly invalid) and garbage actions."""
+    import torch
+    cfg, T = workloads.config("c1_8x8")
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    rng = np.random.default_rng(5)
+    for t in range(120):
+        if t % 3 == 0:
+            a = workloads.random_actions(rng, 64, 2, 8, 8)
+        else:                                              # valid moves, so that the boards evolve
+            a = o.sample()
+            o.global_step += 1
+            flip = rng.random(a.shape) < 0.1
+            a = np.where(flip, workloads.random_actions(rng, 64, 2, 8, 8), a).astype(np.int32)
+        env.step(torch.from_numpy(a).to(env.device))
+        o.step(a)
+        compare(env, o, where=f"step {t}")
+
+
+# ------------------------------------------------------------------------------- configs 2..5, shrunk N
+@pytest.mark.parametrize("name,N,T,over", [
+    ("c2_24x24", 96, 260, dict(max_turns=120)),
+    ("c4_curriculum", 80, 400, dict(max_turns=300)),
+    ("c5a_2v2", 40, 260, dict(max_turns=200)),
+    ("c5b_ffa8", 40, 260, dict(max_turns=200)),
+    ("c5b_ffa8", 24, 200, dict(n_players=3, height=12, width=13, spawn_dmin=5, n_cities=4, max_turns=150)),
+    ("c2_24x24", 33, 200, dict(height=5, width=7, spawn_dmin=3, n_cities=2, max_turns=90)),
+    ("c2_24x24", 20, 150, dict(height=32, width=32, rule_flags=7, max_turns=100)),
+    ("c1_8x8", 20, 150, dict(height=1, width=32, spawn_dmin=8, n_cities=2)),
+    ("c1_8x8", 20, 150, dict(height=31, width=3, spawn_dmin=8, n_cities=2, auto_reset=1, max_turns=70)),
+])
+def test_sampled_play_matches_oracle(gpu, oracle_mod, name, N, T, over):
+    """Configs 2-5 at reduced N (several CTAs plus a ragged tail), every tensor compared every step."""
+    cfg, _ = workloads.config(name, n_games=N, **over)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    compare(env, o, where="reset")
+    for t in range(T):
+        env.step()
+        o.step()
+        compare(env, o, where=f"{name} step {t}")
+    assert int(o.episodes_done.sum()) > 0
+
+
+def test_captures_happen_and_match(gpu, oracle_mod):
+    """Config 4's biased policy at short spawn distances drives general captures + land transfer."""
+    cfg, _ = workloads.config("c4_curriculum", n_games=128, spawn_dmin=3, spawn_dmax=5, height=10, width=10,
+                              n_cities=3, max_turns=400)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    for t in range(500):
+        env.step()
+        o.step()
+        if t % 10 == 0:
+            compare(env, o, where=f"step {t}")
+    compare(env, o, where="end")
+    assert int(o.wins.sum()) > 20                          # real captures, not truncations
+
+
+# ------------------------------------------------------------------------------- rollout == steps
+@pytest.mark.parametrize("mode", ["digest", "none"])
+def test_rollout_equals_steps(gpu, oracle_mod, mode):
+    cfg, _ = workloads.config("c2_24x24", n_games=70, max_turns=90)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    K = 32
+    for it in range(5):
+        env.rollout(K, gpu.OBS_DIGEST if mode == "digest" else gpu.OBS_NONE)
+        o.rollout(K)
+        if mode == "digest":
+            compare(env, o, where=f"rollout {it}")
+        else:
+            compare(env, o, fields=STATE_FIELDS + ["reward", "done", "winner"], digest=False, where=f"rollout {it}")
+    assert env.global_step == 5 * K
+
+
+def test_rollout_every_step_slots(gpu, oracle_mod):
+    K = 12
+    cfg, _ = workloads.config("c2_24x24", n_games=37, max_turns=20)
+    env, o = make_pair(gpu, oracle_mod, cfg, k_slots=K)
+    env.reset()
+    o.reset()
+    for it in range(3):
+        env.rollout(K, gpu.OBS_EVERY_STEP)
+        o.rollout(K, oracle_mod.OBS_EVERY_STEP)
+        env.torch.cuda.synchronize()
+        for k in range(K):
+            compare(env, o, fields=OUT_FIELDS, digest=False, slot=k, oslot=k, where=f"it {it} slot {k}")
+        compare(env, o, fields=STATE_FIELDS, where=f"it {it}")
+
+
+def test_K_split_and_batch_split_independence(gpu, oracle_mod):
+    """M2: rollout(48) == rollout(16) x 3 == 48 steps; a game_id_base split reproduces the same games."""
+    cfg, _ = workloads.config("c2_24x24", n_games=50, max_turns=40)
+    a = gpu.GeneralsEnv(cfg)
+    a.reset()
+    a.rollout(48)
+    b = gpu.GeneralsEnv(cfg)
+    b.reset()
+    for _ in range(3):
+        b.rollout(16)
+    c0 = gpu.GeneralsEnv(dict(cfg, n_games=19))
+    c1 = gpu.GeneralsEnv(dict(cfg, n_games=31, game_id_base=19))
+    for c in (c0, c1):
+        c.set_launch(4)
+        c.reset()
+        for _ in range(48):
+            c.step()
+    for f in STATE_FIELDS + ["obs_digest", "obs_army", "obs_owner", "obs_terrain", "obs_vis", "reward", "done"]:
+        assert np.array_equal(a.field(f), b.field(f)), f
+        assert np.array_equal(a.field(f), np.concatenate([c0.field(f), c1.field(f)], axis=0)), f
+
+
+@pytest.mark.parametrize("wpc", [1, 2, 4, 8, 16])
+def test_launch_geometry_does_not_change_results(gpu, oracle_mod, wpc):
+    cfg, _ = workloads.config("c1_8x8", n_games=45, auto_reset=1, max_turns=50)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.set_launch(wpc)
+    env.reset()
+    o.reset()
+    for _ in range(4):
+        env.rollout(30)
+        o.rollout(30)
+    compare(env, o, where=f"wpc {wpc}")
+
+
+# ------------------------------------------------------------------------------- hand-built boards
+def put_board(env, o):
+    """Copy a hand-built oracle state into the device buffers and let the library observe it."""
+    import torch
+    for f in ("army", "owner", "terrain", "turn", "alive", "general_cell", "done", "winner"):
+        src = np.asarray(getattr(o, f))
+        if f in ("done", "winner"):
+            src = src[0]
+        env.tensors[f].view(-1).copy_(torch.from_numpy(src.reshape(-1).copy()).to(env.device))
+    env.observe()
+
+
+def run_hand_case(gpu, oracle_mod, H, W, P, cells, actions, turn=0, team_size=1, steps=1, **cfg):
+    import torch
+    from helpers import hand_board
+    o = hand_board(oracle_mod, H, W, P, cells, turn=turn, team_size=team_size, **cfg)
+    base = dict(n_games=1, height=H, width=W, n_players=P, team_size=team_size)
+    base.update(cfg)
+    env = gpu.GeneralsEnv(base, digest=False)
+    put_board(env, o)
+    compare(env, o, fields=["land", "army_total"] + OUT_FIELDS[3:], digest=False, where="observe")
+    for s in range(steps):
+        a = np.asarray(actions[s] if steps > 1 else actions, dtype=np.int32).reshape(1, P)
+        env.step(torch.from_numpy(a).to(env.device))
+        o.step(a)
+        compare(env, o, digest=False, where=f"hand step {s}")
+    return env, o
+
+
+W8_CELLS = {(0, 0): (GN, 0, 3), (3, 2): (PL, 0, 10), (3, 3): (GN, 1, 4), (2, 3): (PL, 1, 7),
+            (1, 3): (PL, 1, 1), (2, 2): (PL, 1, 2), (0, 3): (CT, -1, 45), (1, 1): (MT, -1, 0)}
+
+
+@pytest.mark.parametrize("flags", [0, 2])
+def test_W8_capture_on_gpu(gpu, oracle_mod, flags):
+    env, o = run_hand_case(gpu, oracle_mod, 4, 4, 2, W8_CELLS, [act(3, 2, 4, RIGHT), act(2, 3, 4, LEFT)],
+                           turn=10, rule_flags=flags)
+    assert env.field("army_total")[0].tolist() == [13 if flags else 15, 0]     # the paper-derived value
+    assert env.field("reward")[0].tolist() == [1, -1] and int(env.field("done")[0]) == 1
+
+
+def test_hand_cases_on_gpu(gpu, oracle_mod):
+    g2 = {(0, 0): (GN, 0, 1), (2, 2): (GN, 1, 1)}
+    # W1, W3, W4 (three outcomes), W5 (castle), W6 / W7 (simultaneous), W11 (saturation)
+    cases = [
+        (dict(g2, **{(1, 0): (PL, 0, 5)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 0, 3)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 3)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 4)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 7)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict(g2, **{(1, 0): (PL, 0, 51), (1, 1): (CT, -1, 45)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict(g2, **{(1, 0): (PL, 0, 46), (1, 1): (CT, -1, 45)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict(g2, **{(1, 0): (PL, 0, 4), (1, 2): (PL, 1, 6)}), [act(1, 0, 3, RIGHT), act(1, 2, 3, LEFT)]),
+        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 5)}), [act(1, 0, 3, RIGHT), act(1, 1, 3, LEFT)]),
+        (dict(g2, **{(1, 0): (PL, 0, 21), (1, 1): (PL, 0, 32760)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict(g2, **{(1, 0): (PL, 0, 7)}), [act(1, 0, 3, RIGHT, half=1), PASS]),
+        (dict(g2, **{(1, 1): (PL, 0, 5), (0, 1): (MT, -1, 0)}), [act(1, 1, 3, UP), PASS]),
+        (dict(g2, **{(1, 1): (PL, 0, 5)}), [act(1, 1, 3, DOWN), act(2, 2, 3, UP)]),
+    ]
+    for cells, a in cases:
+        for turn in (0, 1, 49, 99):
+            run_hand_case(gpu, oracle_mod, 3, 3, 2, cells, a, turn=turn)
+            run_hand_case(gpu, oracle_mod, 3, 3, 2, cells, a, turn=turn, rule_flags=4)
+    env, _ = run_hand_case(gpu, oracle_mod, 3, 3, 2, cases[9][0], cases[9][1])
+    assert int(env.field("sat_events")[0]) == 1
+
+
+def test_saturating_growth_on_gpu(gpu, oracle_mod):
+    cells = {(0, 0): (GN, 0, 32766), (2, 2): (GN, 1, 1), (1, 1): (CT, 0, 32767), (0, 1): (PL, 0, 32767)}
+    seq = [[PASS, PASS]] * 4
+    env, o = run_hand_case(gpu, oracle_mod, 3, 3, 2, cells, seq, turn=47, steps=4)
+    assert int(env.field("sat_events")[0]) == int(o.sat_events[0]) > 0
+
+
+def test_team_rules_on_gpu(gpu, oracle_mod):
+    base = {(0, 0): (GN, 0, 1), (0, 4): (GN, 2, 1), (4, 0): (GN, 3, 1), (2, 0): (PL, 0, 6)}
+    run_hand_case(gpu, oracle_mod, 5, 5, 4, dict(base, **{(2, 1): (PL, 1, 3), (4, 4): (GN, 1, 1)}),
+                  [act(2, 0, 5, RIGHT), PASS, PASS, PASS], team_size=2)
+    run_hand_case(gpu, oracle_mod, 5, 5, 4, dict(base, **{(2, 1): (GN, 1, 3)}),
+                  [act(2, 0, 5, RIGHT), PASS, PASS, PASS], team_size=2)
+    cells = {(0, 0): (GN, 0, 1), (0, 2): (GN, 2, 1), (0, 1): (PL, 0, 9), (2, 2): (GN, 3, 1),
+             (2, 1): (PL, 1, 9), (2, 0): (GN, 1, 1), (1, 2): (PL, 3, 4)}
+    env, o = run_hand_case(gpu, oracle_mod, 3, 3, 4, cells,
+                           [[act(0, 1, 3, RIGHT), PASS, PASS, PASS], [PASS, act(2, 1, 3, RIGHT), PASS, PASS]],
+                           team_size=2, steps=2)
+    assert env.field("reward")[0].tolist() == [1, 1, -1, -1]
+
+
+def test_B3_exhaustive_joint_actions_3x3(gpu, oracle_mod):
+    """B3: every joint action pair (81 x 81) on a 3x3 board, one game per pair, in one batch."""
+    import torch
+    from helpers import hand_board
+    cells = {(0, 0): (GN, 0, 4), (2, 2): (GN, 1, 3), (0, 1): (PL, 0, 3), (1, 1): (PL, 1, 5),
+             (1, 0): (CT, -1, 2), (2, 0): (MT, -1, 0), (1, 2): (PL, 1, 2), (0, 2): (PL, 0, 2)}
+    one = hand_board(oracle_mod, 3, 3, 2, cells, turn=1)
+    N = 81 * 81
+    cfg = dict(n_games=N, height=3, width=3, n_players=2)
+    o = oracle_mod.Oracle(cfg)
+    for f in ("army", "owner", "terrain", "turn", "alive", "general_cell"):
+        getattr(o, f)[...] = getattr(one, f)[0]
+    o.winner[:] = -1
+    o.observe()
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    put_board(env, o)
+    a = np.stack(np.meshgrid(np.arange(81), np.arange(81), indexing="ij"), -1).reshape(N, 2).astype(np.int32)
+    env.step(torch.from_numpy(a).to(env.device))
+    o.step(a)
+    compare(env, o, digest=False, where="B3")
+    assert len({bytes(x) for x in env.field("army")}) > 30      # many distinct outcomes
+
+
+def test_frozen_games_and_empty_batch(gpu, oracle_mod):
+    cfg, _ = workloads.config("c1_8x8", n_games=30, max_turns=12, auto_reset=0)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    for t in range(20):
+        env.step()
+        o.step()
+        compare(env, o, where=f"frozen {t}")
+    assert (env.field("done") == 2).all() and (env.field("turn") == 12).all()
+    env.rollout(5)
+    o.rollout(5)
+    compare(env, o, where="frozen rollout")
+    empty = gpu.GeneralsEnv(dict(cfg, n_games=0))
+    empty.reset()
+    empty.step()
+    empty.rollout(3)
+    assert empty.launch_count == 0
+
+
+def test_sample_only_matches_oracle(gpu, oracle_mod):
+    cfg, _ = workloads.config("c4_curriculum", n_games=64, height=12, width=12, spawn_dmax=9, n_cities=4)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    for t in range(60):
+        got = env.sample().cpu().numpy()
+        assert np.array_equal(got, o.sample()), t
+        env.step()
+        o.step()
+
+
+def test_keep_episode_reset(gpu, oracle_mod):
+    import torch
+    cfg, _ = workloads.config("c1_8x8", n_games=16)
+    env = gpu.GeneralsEnv(cfg)
+    env.reset()
+    first = env.field("terrain").copy()
+    env.tensors["episode"].copy_(torch.arange(16, dtype=torch.int32, device=env.device))
+    env.reset(keep_episode=True)
+    again = env.field("terrain")
+    assert np.array_equal(again[0], first[0]) and not np.array_equal(again[1:], first[1:])
+    assert env.field("episode").tolist() == list(range(16))
+
+
+def test_step_host_end_to_end(gpu, oracle_mod):
+    import torch
+    cfg, _ = workloads.config("c1_8x8", n_games=32)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    h_a = torch.zeros((32, 2), dtype=torch.int32).pin_memory()
+    h_r = torch.zeros((32, 2), dtype=torch.int8).pin_memory()
+    h_d = torch.zeros((32,), dtype=torch.uint8).pin_memory()
+    for t in range(40):
+        a = o.sample()
+        h_a.copy_(torch.from_numpy(a))
+        env.step_host(h_a, h_r, h_d)
+        o.step(a)
+        assert np.array_equal(h_r.numpy(), o.reward[0]) and np.array_equal(h_d.numpy(), o.done[0])
+    compare(env, o, where="step_host")
+
+
+# ------------------------------------------------------------------------------- full-size sampled check
+def test_config2_full_size_sampled_games(gpu, oracle_mod):
+    """BASELINE config 2 at its full N = 16,384 in the launch configuration bench.py times: the oracle
+    replays a sample of global game ids (first / last / strided; legitimate because a game depends on
+    its global id only, M2) and must agree on state, observation and digest."""
+    cfg, _ = workloads.config("c2_24x24")
+    env = gpu.GeneralsEnv(cfg)
+    env.reset()
+    T = 240
+    for _ in range(T):
+        env.step()
+    env.torch.cuda.synchronize()
+    ids = sorted(set(list(range(0, 24)) + list(range(16384 - 24, 16384)) + list(range(5, 16384, 1571))))
+    for gid in ids:
+        o = oracle_mod.Oracle(dict(cfg, n_games=1, game_id_base=gid))
+        o.reset()
+        for _ in range(T):
+            o.step()
+        for f in STATE_FIELDS + OUT_FIELDS:
+            got = env.field(f)[gid]
+            want = np.asarray(o.field(f))[0]
+            assert np.array_equal(got, want), (gid, f)
+        assert int(env.field("obs_digest")[gid]) == int(o.obs_digest[0]), gid
+    # properties that hold at any size
+    owner, terrain, army = env.field("owner"), env.field("terrain"), env.field("army")
+    assert (owner[terrain == MT] == -1).all() and (army >= 0).all()
+    for p in range(2):
+        assert np.array_equal(env.field("land")[:, p], (owner[:, :576] == p).sum(1))
+        assert np.array_equal(env.field("army_total")[:, p],
+                              np.where(owner[:, :576] == p, army[:, :576], 0).astype(np.int64).sum(1))
+    vis = env.field("obs_vis")
+    assert ((owner[:, None, :] == np.arange(2)[None, :, None]) <= vis.astype(bool)).all()
