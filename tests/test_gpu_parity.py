@@ -105,7 +105,8 @@ def test_sampled_play_matches_oracle(gpu, oracle_mod, name, N, T, over):
         env.step()
         o.step()
         compare(env, o, where=f"{name} step {t}")
-    assert int(o.episodes_done.sum()) > 0
+    if cfg["max_turns"]:
+        assert int(o.episodes_done.sum()) > 0
 
 
 def test_captures_happen_and_match(gpu, oracle_mod):
@@ -193,6 +194,12 @@ def test_launch_geometry_does_not_change_results(gpu, oracle_mod, wpc):
 
 
 # ------------------------------------------------------------------------------- hand-built boards
+def dict_(a, b):
+    d = dict(a)
+    d.update(b)
+    return d
+
+
 def put_board(env, o):
     """Copy a hand-built oracle state into the device buffers and let the library observe it."""
     import torch
@@ -237,19 +244,19 @@ def test_hand_cases_on_gpu(gpu, oracle_mod):
     g2 = {(0, 0): (GN, 0, 1), (2, 2): (GN, 1, 1)}
     # W1, W3, W4 (three outcomes), W5 (castle), W6 / W7 (simultaneous), W11 (saturation)
     cases = [
-        (dict(g2, **{(1, 0): (PL, 0, 5)}), [act(1, 0, 3, RIGHT), PASS]),
-        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 0, 3)}), [act(1, 0, 3, RIGHT), PASS]),
-        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 3)}), [act(1, 0, 3, RIGHT), PASS]),
-        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 4)}), [act(1, 0, 3, RIGHT), PASS]),
-        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 7)}), [act(1, 0, 3, RIGHT), PASS]),
-        (dict(g2, **{(1, 0): (PL, 0, 51), (1, 1): (CT, -1, 45)}), [act(1, 0, 3, RIGHT), PASS]),
-        (dict(g2, **{(1, 0): (PL, 0, 46), (1, 1): (CT, -1, 45)}), [act(1, 0, 3, RIGHT), PASS]),
-        (dict(g2, **{(1, 0): (PL, 0, 4), (1, 2): (PL, 1, 6)}), [act(1, 0, 3, RIGHT), act(1, 2, 3, LEFT)]),
-        (dict(g2, **{(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 5)}), [act(1, 0, 3, RIGHT), act(1, 1, 3, LEFT)]),
-        (dict(g2, **{(1, 0): (PL, 0, 21), (1, 1): (PL, 0, 32760)}), [act(1, 0, 3, RIGHT), PASS]),
-        (dict(g2, **{(1, 0): (PL, 0, 7)}), [act(1, 0, 3, RIGHT, half=1), PASS]),
-        (dict(g2, **{(1, 1): (PL, 0, 5), (0, 1): (MT, -1, 0)}), [act(1, 1, 3, UP), PASS]),
-        (dict(g2, **{(1, 1): (PL, 0, 5)}), [act(1, 1, 3, DOWN), act(2, 2, 3, UP)]),
+        (dict_(g2, {(1, 0): (PL, 0, 5)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict_(g2, {(1, 0): (PL, 0, 5), (1, 1): (PL, 0, 3)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict_(g2, {(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 3)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict_(g2, {(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 4)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict_(g2, {(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 7)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict_(g2, {(1, 0): (PL, 0, 51), (1, 1): (CT, -1, 45)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict_(g2, {(1, 0): (PL, 0, 46), (1, 1): (CT, -1, 45)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict_(g2, {(1, 0): (PL, 0, 4), (1, 2): (PL, 1, 6)}), [act(1, 0, 3, RIGHT), act(1, 2, 3, LEFT)]),
+        (dict_(g2, {(1, 0): (PL, 0, 5), (1, 1): (PL, 1, 5)}), [act(1, 0, 3, RIGHT), act(1, 1, 3, LEFT)]),
+        (dict_(g2, {(1, 0): (PL, 0, 21), (1, 1): (PL, 0, 32760)}), [act(1, 0, 3, RIGHT), PASS]),
+        (dict_(g2, {(1, 0): (PL, 0, 7)}), [act(1, 0, 3, RIGHT, half=1), PASS]),
+        (dict_(g2, {(1, 1): (PL, 0, 5), (0, 1): (MT, -1, 0)}), [act(1, 1, 3, UP), PASS]),
+        (dict_(g2, {(1, 1): (PL, 0, 5)}), [act(1, 1, 3, DOWN), act(2, 2, 3, UP)]),
     ]
     for cells, a in cases:
         for turn in (0, 1, 49, 99):
@@ -268,9 +275,9 @@ def test_saturating_growth_on_gpu(gpu, oracle_mod):
 
 def test_team_rules_on_gpu(gpu, oracle_mod):
     base = {(0, 0): (GN, 0, 1), (0, 4): (GN, 2, 1), (4, 0): (GN, 3, 1), (2, 0): (PL, 0, 6)}
-    run_hand_case(gpu, oracle_mod, 5, 5, 4, dict(base, **{(2, 1): (PL, 1, 3), (4, 4): (GN, 1, 1)}),
+    run_hand_case(gpu, oracle_mod, 5, 5, 4, dict_(base, {(2, 1): (PL, 1, 3), (4, 4): (GN, 1, 1)}),
                   [act(2, 0, 5, RIGHT), PASS, PASS, PASS], team_size=2)
-    run_hand_case(gpu, oracle_mod, 5, 5, 4, dict(base, **{(2, 1): (GN, 1, 3)}),
+    run_hand_case(gpu, oracle_mod, 5, 5, 4, dict_(base, {(2, 1): (GN, 1, 3)}),
                   [act(2, 0, 5, RIGHT), PASS, PASS, PASS], team_size=2)
     cells = {(0, 0): (GN, 0, 1), (0, 2): (GN, 2, 1), (0, 1): (PL, 0, 9), (2, 2): (GN, 3, 1),
              (2, 1): (PL, 1, 9), (2, 0): (GN, 1, 1), (1, 2): (PL, 3, 4)}
