@@ -1,0 +1,294 @@
+#!/usr/bin/env python
+"""Benchmark of the batched Generals.io environment step (BASELINE.json metric: 1v1 env steps/s on one B200).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch: gen_step for all N games (sampler -> moves /
+combat / capture -> growth -> scoreboard / reward / done / auto-reset -> fog-of-war planes for both
+players written to HBM).  value = env steps/s = games advanced one turn per second, whole job.
+Workload: BASELINE config 2 (1v1 24x24, 16,384 games, auto-reset, four planes per player every step),
+synthetic seeded boards.  One JSON line on stdout (rank 0).
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same
+workload: a deliberately plain program, reported as a baseline only.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "env steps/sec (1v1, all games) on 1 B200; % of HBM or int-issue roofline"
+UNIT = "env_steps/s"
+WORKLOAD = "c2_24x24"
+HBM_FALLBACK_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def algorithmic_bytes_per_env_step(H, W, P):
+    """SURVEY 8(d) B_min: read state 4*HW, write observations 5*P*HW, O(P) scalars
+    (actions 4P, reward P, done + winner 2, scoreboard 8P, turn 4)."""
+    return 4 * H * W + 5 * P * H * W + 13 * P + 6
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    return HBM_FALLBACK_GBS, "B200_PROFILING.md fallback (of fallback)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+def oracle_throughput(cfg, sample_games, steps, warmup):
+    """The oracle as it stands, single-threaded, on the first `sample_games` global game ids."""
+    from oracle import oracle
+    o = oracle.Oracle(dict(cfg, n_games=sample_games))
+    o.reset()
+    for _ in range(warmup):
+        o.step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step()
+    dt = time.perf_counter() - t0
+    return sample_games * steps / dt, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2606_23348_b200 import workloads
+    cfg, _ = workloads.config(WORKLOAD)
+    sample = 256
+    steps = min(args.steps, 400)
+    value, dt = oracle_throughput(cfg, sample, steps, min(args.warmup, 20))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": min(args.warmup, 20), "ms_per_step": 1e3 * dt / steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int16", "data": "synthetic",
+        "config": {"workload": f"{WORKLOAD}: 1v1 24x24, auto-reset, sampler policy 5% pass; each step = "
+                               f"first {sample} of 16,384 games advanced one turn by the CPU oracle"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": f"first {sample} global game ids x {steps} turns, single thread"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg, _ = workloads.config(WORKLOAD)
+    if args.games:
+        cfg["n_games"] = args.games
+    N, P, H, W = cfg["n_games"], cfg["n_players"], cfg["height"], cfg["width"]
+    cfg["game_id_base"] = rank * N                  # weak scaling: disjoint global game-id ranges, no collective
+    K, Wm = args.steps, args.warmup
+    env = GeneralsEnv(cfg, device=dev, digest=False, actions_out=True)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- record the action stream of warm-up + timed steps for the end-to-end leg (device sampler -> host)
+    env.reset()
+    h_actions = torch.empty((Wm + K, N, P), dtype=torch.int32).pin_memory()
+    for t in range(Wm + K):
+        env.step()
+        h_actions[t].copy_(env.tensors["actions_out"][0], non_blocking=True)
+    torch.cuda.synchronize()
+
+    # ---- device-resident leg: per-step kernel, L2 flushed between timed iterations, CUDA events per step
+    env.reset()
+    for _ in range(Wm):
+        env.step()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    launches0 = env.launch_count
+    barrier()
+    for a, b in ev:
+        flush.fill_(1)
+        a.record()
+        env.step()
+        b.record()
+    barrier()
+    kernel_ms = [a.elapsed_time(b) for a, b in ev]
+    launches = env.launch_count - launches0
+    total_ms = max_over_ranks(sum(kernel_ms))
+
+    # ---- same K steps back to back (no flush; state planes partly L2-resident), one event pair
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(K):
+        env.step()
+    e1.record()
+    barrier()
+    b2b_ms = max_over_ranks(e0.elapsed_time(e1))
+
+    # ---- fused rollout leg (K_r = 32 turns per launch, observation digest chained every turn)
+    renv = GeneralsEnv(cfg, device=dev, digest=True, actions_out=False)
+    renv.reset()
+    renv.rollout(32, OBS_DIGEST)
+    n_roll = max(1, K // 32)
+    barrier()
+    e0.record()
+    for _ in range(n_roll):
+        renv.rollout(32, OBS_DIGEST)
+    e1.record()
+    barrier()
+    roll_ms = max_over_ranks(e0.elapsed_time(e1))
+    clock_info = clocks.stop() if rank == 0 else None
+
+    # ---- end-to-end leg: host actions in (pinned), gen_step_host, host reward + done out, every step
+    env.reset()
+    h_reward = torch.zeros((N, P), dtype=torch.int8).pin_memory()
+    h_done = torch.zeros((N,), dtype=torch.uint8).pin_memory()
+    for t in range(Wm):
+        env.step_host(h_actions[t], h_reward, h_done)
+    barrier()
+    t0 = time.perf_counter()
+    for t in range(Wm, Wm + K):
+        env.step_host(h_actions[t], h_reward, h_done)
+    torch.cuda.synchronize()
+    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    checksum = int(h_done.sum())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_src = measured_peak()
+    bmin = algorithmic_bytes_per_env_step(H, W, P)
+    value = world * N * K / (total_ms * 1e-3)
+    med_ms = statistics.median(kernel_ms)
+    achieved = N * bmin / (sum(kernel_ms) / K * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int16", "data": "synthetic",
+        "config": {"workload": f"{WORKLOAD}: 1v1 24x24, {N} games/GPU, auto-reset, max_turns 1000, device Philox "
+                               "sampler 5% pass, 4 obs planes x 2 players written every step",
+                   "n_games_per_gpu": N, "path": "gen_step (per-step kernel, 1 launch per step)",
+                   "l2": "256 MB flush write between timed iterations; each step timed with its own CUDA event pair",
+                   "parallelism": f"replicas x{world}, disjoint game-id ranges, no collective"},
+        "clocks": clock_info,
+        "gpu_launches": launches,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "kernel": "gen::k_generals<2,8> (gen_step)", "peak_source": peak_src,
+                     "algorithmic_bytes_per_env_step": bmin, "units_per_launch": N,
+                     "median_kernel_us": 1e3 * med_ms},
+        "e2e": {"value": world * N * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": N * P * 4,
+                "d2h_bytes_per_step": N * P + N, "api": "gen_step_host (pinned host actions in, reward + done out)",
+                "done_checksum": checksum},
+        "back_to_back": {"value": world * N * K / (b2b_ms * 1e-3), "unit": UNIT, "ms_per_step": b2b_ms / K,
+                         "note": "no L2 flush, one event pair around K launches (includes launch gaps)"},
+        "rollout": {"value": world * N * 32 * n_roll / (roll_ms * 1e-3), "unit": UNIT, "K": 32, "launches": n_roll,
+                    "obs": "digest every turn, planes of the last turn", "bound": "alu"},
+    }
+    if not args.no_cpu_baseline:
+        sample, steps = 256, 400
+        v, _ = oracle_throughput(dict(cfg, game_id_base=0), sample, steps, 5)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"first {sample} global game ids x {steps} turns of {WORKLOAD}, single thread"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--games", type=int, default=0, help="override games per GPU (default: config 2's 16,384)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
