@@ -169,8 +169,10 @@ int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, vo
 int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
                   uint8_t *h_done, void *cuda_stream);
 
-/* Launch geometry override for tuning: warps (games) per CTA in {1,2,4,8,16}; 0 restores the default. */
-int gen_set_launch(gen_env *env, int32_t warps_per_cta);
+/* Launch geometry override for tuning: games per CTA in {4, 8, 16, 32} (8 threads per game); 0 restores
+ * the default (16, halved while the CTA's boards would not leave room for three CTAs per SM).  Results
+ * do not depend on it. */
+int gen_set_launch(gen_env *env, int32_t games_per_cta);
 
 /* Number of kernels this handle has launched (bench.py's gpu_launches). */
 uint64_t gen_launch_count(const gen_env *env);

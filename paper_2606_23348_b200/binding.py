@@ -207,8 +207,8 @@ class GeneralsEnv:
     def global_step(self, v):
         self._check(self.lib.gen_set_global_step(self._env, int(v)))
 
-    def set_launch(self, warps_per_cta):
-        self._check(self.lib.gen_set_launch(self._env, int(warps_per_cta)))
+    def set_launch(self, games_per_cta):
+        self._check(self.lib.gen_set_launch(self._env, int(games_per_cta)))
 
     @property
     def launch_count(self):

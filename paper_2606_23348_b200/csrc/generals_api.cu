@@ -11,10 +11,10 @@ struct gen_env {
     gen_policy policy;
     gen::KParams base;       // config-derived fields, filled once
     uint32_t global_step;
-    int32_t warps_per_cta;   // 0 = default
+    int32_t games_per_cta;   // 0 = default
     uint64_t launches;
     int last_cuda_error;
-    bool attr_set[3][5];     // cudaFuncSetAttribute done for <NP idx, WPC idx>
+    bool attr_set[3];        // cudaFuncSetAttribute done for <NP idx>
 };
 
 namespace {
@@ -74,32 +74,41 @@ int check_buffers(const gen_buffers *b, bool need_obs) {
     return GEN_OK;
 }
 
-template <int NP, int WPC>
-int launch_one(gen_env *env, const gen::KParams &kp, int np_idx, int wpc_idx, cudaStream_t stream) {
-    const size_t smem = (size_t)kp.key_bytes + (size_t)WPC * kp.per_warp_bytes;
-    auto kernel = gen::k_generals<NP, WPC>;
-    if (!env->attr_set[np_idx][wpc_idx]) {
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+constexpr size_t kMaxSmem = 200 * 1024;
+
+inline uint32_t align_up(uint32_t x, uint32_t a) { return (x + a - 1) / a * a; }
+
+// shared-memory layout of one CTA of G games (see generals_kernels.cuh)
+void layout(gen::KParams &k, int G, bool digest) {
+    k.G = G;
+    k.MSW = k.NW | 1;
+    const uint32_t cells = (uint32_t)G * (uint32_t)k.S;
+    uint32_t off = 2 * cells;
+    k.off_owner = off; off += cells;
+    k.off_terr = off; off += cells;
+    k.off_mask = off; off += (uint32_t)(2 * k.P + 3) * (uint32_t)G * (uint32_t)k.MSW * 4u;
+    off = align_up(off, 16);
+    k.off_key = off; off += digest ? 8u * (uint32_t)k.S : 0u;
+    k.off_game = off; off += (uint32_t)G * (uint32_t)sizeof(gen::GameS);
+    off = align_up(off, 8);
+    k.off_bar = off; off += 8;
+    k.smem_bytes = off;
+}
+
+template <int NP>
+int launch_np(gen_env *env, const gen::KParams &kp, int np_idx, cudaStream_t stream) {
+    auto kernel = gen::k_generals<NP>;
+    if (!env->attr_set[np_idx]) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
         if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
-        env->attr_set[np_idx][wpc_idx] = true;
+        env->attr_set[np_idx] = true;
     }
-    const int grid = (kp.N + WPC - 1) / WPC;
-    kernel<<<grid, WPC * 32, smem, stream>>>(kp);
+    const int grid = (kp.N + kp.G - 1) / kp.G;
+    kernel<<<grid, gen::LANES_PER_GAME * kp.G, kp.smem_bytes, stream>>>(kp);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
     env->launches += 1;
     return GEN_OK;
-}
-
-template <int NP>
-int launch_np(gen_env *env, const gen::KParams &kp, int np_idx, int wpc, cudaStream_t stream) {
-    switch (wpc) {
-        case 1: return launch_one<NP, 1>(env, kp, np_idx, 0, stream);
-        case 2: return launch_one<NP, 2>(env, kp, np_idx, 1, stream);
-        case 4: return launch_one<NP, 4>(env, kp, np_idx, 2, stream);
-        case 16: return launch_one<NP, 16>(env, kp, np_idx, 4, stream);
-        default: return launch_one<NP, 8>(env, kp, np_idx, 3, stream);
-    }
 }
 
 int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, const int32_t *actions,
@@ -115,15 +124,24 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     kp.b = *bufs;
     kp.actions = actions;
     kp.sample_out = sample_out;
-    kp.key_bytes = (flags & gen::F_DIGEST) ? (uint32_t)(8 * kp.S) : 0u;
-    const int np = kp.P <= 2 ? 2 : (kp.P <= 4 ? 4 : 8);
-    kp.per_warp_bytes = (uint32_t)(4 * kp.S + (np + 3) * gen::MASK_STRIDE);
-    int wpc = env->warps_per_cta ? env->warps_per_cta : 8;
-    while (wpc > 1 && kp.key_bytes + (size_t)wpc * kp.per_warp_bytes > 200u * 1024u) wpc >>= 1;
+    // games per CTA: 16 by default; fewer when the boards are large, so that >= 3 CTAs share an SM
+    int G = env->games_per_cta ? env->games_per_cta : 16;
+    layout(kp, G, (flags & gen::F_DIGEST) != 0);
+    while (G > 4 && (kp.smem_bytes > kMaxSmem || (!env->games_per_cta && kp.smem_bytes > 72u * 1024u))) {
+        G >>= 1;
+        layout(kp, G, (flags & gen::F_DIGEST) != 0);
+    }
+    if (kp.smem_bytes > kMaxSmem) return GEN_ERR_CONFIG;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    if (np == 2) return launch_np<2>(env, kp, 0, wpc, s);
-    if (np == 4) return launch_np<4>(env, kp, 1, wpc, s);
-    return launch_np<8>(env, kp, 2, wpc, s);
+    if (kp.P <= 2) return launch_np<2>(env, kp, 0, s);
+    if (kp.P <= 4) return launch_np<4>(env, kp, 1, s);
+    return launch_np<8>(env, kp, 2, s);
+}
+
+uint64_t host_mix64(uint64_t z) {  // splitmix64 finaliser: the digest keys of R28
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ull;
+    z ^= z >> 27; z *= 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
 }
 
 }  // namespace
@@ -164,6 +182,8 @@ int gen_init(const gen_config *cfg, gen_env **out) {
     k.recipW = 65536u / (uint32_t)k.W + 1u;
     for (uint32_t c = 0; c < 1024u; ++c)
         if (((c * k.recipW) >> 16) != c / (uint32_t)k.W) { delete env; return GEN_ERR_CONFIG; }
+    k.key_sum = 0;
+    for (int c = 0; c < k.HW; ++c) k.key_sum += host_mix64((uint64_t)(c + 1) * 0x9E3779B97F4A7C15ull) | 1ull;
     for (int j = 0; j < 32; ++j) {
         uint32_t n0 = 0, nl = 0, in = 0;
         for (int b = 0; b < 32; ++b) {
@@ -263,12 +283,12 @@ int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_action
     return GEN_OK;
 }
 
-int gen_set_launch(gen_env *env, int32_t warps_per_cta) {
+int gen_set_launch(gen_env *env, int32_t games_per_cta) {
     if (!env) return GEN_ERR_NULL;
-    if (warps_per_cta != 0 && warps_per_cta != 1 && warps_per_cta != 2 && warps_per_cta != 4 &&
-        warps_per_cta != 8 && warps_per_cta != 16)
+    if (games_per_cta != 0 && games_per_cta != 4 && games_per_cta != 8 && games_per_cta != 16 &&
+        games_per_cta != 32)
         return GEN_ERR_ARG;
-    env->warps_per_cta = warps_per_cta;
+    env->games_per_cta = games_per_cta;
     return GEN_OK;
 }
 
@@ -289,6 +309,6 @@ const char *gen_error_string(int code) {
     }
 }
 
-const char *gen_version(void) { return "generals-b200 0.1 (sm_100a)"; }
+const char *gen_version(void) { return "generals-b200 0.2 (sm_100a)"; }
 
 }  // extern "C"
