@@ -78,21 +78,23 @@ constexpr size_t kMaxSmem = 200 * 1024;
 
 inline uint32_t align_up(uint32_t x, uint32_t a) { return (x + a - 1) / a * a; }
 
-// shared-memory layout of one CTA of G games (see generals_kernels.cuh)
-void layout(gen::KParams &k, int G, bool digest) {
-    k.G = G;
-    k.MSW = k.NW | 1;
-    const uint32_t cells = (uint32_t)G * (uint32_t)k.S;
-    uint32_t off = 2 * cells;
-    k.off_owner = off; off += cells;
-    k.off_terr = off; off += cells;
-    k.off_mask = off; off += (uint32_t)(2 * k.P + 3) * (uint32_t)G * (uint32_t)k.MSW * 4u;
-    off = align_up(off, 16);
-    k.off_key = off; off += digest ? 8u * (uint32_t)k.S : 0u;
-    k.off_game = off; off += (uint32_t)G * (uint32_t)sizeof(gen::GameS);
+// shared-memory layout of one CTA of WPC warps (see generals_kernels.cuh):
+// [column / in-bounds tables | digest keys | warp 0 slice | warp 1 slice | ...]
+void layout(gen::KParams &k, int WPC, bool digest) {
+    k.WPC = WPC;
+    const uint32_t GW = (uint32_t)gen::GW, S = (uint32_t)k.S;
+    k.off_key = 3u * 32u * 4u;
+    k.off_warp0 = align_up(k.off_key + (digest ? 8u * S : 0u), 128);
+    uint32_t off = 2 * GW * S;
+    k.w_owner = off; off += GW * S;
+    k.w_terr = off; off += GW * S;
+    k.w_mask = off; off += GW * (uint32_t)k.M * (uint32_t)k.RW * 4u;
     off = align_up(off, 8);
-    k.off_bar = off; off += 8;
-    k.smem_bytes = off;
+    k.w_game = off; off += GW * (uint32_t)sizeof(gen::GameS);
+    off = align_up(off, 8);
+    k.w_bar = off; off += 8;
+    k.warp_bytes = align_up(off, 128);
+    k.smem_bytes = k.off_warp0 + (uint32_t)WPC * k.warp_bytes;
 }
 
 template <int NP>
@@ -103,8 +105,9 @@ int launch_np(gen_env *env, const gen::KParams &kp, int np_idx, cudaStream_t str
         if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
         env->attr_set[np_idx] = true;
     }
-    const int grid = (kp.N + kp.G - 1) / kp.G;
-    kernel<<<grid, gen::LANES_PER_GAME * kp.G, kp.smem_bytes, stream>>>(kp);
+    const int per_cta = gen::GW * kp.WPC;
+    const int grid = (kp.N + per_cta - 1) / per_cta;
+    kernel<<<grid, 32 * kp.WPC, kp.smem_bytes, stream>>>(kp);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
     env->launches += 1;
@@ -124,12 +127,12 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     kp.b = *bufs;
     kp.actions = actions;
     kp.sample_out = sample_out;
-    // games per CTA: 16 by default; fewer when the boards are large, so that >= 3 CTAs share an SM
-    int G = env->games_per_cta ? env->games_per_cta : 16;
-    layout(kp, G, (flags & gen::F_DIGEST) != 0);
-    while (G > 4 && (kp.smem_bytes > kMaxSmem || (!env->games_per_cta && kp.smem_bytes > 72u * 1024u))) {
-        G >>= 1;
-        layout(kp, G, (flags & gen::F_DIGEST) != 0);
+    // warps per CTA (4 games each): 2 by default; fewer while the CTA would not fit
+    int WPC = env->games_per_cta ? env->games_per_cta / gen::GW : 2;
+    layout(kp, WPC, (flags & gen::F_DIGEST) != 0);
+    while (WPC > 1 && kp.smem_bytes > kMaxSmem) {
+        WPC >>= 1;
+        layout(kp, WPC, (flags & gen::F_DIGEST) != 0);
     }
     if (kp.smem_bytes > kMaxSmem) return GEN_ERR_CONFIG;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -170,6 +173,7 @@ int gen_init(const gen_config *cfg, gen_env **out) {
     gen::KParams &k = env->base;
     k.N = cfg->n_games; k.H = cfg->height; k.W = cfg->width; k.P = cfg->n_players;
     k.HW = k.H * k.W; k.S = round_up(k.HW, 16); k.NW = (k.HW + 31) / 32; k.NC8 = k.S / 8;
+    k.NCH = 4 * k.NW; k.WPL = (k.NW + gen::LPG - 1) / gen::LPG; k.RW = k.NW | 1; k.M = 2 * k.P + 3;
     k.team_size = cfg->team_size;
     k.n_teams = (cfg->n_players + cfg->team_size - 1) / cfg->team_size;
     k.n_cities = cfg->n_cities; k.city_lo = cfg->city_army_lo;

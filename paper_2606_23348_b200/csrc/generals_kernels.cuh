@@ -1,20 +1,25 @@
 // generals_kernels.cuh -- device code of the batched Generals.io step for sm_100a.
 //
-// One CTA owns G consecutive games (G = 8, 16 or 32; 8 threads per game).  Their three state planes
-// (int16 army, int8 owner, int8 terrain) are contiguous in HBM and are staged in shared memory with
-// three TMA bulk copies (cp.async.bulk + mbarrier).  The work then alternates between two mappings:
+// WARP-AUTONOMOUS design.  A warp owns GW = 4 consecutive games; an OCTET of 8 lanes owns one game
+// from load to store.  The warp's three state planes (int16 army, int8 owner, int8 terrain of its 4
+// games) are contiguous in HBM and are staged in the warp's own slice of shared memory with three TMA
+// bulk copies (cp.async.bulk + the warp's own mbarrier).  After one CTA barrier in the prologue (small
+// constant tables) no warp ever waits for another one: phases are separated by __syncwarp() only, so
+// while one warp waits for its loads or drains its observation stores the others compute.
 //
-//   * CELL passes -- an "octet" of 8 lanes per game walks the board in 8-cell chunks with
+//   * CELL passes -- the octet walks its board in 8-cell chunks (lane l: chunks l, l+8, ...) with
 //     SIMD-in-register byte arithmetic and 16 / 8-byte shared and global accesses: bitboard
-//     construction, growth, observation planes (the dominant HBM traffic, streaming stores),
-//     observation digest, write-back of the dirty 32-byte sectors of the state.
-//   * GAME passes -- one thread per game (or per game x player) runs the scalar rules on FLAT
-//     BITBOARDS (one bit per cell, word j = cells 32j..32j+31) held in shared memory: the Philox
-//     valid-action sampler (popcount enumeration), move / combat / capture, termination, fog-of-war
-//     dilation (funnel shifts).  32 games advance per warp instruction instead of one.
+//     construction, tick growth, observation planes (the dominant HBM traffic, full-sector streaming
+//     stores), observation digest.
+//   * WORD passes -- flat bitboards (one bit per cell, word j = cells 32j..32j+31: own[p], mountain,
+//     structure, army >= 2, vis[p]) live in shared memory; lane l of the octet owns the WPL
+//     consecutive words l*WPL.. of each row: Philox valid-action sampler (popcount enumeration,
+//     octet scan), structure growth (bit iteration), fog-of-war dilation (funnel shifts).
+//   * SERIAL passes -- lane 0 of the octet runs the scalar rules: move / combat / capture,
+//     termination, reward; four games advance per warp instruction.
 //
-// Rare heavy paths (board generation at reset, general capture with land transfer, int16 saturation)
-// are taken per game and never tax the common path.
+// Rare heavy paths (board generation at reset: the whole warp per game; general capture with land
+// transfer; int16 saturation) never tax the common path.
 //
 // Rules: PAPER.md section IV, readings R1..R32 of DESIGN.md.  This file shares nothing
 // with oracle/ (the CPU checker); it is written from the same rules text.
@@ -27,7 +32,9 @@
 namespace gen {
 
 constexpr uint32_t FULL = 0xffffffffu;
-constexpr int LANES_PER_GAME = 8;  // the octet
+constexpr int LPG = 8;            // lanes per game: the octet
+constexpr int GW = 32 / LPG;      // games per warp
+constexpr int MAXWPL = 32 / LPG;  // bitboard words per lane (NW <= 32 words)
 
 enum : uint32_t {
     F_RESET = 1u << 0,         // generate every board first (gen_reset)
@@ -42,7 +49,7 @@ enum : uint32_t {
 
 enum : int { T_PLAIN = 0, T_MOUNTAIN = 1, T_CITY = 2, T_GENERAL = 3, T_FOG = 4 };
 
-// per-game flags raised by the game passes for the next cell pass
+// per-game flags raised by the serial passes for the following parallel pass
 enum : uint32_t {
     GF_REBUILD = 1u << 0,        // planes changed wholesale: rebuild the bitboards
     GF_RECOUNT = 1u << 1,        // recount army totals from the planes
@@ -54,26 +61,27 @@ enum : uint32_t {
     GF_ALL_DIRTY = 1u << 7,      // write back the whole army / owner planes
 };
 
-// per-game scalars in shared memory (one thread owns a game during the game passes)
+// per-game scalars in shared memory
 struct GameS {
     int32_t turn, winner;
-    uint32_t alive, done, episode, flags, dirtyO, sat;
-    uint32_t dirtyA[2];
+    uint32_t alive, done, episode, flags, sat, dirtyO;  // dirtyO bit u: owner cells 32u..32u+31 changed
+    uint32_t dirtyA[2];                                 // bit u: army cells 16u..16u+15 changed
     unsigned long long digest;
     int32_t tot[8], land[8], act[8];
     int32_t rew_bits, pad_;
 };
 
 struct KParams {
-    int32_t N, H, W, P, HW, S, NW, NC8;
+    int32_t N, H, W, P, HW, S, NW, NC8, NCH, WPL, RW, M;
     int32_t team_size, n_teams;
     int32_t n_cities, city_lo, city_span;
     int32_t dmin, dmax, spawn_exact, max_turns, auto_reset;
     uint32_t rule_flags, gid_base, mountain_thr, key0, key1;
     uint32_t pass_thr, half_thr, bias_thr;
     uint32_t global_step0, flags, recipW;
-    int32_t K, G, MSW;  // games per CTA; mask row stride in words (odd)
-    uint32_t off_owner, off_terr, off_mask, off_key, off_game, off_bar, smem_bytes;
+    int32_t K, WPC;  // turns per launch; warps per CTA
+    // shared memory: [tables | digest keys | warp 0 | warp 1 | ...]; w_* are offsets inside a warp's slice
+    uint32_t off_key, off_warp0, warp_bytes, w_owner, w_terr, w_mask, w_game, w_bar, smem_bytes;
     unsigned long long key_sum;  // sum of the digest keys of cells 0..HW-1
     gen_buffers b;
     const int32_t *actions;
@@ -137,9 +145,15 @@ __device__ __forceinline__ int select_kth(uint32_t word, uint32_t k, uint32_t la
 }
 
 // SIMD-in-register byte helpers
-__device__ __forceinline__ uint32_t nib_to_bytes(uint32_t nib) {  // 4 bits -> 4 bytes 0x00 / 0xFF
-    return ((nib * 0x00204081u) & 0x01010101u) * 0xFFu;
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
+    return d;
 }
+// 4 bits -> a word whose byte i has bit i of the nibble in its MSB (other bits are don't-care);
+// prmt's sign-replicate selectors (8 | byte index) then expand it: 0xBA98 -> four 0x00 / 0xFF byte
+// masks, 0x9988 / 0xBBAA -> the two int16-pair masks of cells (0, 1) / (2, 3).
+__device__ __forceinline__ uint32_t nib_sign(uint32_t nib) { return nib * 0x10204080u; }
 // bytes holding 0/1 in bit 0: x0 = cells 0..3, x1 = cells 4..7 -> 8 bits
 __device__ __forceinline__ uint32_t gather8(uint32_t x0, uint32_t x1) {
     return ((x1 * 16u + x0) * 0x01020408u) >> 24;
@@ -184,34 +198,37 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 template <int NP>
 __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParams kp) {
     extern __shared__ __align__(128) unsigned char smem[];
-    const int tid = threadIdx.x, nthreads = blockDim.x;
+    const int tid = threadIdx.x;
     const uint32_t lane = tid & 31u;
-    const int warp = tid >> 5, nwarps = nthreads >> 5;
-    const int H = kp.H, W = kp.W, P = kp.P, HW = kp.HW, S = kp.S, NW = kp.NW, NC8 = kp.NC8, G = kp.G;
-    const int MSW = kp.MSW, NCH = 4 * NW;  // mask bytes per row that hold board cells
+    const int wic = tid >> 5;
+    const int ol = (int)(lane & (LPG - 1)), sub = (int)(lane / LPG);  // lane of the octet, game of the warp
+    const uint32_t gmask = ((1u << LPG) - 1u) << (sub * LPG);         // the lanes of this octet
+    const int H = kp.H, W = kp.W, P = kp.P, HW = kp.HW, S = kp.S, NW = kp.NW, NC8 = kp.NC8;
+    const int RW = kp.RW, WPL = kp.WPL, M = kp.M;
     const uint32_t flags = kp.flags;
     const gen_buffers &B = kp.b;
-    const int g0 = blockIdx.x * G;
-    const int ng = min(G, kp.N - g0);
+    const int wg0 = (blockIdx.x * kp.WPC + wic) * GW;  // first game of this warp
+    const int nwg = min(GW, kp.N - wg0);               // games of this warp (<= 0: nothing to do)
+    const bool gvalid = sub < nwg;
+    const int g = wg0 + sub;
     const uint32_t allp = (1u << P) - 1u;
 
-    int16_t *s_army = reinterpret_cast<int16_t *>(smem);
-    int8_t *s_owner = reinterpret_cast<int8_t *>(smem + kp.off_owner);
-    int8_t *s_terr = reinterpret_cast<int8_t *>(smem + kp.off_terr);
-    uint32_t *s_mask = reinterpret_cast<uint32_t *>(smem + kp.off_mask);
+    // CTA-wide tables: column / in-bounds masks of the flat bitboard words, digest keys
+    uint32_t *s_nc0 = reinterpret_cast<uint32_t *>(smem), *s_ncL = s_nc0 + 32, *s_inb = s_nc0 + 64;
     uint64_t *s_key = reinterpret_cast<uint64_t *>(smem + kp.off_key);
-    GameS *s_game = reinterpret_cast<GameS *>(smem + kp.off_game);
-    unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(smem + kp.off_bar);
+    // this warp's slice
+    unsigned char *wb = smem + kp.off_warp0 + (size_t)wic * kp.warp_bytes;
+    int16_t *s_army = reinterpret_cast<int16_t *>(wb);
+    int8_t *s_owner = reinterpret_cast<int8_t *>(wb + kp.w_owner);
+    int8_t *s_terr = reinterpret_cast<int8_t *>(wb + kp.w_terr);
+    uint32_t *s_mask = reinterpret_cast<uint32_t *>(wb + kp.w_mask);
+    GameS *s_game = reinterpret_cast<GameS *>(wb + kp.w_game);
+    const uint32_t bar = smem_u32(wb + kp.w_bar);
 
-    // mask rows: own[0..P-1], mountain, structure (city / general), army >= 2, vis[0..P-1]
+    // mask rows of a game: own[0..P-1], mountain, structure (city / general), army >= 2, vis[0..P-1]
     const int M_MTN = P, M_STR = P + 1, M_A2 = P + 2, M_VIS = P + 3;
-    auto mrow = [&](int m, int lg) -> uint32_t * { return s_mask + (m * G + lg) * MSW; };
+    auto mrow = [&](int m, int lg) -> uint32_t * { return s_mask + (lg * M + m) * RW; };
     auto mrow8 = [&](int m, int lg) -> unsigned char * { return reinterpret_cast<unsigned char *>(mrow(m, lg)); };
-
-    // octet identity for the cell passes
-    const int og = tid >> 3, ol = tid & 7;
-    const bool ovalid = og < ng;
-    const uint32_t omask = 0xFFu << (lane & 24u);  // the lanes of this octet
 
     auto team_mask = [&](int p) -> uint32_t {
         const int t = p / kp.team_size;
@@ -225,8 +242,8 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         int16_t *A = s_army + (size_t)lg * S;
         int8_t *O = s_owner + (size_t)lg * S, *Tr = s_terr + (size_t)lg * S;
         GameS &gs = s_game[lg];
-        const int g = g0 + lg;
-        const uint32_t gid = kp.gid_base + (uint32_t)g, episode = gs.episode;
+        const int gg = wg0 + lg;
+        const uint32_t gid = kp.gid_base + (uint32_t)gg, episode = gs.episode;
         __syncwarp();
         for (int i = lane; i < S / 4; i += 32) {
             reinterpret_cast<uint32_t *>(O)[i] = 0xFFFFFFFFu;
@@ -290,7 +307,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 Tr[cell] = (int8_t)T_GENERAL;
                 O[cell] = (int8_t)p;
                 A[cell] = 1;
-                B.general_cell[(size_t)g * P + p] = (int16_t)cell;
+                B.general_cell[(size_t)gg * P + p] = (int16_t)cell;
             }
         }
         __syncwarp();
@@ -322,7 +339,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
 
     // ---------------------------------------------------------------- cell pass: bitboards of one chunk
     auto build_chunk = [&](int lg, int ch) {
-        unsigned char mb[NP + 3];
+        uint32_t mb[NP + 3];
 #pragma unroll
         for (int i = 0; i < NP + 3; ++i) mb[i] = 0;
         if (ch < NC8) {
@@ -332,70 +349,99 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             if (NP == 2) {
                 // owner in {-1, 0, 1}: bit 7 = neutral, bit 0 = player
                 const uint32_t nx = o.x >> 7, ny = o.y >> 7;
-                mb[0] = (unsigned char)gather8(~o.x & ~nx & 0x01010101u, ~o.y & ~ny & 0x01010101u);
-                mb[1] = (unsigned char)gather8(o.x & ~nx & 0x01010101u, o.y & ~ny & 0x01010101u);
+                mb[0] = gather8(~(o.x | nx) & 0x01010101u, ~(o.y | ny) & 0x01010101u);
+                mb[1] = gather8(o.x & ~nx & 0x01010101u, o.y & ~ny & 0x01010101u);
             } else {
 #pragma unroll
                 for (int p = 0; p < NP; ++p)
                     if (p < P) {
                         const uint32_t pat = 0x01010101u * (uint32_t)p;
-                        mb[p] = (unsigned char)gather8(eq_bytes(o.x, pat), eq_bytes(o.y, pat));
+                        mb[p] = gather8(eq_bytes(o.x, pat), eq_bytes(o.y, pat));
                     }
             }
             // terrain in {0,1,2,3}: mountain = 01, structure (city / general) = 1x
             const uint32_t hx = t.x >> 1, hy = t.y >> 1;
-            mb[NP] = (unsigned char)gather8(t.x & ~hx & 0x01010101u, t.y & ~hy & 0x01010101u);
-            mb[NP + 1] = (unsigned char)gather8(hx & 0x01010101u, hy & 0x01010101u);
-            mb[NP + 2] = (unsigned char)ge2_bits(a);
+            mb[NP] = gather8(t.x & ~hx & 0x01010101u, t.y & ~hy & 0x01010101u);
+            mb[NP + 1] = gather8(hx & 0x01010101u, hy & 0x01010101u);
+            mb[NP + 2] = ge2_bits(a);
         }
 #pragma unroll
         for (int p = 0; p < NP; ++p)
-            if (p < P) mrow8(p, lg)[ch] = mb[p];
-        mrow8(M_MTN, lg)[ch] = mb[NP];
-        mrow8(M_STR, lg)[ch] = mb[NP + 1];
-        mrow8(M_A2, lg)[ch] = mb[NP + 2];
+            if (p < P) mrow8(p, lg)[ch] = (unsigned char)mb[p];
+        mrow8(M_MTN, lg)[ch] = (unsigned char)mb[NP];
+        mrow8(M_STR, lg)[ch] = (unsigned char)mb[NP + 1];
+        mrow8(M_A2, lg)[ch] = (unsigned char)mb[NP + 2];
     };
-
-    // octet: rebuild all bitboards of game lg, then land (and army totals if asked) from them
-    auto rebuild_game = [&](int lg, bool recount) {
+    // octet: all bitboards of game lg (the caller syncs the warp afterwards)
+    auto build_game = [&](int lg) {
+#pragma unroll 3
+        for (int ch = ol; ch < kp.NCH; ch += LPG) build_chunk(lg, ch);
+    };
+    // octet: scoreboard from the planes / bitboards (after a capture, a saturation, a reset; gen_observe)
+    auto recount = [&](int lg, bool do_land, bool do_tot) {
         GameS &gs = s_game[lg];
-        for (int ch = ol; ch < NCH; ch += LANES_PER_GAME) build_chunk(lg, ch);
-        if (ol == 0) {
-            for (int p = 0; p < P; ++p) { gs.land[p] = 0; if (recount) gs.tot[p] = 0; }
-        }
-        __syncwarp(omask);
+        const int16_t *A = s_army + (size_t)lg * S;
         for (int p = 0; p < P; ++p) {
-            int l = 0;
-            for (int j = ol; j < NW; j += LANES_PER_GAME) l += __popc(mrow(p, lg)[j] & kp.inb[j]);
-            if (l) atomicAdd(&gs.land[p], l);
-        }
-        if (recount) {
-            for (int ch = ol; ch < NC8; ch += LANES_PER_GAME) {
-                const int16_t *A = s_army + (size_t)lg * S + 8 * ch;
-                for (int p = 0; p < P; ++p) {
-                    uint32_t m = mrow8(p, lg)[ch];
-                    int sum = 0;
+            int l = 0, sum = 0;
+            for (int i = 0; i < WPL; ++i) {
+                const int j = ol * WPL + i;
+                if (j >= NW) break;
+                uint32_t m = mrow(p, lg)[j] & s_inb[j];
+                l += __popc(m);
+                if (do_tot)
                     while (m) {
                         const int b = __ffs(m) - 1;
                         m &= m - 1;
-                        sum += A[b];
+                        sum += A[32 * j + b];
                     }
-                    if (sum) atomicAdd(&gs.tot[p], sum);
-                }
+            }
+            l = __reduce_add_sync(gmask, l);
+            sum = __reduce_add_sync(gmask, sum);
+            if (ol == 0) {
+                if (do_land) gs.land[p] = l;
+                if (do_tot) gs.tot[p] = sum;
             }
         }
-        __syncwarp(omask);
     };
 
-    // ================================================================ load
+    // ================================================================ prologue
+    if (tid < 32) {
+        s_nc0[tid] = kp.notcol0[tid];
+        s_ncL[tid] = kp.notcolL[tid];
+        s_inb[tid] = kp.inb[tid];
+    }
     if (flags & F_DIGEST) {
-        for (int c = tid; c < S; c += nthreads)
+        for (int c = tid; c < S; c += blockDim.x)
             s_key[c] = (c < HW) ? (mix64((uint64_t)(c + 1) * 0x9E3779B97F4A7C15ull) | 1ull) : 0ull;
     }
+    const bool loading = !(flags & F_RESET) && nwg > 0;
+    if (loading && lane == 0) {
+        mbar_init(bar, 1);
+        const uint32_t cells = (uint32_t)nwg * (uint32_t)S;
+        mbar_expect_tx(bar, 4u * cells);
+        bulk_g2s(smem_u32(s_army), B.army + (size_t)wg0 * S, 2u * cells, bar);
+        bulk_g2s(smem_u32(s_owner), B.owner + (size_t)wg0 * S, cells, bar);
+        bulk_g2s(smem_u32(s_terr), B.terrain + (size_t)wg0 * S, cells, bar);
+    }
+    if (loading && gvalid) {  // per-game scalars, spread over the octet
+        GameS &gs = s_game[sub];
+        if (ol < P) {
+            gs.tot[ol] = B.army_total[(size_t)g * P + ol];
+            gs.land[ol] = B.land[(size_t)g * P + ol];
+        }
+        if (ol == 0) { gs.turn = B.turn[g]; gs.episode = B.episode[g]; }
+        if (ol == 1) { gs.alive = B.alive[g]; gs.done = B.done[g]; gs.winner = B.winner[g]; }
+        if (ol == 2) {
+            gs.flags = 0; gs.sat = 0; gs.dirtyO = 0; gs.dirtyA[0] = 0; gs.dirtyA[1] = 0; gs.rew_bits = 0;
+            gs.digest = ((flags & F_DIGEST) && B.obs_digest) ? B.obs_digest[g] : 0ull;
+        }
+    }
+    __syncthreads();  // the only CTA barrier: tables (and the mbarrier init) are visible
+    if (nwg <= 0) return;
+
     if (flags & F_RESET) {
-        if (tid < ng) {
-            GameS &gs = s_game[tid];
-            const int g = g0 + tid;
+        if (gvalid && ol == 0) {
+            GameS &gs = s_game[sub];
             gs.episode = (flags & F_KEEP_EPISODE) ? B.episode[g] : 0u;
             gs.flags = 0; gs.done = 0; gs.winner = -1; gs.digest = 0; gs.sat = 0;
             gs.dirtyO = 0; gs.dirtyA[0] = 0; gs.dirtyA[1] = 0; gs.rew_bits = 0;
@@ -403,95 +449,80 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             B.episodes_done[g] = 0; B.truncations[g] = 0; B.sat_events[g] = 0;
             for (int p = 0; p < P; ++p) B.wins[(size_t)g * P + p] = 0;
         }
-        __syncthreads();
-        for (int lg = warp; lg < ng; lg += nwarps) generate(lg);
-        __syncthreads();
+        __syncwarp();
+        for (int lg = 0; lg < nwg; ++lg) generate(lg);
     } else {
-        const uint32_t bar = smem_u32(s_bar);
-        if (tid == 0) mbar_init(bar, 1);
-        __syncthreads();
-        if (tid == 0) {
-            const uint32_t cells = (uint32_t)ng * (uint32_t)S;
-            mbar_expect_tx(bar, 4u * cells);
-            bulk_g2s(smem_u32(s_army), B.army + (size_t)g0 * S, 2u * cells, bar);
-            bulk_g2s(smem_u32(s_owner), B.owner + (size_t)g0 * S, cells, bar);
-            bulk_g2s(smem_u32(s_terr), B.terrain + (size_t)g0 * S, cells, bar);
-        }
-        if (tid < ng) {
-            GameS &gs = s_game[tid];
-            const int g = g0 + tid;
-            gs.turn = B.turn[g];
-            gs.alive = B.alive[g];
-            gs.done = B.done[g];
-            gs.winner = B.winner[g];
-            gs.episode = B.episode[g];
-            gs.flags = 0; gs.sat = 0; gs.dirtyO = 0; gs.dirtyA[0] = 0; gs.dirtyA[1] = 0; gs.rew_bits = 0;
-            for (int p = 0; p < P; ++p) {
-                gs.tot[p] = B.army_total[(size_t)g * P + p];
-                gs.land[p] = B.land[(size_t)g * P + p];
-            }
-            gs.digest = ((flags & F_DIGEST) && B.obs_digest) ? B.obs_digest[g] : 0ull;
-        }
         mbar_wait(bar, 0);
-        __syncthreads();  // the scalars above were written by thread lg, the octet of game lg reads them
     }
-    // bitboards of every game (land is recounted from them; army totals only for gen_observe)
-    if (ovalid) rebuild_game(og, (flags & F_OBSERVE_ONLY) != 0);
-    __syncthreads();
+    if (gvalid) build_game(sub);
+    __syncwarp();
+    if ((flags & F_OBSERVE_ONLY) && gvalid) recount(sub, true, true);
 
     // ---------------------------------------------------------------- a12: valid-action sampler (R24, R25)
-    // one thread per (game, player); the valid list is ordered (direction, cell)
+    // the whole octet of a game draws player p's action; the valid list is ordered (direction, cell);
+    // lane l owns words l*WPL.. of every bitboard row.  Every lane returns the same action.
     auto sample = [&](int lg, int p, uint32_t gstep) -> int {
-        const uint32_t gid = kp.gid_base + (uint32_t)(g0 + lg);
+        const uint32_t gid = kp.gid_base + (uint32_t)(wg0 + lg);
         uint32_t w[4];
         philox(0u, gid, gstep, (DOM_ACTION << 24) | (uint32_t)p, kp.key0, kp.key1, w);
         if (w[0] < kp.pass_thr) return 0;
         const uint32_t *own = mrow(p, lg), *a2 = mrow(M_A2, lg), *mtn = mrow(M_MTN, lg);
-        // the four "target is on the board and not a mountain" words of word j
-        uint32_t n[4] = {0, 0, 0, 0};
-        {
-            uint32_t prev = 0, cur = ~mtn[0] & kp.inb[0];
-            for (int j = 0; j < NW; ++j) {
-                const uint32_t next = (j + 1 < NW) ? (~mtn[j + 1] & kp.inb[j + 1]) : 0u;
-                const uint32_t M = own[j] & a2[j];
-                n[0] += __popc(M & __funnelshift_lc(prev, cur, W));                   // up:    c - W
-                n[1] += __popc(M & __funnelshift_rc(cur, next, W));                   // down:  c + W
-                n[2] += __popc(M & __funnelshift_l(prev, cur, 1) & kp.notcol0[j]);    // left:  c - 1
-                n[3] += __popc(M & __funnelshift_r(cur, next, 1) & kp.notcolL[j]);    // right: c + 1
-                prev = cur;
-                cur = next;
-            }
-        }
-        const uint32_t total = n[0] + n[1] + n[2] + n[3];
-        if (total == 0) return 0;
-        const int half = (w[2] < kp.half_thr) ? 1 : 0;
-        auto dir_word = [&](int d, int j) -> uint32_t {
-            const uint32_t prev = j > 0 ? (~mtn[j - 1] & kp.inb[j - 1]) : 0u;
-            const uint32_t cur = ~mtn[j] & kp.inb[j];
-            const uint32_t next = (j + 1 < NW) ? (~mtn[j + 1] & kp.inb[j + 1]) : 0u;
-            const uint32_t M = own[j] & a2[j];
-            if (d == 0) return M & __funnelshift_lc(prev, cur, W);
-            if (d == 1) return M & __funnelshift_rc(cur, next, W);
-            if (d == 2) return M & __funnelshift_l(prev, cur, 1) & kp.notcol0[j];
-            return M & __funnelshift_r(cur, next, 1) & kp.notcolL[j];
+        auto freew = [&](int j) -> uint32_t { return (j >= 0 && j < NW) ? (~mtn[j] & s_inb[j]) : 0u; };
+        // the four "source is mine with army >= 2, target is on the board and not a mountain" words
+        auto dir_words = [&](int j, uint32_t prev, uint32_t cur, uint32_t next, uint32_t (&v)[4]) {
+            const uint32_t Mv = own[j] & a2[j];
+            v[0] = Mv & __funnelshift_lc(prev, cur, W);               // up:    c - W
+            v[1] = Mv & __funnelshift_rc(cur, next, W);               // down:  c + W
+            v[2] = Mv & __funnelshift_l(prev, cur, 1) & s_nc0[j];     // left:  c - 1
+            v[3] = Mv & __funnelshift_r(cur, next, 1) & s_ncL[j];     // right: c + 1
         };
-        if (w[3] < kp.bias_thr) {
-            // largest owned stack, ties -> lowest cell index
-            const int16_t *A = s_army + (size_t)lg * S;
-            int best = -1, bc = 0;
-            for (int j = 0; j < NW; ++j) {
-                uint32_t m = own[j] & kp.inb[j];
-                while (m) {
-                    const int b = __ffs(m) - 1;
-                    m &= m - 1;
-                    const int a = A[32 * j + b];
-                    if (a > best) { best = a; bc = 32 * j + b; }
+        const int j0 = ol * WPL;
+        uint32_t v[MAXWPL][4];
+        uint32_t n01 = 0, n23 = 0;
+        {
+            uint32_t prev = freew(j0 - 1), cur = freew(j0);
+#pragma unroll
+            for (int i = 0; i < MAXWPL; ++i) {
+                const int j = j0 + i;
+                v[i][0] = v[i][1] = v[i][2] = v[i][3] = 0;
+                if (i < WPL && j < NW) {
+                    const uint32_t next = freew(j + 1);
+                    dir_words(j, prev, cur, next, v[i]);
+                    n01 += (uint32_t)__popc(v[i][0]) | ((uint32_t)__popc(v[i][1]) << 16);
+                    n23 += (uint32_t)__popc(v[i][2]) | ((uint32_t)__popc(v[i][3]) << 16);
+                    prev = cur;
+                    cur = next;
                 }
             }
-            if (best >= 0) {
+        }
+        n01 = __reduce_add_sync(gmask, n01);
+        n23 = __reduce_add_sync(gmask, n23);
+        const uint32_t n0 = n01 & 0xFFFFu, n1 = n01 >> 16, n2 = n23 & 0xFFFFu, n3 = n23 >> 16;
+        const uint32_t total = n0 + n1 + n2 + n3;
+        if (total == 0) return 0;
+        const int half = (w[2] < kp.half_thr) ? 1 : 0;
+        if (w[3] < kp.bias_thr) {
+            // largest owned stack, ties -> lowest cell index: max of (army + 1) << 10 | (1023 - cell)
+            const int16_t *A = s_army + (size_t)lg * S;
+            uint32_t best = 0;
+            for (int i = 0; i < WPL; ++i) {
+                const int j = j0 + i;
+                if (j >= NW) break;
+                uint32_t m = own[j] & s_inb[j];
+                while (m) {
+                    const int c = 32 * j + __ffs(m) - 1;
+                    m &= m - 1;
+                    best = max(best, (((uint32_t)A[c] + 1u) << 10) | (uint32_t)(1023 - c));
+                }
+            }
+            best = __reduce_max_sync(gmask, best);
+            if (best) {
+                const int bc = 1023 - (int)(best & 1023u), jb = bc >> 5;
+                uint32_t vv[4];
+                dir_words(jb, freew(jb - 1), freew(jb), freew(jb + 1), vv);
                 uint32_t vb = 0;
 #pragma unroll
-                for (int d = 0; d < 4; ++d) vb |= ((dir_word(d, bc >> 5) >> (bc & 31)) & 1u) << d;
+                for (int d = 0; d < 4; ++d) vb |= ((vv[d] >> (bc & 31)) & 1u) << d;
                 if (vb) {
                     const int d = nth_bit(vb, mulhi32(w[1], (uint32_t)__popc(vb)));
                     return bc * 9 + 1 + 2 * d + half;
@@ -500,20 +531,39 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         }
         uint32_t idx = mulhi32(w[1], total);
         int d = 0;
-        if (idx >= n[0]) { idx -= n[0]; d = 1;
-            if (idx >= n[1]) { idx -= n[1]; d = 2;
-                if (idx >= n[2]) { idx -= n[2]; d = 3; } } }
-        int cell = 0;
-        for (int j = 0; j < NW; ++j) {
-            const uint32_t v = dir_word(d, j);
-            const uint32_t c = __popc(v);
-            if (idx < c) { cell = 32 * j + nth_bit(v, idx); break; }
-            idx -= c;
+        if (idx >= n0) { idx -= n0; d = 1;
+            if (idx >= n1) { idx -= n1; d = 2;
+                if (idx >= n2) { idx -= n2; d = 3; } } }
+        uint32_t vd[MAXWPL], cnt = 0;
+#pragma unroll
+        for (int i = 0; i < MAXWPL; ++i) {
+            vd[i] = d == 0 ? v[i][0] : d == 1 ? v[i][1] : d == 2 ? v[i][2] : v[i][3];
+            cnt += (uint32_t)__popc(vd[i]);
         }
+        uint32_t incl = cnt;
+#pragma unroll
+        for (int o = 1; o < LPG; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(gmask, incl, o, LPG);
+            if (ol >= o) incl += t;
+        }
+        int cell = -1;
+        if (idx < incl && idx >= incl - cnt) {
+            uint32_t r = idx - (incl - cnt);
+#pragma unroll
+            for (int i = 0; i < MAXWPL; ++i) {
+                const uint32_t c = (uint32_t)__popc(vd[i]);
+                if (cell < 0) {
+                    if (r < c) cell = 32 * (j0 + i) + nth_bit(vd[i], r);
+                    else r -= c;
+                }
+            }
+        }
+        const uint32_t bal = __ballot_sync(gmask, cell >= 0);
+        cell = __shfl_sync(gmask, cell, __ffs(bal) - 1);
         return cell * 9 + 1 + 2 * d + half;
     };
 
-    // ---------------------------------------------------------------- a2-a5: moves of one game, one thread
+    // ---------------------------------------------------------------- a2-a5: moves of one game, one lane
     auto set_bit = [&](uint32_t *row, int c, bool on) {
         const uint32_t bit = 1u << (c & 31);
         if (on) row[c >> 5] |= bit; else row[c >> 5] &= ~bit;
@@ -524,7 +574,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         GameS &gs = s_game[lg];
         int16_t *A = s_army + (size_t)lg * S;
         int8_t *O = s_owner + (size_t)lg * S, *Tr = s_terr + (size_t)lg * S;
-        const int g = g0 + lg;
+        const int gg = wg0 + lg;
         const int first = (kp.rule_flags & GEN_RULE_ROTATE_PRIORITY) ? (gs.turn % P) : 0;
         for (int i = 0; i < P; ++i) {
             int p = first + i;
@@ -544,6 +594,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             if (!ok) continue;
             const int asrc = A[cell];
             if (O[cell] != p || asrc < 2 || Tr[dst] == T_MOUNTAIN) continue;
+            if (!((gs.alive >> p) & 1u)) continue;  // R7: an eliminated player's move is void
             const int m = half ? (asrc >> 1) : (asrc - 1);  // R4
             const int nsrc = asrc - m;
             const int t = O[dst], d = A[dst];
@@ -586,7 +637,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 const int q = t;
                 Tr[dst] = (int8_t)T_CITY;
                 gs.alive &= ~(1u << q);
-                B.general_cell[(size_t)g * P + q] = -1;
+                B.general_cell[(size_t)gg * P + q] = -1;
                 const bool fl = (kp.rule_flags & GEN_RULE_CAPTURE_HALF_FLOOR) != 0;
                 uint32_t *oq = mrow(q, lg), *op = mrow(p, lg);
                 for (int j = 0; j < NW; ++j) {
@@ -604,13 +655,14 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 gs.flags |= GF_REBUILD | GF_RECOUNT | GF_TERRAIN_DIRTY | GF_ALL_DIRTY;
             }
         }
-        // a6: turn counter; growth itself is applied by the next cell pass (R1, R2, R3)
+        // a6: turn counter; growth itself is applied by the next parallel pass (R1, R2, R3)
         gs.turn += 1;
         if ((gs.turn & 1) == 0) gs.flags |= GF_GROW_EVEN;
         if (gs.turn % 50 == 0) gs.flags |= GF_GROW_TICK;
     };
 
-    // ---------------------------------------------------------------- a6: growth of one chunk (octet lane)
+    // ---------------------------------------------------------------- a6: growth
+    // tick turns (every 50th): cell pass over one chunk, +1 on owned cells (+2 on owned structures)
     auto grow_chunk = [&](int lg, int ch, uint32_t gflags) {
         GameS &gs = s_game[lg];
         const uint32_t sb = mrow8(M_STR, lg)[ch];
@@ -653,12 +705,45 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             if (inc) atomicAdd(&gs.tot[p], inc);
         }
     };
+    // even turns that are no tick: +1 on the few owned structures, found by bit iteration
+    auto grow_structures = [&](int lg) {
+        GameS &gs = s_game[lg];
+        int16_t *A = s_army + (size_t)lg * S;
+        uint32_t dA0 = 0, dA1 = 0;
+        for (int i = 0; i < WPL; ++i) {
+            const int j = ol * WPL + i;
+            if (j >= NW) break;
+            const uint32_t sw = mrow(M_STR, lg)[j] & s_inb[j];
+            if (sw == 0) continue;
+            uint32_t a2w = mrow(M_A2, lg)[j];
+            bool changed = false;
+            for (int p = 0; p < P; ++p) {
+                uint32_t m = sw & mrow(p, lg)[j];
+                if (m == 0) continue;
+                int inc = 0;
+                while (m) {
+                    const int b = __ffs(m) - 1;
+                    m &= m - 1;
+                    const int c = 32 * j + b, av = A[c];
+                    if (av >= 32767) { atomicAdd(&gs.sat, 1u); continue; }  // R21
+                    A[c] = (int16_t)(av + 1);
+                    inc += 1;
+                    if (av == 1) { a2w |= 1u << b; changed = true; }
+                    if (c < 512) dA0 |= 1u << (c >> 4); else dA1 |= 1u << ((c >> 4) & 31);
+                }
+                if (inc) atomicAdd(&gs.tot[p], inc);
+            }
+            if (changed) mrow(M_A2, lg)[j] = a2w;
+        }
+        if (dA0) atomicOr(&gs.dirtyA[0], dA0);
+        if (dA1) atomicOr(&gs.dirtyA[1], dA1);
+    };
 
-    // ---------------------------------------------------------------- a7-a9: end of turn, one thread per game
+    // ---------------------------------------------------------------- a7-a9: end of turn, one lane per game
     auto finish_turn = [&](int lg, size_t slot, bool write_out) {
         GameS &gs = s_game[lg];
-        const int g = g0 + lg;
-        if (gs.sat) { B.sat_events[g] += gs.sat; gs.sat = 0; }
+        const int gg = wg0 + lg;
+        if (gs.sat) { B.sat_events[gg] += gs.sat; gs.sat = 0; }
         int living = 0, last = -1;
         for (int t = 0; t < kp.n_teams; ++t) {
             const uint32_t tm = (((1u << kp.team_size) - 1u) << (t * kp.team_size)) & allp;
@@ -672,26 +757,28 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         for (int p = 0; p < P; ++p) {
             const int r = terminated ? ((p / kp.team_size == last) ? 1 : -1) : 0;
             rew_bits |= (r + 1) << (2 * p);
-            if (write_out) B.reward[(slot * kp.N + g) * P + p] = (int8_t)r;
-            if (r > 0) B.wins[(size_t)g * P + p] += 1;
+            if (write_out) B.reward[(slot * kp.N + gg) * P + p] = (int8_t)r;
+            if (r > 0) B.wins[(size_t)gg * P + p] += 1;
         }
         gs.rew_bits = rew_bits;
         if (write_out) {
-            B.done[slot * kp.N + g] = (uint8_t)gs.done;
-            B.winner[slot * kp.N + g] = (int8_t)gs.winner;
+            B.done[slot * kp.N + gg] = (uint8_t)gs.done;
+            B.winner[slot * kp.N + gg] = (int8_t)gs.winner;
         }
         if (gs.done) {
-            B.episodes_done[g] += 1;
-            if (truncated) B.truncations[g] += 1;
+            B.episodes_done[gg] += 1;
+            if (truncated) B.truncations[gg] += 1;
             if (kp.auto_reset) {  // a9 (R17): reward / done describe the finished episode, state + obs the new one
                 gs.episode += 1;
-                B.episode[g] = gs.episode;
+                B.episode[gg] = gs.episode;
                 gs.flags |= GF_RESET;
             }
         }
     };
 
-    // ---------------------------------------------------------------- a10: fog of war, one thread per (game, player)
+    // ---------------------------------------------------------------- a10: fog of war (octet, player p)
+    // vis = 3x3 dilation of the team's cells.  Lane l produces words l*WPL..; the horizontally dilated
+    // neighbour words are recomputed in registers, so the pass needs no scratch row and no sync.
     auto compute_vis = [&](int lg, int p) {
         uint32_t *vr = mrow(M_VIS + p, lg);
         const uint32_t members = team_mask(p);
@@ -703,48 +790,61 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 if ((members >> q) & 1u) tm |= mrow(q, lg)[j];
             return tm;
         };
-        // horizontal dilation into the vis row, then vertical in place (prev kept in a register)
-        uint32_t prev = 0, cur = team_word(0);
-        for (int j = 0; j < NW; ++j) {
-            const uint32_t next = team_word(j + 1);
-            vr[j] = cur | (__funnelshift_l(prev, cur, 1) & kp.notcol0[j]) | (__funnelshift_r(cur, next, 1) & kp.notcolL[j]);
-            prev = cur;
-            cur = next;
+        const int j0 = ol * WPL;
+        if (j0 >= NW) return;
+        uint32_t tw[MAXWPL + 4], hh[MAXWPL + 2];
+#pragma unroll
+        for (int i = 0; i < MAXWPL + 4; ++i) tw[i] = (i < WPL + 4) ? team_word(j0 - 2 + i) : 0u;
+#pragma unroll
+        for (int i = 0; i < MAXWPL + 2; ++i) {
+            const int j = j0 - 1 + i;
+            hh[i] = 0;
+            if (i < WPL + 2 && j >= 0 && j < NW)
+                hh[i] = tw[i + 1] | (__funnelshift_l(tw[i], tw[i + 1], 1) & s_nc0[j]) |
+                        (__funnelshift_r(tw[i + 1], tw[i + 2], 1) & s_ncL[j]);
         }
-        prev = 0;
-        cur = vr[0];
-        for (int j = 0; j < NW; ++j) {
-            const uint32_t next = (j + 1 < NW) ? vr[j + 1] : 0u;
-            vr[j] = (cur | __funnelshift_lc(prev, cur, W) | __funnelshift_rc(cur, next, W)) & kp.inb[j];
-            prev = cur;
-            cur = next;
+#pragma unroll
+        for (int i = 0; i < MAXWPL; ++i) {
+            const int j = j0 + i;
+            if (i < WPL && j < NW)
+                vr[j] = (hh[i + 1] | __funnelshift_lc(hh[i], hh[i + 1], W) | __funnelshift_rc(hh[i + 1], hh[i + 2], W)) &
+                        s_inb[j];
         }
     };
 
-    // ---------------------------------------------------------------- a11: observation planes (octet lane)
+    // ---------------------------------------------------------------- a11: observation planes (octet)
+    // per 8-cell chunk and player: one 16-byte and three 8-byte streaming stores; the 8 lanes of the octet
+    // write 128 / 64 contiguous bytes per instruction (full 32-byte sectors)
     auto emit_planes = [&](int lg, size_t slot) {
-        const size_t base = (slot * (size_t)kp.N + (size_t)(g0 + lg)) * (size_t)P * (size_t)S;
-        for (int ch = ol; ch < NC8; ch += LANES_PER_GAME) {
-            const uint4 a = *reinterpret_cast<const uint4 *>(s_army + (size_t)lg * S + 8 * ch);
-            const uint2 o = *reinterpret_cast<const uint2 *>(s_owner + (size_t)lg * S + 8 * ch);
-            const uint2 t = *reinterpret_cast<const uint2 *>(s_terr + (size_t)lg * S + 8 * ch);
+        const size_t base = (slot * (size_t)kp.N + (size_t)(wg0 + lg)) * (size_t)P * (size_t)S;
+        int16_t *pa = B.obs_army + base;
+        int8_t *po = B.obs_owner + base, *pt = B.obs_terrain + base;
+        uint8_t *pv = B.obs_vis + base;
+        const int16_t *sa = s_army + (size_t)lg * S;
+        const int8_t *so = s_owner + (size_t)lg * S, *st = s_terr + (size_t)lg * S;
+#pragma unroll 3
+        for (int ch = ol; ch < NC8; ch += LPG) {
+            const uint4 a = *reinterpret_cast<const uint4 *>(sa + 8 * ch);
+            const uint2 o = *reinterpret_cast<const uint2 *>(so + 8 * ch);
+            const uint2 t = *reinterpret_cast<const uint2 *>(st + 8 * ch);
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
-                if (p >= P) break;
+                if (NP > 2 && p >= P) break;
                 const uint32_t vb = mrow8(M_VIS + p, lg)[ch];
-                const uint32_t m0 = nib_to_bytes(vb & 15u), m1 = nib_to_bytes(vb >> 4);
+                const uint32_t s0 = nib_sign(vb & 15u), s1 = nib_sign(vb >> 4);
+                const uint32_t m0 = prmt(s0, 0u, 0xBA98u), m1 = prmt(s1, 0u, 0xBA98u);
                 uint4 oa;
-                oa.x = a.x & __byte_perm(m0, 0, 0x1100); oa.y = a.y & __byte_perm(m0, 0, 0x3322);
-                oa.z = a.z & __byte_perm(m1, 0, 0x1100); oa.w = a.w & __byte_perm(m1, 0, 0x3322);
+                oa.x = a.x & prmt(s0, 0u, 0x9988u); oa.y = a.y & prmt(s0, 0u, 0xBBAAu);
+                oa.z = a.z & prmt(s1, 0u, 0x9988u); oa.w = a.w & prmt(s1, 0u, 0xBBAAu);
                 uint2 oo, ot, ov;
                 oo.x = (o.x & m0) | (~m0 & 0xFEFEFEFEu); oo.y = (o.y & m1) | (~m1 & 0xFEFEFEFEu);
                 ot.x = (t.x & m0) | (~m0 & 0x04040404u); ot.y = (t.y & m1) | (~m1 & 0x04040404u);
                 ov.x = m0 & 0x01010101u; ov.y = m1 & 0x01010101u;
-                const size_t off = base + (size_t)p * S + 8 * (size_t)ch;
-                __stcs(reinterpret_cast<uint4 *>(B.obs_army + off), oa);
-                __stcs(reinterpret_cast<uint2 *>(B.obs_owner + off), oo);
-                __stcs(reinterpret_cast<uint2 *>(B.obs_terrain + off), ot);
-                __stcs(reinterpret_cast<uint2 *>(B.obs_vis + off), ov);
+                const int off = p * S + 8 * ch;
+                __stcs(reinterpret_cast<uint4 *>(pa + off), oa);
+                __stcs(reinterpret_cast<uint2 *>(po + off), oo);
+                __stcs(reinterpret_cast<uint2 *>(pt + off), ot);
+                __stcs(reinterpret_cast<uint2 *>(pv + off), ov);
             }
         }
     };
@@ -753,12 +853,16 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     // A fogged cell packs to 0x400000, a visible one to x | 0x1000000, so
     // pack - 0x400000 = vis ? (x | 0xC00000) : 0 (terrain <= 3 leaves bits 22, 23 clear) and
     // h_p = 0x400000 * sum(key) + sum_c vis & (x | 0xC00000) * key(c).  All 8 lanes of the octet call this.
-    auto chain_digest = [&](int lg) {
+    auto chain_digest = [&](int lg, bool active) {
         uint64_t h[NP];
 #pragma unroll
         for (int p = 0; p < NP; ++p) h[p] = 0;
-        if (lg < ng) {
-            for (int ch = ol; ch < NC8; ch += LANES_PER_GAME) {
+        if (active) {
+            for (int ch = ol; ch < NC8; ch += LPG) {
+                uint32_t vb[NP], any = 0;
+#pragma unroll
+                for (int p = 0; p < NP; ++p) { vb[p] = (p < P) ? mrow8(M_VIS + p, lg)[ch] : 0u; any |= vb[p]; }
+                if (any == 0) continue;
                 const uint4 a = *reinterpret_cast<const uint4 *>(s_army + (size_t)lg * S + 8 * ch);
                 const uint2 o = *reinterpret_cast<const uint2 *>(s_owner + (size_t)lg * S + 8 * ch);
                 const uint2 t = *reinterpret_cast<const uint2 *>(s_terr + (size_t)lg * S + 8 * ch);
@@ -766,9 +870,6 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 const uint32_t otx = (((o.x & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu) | (t.x << 4);
                 const uint32_t oty = (((o.y & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu) | (t.y << 4);
                 const uint32_t aw[4] = {a.x, a.y, a.z, a.w};
-                uint32_t vb[NP];
-#pragma unroll
-                for (int p = 0; p < NP; ++p) vb[p] = (p < P) ? mrow8(M_VIS + p, lg)[ch] : 0u;
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
                     const uint32_t half = (i & 1) ? (aw[i >> 1] >> 16) : (aw[i >> 1] & 0xFFFFu);
@@ -783,9 +884,9 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
 #pragma unroll
         for (int p = 0; p < NP; ++p) {
 #pragma unroll
-            for (int o = 4; o >= 1; o >>= 1) h[p] += __shfl_xor_sync(FULL, h[p], o);
+            for (int o = LPG / 2; o >= 1; o >>= 1) h[p] += __shfl_xor_sync(FULL, h[p], o);
         }
-        if (lg < ng && ol == 0) {
+        if (active && ol == 0) {
             GameS &gs = s_game[lg];
             const uint64_t c0 = 0x400000ull * kp.key_sum;
             uint64_t dg = gs.digest;
@@ -798,15 +899,14 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         }
     };
 
-    // game-pass thread identities
-    const int sp = tid / G, sg = tid - sp * G;          // sampler / vis: (player, game), tid < P * G
-    const bool svalid = sp < P && sg < ng;
-
     if (flags & F_SAMPLE_ONLY) {
-        if (svalid) {
-            const GameS &gs = s_game[sg];
+        if (gvalid) {
+            const GameS &gs = s_game[sub];
             const bool frozen = !kp.auto_reset && gs.done != 0;
-            kp.sample_out[(size_t)(g0 + sg) * P + sp] = frozen ? 0 : sample(sg, sp, kp.global_step0);
+            for (int p = 0; p < P; ++p) {
+                const int a = frozen ? 0 : sample(sub, p, kp.global_step0);
+                if (ol == 0) kp.sample_out[(size_t)g * P + p] = a;
+            }
         }
         return;
     }
@@ -817,126 +917,158 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         const size_t slot = every ? (size_t)k : 0;
         const uint32_t gstep = kp.global_step0 + (uint32_t)k;
         const bool last_step = (k == kp.K - 1);
-        // ---- actions
-        if (svalid) {
-            GameS &gs = s_game[sg];
+        // ---- actions, then the moves (lane 0 of the octet)
+        if (gvalid) {
+            GameS &gs = s_game[sub];
             const bool frozen = !kp.auto_reset && gs.done != 0;  // R31
-            int a = 0;
-            if (!frozen) a = (flags & F_SAMPLER) ? sample(sg, sp, gstep) : kp.actions[(size_t)(g0 + sg) * P + sp];
-            gs.act[sp] = a;
-            if (B.actions_out) B.actions_out[(slot * kp.N + (g0 + sg)) * P + sp] = a;
+            if (flags & F_SAMPLER) {
+                for (int p = 0; p < P; ++p) {
+                    const int a = frozen ? 0 : sample(sub, p, gstep);
+                    if (ol == 0) {
+                        gs.act[p] = a;
+                        if (B.actions_out) B.actions_out[(slot * kp.N + g) * P + p] = a;
+                    }
+                }
+            } else if (ol == 0) {
+                for (int p = 0; p < P; ++p) {
+                    const int a = frozen ? 0 : kp.actions[(size_t)g * P + p];
+                    gs.act[p] = a;
+                    if (B.actions_out) B.actions_out[(slot * kp.N + g) * P + p] = a;
+                }
+            }
+            if (ol == 0) {
+                if (frozen) gs.flags |= GF_FROZEN;
+                else play_moves(sub);
+            }
         }
-        __syncthreads();
-        // ---- moves
-        if (tid < ng) {
-            GameS &gs = s_game[tid];
-            if (!kp.auto_reset && gs.done != 0) gs.flags |= GF_FROZEN;
-            else play_moves(tid);
-        }
-        __syncthreads();
-        // ---- cell pass: rebuild after a capture, growth, recount after a saturation
-        if (ovalid) {
-            GameS &gs = s_game[og];
+        __syncwarp();
+        // ---- parallel pass: rebuild after a capture, growth, recount after a saturation
+        if (gvalid) {
+            GameS &gs = s_game[sub];
             const uint32_t gf = gs.flags;
             if (gf & (GF_GROW_EVEN | GF_GROW_TICK | GF_REBUILD | GF_RECOUNT)) {
-                if (gf & GF_REBUILD) rebuild_game(og, false);
-                if (gf & (GF_GROW_EVEN | GF_GROW_TICK)) {
-                    for (int ch = ol; ch < NC8; ch += LANES_PER_GAME) grow_chunk(og, ch, gf);
-                    __syncwarp(omask);
+                if (gf & GF_REBUILD) {
+                    build_game(sub);
+                    __syncwarp(gmask);
+                    recount(sub, true, false);
                 }
-                if (gs.flags & GF_RECOUNT) rebuild_game(og, true);
-                __syncwarp(omask);
+                if (gf & GF_GROW_TICK) {
+                    for (int ch = ol; ch < NC8; ch += LPG) grow_chunk(sub, ch, gf);
+                } else if (gf & GF_GROW_EVEN) {
+                    grow_structures(sub);
+                }
+                __syncwarp(gmask);
+                if (gs.flags & GF_RECOUNT) recount(sub, false, true);
+                __syncwarp(gmask);
                 if (ol == 0) gs.flags &= ~(GF_GROW_EVEN | GF_GROW_TICK | GF_REBUILD | GF_RECOUNT);
             }
         }
-        __syncthreads();
+        __syncwarp();
         // ---- end of turn
-        int any_reset = 0;
-        if (tid < ng) {
-            GameS &gs = s_game[tid];
-            if (gs.flags & GF_FROZEN) {
-                gs.rew_bits = 0;
-                for (int p = 0; p < P; ++p) gs.rew_bits |= 1 << (2 * p);
-                if (every || last_step) {
-                    for (int p = 0; p < P; ++p) B.reward[(slot * kp.N + g0 + tid) * P + p] = 0;
-                    B.done[slot * kp.N + g0 + tid] = (uint8_t)gs.done;
-                    B.winner[slot * kp.N + g0 + tid] = (int8_t)gs.winner;
+        bool want_reset = false;
+        if (gvalid) {
+            GameS &gs = s_game[sub];
+            if (ol == 0) {
+                if (gs.flags & GF_FROZEN) {
+                    gs.rew_bits = 0;
+                    for (int p = 0; p < P; ++p) gs.rew_bits |= 1 << (2 * p);
+                    if (every || last_step) {
+                        for (int p = 0; p < P; ++p) B.reward[(slot * kp.N + g) * P + p] = 0;
+                        B.done[slot * kp.N + g] = (uint8_t)gs.done;
+                        B.winner[slot * kp.N + g] = (int8_t)gs.winner;
+                    }
+                } else {
+                    finish_turn(sub, slot, every || last_step);
                 }
-            } else {
-                finish_turn(tid, slot, every || last_step);
+                want_reset = (gs.flags & GF_RESET) != 0;
             }
-            any_reset = (gs.flags & GF_RESET) ? 1 : 0;
         }
-        if (__syncthreads_or(any_reset)) {
-            for (int lg = warp; lg < ng; lg += nwarps)
-                if (s_game[lg].flags & GF_RESET) generate(lg);
-            __syncthreads();
-            if (ovalid && (s_game[og].flags & GF_RESET)) {
-                rebuild_game(og, false);
-                if (ol == 0) s_game[og].flags &= ~GF_RESET;
+        const uint32_t rs = __ballot_sync(FULL, want_reset);  // bit sub * LPG: game sub must be regenerated
+        if (rs) {
+            for (int lg = 0; lg < nwg; ++lg)
+                if ((rs >> (lg * LPG)) & 1u) generate(lg);
+            if (gvalid && ((rs >> (sub * LPG)) & 1u)) {
+                build_game(sub);
+                if (ol == 0) s_game[sub].flags &= ~GF_RESET;
             }
-            __syncthreads();
         }
+        __syncwarp();
         // ---- a10 + a11 (R32: the state at the end of the call)
         const bool planes = (flags & F_OBS_PLANES) && (every || last_step);
         if (planes || (flags & F_DIGEST)) {
-            if (svalid) compute_vis(sg, sp);
-            __syncthreads();
-            if (planes && ovalid) emit_planes(og, slot);
-            if (flags & F_DIGEST) {
-                const bool frozen = ovalid && (s_game[og].flags & GF_FROZEN);
-                chain_digest(frozen ? ng : og);
-            }
+            if (gvalid)
+                for (int p = 0; p < P; ++p) compute_vis(sub, p);
+            __syncwarp();
+            if (planes && gvalid) emit_planes(sub, slot);
+            if (flags & F_DIGEST) chain_digest(sub, gvalid && !(s_game[sub].flags & GF_FROZEN));
         }
     }
 
     if (kp.K == 0) {  // gen_reset / gen_observe: observation of the state as it stands
-        if (svalid) compute_vis(sg, sp);
-        if ((flags & F_RESET) && tid < ng) {
-            GameS &gs = s_game[tid];
-            const int g = g0 + tid;
-            gs.rew_bits = 0;
-            for (int p = 0; p < P; ++p) { B.reward[(size_t)g * P + p] = 0; gs.rew_bits |= 1 << (2 * p); }
-            B.done[g] = 0;
-            B.winner[g] = -1;
+        if (gvalid) {
+            for (int p = 0; p < P; ++p) compute_vis(sub, p);
+            if ((flags & F_RESET) && ol == 0) {
+                GameS &gs = s_game[sub];
+                gs.rew_bits = 0;
+                for (int p = 0; p < P; ++p) { B.reward[(size_t)g * P + p] = 0; gs.rew_bits |= 1 << (2 * p); }
+                B.done[g] = 0;
+                B.winner[g] = -1;
+            }
         }
-        __syncthreads();
-        if ((flags & F_OBS_PLANES) && ovalid) emit_planes(og, 0);
-        if ((flags & F_RESET) && (flags & F_DIGEST)) chain_digest(og);
+        __syncwarp();
+        if ((flags & F_OBS_PLANES) && gvalid) emit_planes(sub, 0);
+        if ((flags & F_RESET) && (flags & F_DIGEST)) chain_digest(sub, gvalid);
     }
 
     // ================================================================ store state
-    __syncthreads();
-    if (ovalid) {
-        const GameS &gs = s_game[og];
-        const size_t gbase = (size_t)(g0 + og) * S;
-        const bool all = (gs.flags & GF_ALL_DIRTY) != 0;
-        // dirty 32-byte sectors of the army plane (16 cells), dirty 32-cell groups of the owner plane
-        for (int u = ol; u < S / 16; u += LANES_PER_GAME) {
-            if (all || ((gs.dirtyA[u >> 5] >> (u & 31)) & 1u)) {
-                const uint4 *src = reinterpret_cast<const uint4 *>(s_army + (size_t)og * S + 16 * u);
-                uint4 *dst = reinterpret_cast<uint4 *>(B.army + gbase + 16 * u);
-                dst[0] = src[0];
-                dst[1] = src[1];
-            }
-            if (all || ((gs.dirtyO >> (u >> 1)) & 1u))
+    __syncwarp();
+    if (gvalid) {
+        const GameS &gs = s_game[sub];
+        const size_t gbase = (size_t)g * S;
+        const uint32_t gf = gs.flags;
+        if (gf & GF_ALL_DIRTY) {
+            for (int u = ol; u < S / 8; u += LPG)
+                *reinterpret_cast<uint4 *>(B.army + gbase + 8 * u) =
+                    *reinterpret_cast<const uint4 *>(s_army + (size_t)sub * S + 8 * u);
+            for (int u = ol; u < S / 16; u += LPG)
                 *reinterpret_cast<uint4 *>(B.owner + gbase + 16 * u) =
-                    *reinterpret_cast<const uint4 *>(s_owner + (size_t)og * S + 16 * u);
-            if (gs.flags & GF_TERRAIN_DIRTY)
+                    *reinterpret_cast<const uint4 *>(s_owner + (size_t)sub * S + 16 * u);
+        } else {
+            // dirty 32-byte sectors of the army plane (16 cells): lane l takes the sectors u = l (mod 8)
+#pragma unroll
+            for (int hw = 0; hw < 2; ++hw) {
+                uint32_t m = gs.dirtyA[hw] & (0x01010101u << ol);
+                while (m) {
+                    const int u = 32 * hw + __ffs(m) - 1;
+                    m &= m - 1;
+                    const uint4 *src = reinterpret_cast<const uint4 *>(s_army + (size_t)sub * S + 16 * u);
+                    uint4 *dst = reinterpret_cast<uint4 *>(B.army + gbase + 16 * u);
+                    dst[0] = src[0];
+                    dst[1] = src[1];
+                }
+            }
+            // dirty 32-cell groups of the owner plane
+            uint32_t m = gs.dirtyO & (0x01010101u << ol);
+            while (m) {
+                const int u = __ffs(m) - 1;
+                m &= m - 1;
+                const uint4 *src = reinterpret_cast<const uint4 *>(s_owner + (size_t)sub * S + 32 * u);
+                uint4 *dst = reinterpret_cast<uint4 *>(B.owner + gbase + 32 * u);
+                dst[0] = src[0];
+                if (32 * u + 16 < S) dst[1] = src[1];
+            }
+        }
+        if (gf & GF_TERRAIN_DIRTY)
+            for (int u = ol; u < S / 16; u += LPG)
                 *reinterpret_cast<uint4 *>(B.terrain + gbase + 16 * u) =
-                    *reinterpret_cast<const uint4 *>(s_terr + (size_t)og * S + 16 * u);
+                    *reinterpret_cast<const uint4 *>(s_terr + (size_t)sub * S + 16 * u);
+        // scalars, spread over the octet
+        if (ol < P) {
+            B.land[(size_t)g * P + ol] = gs.land[ol];
+            B.army_total[(size_t)g * P + ol] = gs.tot[ol];
         }
-    }
-    if (tid < ng) {
-        const GameS &gs = s_game[tid];
-        const int g = g0 + tid;
-        B.turn[g] = gs.turn;
-        B.alive[g] = (uint8_t)gs.alive;
-        for (int p = 0; p < P; ++p) {
-            B.land[(size_t)g * P + p] = gs.land[p];
-            B.army_total[(size_t)g * P + p] = gs.tot[p];
-        }
-        if ((flags & F_DIGEST) && B.obs_digest) B.obs_digest[g] = gs.digest;
+        if (ol == (P & 7)) { B.turn[g] = gs.turn; B.alive[g] = (uint8_t)gs.alive; }
+        if (ol == ((P + 1) & 7) && (flags & F_DIGEST) && B.obs_digest) B.obs_digest[g] = gs.digest;
     }
 }
 
