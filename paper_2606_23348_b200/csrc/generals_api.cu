@@ -83,7 +83,7 @@ inline uint32_t align_up(uint32_t x, uint32_t a) { return (x + a - 1) / a * a; }
 void layout(gen::KParams &k, int WPC, bool digest) {
     k.WPC = WPC;
     const uint32_t GW = (uint32_t)gen::GW, S = (uint32_t)k.S;
-    k.off_key = 3u * 32u * 4u;
+    k.off_key = 416;  // three tables of 34 words (zero guards at both ends), 16-byte aligned
     k.off_warp0 = align_up(k.off_key + (digest ? 8u * S : 0u), 128);
     uint32_t off = 2 * GW * S;
     k.w_owner = off; off += GW * S;
@@ -173,7 +173,7 @@ int gen_init(const gen_config *cfg, gen_env **out) {
     gen::KParams &k = env->base;
     k.N = cfg->n_games; k.H = cfg->height; k.W = cfg->width; k.P = cfg->n_players;
     k.HW = k.H * k.W; k.S = round_up(k.HW, 16); k.NW = (k.HW + 31) / 32; k.NC8 = k.S / 8;
-    k.NCH = 4 * k.NW; k.WPL = (k.NW + gen::LPG - 1) / gen::LPG; k.RW = k.NW | 1; k.M = 2 * k.P + 3;
+    k.NCH = 4 * k.NW; k.RW = k.NW | 1; k.M = 2 * k.P + 6;
     k.team_size = cfg->team_size;
     k.n_teams = (cfg->n_players + cfg->team_size - 1) / cfg->team_size;
     k.n_cities = cfg->n_cities; k.city_lo = cfg->city_army_lo;

@@ -11,10 +11,12 @@
 //     SIMD-in-register byte arithmetic and 16 / 8-byte shared and global accesses: bitboard
 //     construction, tick growth, observation planes (the dominant HBM traffic, full-sector streaming
 //     stores), observation digest.
-//   * WORD passes -- flat bitboards (one bit per cell, word j = cells 32j..32j+31: own[p], mountain,
-//     structure, army >= 2, vis[p]) live in shared memory; lane l of the octet owns the WPL
-//     consecutive words l*WPL.. of each row: Philox valid-action sampler (popcount enumeration,
-//     octet scan), structure growth (bit iteration), fog-of-war dilation (funnel shifts).
+//   * WORD passes -- flat bitboards (one bit per cell, word j = cells 32j..32j+31: own[p], structure,
+//     army >= 2, the four static "target is free" rows, vis[p]) live in shared memory.  The octet is
+//     split by player: LPP = 8 / NP lanes serve one (game, player) pair and each of them streams
+//     through WS consecutive words: Philox valid-action sampler (popcount enumeration, scan over the
+//     LPP lanes), fog-of-war dilation (funnel shifts, sliding window).  All players advance in the
+//     same instruction stream.
 //   * SERIAL passes -- lane 0 of the octet runs the scalar rules: move / combat / capture,
 //     termination, reward; four games advance per warp instruction.
 //
@@ -34,7 +36,6 @@ namespace gen {
 constexpr uint32_t FULL = 0xffffffffu;
 constexpr int LPG = 8;            // lanes per game: the octet
 constexpr int GW = 32 / LPG;      // games per warp
-constexpr int MAXWPL = 32 / LPG;  // bitboard words per lane (NW <= 32 words)
 
 enum : uint32_t {
     F_RESET = 1u << 0,         // generate every board first (gen_reset)
@@ -72,7 +73,7 @@ struct GameS {
 };
 
 struct KParams {
-    int32_t N, H, W, P, HW, S, NW, NC8, NCH, WPL, RW, M;
+    int32_t N, H, W, P, HW, S, NW, NC8, NCH, RW, M;
     int32_t team_size, n_teams;
     int32_t n_cities, city_lo, city_span;
     int32_t dmin, dmax, spawn_exact, max_turns, auto_reset;
@@ -86,7 +87,7 @@ struct KParams {
     gen_buffers b;
     const int32_t *actions;
     int32_t *sample_out;
-    uint32_t notcol0[32], notcolL[32], inb[32];
+    uint32_t notcol0[32], notcolL[32], inb[32];  // column / in-bounds masks of bitboard word j
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -154,22 +155,24 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
 // prmt's sign-replicate selectors (8 | byte index) then expand it: 0xBA98 -> four 0x00 / 0xFF byte
 // masks, 0x9988 / 0xBBAA -> the two int16-pair masks of cells (0, 1) / (2, 3).
 __device__ __forceinline__ uint32_t nib_sign(uint32_t nib) { return nib * 0x10204080u; }
-// bytes holding 0/1 in bit 0: x0 = cells 0..3, x1 = cells 4..7 -> 8 bits
+// Bit gathering.  x0 / x1 hold one flag per byte (cells 0..3 / 4..7) at bit position B; bit B + 4 of
+// every byte must be clear, the other bits are don't-care.  nib8 moves them to bits 0, 4, ..., 28 (cell c < 4 at bit 8c, cell 4 + c at bit
+// 8c + 4); one multiply then lines the eight flags up in the top byte.
+template <int B>
 __device__ __forceinline__ uint32_t gather8(uint32_t x0, uint32_t x1) {
-    return ((x1 * 16u + x0) * 0x01020408u) >> 24;
+    const uint32_t z = (B <= 4 ? ((x1 << (4 - B)) | (x0 >> B)) : ((x1 >> (B - 4)) | (x0 >> B))) & 0x11111111u;
+    return (z * 0x01020408u) >> 24;
 }
 __device__ __forceinline__ uint32_t eq_bytes(uint32_t w, uint32_t pat) {  // 0x01 where byte == pat byte
     const uint32_t x = w ^ pat;
     const uint32_t y = ((x & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) | x;
     return (~y >> 7) & 0x01010101u;
 }
-// 8 int16 armies (all in [0, 32767]) -> 8 bits "army >= 2"
+// 8 int16 armies (all in [0, 32767]) -> 8 bits "army >= 2": min(a, 2) has bit 1 set iff a >= 2
 __device__ __forceinline__ uint32_t ge2_bits(const uint4 &a) {
-    const uint32_t y0 = (a.x & 0x7FFE7FFEu) + 0x7FFE7FFEu, y1 = (a.y & 0x7FFE7FFEu) + 0x7FFE7FFEu;
-    const uint32_t y2 = (a.z & 0x7FFE7FFEu) + 0x7FFE7FFEu, y3 = (a.w & 0x7FFE7FFEu) + 0x7FFE7FFEu;
-    const uint32_t u = (__byte_perm(y0, y1, 0x7531) >> 7) & 0x01010101u;
-    const uint32_t v = (__byte_perm(y2, y3, 0x7531) >> 7) & 0x01010101u;
-    return gather8(u, v);
+    const uint32_t y0 = __vminu2(a.x, 0x00020002u), y1 = __vminu2(a.y, 0x00020002u);
+    const uint32_t y2 = __vminu2(a.z, 0x00020002u), y3 = __vminu2(a.w, 0x00020002u);
+    return gather8<1>(__byte_perm(y0, y1, 0x6420), __byte_perm(y2, y3, 0x6420));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -197,14 +200,17 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 // ================================================================================================
 template <int NP>
 __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParams kp) {
+    constexpr int LPP = LPG / NP;  // lanes serving one (game, player) pair in the word passes
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x;
     const uint32_t lane = tid & 31u;
     const int wic = tid >> 5;
     const int ol = (int)(lane & (LPG - 1)), sub = (int)(lane / LPG);  // lane of the octet, game of the warp
     const uint32_t gmask = ((1u << LPG) - 1u) << (sub * LPG);         // the lanes of this octet
+    const int pl = ol / LPP, sl = ol % LPP;                           // word passes: my player, my sub-lane
     const int H = kp.H, W = kp.W, P = kp.P, HW = kp.HW, S = kp.S, NW = kp.NW, NC8 = kp.NC8;
-    const int RW = kp.RW, WPL = kp.WPL, M = kp.M;
+    const int RW = kp.RW, M = kp.M;
+    const int WS = (NW + LPP - 1) / LPP;  // words per sub-lane
     const uint32_t flags = kp.flags;
     const gen_buffers &B = kp.b;
     const int wg0 = (blockIdx.x * kp.WPC + wic) * GW;  // first game of this warp
@@ -212,9 +218,11 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     const bool gvalid = sub < nwg;
     const int g = wg0 + sub;
     const uint32_t allp = (1u << P) - 1u;
+    const bool teams = kp.team_size > 1;
 
-    // CTA-wide tables: column / in-bounds masks of the flat bitboard words, digest keys
-    uint32_t *s_nc0 = reinterpret_cast<uint32_t *>(smem), *s_ncL = s_nc0 + 32, *s_inb = s_nc0 + 64;
+    // CTA-wide tables, index j + 1 for bitboard word j (entries 0 and 33 are zero guards): column masks,
+    // in-bounds mask; digest keys
+    uint32_t *s_nc0 = reinterpret_cast<uint32_t *>(smem) + 1, *s_ncL = s_nc0 + 34, *s_inb = s_nc0 + 68;
     uint64_t *s_key = reinterpret_cast<uint64_t *>(smem + kp.off_key);
     // this warp's slice
     unsigned char *wb = smem + kp.off_warp0 + (size_t)wic * kp.warp_bytes;
@@ -225,8 +233,10 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     GameS *s_game = reinterpret_cast<GameS *>(wb + kp.w_game);
     const uint32_t bar = smem_u32(wb + kp.w_bar);
 
-    // mask rows of a game: own[0..P-1], mountain, structure (city / general), army >= 2, vis[0..P-1]
-    const int M_MTN = P, M_STR = P + 1, M_A2 = P + 2, M_VIS = P + 3;
+    // bitboard rows of a game: own[0..P-1], structure (city / general), army >= 2, ok[4] (source cells whose
+    // up / down / left / right target is on the board and no mountain: static per board), vis[0..P-1].
+    // vis[0] doubles as the mountain row while the ok rows are being built.
+    const int R_STR = P, R_A2 = P + 1, R_OK = P + 2, R_VIS = P + 6, R_MTN = P + 6;
     auto mrow = [&](int m, int lg) -> uint32_t * { return s_mask + (lg * M + m) * RW; };
     auto mrow8 = [&](int m, int lg) -> unsigned char * { return reinterpret_cast<unsigned char *>(mrow(m, lg)); };
 
@@ -337,45 +347,57 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         __syncwarp();
     };
 
-    // ---------------------------------------------------------------- cell pass: bitboards of one chunk
-    auto build_chunk = [&](int lg, int ch) {
-        uint32_t mb[NP + 3];
-#pragma unroll
-        for (int i = 0; i < NP + 3; ++i) mb[i] = 0;
-        if (ch < NC8) {
-            const uint2 o = *reinterpret_cast<const uint2 *>(s_owner + (size_t)lg * S + 8 * ch);
-            const uint2 t = *reinterpret_cast<const uint2 *>(s_terr + (size_t)lg * S + 8 * ch);
-            const uint4 a = *reinterpret_cast<const uint4 *>(s_army + (size_t)lg * S + 8 * ch);
+    // ---------------------------------------------------------------- cell pass: bitboards of one game (octet)
+    // chunk ch = cells 8ch..8ch+7 -> byte ch of the rows own[p], mountain, structure, army >= 2
+    auto build_game = [&](int lg) {
+        const unsigned char *sa = reinterpret_cast<const unsigned char *>(s_army + (size_t)lg * S);
+        const unsigned char *so = reinterpret_cast<const unsigned char *>(s_owner + (size_t)lg * S);
+        const unsigned char *st = reinterpret_cast<const unsigned char *>(s_terr + (size_t)lg * S);
+        unsigned char *rows = mrow8(0, lg);
+        const int rb = 4 * RW;  // row stride in bytes
+#pragma unroll 3
+        for (int ch = ol; ch < NC8; ch += LPG) {
+            const uint2 o = *reinterpret_cast<const uint2 *>(so + 8 * ch);
+            const uint2 t = *reinterpret_cast<const uint2 *>(st + 8 * ch);
+            const uint4 a = *reinterpret_cast<const uint4 *>(sa + 16 * ch);
             if (NP == 2) {
-                // owner in {-1, 0, 1}: bit 7 = neutral, bit 0 = player
-                const uint32_t nx = o.x >> 7, ny = o.y >> 7;
-                mb[0] = gather8(~(o.x | nx) & 0x01010101u, ~(o.y | ny) & 0x01010101u);
-                mb[1] = gather8(o.x & ~nx & 0x01010101u, o.y & ~ny & 0x01010101u);
+                // owner in {-1, 0, 1}: bit 7 = neutral, bit 0 = player (bits 1..6 cleared: gather8 wants bit 4 clean)
+                const uint32_t ox = o.x & 0x81818181u, oy = o.y & 0x81818181u;
+                const uint32_t nx = ox >> 7, ny = oy >> 7;
+                rows[ch] = (unsigned char)gather8<0>(~(ox | nx) & 0x01010101u, ~(oy | ny) & 0x01010101u);
+                rows[rb + ch] = (unsigned char)gather8<0>(ox & ~nx, oy & ~ny);
             } else {
 #pragma unroll
                 for (int p = 0; p < NP; ++p)
                     if (p < P) {
                         const uint32_t pat = 0x01010101u * (uint32_t)p;
-                        mb[p] = gather8(eq_bytes(o.x, pat), eq_bytes(o.y, pat));
+                        rows[p * rb + ch] = (unsigned char)gather8<0>(eq_bytes(o.x, pat), eq_bytes(o.y, pat));
                     }
             }
             // terrain in {0,1,2,3}: mountain = 01, structure (city / general) = 1x
             const uint32_t hx = t.x >> 1, hy = t.y >> 1;
-            mb[NP] = gather8(t.x & ~hx & 0x01010101u, t.y & ~hy & 0x01010101u);
-            mb[NP + 1] = gather8(hx & 0x01010101u, hy & 0x01010101u);
-            mb[NP + 2] = ge2_bits(a);
+            rows[R_MTN * rb + ch] = (unsigned char)gather8<0>(t.x & ~hx, t.y & ~hy);
+            rows[R_STR * rb + ch] = (unsigned char)gather8<0>(hx, hy);
+            rows[R_A2 * rb + ch] = (unsigned char)ge2_bits(a);
         }
-#pragma unroll
-        for (int p = 0; p < NP; ++p)
-            if (p < P) mrow8(p, lg)[ch] = (unsigned char)mb[p];
-        mrow8(M_MTN, lg)[ch] = (unsigned char)mb[NP];
-        mrow8(M_STR, lg)[ch] = (unsigned char)mb[NP + 1];
-        mrow8(M_A2, lg)[ch] = (unsigned char)mb[NP + 2];
+        for (int ch = NC8 + ol; ch < kp.NCH; ch += LPG) {  // bytes of the last word past the plane stride
+            for (int p = 0; p < P; ++p) rows[p * rb + ch] = 0;
+            rows[R_MTN * rb + ch] = 0xFF;
+            rows[R_STR * rb + ch] = 0;
+            rows[R_A2 * rb + ch] = 0;
+        }
     };
-    // octet: all bitboards of game lg (the caller syncs the warp afterwards)
-    auto build_game = [&](int lg) {
-#pragma unroll 3
-        for (int ch = ol; ch < kp.NCH; ch += LPG) build_chunk(lg, ch);
+    // word pass (octet): the four static "target is free" rows from the mountain row
+    auto build_ok = [&](int lg) {
+        const uint32_t *mtn = mrow(R_MTN, lg);
+        auto freew = [&](int j) -> uint32_t { return ((unsigned)j < (unsigned)NW) ? (~mtn[j] & s_inb[j]) : 0u; };
+        for (int j = ol; j < NW; j += LPG) {
+            const uint32_t prev = freew(j - 1), cur = freew(j), next = freew(j + 1), in = s_inb[j];
+            mrow(R_OK + 0, lg)[j] = __funnelshift_lc(prev, cur, W) & in;             // up:    c - W
+            mrow(R_OK + 1, lg)[j] = __funnelshift_rc(cur, next, W) & in;             // down:  c + W
+            mrow(R_OK + 2, lg)[j] = __funnelshift_l(prev, cur, 1) & s_nc0[j] & in;   // left:  c - 1
+            mrow(R_OK + 3, lg)[j] = __funnelshift_r(cur, next, 1) & s_ncL[j] & in;   // right: c + 1
+        }
     };
     // octet: scoreboard from the planes / bitboards (after a capture, a saturation, a reset; gen_observe)
     auto recount = [&](int lg, bool do_land, bool do_tot) {
@@ -383,9 +405,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         const int16_t *A = s_army + (size_t)lg * S;
         for (int p = 0; p < P; ++p) {
             int l = 0, sum = 0;
-            for (int i = 0; i < WPL; ++i) {
-                const int j = ol * WPL + i;
-                if (j >= NW) break;
+            for (int j = ol; j < NW; j += LPG) {
                 uint32_t m = mrow(p, lg)[j] & s_inb[j];
                 l += __popc(m);
                 if (do_tot)
@@ -395,8 +415,11 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                         sum += A[32 * j + b];
                     }
             }
-            l = __reduce_add_sync(gmask, l);
-            sum = __reduce_add_sync(gmask, sum);
+#pragma unroll
+            for (int o = LPG / 2; o >= 1; o >>= 1) {
+                l += __shfl_xor_sync(gmask, l, o);
+                sum += __shfl_xor_sync(gmask, sum, o);
+            }
             if (ol == 0) {
                 if (do_land) gs.land[p] = l;
                 if (do_tot) gs.tot[p] = sum;
@@ -405,10 +428,12 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     };
 
     // ================================================================ prologue
-    if (tid < 32) {
-        s_nc0[tid] = kp.notcol0[tid];
-        s_ncL[tid] = kp.notcolL[tid];
-        s_inb[tid] = kp.inb[tid];
+    for (int t = tid; t < 34; t += blockDim.x) {
+        const int j = t - 1;
+        const bool in = j >= 0 && j < 32;
+        s_nc0[j] = in ? kp.notcol0[j & 31] : 0u;
+        s_ncL[j] = in ? kp.notcolL[j & 31] : 0u;
+        s_inb[j] = in ? kp.inb[j & 31] : 0u;
     }
     if (flags & F_DIGEST) {
         for (int c = tid; c < S; c += blockDim.x)
@@ -456,58 +481,47 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     }
     if (gvalid) build_game(sub);
     __syncwarp();
-    if ((flags & F_OBSERVE_ONLY) && gvalid) recount(sub, true, true);
+    if (gvalid) {
+        build_ok(sub);
+        if (flags & F_OBSERVE_ONLY) recount(sub, true, true);
+    }
+    __syncwarp();
 
     // ---------------------------------------------------------------- a12: valid-action sampler (R24, R25)
-    // the whole octet of a game draws player p's action; the valid list is ordered (direction, cell);
-    // lane l owns words l*WPL.. of every bitboard row.  Every lane returns the same action.
-    auto sample = [&](int lg, int p, uint32_t gstep) -> int {
+    // All players of a game are drawn in one instruction stream: the LPP lanes (pl, 0..LPP-1) of the octet
+    // serve player pl and split the NW bitboard words among themselves (WS consecutive words each).  The valid
+    // list is ordered (direction, cell).  Returns player pl's action on every lane serving pl.  No lane leaves
+    // early, so the octet stays converged for the shuffles.
+    auto sample = [&](int lg, uint32_t gstep) -> int {
+        const int p = min(pl, P - 1);  // lanes past the last player shadow it (their result is ignored)
         const uint32_t gid = kp.gid_base + (uint32_t)(wg0 + lg);
         uint32_t w[4];
         philox(0u, gid, gstep, (DOM_ACTION << 24) | (uint32_t)p, kp.key0, kp.key1, w);
-        if (w[0] < kp.pass_thr) return 0;
-        const uint32_t *own = mrow(p, lg), *a2 = mrow(M_A2, lg), *mtn = mrow(M_MTN, lg);
-        auto freew = [&](int j) -> uint32_t { return (j >= 0 && j < NW) ? (~mtn[j] & s_inb[j]) : 0u; };
-        // the four "source is mine with army >= 2, target is on the board and not a mountain" words
-        auto dir_words = [&](int j, uint32_t prev, uint32_t cur, uint32_t next, uint32_t (&v)[4]) {
-            const uint32_t Mv = own[j] & a2[j];
-            v[0] = Mv & __funnelshift_lc(prev, cur, W);               // up:    c - W
-            v[1] = Mv & __funnelshift_rc(cur, next, W);               // down:  c + W
-            v[2] = Mv & __funnelshift_l(prev, cur, 1) & s_nc0[j];     // left:  c - 1
-            v[3] = Mv & __funnelshift_r(cur, next, 1) & s_ncL[j];     // right: c + 1
-        };
-        const int j0 = ol * WPL;
-        uint32_t v[MAXWPL][4];
-        uint32_t n01 = 0, n23 = 0;
-        {
-            uint32_t prev = freew(j0 - 1), cur = freew(j0);
-#pragma unroll
-            for (int i = 0; i < MAXWPL; ++i) {
-                const int j = j0 + i;
-                v[i][0] = v[i][1] = v[i][2] = v[i][3] = 0;
-                if (i < WPL && j < NW) {
-                    const uint32_t next = freew(j + 1);
-                    dir_words(j, prev, cur, next, v[i]);
-                    n01 += (uint32_t)__popc(v[i][0]) | ((uint32_t)__popc(v[i][1]) << 16);
-                    n23 += (uint32_t)__popc(v[i][2]) | ((uint32_t)__popc(v[i][3]) << 16);
-                    prev = cur;
-                    cur = next;
-                }
-            }
+        const uint32_t *own = mrow(p, lg), *a2 = mrow(R_A2, lg), *ok = mrow(R_OK, lg);
+        const int js = sl * WS, je = min(js + WS, NW);
+        // count pass: my words' valid moves per direction, packed 2 x 16 bits
+        uint32_t ln01 = 0, ln23 = 0;
+        for (int j = js; j < je; ++j) {
+            const uint32_t src = own[j] & a2[j];
+            ln01 += (uint32_t)__popc(src & ok[j]) | ((uint32_t)__popc(src & ok[RW + j]) << 16);
+            ln23 += (uint32_t)__popc(src & ok[2 * RW + j]) | ((uint32_t)__popc(src & ok[3 * RW + j]) << 16);
         }
-        n01 = __reduce_add_sync(gmask, n01);
-        n23 = __reduce_add_sync(gmask, n23);
+        uint32_t n01 = ln01, n23 = ln23;
+#pragma unroll
+        for (int o = LPP / 2; o >= 1; o >>= 1) {
+            n01 += __shfl_xor_sync(gmask, n01, o);
+            n23 += __shfl_xor_sync(gmask, n23, o);
+        }
         const uint32_t n0 = n01 & 0xFFFFu, n1 = n01 >> 16, n2 = n23 & 0xFFFFu, n3 = n23 >> 16;
         const uint32_t total = n0 + n1 + n2 + n3;
-        if (total == 0) return 0;
         const int half = (w[2] < kp.half_thr) ? 1 : 0;
-        if (w[3] < kp.bias_thr) {
+        int action = 0;
+        bool decided = (w[0] < kp.pass_thr) || total == 0;
+        if (kp.bias_thr) {  // uniform: config 4's policy
             // largest owned stack, ties -> lowest cell index: max of (army + 1) << 10 | (1023 - cell)
             const int16_t *A = s_army + (size_t)lg * S;
             uint32_t best = 0;
-            for (int i = 0; i < WPL; ++i) {
-                const int j = j0 + i;
-                if (j >= NW) break;
+            for (int j = js; j < je; ++j) {
                 uint32_t m = own[j] & s_inb[j];
                 while (m) {
                     const int c = 32 * j + __ffs(m) - 1;
@@ -515,52 +529,50 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                     best = max(best, (((uint32_t)A[c] + 1u) << 10) | (uint32_t)(1023 - c));
                 }
             }
-            best = __reduce_max_sync(gmask, best);
-            if (best) {
+#pragma unroll
+            for (int o = LPP / 2; o >= 1; o >>= 1) best = max(best, __shfl_xor_sync(gmask, best, o));
+            if (!decided && w[3] < kp.bias_thr && best) {
                 const int bc = 1023 - (int)(best & 1023u), jb = bc >> 5;
-                uint32_t vv[4];
-                dir_words(jb, freew(jb - 1), freew(jb), freew(jb + 1), vv);
+                const uint32_t src = (own[jb] & a2[jb]) >> (bc & 31);
                 uint32_t vb = 0;
 #pragma unroll
-                for (int d = 0; d < 4; ++d) vb |= ((vv[d] >> (bc & 31)) & 1u) << d;
+                for (int d = 0; d < 4; ++d) vb |= ((src & (ok[d * RW + jb] >> (bc & 31))) & 1u) << d;
                 if (vb) {
                     const int d = nth_bit(vb, mulhi32(w[1], (uint32_t)__popc(vb)));
-                    return bc * 9 + 1 + 2 * d + half;
+                    action = bc * 9 + 1 + 2 * d + half;
+                    decided = true;
                 }
             }
         }
         uint32_t idx = mulhi32(w[1], total);
         int d = 0;
-        if (idx >= n0) { idx -= n0; d = 1;
-            if (idx >= n1) { idx -= n1; d = 2;
-                if (idx >= n2) { idx -= n2; d = 3; } } }
-        uint32_t vd[MAXWPL], cnt = 0;
-#pragma unroll
-        for (int i = 0; i < MAXWPL; ++i) {
-            vd[i] = d == 0 ? v[i][0] : d == 1 ? v[i][1] : d == 2 ? v[i][2] : v[i][3];
-            cnt += (uint32_t)__popc(vd[i]);
-        }
+        uint32_t cnt = ln01 & 0xFFFFu;
+        if (idx >= n0) { idx -= n0; d = 1; cnt = ln01 >> 16;
+            if (idx >= n1) { idx -= n1; d = 2; cnt = ln23 & 0xFFFFu;
+                if (idx >= n2) { idx -= n2; d = 3; cnt = ln23 >> 16; } } }
         uint32_t incl = cnt;
 #pragma unroll
-        for (int o = 1; o < LPG; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(gmask, incl, o, LPG);
-            if (ol >= o) incl += t;
+        for (int o = 1; o < LPP; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(gmask, incl, o, LPP);
+            if (sl >= o) incl += t;
         }
         int cell = -1;
-        if (idx < incl && idx >= incl - cnt) {
-            uint32_t r = idx - (incl - cnt);
-#pragma unroll
-            for (int i = 0; i < MAXWPL; ++i) {
-                const uint32_t c = (uint32_t)__popc(vd[i]);
-                if (cell < 0) {
-                    if (r < c) cell = 32 * (j0 + i) + nth_bit(vd[i], r);
-                    else r -= c;
-                }
+        if (!decided && idx < incl && idx >= incl - cnt) {  // the idx-th move of direction d starts in my words
+            uint32_t r = idx - (incl - cnt), vw = 0;
+            int j = js;
+            for (; j < je; ++j) {
+                vw = own[j] & a2[j] & ok[d * RW + j];
+                const uint32_t c = (uint32_t)__popc(vw);
+                if (r < c) break;
+                r -= c;
             }
+            cell = 32 * j + nth_bit(vw, r);
         }
-        const uint32_t bal = __ballot_sync(gmask, cell >= 0);
-        cell = __shfl_sync(gmask, cell, __ffs(bal) - 1);
-        return cell * 9 + 1 + 2 * d + half;
+        const int leader = (int)(lane & ~(uint32_t)(LPP - 1));
+        const uint32_t mine = (__ballot_sync(gmask, cell >= 0) >> leader) & ((1u << LPP) - 1u);
+        cell = __shfl_sync(gmask, cell, mine ? leader + __ffs(mine) - 1 : (int)lane);
+        if (mine) action = cell * 9 + 1 + 2 * d + half;
+        return action;
     };
 
     // ---------------------------------------------------------------- a2-a5: moves of one game, one lane
@@ -568,20 +580,22 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         const uint32_t bit = 1u << (c & 31);
         if (on) row[c >> 5] |= bit; else row[c >> 5] &= ~bit;
     };
-    auto touch = [&](GameS &gs, int c) { gs.dirtyA[c >> 9] |= 1u << ((c >> 4) & 31); };
 
     auto play_moves = [&](int lg) {
         GameS &gs = s_game[lg];
         int16_t *A = s_army + (size_t)lg * S;
         int8_t *O = s_owner + (size_t)lg * S, *Tr = s_terr + (size_t)lg * S;
+        uint32_t *a2row = mrow(R_A2, lg);
         const int gg = wg0 + lg;
         const int first = (kp.rule_flags & GEN_RULE_ROTATE_PRIORITY) ? (gs.turn % P) : 0;
+        uint32_t dA0 = 0, dA1 = 0, dO = 0, gflags = 0;
         for (int i = 0; i < P; ++i) {
             int p = first + i;
             if (p >= P) p -= P;
             const int a = gs.act[p];
             if (a <= 0 || a >= 9 * HW) continue;
-            const int cell = a / 9, kk = a - 9 * cell;
+            const int cell = (int)(((uint32_t)a * 7282u) >> 16);  // a / 9 for a < 9 * 1024
+            const int kk = a - 9 * cell;
             if (kk == 0) continue;
             const int dir = (kk - 1) >> 1, half = (kk - 1) & 1;
             const int r = row_of(cell), col = cell - r * W;
@@ -594,17 +608,16 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             if (!ok) continue;
             const int asrc = A[cell];
             if (O[cell] != p || asrc < 2 || Tr[dst] == T_MOUNTAIN) continue;
-            if (!((gs.alive >> p) & 1u)) continue;  // R7: an eliminated player's move is void
             const int m = half ? (asrc >> 1) : (asrc - 1);  // R4
             const int nsrc = asrc - m;
             const int t = O[dst], d = A[dst];
             const bool dst_general = Tr[dst] == T_GENERAL;
             int ndst, nown = t;
             bool captured = false;
-            const bool ally = t >= 0 && t != p && ((team_mask(p) >> t) & 1u);
+            const bool ally = teams && t >= 0 && t != p && ((team_mask(p) >> t) & 1u);
             if (t == p || ally) {  // R8 / P:L97, R19
                 ndst = d + m;
-                if (ndst > 32767) { ndst = 32767; gs.sat += 1; gs.flags |= GF_RECOUNT; }
+                if (ndst > 32767) { ndst = 32767; gs.sat += 1; gflags |= GF_RECOUNT; }
                 if (ally) {
                     if (!dst_general) { nown = p; gs.tot[p] += d; gs.tot[t] -= d; }
                     else { gs.tot[p] -= m; gs.tot[t] += m; }
@@ -622,13 +635,13 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             }
             A[cell] = (int16_t)nsrc;
             A[dst] = (int16_t)ndst;
-            touch(gs, cell);
-            touch(gs, dst);
-            set_bit(mrow(M_A2, lg), cell, nsrc >= 2);
-            set_bit(mrow(M_A2, lg), dst, ndst >= 2);
+            if (cell < 512) dA0 |= 1u << (cell >> 4); else dA1 |= 1u << ((cell >> 4) & 31);
+            if (dst < 512) dA0 |= 1u << (dst >> 4); else dA1 |= 1u << ((dst >> 4) & 31);
+            set_bit(a2row, cell, nsrc >= 2);
+            set_bit(a2row, dst, ndst >= 2);
             if (nown != t) {
                 O[dst] = (int8_t)nown;
-                gs.dirtyO |= 1u << (dst >> 5);
+                dO |= 1u << (dst >> 5);
                 set_bit(mrow(nown, lg), dst, true);
                 gs.land[nown] += 1;
                 if (t >= 0) { set_bit(mrow(t, lg), dst, false); gs.land[t] -= 1; }
@@ -652,20 +665,25 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                         A[c] = (int16_t)(fl ? (av >> 1) : ((av + 1) >> 1));
                     }
                 }
-                gs.flags |= GF_REBUILD | GF_RECOUNT | GF_TERRAIN_DIRTY | GF_ALL_DIRTY;
+                gflags |= GF_REBUILD | GF_RECOUNT | GF_TERRAIN_DIRTY | GF_ALL_DIRTY;
             }
         }
         // a6: turn counter; growth itself is applied by the next parallel pass (R1, R2, R3)
-        gs.turn += 1;
-        if ((gs.turn & 1) == 0) gs.flags |= GF_GROW_EVEN;
-        if (gs.turn % 50 == 0) gs.flags |= GF_GROW_TICK;
+        const int turn = gs.turn + 1;
+        gs.turn = turn;
+        if ((turn & 1) == 0) gflags |= GF_GROW_EVEN;
+        if (turn % 50 == 0) gflags |= GF_GROW_TICK;
+        if (gflags) gs.flags |= gflags;
+        if (dA0) gs.dirtyA[0] |= dA0;
+        if (dA1) gs.dirtyA[1] |= dA1;
+        if (dO) gs.dirtyO |= dO;
     };
 
     // ---------------------------------------------------------------- a6: growth
     // tick turns (every 50th): cell pass over one chunk, +1 on owned cells (+2 on owned structures)
     auto grow_chunk = [&](int lg, int ch, uint32_t gflags) {
         GameS &gs = s_game[lg];
-        const uint32_t sb = mrow8(M_STR, lg)[ch];
+        const uint32_t sb = mrow8(R_STR, lg)[ch];
         uint32_t ownedb = 0;
         for (int p = 0; p < P; ++p) ownedb |= mrow8(p, lg)[ch];
         const uint32_t e = (gflags & GF_GROW_EVEN) ? (sb & ownedb) : 0u;
@@ -697,7 +715,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         }
         a.x = aw[0]; a.y = aw[1]; a.z = aw[2]; a.w = aw[3];
         *ap = a;
-        mrow8(M_A2, lg)[ch] = (unsigned char)ge2_bits(a);
+        mrow8(R_A2, lg)[ch] = (unsigned char)ge2_bits(a);
         atomicOr(&gs.dirtyA[ch >> 6], 1u << ((ch >> 1) & 31));
         for (int p = 0; p < P; ++p) {
             const uint32_t ob = mrow8(p, lg)[ch];
@@ -705,17 +723,15 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             if (inc) atomicAdd(&gs.tot[p], inc);
         }
     };
-    // even turns that are no tick: +1 on the few owned structures, found by bit iteration
+    // even turns that are no tick: +1 on the few owned structures, found by bit iteration (octet)
     auto grow_structures = [&](int lg) {
         GameS &gs = s_game[lg];
         int16_t *A = s_army + (size_t)lg * S;
         uint32_t dA0 = 0, dA1 = 0;
-        for (int i = 0; i < WPL; ++i) {
-            const int j = ol * WPL + i;
-            if (j >= NW) break;
-            const uint32_t sw = mrow(M_STR, lg)[j] & s_inb[j];
+        for (int j = ol; j < NW; j += LPG) {
+            const uint32_t sw = mrow(R_STR, lg)[j];
             if (sw == 0) continue;
-            uint32_t a2w = mrow(M_A2, lg)[j];
+            uint32_t a2w = mrow(R_A2, lg)[j];
             bool changed = false;
             for (int p = 0; p < P; ++p) {
                 uint32_t m = sw & mrow(p, lg)[j];
@@ -733,38 +749,55 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 }
                 if (inc) atomicAdd(&gs.tot[p], inc);
             }
-            if (changed) mrow(M_A2, lg)[j] = a2w;
+            if (changed) mrow(R_A2, lg)[j] = a2w;
         }
         if (dA0) atomicOr(&gs.dirtyA[0], dA0);
         if (dA1) atomicOr(&gs.dirtyA[1], dA1);
     };
 
     // ---------------------------------------------------------------- a7-a9: end of turn, one lane per game
+    auto write_result = [&](size_t slot, int gg, int rew_bits, uint32_t done, int winner) {
+        int8_t *rw = B.reward + (slot * kp.N + gg) * P;
+        if (rew_bits == 0x5555 >> (16 - 2 * P) && (P == 2 || P == 4 || P == 8)) {  // all zero: one store
+            if (P == 2) *reinterpret_cast<uint16_t *>(rw) = 0;
+            else if (P == 4) *reinterpret_cast<uint32_t *>(rw) = 0;
+            else *reinterpret_cast<uint2 *>(rw) = make_uint2(0u, 0u);
+        } else {
+            for (int p = 0; p < P; ++p) rw[p] = (int8_t)(((rew_bits >> (2 * p)) & 3) - 1);
+        }
+        B.done[slot * kp.N + gg] = (uint8_t)done;
+        B.winner[slot * kp.N + gg] = (int8_t)winner;
+    };
     auto finish_turn = [&](int lg, size_t slot, bool write_out) {
         GameS &gs = s_game[lg];
         const int gg = wg0 + lg;
         if (gs.sat) { B.sat_events[gg] += gs.sat; gs.sat = 0; }
+        const int zero_bits = 0x5555 >> (16 - 2 * P);
+        const bool truncated_now = kp.max_turns > 0 && gs.turn >= kp.max_turns;
+        if (gs.alive == allp && !truncated_now && kp.n_teams > 1) {  // the common case: nothing ends
+            gs.done = 0;
+            gs.winner = -1;
+            gs.rew_bits = zero_bits;
+            if (write_out) write_result(slot, gg, zero_bits, 0u, -1);
+            return;
+        }
         int living = 0, last = -1;
         for (int t = 0; t < kp.n_teams; ++t) {
             const uint32_t tm = (((1u << kp.team_size) - 1u) << (t * kp.team_size)) & allp;
             if (gs.alive & tm) { ++living; last = t; }
         }
         const bool terminated = living <= 1;
-        const bool truncated = !terminated && kp.max_turns > 0 && gs.turn >= kp.max_turns;
+        const bool truncated = !terminated && truncated_now;
         gs.done = (terminated ? 1u : 0u) | (truncated ? 2u : 0u);
         gs.winner = terminated ? last : -1;
         int rew_bits = 0;
         for (int p = 0; p < P; ++p) {
             const int r = terminated ? ((p / kp.team_size == last) ? 1 : -1) : 0;
             rew_bits |= (r + 1) << (2 * p);
-            if (write_out) B.reward[(slot * kp.N + gg) * P + p] = (int8_t)r;
             if (r > 0) B.wins[(size_t)gg * P + p] += 1;
         }
         gs.rew_bits = rew_bits;
-        if (write_out) {
-            B.done[slot * kp.N + gg] = (uint8_t)gs.done;
-            B.winner[slot * kp.N + gg] = (int8_t)gs.winner;
-        }
+        if (write_out) write_result(slot, gg, rew_bits, gs.done, gs.winner);
         if (gs.done) {
             B.episodes_done[gg] += 1;
             if (truncated) B.truncations[gg] += 1;
@@ -776,61 +809,58 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         }
     };
 
-    // ---------------------------------------------------------------- a10: fog of war (octet, player p)
-    // vis = 3x3 dilation of the team's cells.  Lane l produces words l*WPL..; the horizontally dilated
-    // neighbour words are recomputed in registers, so the pass needs no scratch row and no sync.
-    auto compute_vis = [&](int lg, int p) {
-        uint32_t *vr = mrow(M_VIS + p, lg);
-        const uint32_t members = team_mask(p);
-        auto team_word = [&](int j) -> uint32_t {
-            if (j < 0 || j >= NW) return 0u;
-            if (kp.team_size == 1) return mrow(p, lg)[j];
+    // ---------------------------------------------------------------- a10: fog of war (all players at once)
+    // vis = 3x3 dilation of the team's cells.  Sub-lane (pl, sl) streams through its WS words of player pl's
+    // row with a sliding window: tw = team-owned words, h = horizontally dilated words, both in registers.
+    auto compute_vis = [&](int lg) {
+        if (pl >= P) return;
+        const int js = sl * WS, je = min(js + WS, NW);
+        if (js >= je) return;
+        uint32_t *vr = mrow(R_VIS + pl, lg);
+        const uint32_t *own = mrow(pl, lg);
+        const uint32_t members = teams ? team_mask(pl) : 0u;
+        auto tw = [&](int j) -> uint32_t {
+            if ((unsigned)j >= (unsigned)NW) return 0u;
+            if (!teams) return own[j];
             uint32_t tm = 0;
             for (int q = 0; q < P; ++q)
                 if ((members >> q) & 1u) tm |= mrow(q, lg)[j];
             return tm;
         };
-        const int j0 = ol * WPL;
-        if (j0 >= NW) return;
-        uint32_t tw[MAXWPL + 4], hh[MAXWPL + 2];
-#pragma unroll
-        for (int i = 0; i < MAXWPL + 4; ++i) tw[i] = (i < WPL + 4) ? team_word(j0 - 2 + i) : 0u;
-#pragma unroll
-        for (int i = 0; i < MAXWPL + 2; ++i) {
-            const int j = j0 - 1 + i;
-            hh[i] = 0;
-            if (i < WPL + 2 && j >= 0 && j < NW)
-                hh[i] = tw[i + 1] | (__funnelshift_l(tw[i], tw[i + 1], 1) & s_nc0[j]) |
-                        (__funnelshift_r(tw[i + 1], tw[i + 2], 1) & s_ncL[j]);
-        }
-#pragma unroll
-        for (int i = 0; i < MAXWPL; ++i) {
-            const int j = j0 + i;
-            if (i < WPL && j < NW)
-                vr[j] = (hh[i + 1] | __funnelshift_lc(hh[i], hh[i + 1], W) | __funnelshift_rc(hh[i + 1], hh[i + 2], W)) &
-                        s_inb[j];
+        auto hdil = [&](uint32_t a, uint32_t b, uint32_t c, int j) -> uint32_t {  // s_nc0 / s_ncL are 0 off the board
+            return b | (__funnelshift_l(a, b, 1) & s_nc0[j]) | (__funnelshift_r(b, c, 1) & s_ncL[j]);
+        };
+        uint32_t t1 = tw(js - 1), t2 = tw(js), t3 = tw(js + 1);
+        uint32_t hm = hdil(tw(js - 2), t1, t2, js - 1), hc = hdil(t1, t2, t3, js);
+        for (int j = js; j < je; ++j) {
+            const uint32_t t4 = tw(j + 2);
+            const uint32_t hn = hdil(t2, t3, t4, j + 1);
+            vr[j] = (hc | __funnelshift_lc(hm, hc, W) | __funnelshift_rc(hc, hn, W)) & s_inb[j];
+            hm = hc; hc = hn; t2 = t3; t3 = t4;
         }
     };
 
     // ---------------------------------------------------------------- a11: observation planes (octet)
-    // per 8-cell chunk and player: one 16-byte and three 8-byte streaming stores; the 8 lanes of the octet
+    // per player, per 8-cell chunk: one 16-byte and three 8-byte streaming stores; the 8 lanes of the octet
     // write 128 / 64 contiguous bytes per instruction (full 32-byte sectors)
     auto emit_planes = [&](int lg, size_t slot) {
         const size_t base = (slot * (size_t)kp.N + (size_t)(wg0 + lg)) * (size_t)P * (size_t)S;
-        int16_t *pa = B.obs_army + base;
-        int8_t *po = B.obs_owner + base, *pt = B.obs_terrain + base;
-        uint8_t *pv = B.obs_vis + base;
-        const int16_t *sa = s_army + (size_t)lg * S;
-        const int8_t *so = s_owner + (size_t)lg * S, *st = s_terr + (size_t)lg * S;
+        const unsigned char *sa = reinterpret_cast<const unsigned char *>(s_army + (size_t)lg * S) + 16 * ol;
+        const unsigned char *so = reinterpret_cast<const unsigned char *>(s_owner + (size_t)lg * S) + 8 * ol;
+        const unsigned char *st = reinterpret_cast<const unsigned char *>(s_terr + (size_t)lg * S) + 8 * ol;
+        const int nit = (NC8 - ol + LPG - 1) / LPG;  // chunks of this lane: ol, ol + 8, ...
+        for (int p = 0; p < P; ++p) {
+            const unsigned char *sv = mrow8(R_VIS + p, lg) + ol;
+            unsigned char *ga = reinterpret_cast<unsigned char *>(B.obs_army + base + (size_t)p * S) + 16 * ol;
+            unsigned char *go = reinterpret_cast<unsigned char *>(B.obs_owner + base + (size_t)p * S) + 8 * ol;
+            unsigned char *gt = reinterpret_cast<unsigned char *>(B.obs_terrain + base + (size_t)p * S) + 8 * ol;
+            unsigned char *gv = reinterpret_cast<unsigned char *>(B.obs_vis + base + (size_t)p * S) + 8 * ol;
 #pragma unroll 3
-        for (int ch = ol; ch < NC8; ch += LPG) {
-            const uint4 a = *reinterpret_cast<const uint4 *>(sa + 8 * ch);
-            const uint2 o = *reinterpret_cast<const uint2 *>(so + 8 * ch);
-            const uint2 t = *reinterpret_cast<const uint2 *>(st + 8 * ch);
-#pragma unroll
-            for (int p = 0; p < NP; ++p) {
-                if (NP > 2 && p >= P) break;
-                const uint32_t vb = mrow8(M_VIS + p, lg)[ch];
+            for (int i = 0; i < nit; ++i) {
+                const uint4 a = *reinterpret_cast<const uint4 *>(sa + 128 * i);
+                const uint2 o = *reinterpret_cast<const uint2 *>(so + 64 * i);
+                const uint2 t = *reinterpret_cast<const uint2 *>(st + 64 * i);
+                const uint32_t vb = sv[8 * i];
                 const uint32_t s0 = nib_sign(vb & 15u), s1 = nib_sign(vb >> 4);
                 const uint32_t m0 = prmt(s0, 0u, 0xBA98u), m1 = prmt(s1, 0u, 0xBA98u);
                 uint4 oa;
@@ -840,11 +870,10 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 oo.x = (o.x & m0) | (~m0 & 0xFEFEFEFEu); oo.y = (o.y & m1) | (~m1 & 0xFEFEFEFEu);
                 ot.x = (t.x & m0) | (~m0 & 0x04040404u); ot.y = (t.y & m1) | (~m1 & 0x04040404u);
                 ov.x = m0 & 0x01010101u; ov.y = m1 & 0x01010101u;
-                const int off = p * S + 8 * ch;
-                __stcs(reinterpret_cast<uint4 *>(pa + off), oa);
-                __stcs(reinterpret_cast<uint2 *>(po + off), oo);
-                __stcs(reinterpret_cast<uint2 *>(pt + off), ot);
-                __stcs(reinterpret_cast<uint2 *>(pv + off), ov);
+                __stcs(reinterpret_cast<uint4 *>(ga + 128 * i), oa);
+                __stcs(reinterpret_cast<uint2 *>(go + 64 * i), oo);
+                __stcs(reinterpret_cast<uint2 *>(gt + 64 * i), ot);
+                __stcs(reinterpret_cast<uint2 *>(gv + 64 * i), ov);
             }
         }
     };
@@ -861,7 +890,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             for (int ch = ol; ch < NC8; ch += LPG) {
                 uint32_t vb[NP], any = 0;
 #pragma unroll
-                for (int p = 0; p < NP; ++p) { vb[p] = (p < P) ? mrow8(M_VIS + p, lg)[ch] : 0u; any |= vb[p]; }
+                for (int p = 0; p < NP; ++p) { vb[p] = (p < P) ? mrow8(R_VIS + p, lg)[ch] : 0u; any |= vb[p]; }
                 if (any == 0) continue;
                 const uint4 a = *reinterpret_cast<const uint4 *>(s_army + (size_t)lg * S + 8 * ch);
                 const uint2 o = *reinterpret_cast<const uint2 *>(s_owner + (size_t)lg * S + 8 * ch);
@@ -903,10 +932,8 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         if (gvalid) {
             const GameS &gs = s_game[sub];
             const bool frozen = !kp.auto_reset && gs.done != 0;
-            for (int p = 0; p < P; ++p) {
-                const int a = frozen ? 0 : sample(sub, p, kp.global_step0);
-                if (ol == 0) kp.sample_out[(size_t)g * P + p] = a;
-            }
+            const int a = frozen ? 0 : sample(sub, kp.global_step0);
+            if (sl == 0 && pl < P) kp.sample_out[(size_t)g * P + pl] = a;
         }
         return;
     }
@@ -917,29 +944,25 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         const size_t slot = every ? (size_t)k : 0;
         const uint32_t gstep = kp.global_step0 + (uint32_t)k;
         const bool last_step = (k == kp.K - 1);
-        // ---- actions, then the moves (lane 0 of the octet)
+        // ---- actions (all players at once), then the moves (lane 0 of the octet)
+        bool frozen = false;
         if (gvalid) {
             GameS &gs = s_game[sub];
-            const bool frozen = !kp.auto_reset && gs.done != 0;  // R31
-            if (flags & F_SAMPLER) {
-                for (int p = 0; p < P; ++p) {
-                    const int a = frozen ? 0 : sample(sub, p, gstep);
-                    if (ol == 0) {
-                        gs.act[p] = a;
-                        if (B.actions_out) B.actions_out[(slot * kp.N + g) * P + p] = a;
-                    }
-                }
-            } else if (ol == 0) {
-                for (int p = 0; p < P; ++p) {
-                    const int a = frozen ? 0 : kp.actions[(size_t)g * P + p];
-                    gs.act[p] = a;
-                    if (B.actions_out) B.actions_out[(slot * kp.N + g) * P + p] = a;
-                }
+            frozen = !kp.auto_reset && gs.done != 0;  // R31
+            int a = 0;
+            if (!frozen) {
+                if (flags & F_SAMPLER) a = sample(sub, gstep);
+                else if (sl == 0 && pl < P) a = kp.actions[(size_t)g * P + pl];
             }
-            if (ol == 0) {
-                if (frozen) gs.flags |= GF_FROZEN;
-                else play_moves(sub);
+            if (sl == 0 && pl < P) {
+                gs.act[pl] = a;
+                if (B.actions_out) B.actions_out[(slot * kp.N + g) * P + pl] = a;
             }
+        }
+        __syncwarp();
+        if (gvalid && ol == 0) {
+            if (frozen) s_game[sub].flags |= GF_FROZEN;
+            else play_moves(sub);
         }
         __syncwarp();
         // ---- parallel pass: rebuild after a capture, growth, recount after a saturation
@@ -966,29 +989,25 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         __syncwarp();
         // ---- end of turn
         bool want_reset = false;
-        if (gvalid) {
+        if (gvalid && ol == 0) {
             GameS &gs = s_game[sub];
-            if (ol == 0) {
-                if (gs.flags & GF_FROZEN) {
-                    gs.rew_bits = 0;
-                    for (int p = 0; p < P; ++p) gs.rew_bits |= 1 << (2 * p);
-                    if (every || last_step) {
-                        for (int p = 0; p < P; ++p) B.reward[(slot * kp.N + g) * P + p] = 0;
-                        B.done[slot * kp.N + g] = (uint8_t)gs.done;
-                        B.winner[slot * kp.N + g] = (int8_t)gs.winner;
-                    }
-                } else {
-                    finish_turn(sub, slot, every || last_step);
-                }
-                want_reset = (gs.flags & GF_RESET) != 0;
+            if (frozen) {
+                gs.rew_bits = 0x5555 >> (16 - 2 * P);
+                if (every || last_step) write_result(slot, g, gs.rew_bits, gs.done, gs.winner);
+            } else {
+                finish_turn(sub, slot, every || last_step);
             }
+            want_reset = (gs.flags & GF_RESET) != 0;
         }
         const uint32_t rs = __ballot_sync(FULL, want_reset);  // bit sub * LPG: game sub must be regenerated
         if (rs) {
             for (int lg = 0; lg < nwg; ++lg)
                 if ((rs >> (lg * LPG)) & 1u) generate(lg);
-            if (gvalid && ((rs >> (sub * LPG)) & 1u)) {
-                build_game(sub);
+            const bool mine = gvalid && ((rs >> (sub * LPG)) & 1u);
+            if (mine) build_game(sub);
+            __syncwarp();
+            if (mine) {
+                build_ok(sub);
                 if (ol == 0) s_game[sub].flags &= ~GF_RESET;
             }
         }
@@ -996,23 +1015,20 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         // ---- a10 + a11 (R32: the state at the end of the call)
         const bool planes = (flags & F_OBS_PLANES) && (every || last_step);
         if (planes || (flags & F_DIGEST)) {
-            if (gvalid)
-                for (int p = 0; p < P; ++p) compute_vis(sub, p);
+            if (gvalid) compute_vis(sub);
             __syncwarp();
             if (planes && gvalid) emit_planes(sub, slot);
-            if (flags & F_DIGEST) chain_digest(sub, gvalid && !(s_game[sub].flags & GF_FROZEN));
+            if (flags & F_DIGEST) chain_digest(sub, gvalid && !frozen);
         }
     }
 
     if (kp.K == 0) {  // gen_reset / gen_observe: observation of the state as it stands
         if (gvalid) {
-            for (int p = 0; p < P; ++p) compute_vis(sub, p);
+            compute_vis(sub);
             if ((flags & F_RESET) && ol == 0) {
                 GameS &gs = s_game[sub];
-                gs.rew_bits = 0;
-                for (int p = 0; p < P; ++p) { B.reward[(size_t)g * P + p] = 0; gs.rew_bits |= 1 << (2 * p); }
-                B.done[g] = 0;
-                B.winner[g] = -1;
+                gs.rew_bits = 0x5555 >> (16 - 2 * P);
+                write_result(0, g, gs.rew_bits, 0u, -1);
             }
         }
         __syncwarp();
