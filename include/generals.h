@@ -170,9 +170,19 @@ int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_action
                   uint8_t *h_done, void *cuda_stream);
 
 /* Launch geometry override for tuning: games per CTA in {4, 8, 16, 32} (8 threads per game); 0 restores
- * the default (16, halved while the CTA's boards would not leave room for three CTAs per SM).  Results
- * do not depend on it. */
+ * the default (8).  Results do not depend on it. */
 int gen_set_launch(gen_env *env, int32_t games_per_cta);
+
+/* Kernel selection override for tests: the library holds board-specialised instantiations of its one
+ * kernel for the paper-sized configurations (1v1 8x8 and 24x24, 4 and 8 players on 32x32) next to the
+ * generic one that serves every board up to 32x32.  force_generic != 0 makes this handle always launch the
+ * generic kernel.  Results do not depend on it. */
+int gen_set_generic(gen_env *env, int32_t force_generic);
+
+/* Which instantiation the last launch of this handle used: returns its index in the library's variant
+ * table (-1 before the first launch) and, if board_specialised is non-NULL, stores 1 there when that
+ * kernel was compiled for this exact board size and mode, 0 for the generic one.  Diagnostic only. */
+int32_t gen_last_variant(const gen_env *env, int32_t *board_specialised);
 
 /* Number of kernels this handle has launched (bench.py's gpu_launches). */
 uint64_t gen_launch_count(const gen_env *env);

@@ -15,7 +15,8 @@ RULE_TICK_PLAIN_ONLY, RULE_CAPTURE_HALF_FLOOR, RULE_ROTATE_PRIORITY = 1, 2, 4
 
 EXPORTS = ["gen_query_sizes", "gen_init", "gen_set_policy", "gen_global_step", "gen_set_global_step",
            "gen_reset", "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host",
-           "gen_set_launch", "gen_launch_count", "gen_last_cuda_error", "gen_destroy",
+           "gen_set_launch", "gen_set_generic", "gen_last_variant",
+           "gen_launch_count", "gen_last_cuda_error", "gen_destroy",
            "gen_error_string", "gen_version"]
 
 
@@ -96,6 +97,9 @@ def load_library(path=None):
     lib.gen_sample.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
     lib.gen_step_host.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.gen_set_launch.argtypes = [env_p, C.c_int32]
+    lib.gen_set_generic.argtypes = [env_p, C.c_int32]
+    lib.gen_last_variant.argtypes = [env_p, C.POINTER(C.c_int32)]
+    lib.gen_last_variant.restype = C.c_int32
     lib.gen_launch_count.argtypes = [env_p]
     lib.gen_launch_count.restype = C.c_uint64
     lib.gen_last_cuda_error.argtypes = [env_p]
@@ -106,7 +110,7 @@ def load_library(path=None):
     lib.gen_version.restype = C.c_char_p
     for name in ("gen_query_sizes", "gen_init", "gen_set_policy", "gen_set_global_step", "gen_reset",
                  "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host", "gen_set_launch",
-                 "gen_last_cuda_error"):
+                 "gen_set_generic", "gen_last_cuda_error"):
         getattr(lib, name).restype = C.c_int
     if path == LIB_PATH:
         _lib = lib
@@ -209,6 +213,16 @@ class GeneralsEnv:
 
     def set_launch(self, games_per_cta):
         self._check(self.lib.gen_set_launch(self._env, int(games_per_cta)))
+
+    def set_generic(self, force_generic=True):
+        self._check(self.lib.gen_set_generic(self._env, 1 if force_generic else 0))
+
+    @property
+    def last_launch_specialised(self):
+        """True when the last launch used a kernel compiled for this exact board size and mode."""
+        flag = C.c_int32(0)
+        self.lib.gen_last_variant(self._env, C.byref(flag))
+        return bool(flag.value)
 
     @property
     def launch_count(self):

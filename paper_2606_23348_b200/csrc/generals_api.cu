@@ -4,7 +4,7 @@
 #include <cstring>
 #include <new>
 
-#include "generals_kernels.cuh"
+#include "generals_variants.h"
 
 struct gen_env {
     gen_config cfg;
@@ -14,7 +14,8 @@ struct gen_env {
     int32_t games_per_cta;   // 0 = default
     uint64_t launches;
     int last_cuda_error;
-    bool attr_set[3];        // cudaFuncSetAttribute done for <NP idx>
+    int32_t force_generic;   // 1: never pick a board-specialised kernel (tests)
+    int32_t last_variant;    // index into GEN_VARIANTS of the last launch (-1: none yet)
 };
 
 namespace {
@@ -74,7 +75,7 @@ int check_buffers(const gen_buffers *b, bool need_obs) {
     return GEN_OK;
 }
 
-constexpr size_t kMaxSmem = 200 * 1024;
+using gen::kMaxSmem;
 
 inline uint32_t align_up(uint32_t x, uint32_t a) { return (x + a - 1) / a * a; }
 
@@ -97,20 +98,42 @@ void layout(gen::KParams &k, int WPC, bool digest) {
     k.smem_bytes = k.off_warp0 + (uint32_t)WPC * k.warp_bytes;
 }
 
-template <int NP>
-int launch_np(gen_env *env, const gen::KParams &kp, int np_idx, cudaStream_t stream) {
-    auto kernel = gen::k_generals<NP>;
-    if (!env->attr_set[np_idx]) {
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
-        if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
-        env->attr_set[np_idx] = true;
+using gen::F_RUNTIME;
+using gen::FF_ROLL_DIGEST;
+using gen::FF_STEP;
+const gen::Variant kVariants[gen::N_VARIANTS] = {
+#define GEN_ROW(id, np, h, w, ff) {np, h, w, ff, gen::launch_variant_##id},
+    GEN_VARIANTS(GEN_ROW)
+#undef GEN_ROW
+};
+
+// the most specialised instantiation that serves this launch: exact board + exact mode first, else the
+// generic kernel of the smallest NP >= P
+const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp) {
+    const gen::Variant *generic = nullptr;
+    const uint32_t mode = (kp.flags & ~gen::F_SAMPLER) | (kp.K == 1 ? gen::F_K1 : 0u);
+    for (const gen::Variant &v : kVariants) {
+        if (v.h == 0) {
+            if (kp.P <= v.np && (!generic || v.np < generic->np)) generic = &v;
+            continue;
+        }
+        if (env->force_generic || v.np != kp.P || v.h != kp.H || v.w != kp.W) continue;
+        if (v.np == 2 && kp.team_size > 1) continue;
+        const uint32_t want = (v.ff & gen::F_K1) ? mode : (mode & ~gen::F_K1);
+        if (v.ff == want) return &v;
     }
+    return generic;
+}
+
+int launch_kernel(gen_env *env, const gen::KParams &kp, cudaStream_t stream) {
+    const gen::Variant *v = pick_variant(env, kp);
+    if (!v) return GEN_ERR_CONFIG;
     const int per_cta = gen::GW * kp.WPC;
     const int grid = (kp.N + per_cta - 1) / per_cta;
-    kernel<<<grid, 32 * kp.WPC, kp.smem_bytes, stream>>>(kp);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = v->launch(kp, grid, 32 * kp.WPC, kp.smem_bytes, stream);
     if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
     env->launches += 1;
+    env->last_variant = (int32_t)(v - kVariants);
     return GEN_OK;
 }
 
@@ -135,10 +158,7 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
         layout(kp, WPC, (flags & gen::F_DIGEST) != 0);
     }
     if (kp.smem_bytes > kMaxSmem) return GEN_ERR_CONFIG;
-    cudaStream_t s = static_cast<cudaStream_t>(stream);
-    if (kp.P <= 2) return launch_np<2>(env, kp, 0, s);
-    if (kp.P <= 4) return launch_np<4>(env, kp, 1, s);
-    return launch_np<8>(env, kp, 2, s);
+    return launch_kernel(env, kp, static_cast<cudaStream_t>(stream));
 }
 
 uint64_t host_mix64(uint64_t z) {  // splitmix64 finaliser: the digest keys of R28
@@ -167,6 +187,7 @@ int gen_init(const gen_config *cfg, gen_env **out) {
     if (!env) return GEN_ERR_ARG;
     std::memset(env, 0, sizeof(*env));
     env->cfg = *cfg;
+    env->last_variant = -1;
     env->policy.pass_thr = 0;
     env->policy.half_thr = 0x80000000u;
     env->policy.bias_thr = 0;
@@ -294,6 +315,18 @@ int gen_set_launch(gen_env *env, int32_t games_per_cta) {
         return GEN_ERR_ARG;
     env->games_per_cta = games_per_cta;
     return GEN_OK;
+}
+
+int gen_set_generic(gen_env *env, int32_t force_generic) {
+    if (!env) return GEN_ERR_NULL;
+    env->force_generic = force_generic ? 1 : 0;
+    return GEN_OK;
+}
+
+int32_t gen_last_variant(const gen_env *env, int32_t *board_specialised) {
+    if (!env || env->last_variant < 0) return -1;
+    if (board_specialised) *board_specialised = kVariants[env->last_variant].h > 0 ? 1 : 0;
+    return env->last_variant;
 }
 
 uint64_t gen_launch_count(const gen_env *env) { return env ? env->launches : 0; }

@@ -46,6 +46,8 @@ enum : uint32_t {
     F_OBSERVE_ONLY = 1u << 5,  // gen_observe: recount + planes, no turn
     F_SAMPLE_ONLY = 1u << 6,   // gen_sample: actions only
     F_KEEP_EPISODE = 1u << 7,
+    F_RUNTIME = 0xFFFFFFFFu,   // template argument FF: read the flags word from KParams (generic kernel)
+    F_K1 = 1u << 30,           // template argument FF only: exactly one turn per launch (gen_step)
 };
 
 enum : int { T_PLAIN = 0, T_MOUNTAIN = 1, T_CITY = 2, T_GENERAL = 3, T_FOG = 4 };
@@ -198,8 +200,14 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 }
 
 // ================================================================================================
-template <int NP>
+// Template arguments: NP = bound of the player loops (register arrays).  CH x CW > 0 = the board size is a
+// compile-time constant and P == NP exactly (the paper-sized configs: strides, word counts and the row
+// division fold into immediates and the cell loops unroll); 0 = any board up to 32 x 32, read from KParams.
+// FF = the mode flags as a compile-time constant (dead modes drop out of the instruction stream), or
+// F_RUNTIME.  With FF fixed, F_SAMPLER alone stays a runtime choice.
+template <int NP, int CH, int CW, uint32_t FF>
 __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParams kp) {
+    constexpr bool FIXED = CH > 0;
     constexpr int LPP = LPG / NP;  // lanes serving one (game, player) pair in the word passes
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x;
@@ -208,17 +216,21 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     const int ol = (int)(lane & (LPG - 1)), sub = (int)(lane / LPG);  // lane of the octet, game of the warp
     const uint32_t gmask = ((1u << LPG) - 1u) << (sub * LPG);         // the lanes of this octet
     const int pl = ol / LPP, sl = ol % LPP;                           // word passes: my player, my sub-lane
-    const int H = kp.H, W = kp.W, P = kp.P, HW = kp.HW, S = kp.S, NW = kp.NW, NC8 = kp.NC8;
-    const int RW = kp.RW, M = kp.M;
+    constexpr int cHW = CH * CW, cS = (cHW + 15) / 16 * 16, cNW = (cHW + 31) / 32;
+    const int H = FIXED ? CH : kp.H, W = FIXED ? CW : kp.W, P = FIXED ? NP : kp.P;
+    const int HW = FIXED ? cHW : kp.HW, S = FIXED ? cS : kp.S, NW = FIXED ? cNW : kp.NW;
+    const int NC8 = FIXED ? cS / 8 : kp.NC8, NCH = FIXED ? 4 * cNW : kp.NCH;
+    const int RW = FIXED ? (cNW | 1) : kp.RW, M = FIXED ? 2 * NP + 6 : kp.M;
     const int WS = (NW + LPP - 1) / LPP;  // words per sub-lane
-    const uint32_t flags = kp.flags;
+    const uint32_t flags = (FF == F_RUNTIME) ? kp.flags : ((FF & ~F_K1) | (kp.flags & F_SAMPLER));
+    const int K = (FF != F_RUNTIME && (FF & F_K1)) ? 1 : kp.K;
     const gen_buffers &B = kp.b;
     const int wg0 = (blockIdx.x * kp.WPC + wic) * GW;  // first game of this warp
     const int nwg = min(GW, kp.N - wg0);               // games of this warp (<= 0: nothing to do)
     const bool gvalid = sub < nwg;
     const int g = wg0 + sub;
     const uint32_t allp = (1u << P) - 1u;
-    const bool teams = kp.team_size > 1;
+    const bool teams = (FIXED && NP == 2) ? false : kp.team_size > 1;
 
     // CTA-wide tables, index j + 1 for bitboard word j (entries 0 and 33 are zero guards): column masks,
     // in-bounds mask; digest keys
@@ -244,7 +256,9 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         const int t = p / kp.team_size;
         return (((1u << kp.team_size) - 1u) << (t * kp.team_size)) & allp;
     };
-    auto row_of = [&](int cell) -> int { return (int)(((uint32_t)cell * kp.recipW) >> 16); };
+    auto row_of = [&](int cell) -> int {
+        return FIXED ? (int)((uint32_t)cell / (uint32_t)(FIXED ? CW : 1)) : (int)(((uint32_t)cell * kp.recipW) >> 16);
+    };
 
     // ---------------------------------------------------------------- a1: generator, one warp per game
     // (R13, R14, R29, R30)
@@ -380,7 +394,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             rows[R_STR * rb + ch] = (unsigned char)gather8<0>(hx, hy);
             rows[R_A2 * rb + ch] = (unsigned char)ge2_bits(a);
         }
-        for (int ch = NC8 + ol; ch < kp.NCH; ch += LPG) {  // bytes of the last word past the plane stride
+        for (int ch = NC8 + ol; ch < NCH; ch += LPG) {  // bytes of the last word past the plane stride
             for (int p = 0; p < P; ++p) rows[p * rb + ch] = 0;
             rows[R_MTN * rb + ch] = 0xFF;
             rows[R_STR * rb + ch] = 0;
@@ -940,10 +954,10 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
 
     // ================================================================ K turns
     const bool every = (flags & F_OBS_EVERY) != 0;
-    for (int k = 0; k < kp.K; ++k) {
+    for (int k = 0; k < K; ++k) {
         const size_t slot = every ? (size_t)k : 0;
         const uint32_t gstep = kp.global_step0 + (uint32_t)k;
-        const bool last_step = (k == kp.K - 1);
+        const bool last_step = (k == K - 1);
         // ---- actions (all players at once), then the moves (lane 0 of the octet)
         bool frozen = false;
         if (gvalid) {
@@ -1022,7 +1036,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         }
     }
 
-    if (kp.K == 0) {  // gen_reset / gen_observe: observation of the state as it stands
+    if (K == 0) {  // gen_reset / gen_observe: observation of the state as it stands
         if (gvalid) {
             compute_vis(sub);
             if ((flags & F_RESET) && ol == 0) {

@@ -125,6 +125,49 @@ def test_captures_happen_and_match(gpu, oracle_mod):
     assert int(o.wins.sum()) > 20                          # real captures, not truncations
 
 
+# ------------------------------------------------------------------------------- board-specialised kernels
+@pytest.mark.parametrize("name,N,T,over", [
+    ("c2_24x24", 101, 230, dict(max_turns=110)),
+    ("c4_curriculum", 75, 300, dict(max_turns=200)),
+    ("c1_8x8", 77, 200, dict(auto_reset=1, max_turns=80)),
+    ("c5a_2v2", 37, 230, dict(max_turns=150)),
+    ("c5b_ffa8", 37, 230, dict(max_turns=150)),
+])
+def test_specialised_step_kernels_match_oracle(gpu, oracle_mod, name, N, T, over):
+    """The per-step kernels compiled for the paper-sized boards (what bench.py times: no digest buffer)
+    against the oracle, every tensor every step; the same handle forced onto the generic kernel must
+    agree too."""
+    cfg, _ = workloads.config(name, n_games=N, **over)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    gen = gpu.GeneralsEnv(cfg, digest=False)
+    gen.set_generic(True)
+    o = oracle_mod.Oracle(cfg)
+    for e in (env, gen):
+        e.reset()
+    o.reset()
+    for t in range(T):
+        env.step()
+        gen.step()
+        o.step()
+        compare(env, o, digest=False, where=f"{name} specialised step {t}")
+        if t % 16 == 0:
+            compare(gen, o, digest=False, where=f"{name} generic step {t}")
+    assert env.last_launch_specialised and not gen.last_launch_specialised
+    assert int(o.episodes_done.sum()) > 0
+
+
+def test_specialised_rollout_kernel_matches_oracle(gpu, oracle_mod):
+    cfg, _ = workloads.config("c2_24x24", n_games=70, max_turns=90)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    for it in range(4):
+        env.rollout(32, gpu.OBS_DIGEST)
+        o.rollout(32)
+        compare(env, o, where=f"rollout {it}")
+    assert env.last_launch_specialised
+
+
 # ------------------------------------------------------------------------------- rollout == steps
 @pytest.mark.parametrize("mode", ["digest", "none"])
 def test_rollout_equals_steps(gpu, oracle_mod, mode):
