@@ -29,6 +29,9 @@ METRIC = "env steps/sec (1v1, all games) on 1 B200; % of HBM or int-issue roofli
 UNIT = "env_steps/s"
 WORKLOAD = "c2_24x24"
 HBM_FALLBACK_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+# dram__bytes_read.sum + dram__bytes_write.sum of one gen_step launch, by games per launch, from the
+# `ncu --set full` capture summarised in profiles/ (see profiles/README.md); None where not captured
+NCU_DRAM_BYTES_PER_LAUNCH = {}
 
 
 def algorithmic_bytes_per_env_step(H, W, P):
@@ -134,7 +137,7 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, workloads
+    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, replicas, workloads
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -150,10 +153,14 @@ def run_ours(args):
     if args.games:
         cfg["n_games"] = args.games
     N, P, H, W = cfg["n_games"], cfg["n_players"], cfg["height"], cfg["width"]
-    cfg["game_id_base"] = rank * N                  # weak scaling: disjoint global game-id ranges, no collective
+    bmin = algorithmic_bytes_per_env_step(H, W, P)
+    # Replicas of the batch, stepped round-robin, so that every launch finds its inputs in HBM and not in
+    # the 126 MB L2: between two steps of the same replica the others move (R - 1) * N * bmin bytes.
+    R = args.replicas or max(2, -(-(640 << 20) // (N * bmin)))
     K, Wm = args.steps, args.warmup
-    env = GeneralsEnv(cfg, device=dev, digest=False, actions_out=True)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
+    envs = [GeneralsEnv(dict(cfg, game_id_base=(rank * R + r) * N), device=dev, digest=False, actions_out=(r == 0))
+            for r in range(R)]
+    env = envs[0]
 
     def barrier():
         if world > 1:
@@ -161,11 +168,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(x, dist if world > 1 else None, dev)
 
     # ---- record the action stream of warm-up + timed steps for the end-to-end leg (device sampler -> host)
     env.reset()
@@ -175,15 +178,31 @@ def run_ours(args):
         h_actions[t].copy_(env.tensors["actions_out"][0], non_blocking=True)
     torch.cuda.synchronize()
 
-    # ---- device-resident leg: per-step kernel, L2 flushed between timed iterations, CUDA events per step
-    env.reset()
-    for _ in range(Wm):
-        env.step()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    # ---- device-resident leg: K gen_step launches back to back, replica t % R at step t; one CUDA event pair
+    # on the launching (torch current) stream around the timed region
+    for e in envs:
+        e.reset()
+    for t in range(Wm):
+        envs[t % R].step()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     clocks = ClockSampler(local)
     if rank == 0:
         clocks.start()
-    launches0 = env.launch_count
+    launches0 = sum(e.launch_count for e in envs)
+    barrier()
+    e0.record()
+    for t in range(Wm, Wm + K):
+        envs[t % R].step()
+    e1.record()
+    barrier()
+    launches = sum(e.launch_count for e in envs) - launches0
+    total_ms = max_over_ranks(e0.elapsed_time(e1))
+    specialised = env.last_launch_specialised
+
+    # ---- the same with a 256 MB L2-flush write before every launch and one event pair per launch
+    # (isolated launches: includes the launch latency a back-to-back stream hides)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(min(K, 50))]
     barrier()
     for a, b in ev:
         flush.fill_(1)
@@ -191,19 +210,8 @@ def run_ours(args):
         env.step()
         b.record()
     barrier()
-    kernel_ms = [a.elapsed_time(b) for a, b in ev]
-    launches = env.launch_count - launches0
-    total_ms = max_over_ranks(sum(kernel_ms))
-
-    # ---- same K steps back to back (no flush; state planes partly L2-resident), one event pair
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record()
-    for _ in range(K):
-        env.step()
-    e1.record()
-    barrier()
-    b2b_ms = max_over_ranks(e0.elapsed_time(e1))
+    iso_ms = statistics.median(a.elapsed_time(b) for a, b in ev)
+    del flush
 
     # ---- fused rollout leg (K_r = 32 turns per launch, observation digest chained every turn)
     renv = GeneralsEnv(cfg, device=dev, digest=True, actions_out=False)
@@ -239,10 +247,11 @@ def run_ours(args):
         return 0
 
     peak, peak_src = measured_peak()
-    bmin = algorithmic_bytes_per_env_step(H, W, P)
     value = world * N * K / (total_ms * 1e-3)
-    med_ms = statistics.median(kernel_ms)
-    achieved = N * bmin / (sum(kernel_ms) / K * 1e-3) / 1e9
+    launch_ms = total_ms / K
+    achieved = N * bmin / (launch_ms * 1e-3) / 1e9
+    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(N)
+    kname = f"gen::k_generals<{P}, {H}, {W}, F_OBS_PLANES | F_K1>" if specialised else "gen::k_generals (generic)"
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -250,19 +259,22 @@ def run_ours(args):
         "config": {"workload": f"{WORKLOAD}: 1v1 24x24, {N} games/GPU, auto-reset, max_turns 1000, device Philox "
                                "sampler 5% pass, 4 obs planes x 2 players written every step",
                    "n_games_per_gpu": N, "path": "gen_step (per-step kernel, 1 launch per step)",
-                   "l2": "256 MB flush write between timed iterations; each step timed with its own CUDA event pair",
+                   "l2": f"inputs larger than L2: {R} replicas of the batch stepped round-robin ({R} x "
+                         f"{N * bmin / 1e6:.0f} MB of algorithmic traffic between two steps of one replica; L2 is "
+                         "126 MB); K launches back to back, one CUDA event pair around them",
+                   "replicas_in_rotation": R,
                    "parallelism": f"replicas x{world}, disjoint game-id ranges, no collective"},
         "clocks": clock_info,
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": "gen::k_generals<2,8> (gen_step)", "peak_source": peak_src,
+                     "traffic": traffic, "kernel": kname + " (gen_step)", "peak_source": peak_src,
                      "algorithmic_bytes_per_env_step": bmin, "units_per_launch": N,
-                     "median_kernel_us": 1e3 * med_ms},
+                     "avg_launch_us": 1e3 * launch_ms,
+                     "isolated_launch_us": 1e3 * iso_ms,
+                     "isolated_note": "median of single launches, each after a 256 MB L2-flush write, own event pair"},
         "e2e": {"value": world * N * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": N * P * 4,
                 "d2h_bytes_per_step": N * P + N, "api": "gen_step_host (pinned host actions in, reward + done out)",
                 "done_checksum": checksum},
-        "back_to_back": {"value": world * N * K / (b2b_ms * 1e-3), "unit": UNIT, "ms_per_step": b2b_ms / K,
-                         "note": "no L2 flush, one event pair around K launches (includes launch gaps)"},
         "rollout": {"value": world * N * 32 * n_roll / (roll_ms * 1e-3), "unit": UNIT, "K": 32, "launches": n_roll,
                     "obs": "digest every turn, planes of the last turn", "bound": "alu"},
     }
@@ -284,6 +296,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--games", type=int, default=0, help="override games per GPU (default: config 2's 16,384)")
+    ap.add_argument("--replicas", type=int, default=0, help="replicas in the round-robin (default: enough for 640 MB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
