@@ -109,7 +109,16 @@ typedef struct gen_buffers {
     uint32_t *sat_events;    /* state [N]   int16 saturations (R21) */
     uint64_t *obs_digest;    /* state [N]   may be NULL for gen_reset / gen_step (no digest then) */
     int32_t *actions_out;    /* out   [K][N][P]  the actions actually applied; may be NULL */
+    uint32_t *bitboards;     /* state [N][P+3][BW]  derived cache, may be NULL (see below) */
 } gen_buffers;
+
+/* `bitboards` caches what the rules need of the three planes as one bit per cell (bit c & 31 of word
+ * c >> 5; BW = gen_sizes.bitboard_row_words = ceil(H*W / 32) rounded up to 4 words): rows 0..P-1 "owned by
+ * player p", row P "army >= 2", row P+1 "city or general", row P+2 "mountain or off the board" (all ones
+ * past H*W).  gen_reset and gen_observe build it from the planes; gen_step and gen_rollout keep it
+ * current.  With it, gen_step without a digest buffer runs the register-resident per-step kernel, which
+ * never rebuilds the rows from the planes; without it (NULL) every call stages and scans the planes.
+ * A caller who writes the planes directly must call gen_observe before the next gen_step. */
 
 /* byte sizes of the buffers above for K slots */
 typedef struct gen_sizes {
@@ -117,7 +126,8 @@ typedef struct gen_sizes {
     int32_t alignment;       /* 16 */
     size_t army, owner, terrain, turn, episode, alive, general_cell, land, army_total;
     size_t reward, done, winner, obs_army, obs_owner, obs_terrain, obs_vis;
-    size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out;
+    size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out, bitboards;
+    int32_t bitboard_row_words; /* BW */
 } gen_sizes;
 
 typedef struct gen_env gen_env;
@@ -173,16 +183,19 @@ int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_action
  * the default (8).  Results do not depend on it. */
 int gen_set_launch(gen_env *env, int32_t games_per_cta);
 
-/* Kernel selection override for tests: the library holds board-specialised instantiations of its one
- * kernel for the paper-sized configurations (1v1 8x8 and 24x24, 4 and 8 players on 32x32) next to the
- * generic one that serves every board up to 32x32.  force_generic != 0 makes this handle always launch the
- * generic kernel.  Results do not depend on it. */
-int gen_set_generic(gen_env *env, int32_t force_generic);
+/* Kernel selection overrides for tests.  The library holds two kernels: the STAGED one (planes resident in
+ * shared memory; serves every call) and the REGISTER-RESIDENT per-step one (gen_step with bufs->bitboards
+ * and without a digest buffer, uniform policy), each as a generic instantiation for every board up to
+ * 32x32 and as instantiations compiled for the paper-sized configurations (1v1 8x8 and 24x24, 4 and 8
+ * players on 32x32).  force_generic != 0: never launch a board-specialised instantiation;
+ * force_staged != 0: never launch the register-resident kernel.  Results do not depend on either. */
+int gen_set_generic(gen_env *env, int32_t force_generic, int32_t force_staged);
 
 /* Which instantiation the last launch of this handle used: returns its index in the library's variant
- * table (-1 before the first launch) and, if board_specialised is non-NULL, stores 1 there when that
- * kernel was compiled for this exact board size and mode, 0 for the generic one.  Diagnostic only. */
-int32_t gen_last_variant(const gen_env *env, int32_t *board_specialised);
+ * table (-1 before the first launch); if non-NULL, *board_specialised is set to 1 when that kernel was
+ * compiled for this exact board size, *register_resident to 1 when it was the register-resident per-step
+ * kernel.  Diagnostic only. */
+int32_t gen_last_variant(const gen_env *env, int32_t *board_specialised, int32_t *register_resident);
 
 /* Number of kernels this handle has launched (bench.py's gpu_launches). */
 uint64_t gen_launch_count(const gen_env *env);

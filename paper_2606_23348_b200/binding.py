@@ -59,6 +59,7 @@ BUFFERS = [
     ("sat_events", "int32", lambda N, P, S, K: (N,)),
     ("obs_digest", "int64", lambda N, P, S, K: (N,)),         # bits of uint64
     ("actions_out", "int32", lambda N, P, S, K: (K, N, P)),
+    ("bitboards", "int32", lambda N, P, S, K: (N, P + 3, (-(-S // 32) + 3) // 4 * 4)),   # bits of uint32
 ]
 
 
@@ -67,7 +68,8 @@ class GenBuffers(C.Structure):
 
 
 class GenSizes(C.Structure):
-    _fields_ = [("plane_stride", C.c_int32), ("alignment", C.c_int32)] + [(n, C.c_size_t) for n, _, _ in BUFFERS]
+    _fields_ = ([("plane_stride", C.c_int32), ("alignment", C.c_int32)] + [(n, C.c_size_t) for n, _, _ in BUFFERS]
+                + [("bitboard_row_words", C.c_int32)])
 
 
 _lib = None
@@ -97,8 +99,8 @@ def load_library(path=None):
     lib.gen_sample.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
     lib.gen_step_host.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.gen_set_launch.argtypes = [env_p, C.c_int32]
-    lib.gen_set_generic.argtypes = [env_p, C.c_int32]
-    lib.gen_last_variant.argtypes = [env_p, C.POINTER(C.c_int32)]
+    lib.gen_set_generic.argtypes = [env_p, C.c_int32, C.c_int32]
+    lib.gen_last_variant.argtypes = [env_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     lib.gen_last_variant.restype = C.c_int32
     lib.gen_launch_count.argtypes = [env_p]
     lib.gen_launch_count.restype = C.c_uint64
@@ -143,7 +145,7 @@ class GeneralsEnv:
     k_slots > 1 sizes the output buffers for rollout(K, OBS_EVERY_STEP).
     """
 
-    def __init__(self, cfg, device="cuda:0", k_slots=1, digest=True, actions_out=True):
+    def __init__(self, cfg, device="cuda:0", k_slots=1, digest=True, actions_out=True, bitboards=True):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -162,7 +164,8 @@ class GeneralsEnv:
         self.bufs = GenBuffers()
         self.tensors = {}
         for name, dt, shape in BUFFERS:
-            if (name == "obs_digest" and not digest) or (name == "actions_out" and not actions_out):
+            if ((name == "obs_digest" and not digest) or (name == "actions_out" and not actions_out)
+                    or (name == "bitboards" and not bitboards)):
                 setattr(self.bufs, name, None)
                 continue
             t = torch.zeros(shape(self.N, self.P, self.S, self.K), dtype=getattr(torch, dt), device=self.device)
@@ -214,15 +217,23 @@ class GeneralsEnv:
     def set_launch(self, games_per_cta):
         self._check(self.lib.gen_set_launch(self._env, int(games_per_cta)))
 
-    def set_generic(self, force_generic=True):
-        self._check(self.lib.gen_set_generic(self._env, 1 if force_generic else 0))
+    def set_generic(self, force_generic=True, force_staged=False):
+        """Test hooks: never launch a board-specialised / the register-resident kernel."""
+        self._check(self.lib.gen_set_generic(self._env, 1 if force_generic else 0, 1 if force_staged else 0))
 
     @property
     def last_launch_specialised(self):
         """True when the last launch used a kernel compiled for this exact board size and mode."""
-        flag = C.c_int32(0)
-        self.lib.gen_last_variant(self._env, C.byref(flag))
+        flag, rr = C.c_int32(0), C.c_int32(0)
+        self.lib.gen_last_variant(self._env, C.byref(flag), C.byref(rr))
         return bool(flag.value)
+
+    @property
+    def last_launch_register_resident(self):
+        """True when the last launch was the register-resident per-step kernel (generals_step.cuh)."""
+        flag, rr = C.c_int32(0), C.c_int32(0)
+        self.lib.gen_last_variant(self._env, C.byref(flag), C.byref(rr))
+        return bool(rr.value)
 
     @property
     def launch_count(self):

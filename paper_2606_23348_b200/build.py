@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgenerals.so")
 DEPS = [os.path.join(CSRC, f) for f in ("generals_api.cu", "generals_variant.cu", "generals_variants.h",
-                                        "generals_kernels.cuh")] + [os.path.join(ROOT, "include", "generals.h")]
+                                        "generals_kernels.cuh", "generals_step.cuh")] + [os.path.join(ROOT, "include", "generals.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 

@@ -15,6 +15,7 @@ struct gen_env {
     uint64_t launches;
     int last_cuda_error;
     int32_t force_generic;   // 1: never pick a board-specialised kernel (tests)
+    int32_t force_staged;    // 1: never pick the register-resident step kernel (tests)
     int32_t last_variant;    // index into GEN_VARIANTS of the last launch (-1: none yet)
 };
 
@@ -53,6 +54,9 @@ void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
     s->obs_vis = k * N * P * S;
     s->episodes_done = N * 4; s->wins = N * P * 4; s->truncations = N * 4; s->sat_events = N * 4;
     s->obs_digest = N * 8; s->actions_out = k * N * P * 4;
+    const size_t BW = (size_t)round_up((c->height * c->width + 31) / 32, 4);
+    s->bitboard_row_words = (int32_t)BW;
+    s->bitboards = N * (P + 3) * BW * 4;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -72,6 +76,7 @@ int check_buffers(const gen_buffers *b, bool need_obs) {
     }
     if (b->obs_digest && !aligned16(b->obs_digest)) return GEN_ERR_ALIGN;
     if (b->actions_out && !aligned16(b->actions_out)) return GEN_ERR_ALIGN;
+    if (b->bitboards && !aligned16(b->bitboards)) return GEN_ERR_ALIGN;
     return GEN_OK;
 }
 
@@ -98,43 +103,49 @@ void layout(gen::KParams &k, int WPC, bool digest) {
     k.smem_bytes = k.off_warp0 + (uint32_t)WPC * k.warp_bytes;
 }
 
+// shared-memory layout of one CTA of the register-resident step kernel (generals_step.cuh):
+// [tables | warp 0: cache rows, vis rows, scalars, mbarrier, regeneration scratch | warp 1 | ...]
+void layout_step(gen::KParams &k, int WPC) {
+    k.WPC = WPC;
+    const uint32_t GW = (uint32_t)gen::GW, P = (uint32_t)k.P, BW = (uint32_t)k.BW;
+    k.off_key = 416;
+    k.off_warp0 = 512;
+    uint32_t off = GW * (2 * P + 3) * BW * 4u;
+    k.w_mask = 0;
+    k.w_game = off; off += GW * (uint32_t)sizeof(gen::StepGame);
+    k.w_bar = off; off += 8;
+    off = align_up(off, 16);
+    k.w_scratch = off; off += 4u * (uint32_t)k.S;
+    k.warp_bytes = align_up(off, 128);
+    k.smem_bytes = k.off_warp0 + (uint32_t)WPC * k.warp_bytes;
+}
+
 using gen::F_RUNTIME;
 using gen::FF_ROLL_DIGEST;
-using gen::FF_STEP;
 const gen::Variant kVariants[gen::N_VARIANTS] = {
-#define GEN_ROW(id, np, h, w, ff) {np, h, w, ff, gen::launch_variant_##id},
+#define GEN_ROW(id, kind, np, h, w, ff, maxt, minb) {kind, np, h, w, ff, maxt, gen::launch_variant_##id},
     GEN_VARIANTS(GEN_ROW)
 #undef GEN_ROW
 };
 
-// the most specialised instantiation that serves this launch: exact board + exact mode first, else the
-// generic kernel of the smallest NP >= P
-const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp) {
+// The most specialised instantiation that serves this launch.  step_ok: the register-resident kernel may
+// be used (gen_step with the bitboard cache, no digest, uniform policy).  Within a kind: the exact board
+// (and, for the staged kernel, the exact mode) first, else the generic kernel of the smallest NP >= P.
+const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, bool step_ok) {
+    const int kind = step_ok ? 1 : 0;
     const gen::Variant *generic = nullptr;
-    const uint32_t mode = (kp.flags & ~gen::F_SAMPLER) | (kp.K == 1 ? gen::F_K1 : 0u);
     for (const gen::Variant &v : kVariants) {
+        if (v.kind != kind) continue;
         if (v.h == 0) {
             if (kp.P <= v.np && (!generic || v.np < generic->np)) generic = &v;
             continue;
         }
         if (env->force_generic || v.np != kp.P || v.h != kp.H || v.w != kp.W) continue;
         if (v.np == 2 && kp.team_size > 1) continue;
-        const uint32_t want = (v.ff & gen::F_K1) ? mode : (mode & ~gen::F_K1);
-        if (v.ff == want) return &v;
+        if (kind == 0 && v.ff != (kp.flags & ~gen::F_SAMPLER)) continue;
+        return &v;
     }
     return generic;
-}
-
-int launch_kernel(gen_env *env, const gen::KParams &kp, cudaStream_t stream) {
-    const gen::Variant *v = pick_variant(env, kp);
-    if (!v) return GEN_ERR_CONFIG;
-    const int per_cta = gen::GW * kp.WPC;
-    const int grid = (kp.N + per_cta - 1) / per_cta;
-    cudaError_t e = v->launch(kp, grid, 32 * kp.WPC, kp.smem_bytes, stream);
-    if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
-    env->launches += 1;
-    env->last_variant = (int32_t)(v - kVariants);
-    return GEN_OK;
 }
 
 int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, const int32_t *actions,
@@ -150,15 +161,29 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     kp.b = *bufs;
     kp.actions = actions;
     kp.sample_out = sample_out;
+    // gen_step proper (one turn, planes, no digest) with the bitboard cache and the uniform policy runs the
+    // register-resident kernel; everything else the staged one
+    const bool step_ok = !env->force_staged && K == 1 && bufs->bitboards && kp.bias_thr == 0 &&
+                         (flags & ~gen::F_SAMPLER) == gen::F_OBS_PLANES;
+    const gen::Variant *v = pick_variant(env, kp, step_ok);
+    if (!v) return GEN_ERR_CONFIG;
     // warps per CTA (4 games each): 2 by default; fewer while the CTA would not fit
     int WPC = env->games_per_cta ? env->games_per_cta / gen::GW : 2;
-    layout(kp, WPC, (flags & gen::F_DIGEST) != 0);
+    while (32 * WPC > v->max_threads) WPC >>= 1;
+    const bool digest = (flags & gen::F_DIGEST) != 0;
+    if (v->kind == 1) layout_step(kp, WPC); else layout(kp, WPC, digest);
     while (WPC > 1 && kp.smem_bytes > kMaxSmem) {
         WPC >>= 1;
-        layout(kp, WPC, (flags & gen::F_DIGEST) != 0);
+        if (v->kind == 1) layout_step(kp, WPC); else layout(kp, WPC, digest);
     }
     if (kp.smem_bytes > kMaxSmem) return GEN_ERR_CONFIG;
-    return launch_kernel(env, kp, static_cast<cudaStream_t>(stream));
+    const int per_cta = gen::GW * kp.WPC;
+    const int grid = (kp.N + per_cta - 1) / per_cta;
+    cudaError_t e = v->launch(kp, grid, 32 * kp.WPC, kp.smem_bytes, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
+    env->launches += 1;
+    env->last_variant = (int32_t)(v - kVariants);
+    return GEN_OK;
 }
 
 uint64_t host_mix64(uint64_t z) {  // splitmix64 finaliser: the digest keys of R28
@@ -194,7 +219,7 @@ int gen_init(const gen_config *cfg, gen_env **out) {
     gen::KParams &k = env->base;
     k.N = cfg->n_games; k.H = cfg->height; k.W = cfg->width; k.P = cfg->n_players;
     k.HW = k.H * k.W; k.S = round_up(k.HW, 16); k.NW = (k.HW + 31) / 32; k.NC8 = k.S / 8;
-    k.NCH = 4 * k.NW; k.RW = k.NW | 1; k.M = 2 * k.P + 6;
+    k.NCH = 4 * k.NW; k.RW = k.NW | 1; k.M = 2 * k.P + 7; k.BW = round_up(k.NW, 4);
     k.team_size = cfg->team_size;
     k.n_teams = (cfg->n_players + cfg->team_size - 1) / cfg->team_size;
     k.n_cities = cfg->n_cities; k.city_lo = cfg->city_army_lo;
@@ -317,15 +342,17 @@ int gen_set_launch(gen_env *env, int32_t games_per_cta) {
     return GEN_OK;
 }
 
-int gen_set_generic(gen_env *env, int32_t force_generic) {
+int gen_set_generic(gen_env *env, int32_t force_generic, int32_t force_staged) {
     if (!env) return GEN_ERR_NULL;
     env->force_generic = force_generic ? 1 : 0;
+    env->force_staged = force_staged ? 1 : 0;
     return GEN_OK;
 }
 
-int32_t gen_last_variant(const gen_env *env, int32_t *board_specialised) {
+int32_t gen_last_variant(const gen_env *env, int32_t *board_specialised, int32_t *register_resident) {
     if (!env || env->last_variant < 0) return -1;
     if (board_specialised) *board_specialised = kVariants[env->last_variant].h > 0 ? 1 : 0;
+    if (register_resident) *register_resident = kVariants[env->last_variant].kind == 1 ? 1 : 0;
     return env->last_variant;
 }
 

@@ -75,7 +75,7 @@ struct GameS {
 };
 
 struct KParams {
-    int32_t N, H, W, P, HW, S, NW, NC8, NCH, RW, M;
+    int32_t N, H, W, P, HW, S, NW, NC8, NCH, RW, M, BW;  // BW: words per row of gen_buffers.bitboards
     int32_t team_size, n_teams;
     int32_t n_cities, city_lo, city_span;
     int32_t dmin, dmax, spawn_exact, max_turns, auto_reset;
@@ -84,7 +84,7 @@ struct KParams {
     uint32_t global_step0, flags, recipW;
     int32_t K, WPC;  // turns per launch; warps per CTA
     // shared memory: [tables | digest keys | warp 0 | warp 1 | ...]; w_* are offsets inside a warp's slice
-    uint32_t off_key, off_warp0, warp_bytes, w_owner, w_terr, w_mask, w_game, w_bar, smem_bytes;
+    uint32_t off_key, off_warp0, warp_bytes, w_owner, w_terr, w_mask, w_game, w_bar, w_scratch, smem_bytes;
     unsigned long long key_sum;  // sum of the digest keys of cells 0..HW-1
     gen_buffers b;
     const int32_t *actions;
@@ -220,7 +220,8 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     const int H = FIXED ? CH : kp.H, W = FIXED ? CW : kp.W, P = FIXED ? NP : kp.P;
     const int HW = FIXED ? cHW : kp.HW, S = FIXED ? cS : kp.S, NW = FIXED ? cNW : kp.NW;
     const int NC8 = FIXED ? cS / 8 : kp.NC8, NCH = FIXED ? 4 * cNW : kp.NCH;
-    const int RW = FIXED ? (cNW | 1) : kp.RW, M = FIXED ? 2 * NP + 6 : kp.M;
+    const int RW = FIXED ? (cNW | 1) : kp.RW, M = FIXED ? 2 * NP + 7 : kp.M;
+    const int BW = FIXED ? (cNW + 3) / 4 * 4 : kp.BW;
     const int WS = (NW + LPP - 1) / LPP;  // words per sub-lane
     const uint32_t flags = (FF == F_RUNTIME) ? kp.flags : ((FF & ~F_K1) | (kp.flags & F_SAMPLER));
     const int K = (FF != F_RUNTIME && (FF & F_K1)) ? 1 : kp.K;
@@ -246,9 +247,9 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     const uint32_t bar = smem_u32(wb + kp.w_bar);
 
     // bitboard rows of a game: own[0..P-1], structure (city / general), army >= 2, ok[4] (source cells whose
-    // up / down / left / right target is on the board and no mountain: static per board), vis[0..P-1].
-    // vis[0] doubles as the mountain row while the ok rows are being built.
-    const int R_STR = P, R_A2 = P + 1, R_OK = P + 2, R_VIS = P + 6, R_MTN = P + 6;
+    // up / down / left / right target is on the board and no mountain: static per board), vis[0..P-1],
+    // mountain (or off the board).
+    const int R_STR = P, R_A2 = P + 1, R_OK = P + 2, R_VIS = P + 6, R_MTN = 2 * P + 6;
     auto mrow = [&](int m, int lg) -> uint32_t * { return s_mask + (lg * M + m) * RW; };
     auto mrow8 = [&](int m, int lg) -> unsigned char * { return reinterpret_cast<unsigned char *>(mrow(m, lg)); };
 
@@ -1099,6 +1100,16 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         }
         if (ol == (P & 7)) { B.turn[g] = gs.turn; B.alive[g] = (uint8_t)gs.alive; }
         if (ol == ((P + 1) & 7) && (flags & F_DIGEST) && B.obs_digest) B.obs_digest[g] = gs.digest;
+        // the bitboard cache of the register-resident step kernel (generals_step.cuh): own[p], army >= 2,
+        // structure, mountain; words past the board are 0 (all ones in the mountain row)
+        if (B.bitboards) {
+            uint32_t *bb = B.bitboards + (size_t)g * (size_t)(P + 3) * (size_t)BW;
+            for (int u = ol; u < (P + 3) * BW; u += LPG) {
+                const int row = u / BW, j = u - row * BW;
+                const int m = row < P ? row : (row == P ? R_A2 : (row == P + 1 ? R_STR : R_MTN));
+                bb[u] = j < NW ? mrow(m, sub)[j] : (row == P + 2 ? 0xFFFFFFFFu : 0u);
+            }
+        }
     }
 }
 

@@ -1,0 +1,726 @@
+// generals_step.cuh -- the per-step kernel of gen_step (a2..a12 of SURVEY.md section 8, one turn per launch).
+//
+// REGISTER-RESIDENT design.  The three state planes are never staged in shared memory: what the rules
+// need of them lives in the bitboard cache gen_buffers.bitboards ((P + 3) rows of one bit per cell per
+// game: own[p], army >= 2, structure, mountain), which every kernel of the library keeps current.
+//   * load: one TMA bulk copy per warp brings the cache rows of its 4 games (400 B each at 24x24 1v1)
+//     into shared memory; the planes stay in HBM / L2;
+//   * rules (sampler, moves, capture, growth, termination) run on the rows; the handful of army cells a
+//     move or a structure's growth touches are read and written in global memory directly;
+//   * emit: every lane reads its 8-cell chunks of the planes once, straight into registers (16 / 8-byte
+//     coalesced loads), masks them with each player's fog row and streams the observation planes out.
+// Shared memory per game drops from 3.3 KB to about 0.7 KB, so a whole 16,384-game batch is resident on
+// the 148 SMs at once (one wave), and nothing is rebuilt from the planes per step.
+//
+// Same thread mapping as generals_kernels.cuh: a warp owns 4 consecutive games, an octet of 8 lanes one
+// game; word passes split the octet by player; lane 0 of the octet runs the serial rules.  Same rules
+// text (section IV, readings R1..R32 of DESIGN.md); parity with the oracle is bit-exact.
+// Not served here (the host falls back to the staged kernel): observation digest, K > 1, the biased
+// policy (R25), gen_reset / gen_observe / gen_sample.
+#pragma once
+#include "generals_kernels.cuh"
+
+namespace gen {
+
+struct StepGame {  // per-game scalars in shared memory
+    int32_t turn, winner;
+    uint32_t alive, done, episode, flags, sat;
+    int32_t rew_bits;
+    int32_t tot[8], land[8], act[8], gcell[8];
+};
+
+enum : uint32_t {
+    SG_RESET = 1u << 0,      // auto-reset: regenerate the board in this call
+    SG_FROZEN = 1u << 1,     // finished game without auto-reset (R31)
+    SG_GROW_EVEN = 1u << 2,  // owned structures +1 this turn
+    SG_GROW_TICK = 1u << 3,  // all owned cells +1 this turn
+    SG_STATIC_DIRTY = 1u << 4,  // structure / mountain rows changed (regenerated): write them back too
+};
+
+// ------------------------------------------------------------------------------------------------
+// a1: board generator (R13, R14, R29, R30), one warp per game, planes in shared memory (S cells each).
+// Writes general_cell[p] through gcell_out.  The same procedure as the generator of the staged kernel.
+template <int NP>
+__device__ __noinline__ void generate_board(const KParams &kp, uint32_t lane, uint32_t gid, uint32_t episode,
+                                            int16_t *A, int8_t *O, int8_t *Tr, int16_t *gcell_out) {
+    const int P = kp.P, HW = kp.HW, S = kp.S, NW = kp.NW, W = kp.W;
+    __syncwarp();
+    for (int i = lane; i < S / 4; i += 32) {
+        reinterpret_cast<uint32_t *>(O)[i] = 0xFFFFFFFFu;
+        reinterpret_cast<uint32_t *>(A)[2 * i] = 0;
+        reinterpret_cast<uint32_t *>(A)[2 * i + 1] = 0;
+    }
+    uint32_t w[4];
+    int lo = kp.dmin, hi = kp.dmax > 0 ? kp.dmax : 64;
+    if (kp.spawn_exact) {
+        philox(0, gid, episode, DOM_SPAWN << 24, kp.key0, kp.key1, w);
+        lo = hi = kp.dmin + (int)mulhi32(w[1], (uint32_t)(kp.dmax - kp.dmin + 1));
+    }
+    for (int q = lane; q < S / 4; q += 32) {
+        philox((uint32_t)q, gid, episode, DOM_MOUNTAIN << 24, kp.key0, kp.key1, w);
+        uint32_t tw = 0;
+#pragma unroll
+        for (int b = 0; b < 4; ++b)
+            tw |= (w[b] < kp.mountain_thr || 4 * q + b >= HW) ? (uint32_t)T_MOUNTAIN << (8 * b) : 0u;
+        reinterpret_cast<uint32_t *>(Tr)[q] = tw;
+    }
+    __syncwarp();
+    int gr[NP], gc[NP];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) { gr[p] = 0; gc[p] = 0; }
+    for (int p = 0; p < P; ++p) {
+        philox((uint32_t)p, gid, episode, DOM_SPAWN << 24, kp.key0, kp.key1, w);
+        int cell;
+        if (p == 0) {
+            cell = (int)mulhi32(w[0], (uint32_t)HW);
+        } else {
+            int l = lo, h = hi;
+            uint32_t cand, n;
+            for (;;) {
+                cand = 0;
+                for (int j = 0; j < NW; ++j) {
+                    const int c = 32 * j + (int)lane;
+                    const int r = (int)(((uint32_t)c * kp.recipW) >> 16), col = c - r * W;
+                    int mind = 1 << 20;
+#pragma unroll
+                    for (int q = 0; q < NP; ++q)
+                        if (q < p) mind = min(mind, abs(r - gr[q]) + abs(col - gc[q]));
+                    const uint32_t bal = __ballot_sync(FULL, c < HW && mind >= l && mind <= h && mind > 0);
+                    if ((int)lane == j) cand = bal;
+                }
+                n = __reduce_add_sync(FULL, __popc(cand));
+                if (n > 0) break;
+                if (l > 0) l -= 1;
+                h += 1;
+            }
+            cell = select_kth(cand, mulhi32(w[0], n), lane);
+        }
+        const int r = (int)(((uint32_t)cell * kp.recipW) >> 16);
+#pragma unroll
+        for (int q = 0; q < NP; ++q)
+            if (q == p) { gr[q] = r; gc[q] = cell - r * W; }
+        if (lane == 0) {
+            Tr[cell] = (int8_t)T_GENERAL;
+            O[cell] = (int8_t)p;
+            A[cell] = 1;
+            gcell_out[p] = (int16_t)cell;
+        }
+    }
+    __syncwarp();
+    uint32_t plain = 0;
+    for (int j = 0; j < NW; ++j) {
+        const int c = 32 * j + (int)lane;
+        const uint32_t bal = __ballot_sync(FULL, c < HW && Tr[c] == T_PLAIN);
+        if ((int)lane == j) plain = bal;
+    }
+    uint32_t n = __reduce_add_sync(FULL, __popc(plain));
+    for (int k = 0; k < kp.n_cities && n > 0; ++k, --n) {
+        philox((uint32_t)k, gid, episode, DOM_CITY << 24, kp.key0, kp.key1, w);
+        const int cell = select_kth(plain, mulhi32(w[0], n), lane);
+        if ((int)lane == (cell >> 5)) plain &= ~(1u << (cell & 31));
+        if (lane == 0) {
+            Tr[cell] = (int8_t)T_CITY;
+            A[cell] = (int16_t)(kp.city_lo + (int)mulhi32(w[1], (uint32_t)kp.city_span));
+        }
+    }
+    __syncwarp();
+}
+
+// ================================================================================================
+// NP = bound of the player loops; CH x CW > 0: board size fixed at compile time and P == NP; MAXT / MINB:
+// launch bounds (threads per CTA, resident CTAs per SM the register allocation must allow).
+template <int NP, int CH, int CW, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KParams kp) {
+    constexpr bool FIXED = CH > 0;
+    constexpr int LPP = LPG / NP;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int tid = threadIdx.x;
+    const uint32_t lane = tid & 31u;
+    const int wic = tid >> 5;
+    const int ol = (int)(lane & (LPG - 1)), sub = (int)(lane / LPG);
+    const uint32_t gmask = ((1u << LPG) - 1u) << (sub * LPG);
+    const int pl = ol / LPP, sl = ol % LPP;
+    constexpr int cHW = CH * CW, cS = (cHW + 15) / 16 * 16, cNW = (cHW + 31) / 32;
+    const int H = FIXED ? CH : kp.H, W = FIXED ? CW : kp.W, P = FIXED ? NP : kp.P;
+    const int HW = FIXED ? cHW : kp.HW, S = FIXED ? cS : kp.S, NW = FIXED ? cNW : kp.NW;
+    const int NC8 = FIXED ? cS / 8 : kp.NC8;
+    const int BW = FIXED ? (cNW + 3) / 4 * 4 : kp.BW;
+    const int WS = (NW + LPP - 1) / LPP;
+    const uint32_t flags = kp.flags;  // F_SAMPLER is the only mode bit this kernel looks at
+    const gen_buffers &B = kp.b;
+    const int wg0 = (blockIdx.x * kp.WPC + wic) * GW;
+    const int nwg = min(GW, kp.N - wg0);
+    const bool gvalid = sub < nwg;
+    const int g = wg0 + sub;
+    const uint32_t allp = (1u << P) - 1u;
+    const bool teams = (FIXED && NP == 2) ? false : kp.team_size > 1;
+
+    uint32_t *s_nc0 = reinterpret_cast<uint32_t *>(smem) + 1, *s_ncL = s_nc0 + 34, *s_inb = s_nc0 + 68;
+    unsigned char *wb = smem + kp.off_warp0 + (size_t)wic * kp.warp_bytes;
+    // rows of a game: [cache rows of the warp's games: own[0..P-1], army >= 2, structure, mountain] [vis[0..P-1]]
+    uint32_t *s_rows = reinterpret_cast<uint32_t *>(wb);
+    uint32_t *s_vis = s_rows + GW * (P + 3) * BW;
+    StepGame *s_game = reinterpret_cast<StepGame *>(wb + kp.w_game);
+    const uint32_t bar = smem_u32(wb + kp.w_bar);
+    unsigned char *s_scratch = wb + kp.w_scratch;  // one game's planes while it is regenerated
+    const int R_A2 = P, R_STR = P + 1, R_MTN = P + 2;
+    auto row = [&](int m, int lg) -> uint32_t * { return s_rows + (lg * (P + 3) + m) * BW; };
+    auto row8 = [&](int m, int lg) -> unsigned char * { return reinterpret_cast<unsigned char *>(row(m, lg)); };
+    auto vrow = [&](int p, int lg) -> uint32_t * { return s_vis + (lg * P + p) * BW; };
+    auto team_mask = [&](int p) -> uint32_t {
+        const int t = p / kp.team_size;
+        return (((1u << kp.team_size) - 1u) << (t * kp.team_size)) & allp;
+    };
+    auto row_of = [&](int cell) -> int {
+        return FIXED ? (int)((uint32_t)cell / (uint32_t)(FIXED ? CW : 1)) : (int)(((uint32_t)cell * kp.recipW) >> 16);
+    };
+    auto bit_of = [&](const uint32_t *r, int c) -> bool { return (r[c >> 5] >> (c & 31)) & 1u; };
+    auto set_bit = [&](uint32_t *r, int c, bool on) {
+        const uint32_t bit = 1u << (c & 31);
+        if (on) r[c >> 5] |= bit; else r[c >> 5] &= ~bit;
+    };
+
+    // ================================================================ prologue
+    for (int t = tid; t < 34; t += blockDim.x) {
+        const int j = t - 1;
+        const bool in = j >= 0 && j < 32;
+        s_nc0[j] = in ? kp.notcol0[j & 31] : 0u;
+        s_ncL[j] = in ? kp.notcolL[j & 31] : 0u;
+        s_inb[j] = in ? kp.inb[j & 31] : 0u;
+    }
+    if (nwg > 0 && lane == 0) {
+        mbar_init(bar, 1);
+        const uint32_t bytes = (uint32_t)nwg * (uint32_t)(P + 3) * (uint32_t)BW * 4u;
+        mbar_expect_tx(bar, bytes);
+        bulk_g2s(smem_u32(s_rows), B.bitboards + (size_t)wg0 * (size_t)(P + 3) * (size_t)BW, bytes, bar);
+    }
+    if (gvalid) {  // per-game scalars, spread over the octet
+        StepGame &gs = s_game[sub];
+        if (ol < P) {
+            gs.tot[ol] = B.army_total[(size_t)g * P + ol];
+            gs.land[ol] = B.land[(size_t)g * P + ol];
+            gs.gcell[ol] = B.general_cell[(size_t)g * P + ol];
+        }
+        if (ol == 0) { gs.turn = B.turn[g]; gs.episode = B.episode[g]; }
+        if (ol == 1) { gs.alive = B.alive[g]; gs.done = B.done[g]; gs.winner = B.winner[g]; }
+        if (ol == 2) { gs.flags = 0; gs.sat = 0; gs.rew_bits = 0; }
+    }
+    __syncthreads();  // the only CTA barrier: tables and the mbarrier init are visible
+    if (nwg <= 0) return;
+    mbar_wait(bar, 0);
+
+    // ---------------------------------------------------------------- a12: valid-action sampler (R24)
+    // As in the staged kernel: the LPP lanes (pl, 0..LPP-1) of the octet serve player pl and split the NW
+    // words; the valid list is ordered (direction, cell).  The four "target is free" masks are formed on
+    // the fly from the mountain row (sliding window of three words).
+    auto freew = [&](const uint32_t *mtn, int j) -> uint32_t {
+        return ((unsigned)j < (unsigned)NW) ? (~mtn[j] & s_inb[j]) : 0u;
+    };
+    auto sample = [&](int lg, uint32_t gstep) -> int {
+        const int p = min(pl, P - 1);
+        const uint32_t gid = kp.gid_base + (uint32_t)(wg0 + lg);
+        uint32_t w[4];
+        philox(0u, gid, gstep, (DOM_ACTION << 24) | (uint32_t)p, kp.key0, kp.key1, w);
+        const uint32_t *own = row(p, lg), *a2 = row(R_A2, lg), *mtn = row(R_MTN, lg);
+        const int js = sl * WS, je = min(js + WS, NW);
+        uint32_t ln01 = 0, ln23 = 0;
+        {
+            uint32_t fp = freew(mtn, js - 1), fc = freew(mtn, js);
+            for (int j = js; j < je; ++j) {
+                const uint32_t fn = freew(mtn, j + 1);
+                const uint32_t src = own[j] & a2[j];
+                const uint32_t up = __funnelshift_lc(fp, fc, W), dn = __funnelshift_rc(fc, fn, W);
+                const uint32_t lf = __funnelshift_l(fp, fc, 1) & s_nc0[j], rt = __funnelshift_r(fc, fn, 1) & s_ncL[j];
+                ln01 += (uint32_t)__popc(src & up) | ((uint32_t)__popc(src & dn) << 16);
+                ln23 += (uint32_t)__popc(src & lf) | ((uint32_t)__popc(src & rt) << 16);
+                fp = fc; fc = fn;
+            }
+        }
+        uint32_t n01 = ln01, n23 = ln23;
+#pragma unroll
+        for (int o = LPP / 2; o >= 1; o >>= 1) {
+            n01 += __shfl_xor_sync(gmask, n01, o);
+            n23 += __shfl_xor_sync(gmask, n23, o);
+        }
+        const uint32_t n0 = n01 & 0xFFFFu, n1 = n01 >> 16, n2 = n23 & 0xFFFFu, n3 = n23 >> 16;
+        const uint32_t total = n0 + n1 + n2 + n3;
+        const int half = (w[2] < kp.half_thr) ? 1 : 0;
+        int action = 0;
+        const bool decided = (w[0] < kp.pass_thr) || total == 0;
+        uint32_t idx = mulhi32(w[1], total);
+        int d = 0;
+        uint32_t cnt = ln01 & 0xFFFFu;
+        if (idx >= n0) { idx -= n0; d = 1; cnt = ln01 >> 16;
+            if (idx >= n1) { idx -= n1; d = 2; cnt = ln23 & 0xFFFFu;
+                if (idx >= n2) { idx -= n2; d = 3; cnt = ln23 >> 16; } } }
+        uint32_t incl = cnt;
+#pragma unroll
+        for (int o = 1; o < LPP; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(gmask, incl, o, LPP);
+            if (sl >= o) incl += t;
+        }
+        int cell = -1;
+        if (!decided && idx < incl && idx >= incl - cnt) {  // the idx-th move of direction d starts in my words
+            uint32_t r = idx - (incl - cnt), vw = 0;
+            int j = js;
+            for (; j < je; ++j) {
+                const uint32_t fp = freew(mtn, j - 1), fc = freew(mtn, j), fn = freew(mtn, j + 1);
+                const uint32_t okd = d == 0 ? __funnelshift_lc(fp, fc, W)
+                                   : d == 1 ? __funnelshift_rc(fc, fn, W)
+                                   : d == 2 ? (__funnelshift_l(fp, fc, 1) & s_nc0[j])
+                                            : (__funnelshift_r(fc, fn, 1) & s_ncL[j]);
+                vw = own[j] & a2[j] & okd;
+                const uint32_t c = (uint32_t)__popc(vw);
+                if (r < c) break;
+                r -= c;
+            }
+            cell = 32 * j + nth_bit(vw, r);
+        }
+        const int leader = (int)(lane & ~(uint32_t)(LPP - 1));
+        const uint32_t mine = (__ballot_sync(gmask, cell >= 0) >> leader) & ((1u << LPP) - 1u);
+        cell = __shfl_sync(gmask, cell, mine ? leader + __ffs(mine) - 1 : (int)lane);
+        if (mine) action = cell * 9 + 1 + 2 * d + half;
+        return action;
+    };
+
+    // ---------------------------------------------------------------- a2-a5: moves of one game, one lane
+    // The rows answer every question but the two army values, which are read from and written to the
+    // army plane in global memory (ld.global.cg: L2 only, so that the emit pass of the other lanes sees them).
+    auto owner_of = [&](int lg, int c) -> int {
+        int t = -1;
+#pragma unroll
+        for (int q = 0; q < NP; ++q)
+            if (q < P && bit_of(row(q, lg), c)) t = q;
+        return t;
+    };
+    auto play_moves = [&](int lg) {
+        StepGame &gs = s_game[lg];
+        const int gg = wg0 + lg;
+        int16_t *A = B.army + (size_t)gg * S;
+        int8_t *O = B.owner + (size_t)gg * S, *Tr = B.terrain + (size_t)gg * S;
+        uint32_t *a2row = row(R_A2, lg);
+        const uint32_t *mtn = row(R_MTN, lg);
+        const int first = (kp.rule_flags & GEN_RULE_ROTATE_PRIORITY) ? (gs.turn % P) : 0;
+        for (int i = 0; i < P; ++i) {
+            int p = first + i;
+            if (p >= P) p -= P;
+            const int a = gs.act[p];
+            if (a <= 0 || a >= 9 * HW) continue;
+            const int cell = (int)(((uint32_t)a * 7282u) >> 16);  // a / 9 for a < 9 * 1024
+            const int kk = a - 9 * cell;
+            if (kk == 0) continue;
+            const int dir = (kk - 1) >> 1, half = (kk - 1) & 1;
+            const int r = row_of(cell), col = cell - r * W;
+            int dst;
+            bool ok;
+            if (dir == 0) { dst = cell - W; ok = r > 0; }
+            else if (dir == 1) { dst = cell + W; ok = r < H - 1; }
+            else if (dir == 2) { dst = cell - 1; ok = col > 0; }
+            else { dst = cell + 1; ok = col < W - 1; }
+            if (!ok) continue;
+            // R5, R10: own the source, army >= 2 (the row is exact), target no mountain
+            if (!bit_of(row(p, lg), cell) || !bit_of(a2row, cell) || bit_of(mtn, dst)) continue;
+            const int asrc = __ldcg(A + cell), d = __ldcg(A + dst);
+            const int m = half ? (asrc >> 1) : (asrc - 1);  // R4
+            const int nsrc = asrc - m;
+            const int t = owner_of(lg, dst);
+            const bool dst_general = t >= 0 && gs.gcell[t] == dst;
+            int ndst, nown = t;
+            bool captured = false;
+            const bool ally = teams && t >= 0 && t != p && ((team_mask(p) >> t) & 1u);
+            if (t == p || ally) {  // R8 / P:L97, R19
+                ndst = d + m;
+                int lost = 0;
+                if (ndst > 32767) { lost = ndst - 32767; ndst = 32767; gs.sat += 1; }  // R21
+                int holder = p;
+                if (ally) {
+                    if (!dst_general) { nown = p; gs.tot[p] += d; gs.tot[t] -= d; }
+                    else { gs.tot[p] -= m; gs.tot[t] += m; holder = t; }
+                }
+                if (lost) gs.tot[holder] -= lost;
+            } else if (m > d) {
+                ndst = m - d;
+                nown = p;
+                captured = dst_general;  // R11, R12
+                gs.tot[p] -= d;
+                if (t >= 0) gs.tot[t] -= d;
+            } else {
+                ndst = d - m;  // tie -> 0, previous owner keeps the cell
+                gs.tot[p] -= m;
+                if (t >= 0) gs.tot[t] -= m;
+            }
+            A[cell] = (int16_t)nsrc;
+            A[dst] = (int16_t)ndst;
+            set_bit(a2row, cell, nsrc >= 2);
+            set_bit(a2row, dst, ndst >= 2);
+            if (nown != t) {
+                O[dst] = (int8_t)nown;
+                set_bit(row(nown, lg), dst, true);
+                gs.land[nown] += 1;
+                if (t >= 0) { set_bit(row(t, lg), dst, false); gs.land[t] -= 1; }
+            }
+            if (captured) {  // a4: land transfer (R11); the general becomes a city
+                const int q = t;
+                Tr[dst] = (int8_t)T_CITY;
+                gs.alive &= ~(1u << q);
+                gs.gcell[q] = -1;
+                B.general_cell[(size_t)gg * P + q] = -1;
+                const bool fl = (kp.rule_flags & GEN_RULE_CAPTURE_HALF_FLOOR) != 0;
+                uint32_t *oq = row(q, lg), *op = row(p, lg);
+                int moved = 0;
+                for (int j = 0; j < NW; ++j) {
+                    uint32_t wq = oq[j];
+                    if (wq == 0) continue;
+                    op[j] |= wq;
+                    oq[j] = 0;
+                    uint32_t a2w = a2row[j];
+                    while (wq) {
+                        const int b = __ffs(wq) - 1;
+                        wq &= wq - 1;
+                        const int c = 32 * j + b;
+                        O[c] = (int8_t)p;
+                        const int av = __ldcg(A + c);
+                        const int nv = fl ? (av >> 1) : ((av + 1) >> 1);
+                        A[c] = (int16_t)nv;
+                        moved += nv;
+                        a2w = nv >= 2 ? (a2w | (1u << b)) : (a2w & ~(1u << b));
+                    }
+                    a2row[j] = a2w;
+                }
+                gs.tot[p] += moved;
+                gs.tot[q] = 0;
+                gs.land[p] += gs.land[q];
+                gs.land[q] = 0;
+            }
+        }
+        // a6: turn counter; growth itself is applied by the next parallel pass (R1, R2, R3)
+        const int turn = gs.turn + 1;
+        gs.turn = turn;
+        uint32_t gflags = 0;
+        if ((turn & 1) == 0) gflags |= SG_GROW_EVEN;
+        if (turn % 50 == 0) gflags |= SG_GROW_TICK;
+        if (gflags) gs.flags |= gflags;
+    };
+
+    // ---------------------------------------------------------------- a6: growth (octet), army plane in global
+    // tick turns (every 50th, always even): +1 on owned cells, +1 more on owned structures (R2)
+    auto grow_tick = [&](int lg) {
+        StepGame &gs = s_game[lg];
+        int16_t *A = B.army + (size_t)(wg0 + lg) * S;
+        for (int ch = ol; ch < NC8; ch += LPG) {
+            const uint32_t sb = row8(R_STR, lg)[ch];
+            uint32_t ob[NP], ownedb = 0;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) { ob[p] = p < P ? row8(p, lg)[ch] : 0u; ownedb |= ob[p]; }
+            const uint32_t e = sb & ownedb;
+            const uint32_t t = (kp.rule_flags & GEN_RULE_TICK_PLAIN_ONLY) ? (ownedb & ~sb) : ownedb;
+            if ((e | t) == 0) continue;
+            uint4 *ap = reinterpret_cast<uint4 *>(A + 8 * ch);
+            uint4 a = __ldcg(ap);
+            uint32_t aw[4] = {a.x, a.y, a.z, a.w};
+            bool sat = false;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t lo = ((e >> (2 * k)) & 1u) + ((t >> (2 * k)) & 1u);
+                const uint32_t hi = ((e >> (2 * k + 1)) & 1u) + ((t >> (2 * k + 1)) & 1u);
+                aw[k] += lo | (hi << 16);
+                sat |= (aw[k] & 0x80008000u) != 0;
+            }
+            int lost[NP];
+#pragma unroll
+            for (int p = 0; p < NP; ++p) lost[p] = 0;
+            if (sat) {  // R21: every +1 that would pass 32767 is one saturation event, charged to the owner
+                int ev = 0;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    uint32_t v = (i & 1) ? (aw[i >> 1] >> 16) : (aw[i >> 1] & 0xFFFFu);
+                    if (v > 32767u) {
+                        const int over = (int)(v - 32767u);
+                        ev += over;
+#pragma unroll
+                        for (int p = 0; p < NP; ++p)
+                            if ((ob[p] >> i) & 1u) lost[p] += over;
+                        aw[i >> 1] = (i & 1) ? ((aw[i >> 1] & 0xFFFFu) | (32767u << 16))
+                                             : ((aw[i >> 1] & 0xFFFF0000u) | 32767u);
+                    }
+                }
+                atomicAdd(&gs.sat, (uint32_t)ev);
+            }
+            a.x = aw[0]; a.y = aw[1]; a.z = aw[2]; a.w = aw[3];
+            *ap = a;
+            row8(R_A2, lg)[ch] = (unsigned char)ge2_bits(a);
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                const int inc = __popc(e & ob[p]) + __popc(t & ob[p]) - lost[p];
+                if (p < P && inc) atomicAdd(&gs.tot[p], inc);
+            }
+        }
+    };
+    // even turns that are no tick: +1 on the few owned structures, found by bit iteration
+    auto grow_structures = [&](int lg) {
+        StepGame &gs = s_game[lg];
+        int16_t *A = B.army + (size_t)(wg0 + lg) * S;
+        for (int j = ol; j < NW; j += LPG) {
+            const uint32_t sw = row(R_STR, lg)[j];
+            if (sw == 0) continue;
+            uint32_t a2w = row(R_A2, lg)[j];
+            bool changed = false;
+            for (int p = 0; p < P; ++p) {
+                uint32_t m = sw & row(p, lg)[j];
+                int inc = 0;
+                while (m) {
+                    const int b = __ffs(m) - 1;
+                    m &= m - 1;
+                    const int c = 32 * j + b, av = __ldcg(A + c);
+                    if (av >= 32767) { atomicAdd(&gs.sat, 1u); continue; }  // R21
+                    A[c] = (int16_t)(av + 1);
+                    inc += 1;
+                    if (av == 1) { a2w |= 1u << b; changed = true; }
+                }
+                if (inc) atomicAdd(&gs.tot[p], inc);
+            }
+            if (changed) row(R_A2, lg)[j] = a2w;
+        }
+    };
+
+    // ---------------------------------------------------------------- a7-a9: end of turn, one lane per game
+    auto write_result = [&](int gg, int rew_bits, uint32_t done, int winner) {
+        int8_t *rw = B.reward + (size_t)gg * P;
+        if (rew_bits == 0x5555 >> (16 - 2 * P) && (P == 2 || P == 4 || P == 8)) {  // all zero: one store
+            if (P == 2) *reinterpret_cast<uint16_t *>(rw) = 0;
+            else if (P == 4) *reinterpret_cast<uint32_t *>(rw) = 0;
+            else *reinterpret_cast<uint2 *>(rw) = make_uint2(0u, 0u);
+        } else {
+            for (int p = 0; p < P; ++p) rw[p] = (int8_t)(((rew_bits >> (2 * p)) & 3) - 1);
+        }
+        B.done[gg] = (uint8_t)done;
+        B.winner[gg] = (int8_t)winner;
+    };
+    auto finish_turn = [&](int lg) {
+        StepGame &gs = s_game[lg];
+        const int gg = wg0 + lg;
+        if (gs.sat) { B.sat_events[gg] += gs.sat; gs.sat = 0; }
+        const int zero_bits = 0x5555 >> (16 - 2 * P);
+        const bool truncated_now = kp.max_turns > 0 && gs.turn >= kp.max_turns;
+        if (gs.alive == allp && !truncated_now && kp.n_teams > 1) {  // the common case: nothing ends
+            gs.done = 0;
+            gs.winner = -1;
+            write_result(gg, zero_bits, 0u, -1);
+            return;
+        }
+        int living = 0, last = -1;
+        for (int t = 0; t < kp.n_teams; ++t) {
+            const uint32_t tm = (((1u << kp.team_size) - 1u) << (t * kp.team_size)) & allp;
+            if (gs.alive & tm) { ++living; last = t; }
+        }
+        const bool terminated = living <= 1;
+        const bool truncated = !terminated && truncated_now;
+        gs.done = (terminated ? 1u : 0u) | (truncated ? 2u : 0u);
+        gs.winner = terminated ? last : -1;
+        int rew_bits = 0;
+        for (int p = 0; p < P; ++p) {
+            const int r = terminated ? ((p / kp.team_size == last) ? 1 : -1) : 0;
+            rew_bits |= (r + 1) << (2 * p);
+            if (r > 0) B.wins[(size_t)gg * P + p] += 1;
+        }
+        write_result(gg, rew_bits, gs.done, gs.winner);
+        if (gs.done) {
+            B.episodes_done[gg] += 1;
+            if (truncated) B.truncations[gg] += 1;
+            if (kp.auto_reset) {  // a9 (R17)
+                gs.episode += 1;
+                B.episode[gg] = gs.episode;
+                gs.flags |= SG_RESET;
+            }
+        }
+    };
+
+    // ---------------------------------------------------------------- a9 + a1: regenerate game lg (whole warp)
+    // The generator fills one game's planes in the warp's scratch; the rows are gathered from them and the
+    // planes copied out to HBM.
+    auto regenerate = [&](int lg) {
+        StepGame &gs = s_game[lg];
+        const int gg = wg0 + lg;
+        int16_t *sA = reinterpret_cast<int16_t *>(s_scratch);
+        int8_t *sO = reinterpret_cast<int8_t *>(s_scratch + 2 * S), *sT = reinterpret_cast<int8_t *>(s_scratch + 3 * S);
+        generate_board<NP>(kp, lane, kp.gid_base + (uint32_t)gg, gs.episode, sA, sO, sT,
+                           B.general_cell + (size_t)gg * P);
+        const int rb = 4 * BW;  // row stride in bytes
+        unsigned char *rows = row8(0, lg);
+        for (int ch = (int)lane; ch < rb; ch += 32) {
+            if (ch < NC8) {
+                const uint2 o = *reinterpret_cast<const uint2 *>(sO + 8 * ch);
+                const uint2 t = *reinterpret_cast<const uint2 *>(sT + 8 * ch);
+                const uint4 a = *reinterpret_cast<const uint4 *>(sA + 8 * ch);
+#pragma unroll
+                for (int p = 0; p < NP; ++p)
+                    if (p < P) {
+                        const uint32_t pat = 0x01010101u * (uint32_t)p;
+                        rows[p * rb + ch] = (unsigned char)gather8<0>(eq_bytes(o.x, pat), eq_bytes(o.y, pat));
+                    }
+                const uint32_t hx = t.x >> 1, hy = t.y >> 1;  // terrain: mountain = 01, structure = 1x
+                rows[R_MTN * rb + ch] = (unsigned char)gather8<0>(t.x & ~hx, t.y & ~hy);
+                rows[R_STR * rb + ch] = (unsigned char)gather8<0>(hx, hy);
+                rows[R_A2 * rb + ch] = (unsigned char)ge2_bits(a);
+            } else {
+                for (int p = 0; p < P; ++p) rows[p * rb + ch] = 0;
+                rows[R_MTN * rb + ch] = 0xFF;
+                rows[R_STR * rb + ch] = 0;
+                rows[R_A2 * rb + ch] = 0;
+            }
+        }
+        const size_t gbase = (size_t)gg * S;
+        for (int u = (int)lane; u < S / 8; u += 32)
+            *reinterpret_cast<uint4 *>(B.army + gbase + 8 * u) = *reinterpret_cast<const uint4 *>(sA + 8 * u);
+        for (int u = (int)lane; u < S / 16; u += 32) {
+            *reinterpret_cast<uint4 *>(B.owner + gbase + 16 * u) = *reinterpret_cast<const uint4 *>(sO + 16 * u);
+            *reinterpret_cast<uint4 *>(B.terrain + gbase + 16 * u) = *reinterpret_cast<const uint4 *>(sT + 16 * u);
+        }
+        if (lane == 0) {
+            gs.turn = 0;
+            gs.alive = allp;
+            gs.flags = (gs.flags & ~SG_RESET) | SG_STATIC_DIRTY;
+            for (int p = 0; p < P; ++p) {
+                gs.tot[p] = 1;
+                gs.land[p] = 1;
+                gs.gcell[p] = B.general_cell[(size_t)gg * P + p];
+            }
+        }
+        __syncwarp();
+    };
+
+    // ---------------------------------------------------------------- a10: fog of war (all players at once)
+    auto compute_vis = [&](int lg) {
+        if (pl >= P) return;
+        const int js = sl * WS, je = min(js + WS, NW);
+        if (js >= je) return;
+        uint32_t *vr = vrow(pl, lg);
+        const uint32_t *own = row(pl, lg);
+        const uint32_t members = teams ? team_mask(pl) : 0u;
+        auto tw = [&](int j) -> uint32_t {
+            if ((unsigned)j >= (unsigned)NW) return 0u;
+            if (!teams) return own[j];
+            uint32_t tm = 0;
+            for (int q = 0; q < P; ++q)
+                if ((members >> q) & 1u) tm |= row(q, lg)[j];
+            return tm;
+        };
+        auto hdil = [&](uint32_t a, uint32_t b, uint32_t c, int j) -> uint32_t {  // s_nc0 / s_ncL are 0 off the board
+            return b | (__funnelshift_l(a, b, 1) & s_nc0[j]) | (__funnelshift_r(b, c, 1) & s_ncL[j]);
+        };
+        uint32_t t1 = tw(js - 1), t2 = tw(js), t3 = tw(js + 1);
+        uint32_t hm = hdil(tw(js - 2), t1, t2, js - 1), hc = hdil(t1, t2, t3, js);
+        for (int j = js; j < je; ++j) {
+            const uint32_t t4 = tw(j + 2);
+            const uint32_t hn = hdil(t2, t3, t4, j + 1);
+            vr[j] = (hc | __funnelshift_lc(hm, hc, W) | __funnelshift_rc(hc, hn, W)) & s_inb[j];
+            hm = hc; hc = hn; t2 = t3; t3 = t4;
+        }
+    };
+
+    // ---------------------------------------------------------------- a11: observation planes (octet)
+    // per 8-cell chunk: the state is read once from global memory (16 + 8 + 8 bytes per lane, the octet
+    // covers full 128 / 64-byte lines) and masked once per player: one 16-byte and three 8-byte streaming
+    // stores each
+    auto emit_planes = [&](int lg) {
+        const size_t gbase = (size_t)(wg0 + lg) * (size_t)S;
+        const size_t obase = gbase * (size_t)P;
+        const unsigned char *ga = reinterpret_cast<const unsigned char *>(B.army + gbase) + 16 * ol;
+        const unsigned char *go = reinterpret_cast<const unsigned char *>(B.owner + gbase) + 8 * ol;
+        const unsigned char *gt = reinterpret_cast<const unsigned char *>(B.terrain + gbase) + 8 * ol;
+        unsigned char *oa = reinterpret_cast<unsigned char *>(B.obs_army + obase) + 16 * ol;
+        unsigned char *oo = reinterpret_cast<unsigned char *>(B.obs_owner + obase) + 8 * ol;
+        unsigned char *ot = reinterpret_cast<unsigned char *>(B.obs_terrain + obase) + 8 * ol;
+        unsigned char *ov = reinterpret_cast<unsigned char *>(B.obs_vis + obase) + 8 * ol;
+        const unsigned char *sv = reinterpret_cast<const unsigned char *>(vrow(0, lg)) + ol;
+        const int nit = (NC8 - ol + LPG - 1) / LPG;
+#pragma unroll 3
+        for (int i = 0; i < nit; ++i) {
+            const uint4 a = __ldcg(reinterpret_cast<const uint4 *>(ga + 128 * i));
+            const uint2 o = __ldcg(reinterpret_cast<const uint2 *>(go + 64 * i));
+            const uint2 t = __ldcg(reinterpret_cast<const uint2 *>(gt + 64 * i));
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                if (p >= P) break;
+                const uint32_t vb = sv[4 * BW * p + 8 * i];
+                const uint32_t s0 = nib_sign(vb & 15u), s1 = nib_sign(vb >> 4);
+                const uint32_t m0 = prmt(s0, 0u, 0xBA98u), m1 = prmt(s1, 0u, 0xBA98u);
+                uint4 xa;
+                xa.x = a.x & prmt(s0, 0u, 0x9988u); xa.y = a.y & prmt(s0, 0u, 0xBBAAu);
+                xa.z = a.z & prmt(s1, 0u, 0x9988u); xa.w = a.w & prmt(s1, 0u, 0xBBAAu);
+                uint2 xo, xt, xv;
+                xo.x = (o.x & m0) | (~m0 & 0xFEFEFEFEu); xo.y = (o.y & m1) | (~m1 & 0xFEFEFEFEu);
+                xt.x = (t.x & m0) | (~m0 & 0x04040404u); xt.y = (t.y & m1) | (~m1 & 0x04040404u);
+                xv.x = m0 & 0x01010101u; xv.y = m1 & 0x01010101u;
+                const size_t po = (size_t)p * (size_t)S;
+                __stcs(reinterpret_cast<uint4 *>(oa + 2 * po + 128 * i), xa);
+                __stcs(reinterpret_cast<uint2 *>(oo + po + 64 * i), xo);
+                __stcs(reinterpret_cast<uint2 *>(ot + po + 64 * i), xt);
+                __stcs(reinterpret_cast<uint2 *>(ov + po + 64 * i), xv);
+            }
+        }
+    };
+
+    // ================================================================ the turn
+    const uint32_t gstep = kp.global_step0;
+    bool frozen = false;
+    if (gvalid) {
+        StepGame &gs = s_game[sub];
+        frozen = !kp.auto_reset && gs.done != 0;  // R31
+        int a = 0;
+        if (!frozen) {
+            if (flags & F_SAMPLER) a = sample(sub, gstep);
+            else if (sl == 0 && pl < P) a = kp.actions[(size_t)g * P + pl];
+        }
+        if (sl == 0 && pl < P) {
+            gs.act[pl] = a;
+            if (B.actions_out) B.actions_out[(size_t)g * P + pl] = a;
+        }
+    }
+    __syncwarp();
+    if (gvalid && ol == 0) {
+        if (frozen) s_game[sub].flags |= SG_FROZEN;
+        else play_moves(sub);
+    }
+    __syncwarp();
+    if (gvalid) {
+        const uint32_t gf = s_game[sub].flags;
+        if (gf & SG_GROW_TICK) grow_tick(sub);
+        else if (gf & SG_GROW_EVEN) grow_structures(sub);
+    }
+    __syncwarp();
+    bool want_reset = false;
+    if (gvalid && ol == 0) {
+        StepGame &gs = s_game[sub];
+        if (frozen) write_result(g, 0x5555 >> (16 - 2 * P), gs.done, gs.winner);
+        else finish_turn(sub);
+        want_reset = (gs.flags & SG_RESET) != 0;
+    }
+    const uint32_t rs = __ballot_sync(FULL, want_reset);  // bit sub * LPG: game sub must be regenerated
+    if (rs) {
+        for (int lg = 0; lg < nwg; ++lg)
+            if ((rs >> (lg * LPG)) & 1u) regenerate(lg);
+    }
+    __syncwarp();
+    // ---- a10 + a11 (R32: the state at the end of the call)
+    if (gvalid) compute_vis(sub);
+    __syncwarp();
+    if (gvalid) emit_planes(sub);
+
+    // ================================================================ store: cache rows and scalars
+    if (gvalid) {
+        const StepGame &gs = s_game[sub];
+        const int nrows = (gs.flags & SG_STATIC_DIRTY) ? P + 3 : P + 1;  // own[p] + army >= 2 (+ structure, mountain)
+        const uint4 *src = reinterpret_cast<const uint4 *>(row(0, sub));
+        uint4 *dst = reinterpret_cast<uint4 *>(B.bitboards + (size_t)g * (size_t)(P + 3) * (size_t)BW);
+        if (!frozen)
+            for (int u = ol; u < nrows * BW / 4; u += LPG) dst[u] = src[u];
+        if (ol < P) {
+            B.land[(size_t)g * P + ol] = gs.land[ol];
+            B.army_total[(size_t)g * P + ol] = gs.tot[ol];
+        }
+        if (ol == (P & 7)) { B.turn[g] = gs.turn; B.alive[g] = (uint8_t)gs.alive; }
+    }
+}
+
+}  // namespace gen

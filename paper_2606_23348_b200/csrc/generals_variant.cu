@@ -9,13 +9,22 @@
 namespace gen {
 
 template <int ID> struct Sel;
-#define GEN_DEFINE(id, np, h, w, ff)                                    \
+#define GEN_DEFINE(id, kind, np, h, w, ff, maxt, minb)                  \
     template <> struct Sel<id> {                                        \
-        static constexpr int NP = np, H = h, W = w;                     \
+        static constexpr int KIND = kind, NP = np, H = h, W = w;        \
         static constexpr uint32_t FF = ff;                              \
+        static constexpr int MAXT = maxt, MINB = minb;                  \
     };
 GEN_VARIANTS(GEN_DEFINE)
 #undef GEN_DEFINE
+
+template <typename S, int KIND> struct KernelOf;
+template <typename S> struct KernelOf<S, 0> {
+    static constexpr auto fn = k_generals<S::NP, S::H, S::W, S::FF>;
+};
+template <typename S> struct KernelOf<S, 1> {
+    static constexpr auto fn = k_step<S::NP, S::H, S::W, S::MAXT, S::MINB>;
+};
 
 #define GEN_CAT_(a, b) a##b
 #define GEN_CAT(a, b) GEN_CAT_(a, b)
@@ -23,7 +32,7 @@ GEN_VARIANTS(GEN_DEFINE)
 cudaError_t GEN_CAT(launch_variant_, GEN_VARIANT_ID)(const KParams &kp, int grid, int block, size_t smem,
                                                      cudaStream_t stream) {
     using S = Sel<GEN_VARIANT_ID>;
-    auto kernel = k_generals<S::NP, S::H, S::W, S::FF>;
+    auto kernel = KernelOf<S, S::KIND>::fn;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);

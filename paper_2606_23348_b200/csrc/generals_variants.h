@@ -1,35 +1,42 @@
 // generals_variants.h -- the list of kernel instantiations of libgenerals.so.
 // One translation unit per variant (generals_variant.cu compiled with -DGEN_VARIANT_ID=n) so that the
 // build compiles them in parallel; generals_api.cu picks one per launch from this table.
+//   kind 0: the STAGED kernel k_generals (generals_kernels.cuh): planes resident in shared memory; serves
+//           every call (reset, observe, sample, step, K-step rollout, digest).
+//   kind 1: the REGISTER-RESIDENT per-step kernel k_step (generals_step.cuh): gen_step when the caller
+//           provides the bitboard cache and no digest buffer, uniform policy.
 #pragma once
 #include <cuda_runtime.h>
 
-#include "generals_kernels.cuh"
+#include "generals_step.cuh"
 
 namespace gen {
 
-constexpr uint32_t FF_STEP = F_OBS_PLANES | F_K1;                // gen_step without a digest buffer
 constexpr uint32_t FF_ROLL_DIGEST = F_OBS_PLANES | F_DIGEST;     // gen_rollout(K, GEN_OBS_DIGEST)
 
-//  X(id, NP, H, W, flags)
-#define GEN_VARIANTS(X)            \
-    X(0, 2, 0, 0, F_RUNTIME)       \
-    X(1, 4, 0, 0, F_RUNTIME)       \
-    X(2, 8, 0, 0, F_RUNTIME)       \
-    X(3, 2, 24, 24, FF_STEP)       \
-    X(4, 2, 24, 24, FF_ROLL_DIGEST)\
-    X(5, 2, 8, 8, FF_STEP)         \
-    X(6, 4, 32, 32, FF_STEP)       \
-    X(7, 8, 32, 32, FF_STEP)
-constexpr int N_VARIANTS = 8;
+//  X(id, kind, NP, H, W, flags (kind 0) or 0, max threads per CTA, min CTAs per SM (kind 1))
+#define GEN_VARIANTS(X)                          \
+    X(0, 0, 2, 0, 0, F_RUNTIME, 256, 1)          \
+    X(1, 0, 4, 0, 0, F_RUNTIME, 256, 1)          \
+    X(2, 0, 8, 0, 0, F_RUNTIME, 256, 1)          \
+    X(3, 0, 2, 24, 24, FF_ROLL_DIGEST, 256, 1)   \
+    X(4, 1, 2, 0, 0, 0, 256, 2)                  \
+    X(5, 1, 4, 0, 0, 0, 256, 2)                  \
+    X(6, 1, 8, 0, 0, 0, 256, 2)                  \
+    X(7, 1, 2, 24, 24, 0, 64, 14)                \
+    X(8, 1, 2, 8, 8, 0, 64, 16)                  \
+    X(9, 1, 4, 32, 32, 0, 64, 8)                 \
+    X(10, 1, 8, 32, 32, 0, 64, 6)
+constexpr int N_VARIANTS = 11;
 
 struct Variant {
-    int np, h, w;      // h == 0: any board with n_players <= np
-    uint32_t ff;       // F_RUNTIME: any mode
+    int kind, np, h, w;  // h == 0: any board with n_players <= np
+    uint32_t ff;         // kind 0: F_RUNTIME = any mode, else the exact mode
+    int max_threads;     // largest CTA this instantiation may be launched with
     cudaError_t (*launch)(const KParams &, int grid, int block, size_t smem, cudaStream_t);
 };
 
-#define GEN_DECLARE(id, np, h, w, ff) \
+#define GEN_DECLARE(id, kind, np, h, w, ff, maxt, minb) \
     cudaError_t launch_variant_##id(const KParams &, int grid, int block, size_t smem, cudaStream_t);
 GEN_VARIANTS(GEN_DECLARE)
 #undef GEN_DECLARE

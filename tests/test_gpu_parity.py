@@ -134,25 +134,63 @@ def test_captures_happen_and_match(gpu, oracle_mod):
     ("c5b_ffa8", 37, 230, dict(max_turns=150)),
 ])
 def test_specialised_step_kernels_match_oracle(gpu, oracle_mod, name, N, T, over):
-    """The per-step kernels compiled for the paper-sized boards (what bench.py times: no digest buffer)
-    against the oracle, every tensor every step; the same handle forced onto the generic kernel must
-    agree too."""
+    """gen_step as bench.py times it (bitboard cache, no digest buffer): the register-resident kernel compiled
+    for the paper-sized board against the oracle, every tensor every step; the same kernel's generic
+    instantiation and the staged kernel must agree too."""
     cfg, _ = workloads.config(name, n_games=N, **over)
     env = gpu.GeneralsEnv(cfg, digest=False)
     gen = gpu.GeneralsEnv(cfg, digest=False)
-    gen.set_generic(True)
+    gen.set_generic(True, False)
+    stg = gpu.GeneralsEnv(cfg, digest=False, bitboards=False)
     o = oracle_mod.Oracle(cfg)
-    for e in (env, gen):
+    for e in (env, gen, stg):
         e.reset()
     o.reset()
     for t in range(T):
-        env.step()
-        gen.step()
+        for e in (env, gen, stg):
+            e.step()
         o.step()
         compare(env, o, digest=False, where=f"{name} specialised step {t}")
         if t % 16 == 0:
             compare(gen, o, digest=False, where=f"{name} generic step {t}")
-    assert env.last_launch_specialised and not gen.last_launch_specialised
+            compare(stg, o, digest=False, where=f"{name} staged step {t}")
+    uniform = cfg["bias_thr"] == 0                          # the biased policy (R25) runs on the staged kernel
+    assert env.last_launch_specialised == uniform and env.last_launch_register_resident == uniform
+    assert not gen.last_launch_specialised and gen.last_launch_register_resident == uniform
+    assert not stg.last_launch_register_resident
+    assert int(o.episodes_done.sum()) > 0
+
+
+def test_kernels_interleave_coherently(gpu, oracle_mod):
+    """The bitboard cache stays current across every kind of call: register-resident steps, staged rollouts,
+    staged steps (forced), explicit actions, gen_observe, gen_sample."""
+    import torch
+    cfg, _ = workloads.config("c2_24x24", n_games=53, max_turns=70, spawn_dmin=4)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+    kinds = []
+    for it in range(12):
+        for _ in range(7):
+            env.step()
+            o.step()
+        kinds.append(env.last_launch_register_resident)
+        compare(env, o, digest=False, where=f"it {it} steps")
+        env.rollout(9, gpu.OBS_NONE)
+        o.rollout(9, oracle_mod.OBS_NONE)
+        env.set_generic(False, True)
+        env.step()
+        o.step()
+        kinds.append(env.last_launch_register_resident)
+        env.set_generic(False, False)
+        a = o.sample()
+        assert np.array_equal(env.sample().cpu().numpy(), a)
+        env.step(torch.from_numpy(a).to(env.device))
+        o.step(a)
+        env.observe()
+        compare(env, o, fields=STATE_FIELDS + OUT_FIELDS[3:], digest=False, where=f"it {it} end")
+    assert kinds[0] and not kinds[1]
     assert int(o.episodes_done.sum()) > 0
 
 
@@ -260,14 +298,18 @@ def run_hand_case(gpu, oracle_mod, H, W, P, cells, actions, turn=0, team_size=1,
     o = hand_board(oracle_mod, H, W, P, cells, turn=turn, team_size=team_size, **cfg)
     base = dict(n_games=1, height=H, width=W, n_players=P, team_size=team_size)
     base.update(cfg)
-    env = gpu.GeneralsEnv(base, digest=False)
-    put_board(env, o)
-    compare(env, o, fields=["land", "army_total"] + OUT_FIELDS[3:], digest=False, where="observe")
+    env = gpu.GeneralsEnv(base, digest=False)                      # register-resident step kernel
+    twin = gpu.GeneralsEnv(base, digest=False, bitboards=False)    # staged kernel
+    for e in (env, twin):
+        put_board(e, o)
+        compare(e, o, fields=["land", "army_total"] + OUT_FIELDS[3:], digest=False, where="observe")
     for s in range(steps):
         a = np.asarray(actions[s] if steps > 1 else actions, dtype=np.int32).reshape(1, P)
-        env.step(torch.from_numpy(a).to(env.device))
         o.step(a)
-        compare(env, o, digest=False, where=f"hand step {s}")
+        for e in (env, twin):
+            e.step(torch.from_numpy(a).to(e.device))
+            compare(e, o, digest=False, where=f"hand step {s}")
+    assert env.last_launch_register_resident and not twin.last_launch_register_resident
     return env, o
 
 
@@ -417,12 +459,14 @@ def test_step_host_end_to_end(gpu, oracle_mod):
 
 
 # ------------------------------------------------------------------------------- full-size sampled check
-def test_config2_full_size_sampled_games(gpu, oracle_mod):
-    """BASELINE config 2 at its full N = 16,384 in the launch configuration bench.py times: the oracle
+@pytest.mark.parametrize("digest", [False, True])
+def test_config2_full_size_sampled_games(gpu, oracle_mod, digest):
+    """BASELINE config 2 at its full N = 16,384 in the launch configuration bench.py times (digest False:
+    the register-resident step kernel; True: the staged kernel with the digest chained): the oracle
     replays a sample of global game ids (first / last / strided; legitimate because a game depends on
     its global id only, M2) and must agree on state, observation and digest."""
     cfg, _ = workloads.config("c2_24x24")
-    env = gpu.GeneralsEnv(cfg)
+    env = gpu.GeneralsEnv(cfg, digest=digest)
     env.reset()
     T = 240
     for _ in range(T):
@@ -438,7 +482,9 @@ def test_config2_full_size_sampled_games(gpu, oracle_mod):
             got = env.field(f)[gid]
             want = np.asarray(o.field(f))[0]
             assert np.array_equal(got, want), (gid, f)
-        assert int(env.field("obs_digest")[gid]) == int(o.obs_digest[0]), gid
+        if digest:
+            assert int(env.field("obs_digest")[gid]) == int(o.obs_digest[0]), gid
+    assert env.last_launch_register_resident == (not digest) and env.last_launch_specialised
     # properties that hold at any size
     owner, terrain, army = env.field("owner"), env.field("terrain"), env.field("army")
     assert (owner[terrain == MT] == -1).all() and (army >= 0).all()
