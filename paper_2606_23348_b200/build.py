@@ -40,6 +40,7 @@ def build(force=False, verbose=False):
     os.makedirs(OBJ, exist_ok=True)
     base = [nvcc_path(), "-std=c++17", "-O3", *ARCH, "-lineinfo", "-Xcompiler", "-fPIC",
             "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+    base += os.environ.get("GEN_NVCC_FLAGS", "").split()      # development only (e.g. -DGEN_EXPERIMENT=...)
     if verbose:
         base += ["-Xptxas", "-v"]
     jobs = [(base + ["-c", os.path.join(CSRC, "generals_api.cu"), "-o", os.path.join(OBJ, "api.o")])]

@@ -191,6 +191,10 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(bar) : "memory");
 }
+__device__ __forceinline__ void l2_prefetch(const void *src, uint32_t bytes) {  // TMA bulk prefetch HBM -> L2
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes)
+                 : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t ok;
     do {
@@ -463,17 +467,20 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         bulk_g2s(smem_u32(s_owner), B.owner + (size_t)wg0 * S, cells, bar);
         bulk_g2s(smem_u32(s_terr), B.terrain + (size_t)wg0 * S, cells, bar);
     }
-    if (loading && gvalid) {  // per-game scalars, spread over the octet
+    if (loading && gvalid) {  // per-game scalars: every lane issues all loads (one round trip), then the octet scatters
         GameS &gs = s_game[sub];
-        if (ol < P) {
-            gs.tot[ol] = B.army_total[(size_t)g * P + ol];
-            gs.land[ol] = B.land[(size_t)g * P + ol];
-        }
-        if (ol == 0) { gs.turn = B.turn[g]; gs.episode = B.episode[g]; }
-        if (ol == 1) { gs.alive = B.alive[g]; gs.done = B.done[g]; gs.winner = B.winner[g]; }
+        const size_t gp = (size_t)g * P + (size_t)min(ol, P - 1);
+        const int32_t v_tot = __ldcg(B.army_total + gp), v_land = __ldcg(B.land + gp);
+        const int32_t v_turn = __ldcg(B.turn + g);
+        const uint32_t v_ep = __ldcg(B.episode + g), v_alive = __ldcg(B.alive + g), v_done = __ldcg(B.done + g);
+        const int32_t v_win = __ldcg(B.winner + g);
+        const unsigned long long v_dg = ((flags & F_DIGEST) && B.obs_digest) ? __ldcg(B.obs_digest + g) : 0ull;
+        if (ol < P) { gs.tot[ol] = v_tot; gs.land[ol] = v_land; }
+        if (ol == 0) { gs.turn = v_turn; gs.episode = v_ep; }
+        if (ol == 1) { gs.alive = v_alive; gs.done = v_done; gs.winner = v_win; }
         if (ol == 2) {
             gs.flags = 0; gs.sat = 0; gs.dirtyO = 0; gs.dirtyA[0] = 0; gs.dirtyA[1] = 0; gs.rew_bits = 0;
-            gs.digest = ((flags & F_DIGEST) && B.obs_digest) ? B.obs_digest[g] : 0ull;
+            gs.digest = v_dg;
         }
     }
     __syncthreads();  // the only CTA barrier: tables (and the mbarrier init) are visible

@@ -22,6 +22,26 @@
 
 namespace gen {
 
+#ifdef GEN_TRACE  // development only: mean time per phase and warp (globaltimer), read by gen_debug_trace_<id>
+static __device__ unsigned long long g_trace[32];
+__device__ __forceinline__ unsigned long long gtimer() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define GEN_TRACE_MARK(k)                                                            \
+    do {                                                                             \
+        __syncwarp();                                                                \
+        if (lane == 0) {                                                             \
+            const unsigned long long t_ = gtimer();                                  \
+            atomicAdd(&g_trace[k], t_ - t_prev);                                     \
+            t_prev = t_;                                                             \
+        }                                                                            \
+    } while (0)
+#else
+#define GEN_TRACE_MARK(k)
+#endif
+
 struct StepGame {  // per-game scalars in shared memory
     int32_t turn, winner;
     uint32_t alive, done, episode, flags, sat;
@@ -181,6 +201,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     };
 
     // ================================================================ prologue
+#ifdef GEN_TRACE
+    unsigned long long t_prev = gtimer();
+    if (lane == 0) atomicAdd(&g_trace[31], 1ull);
+#endif
     for (int t = tid; t < 34; t += blockDim.x) {
         const int j = t - 1;
         const bool in = j >= 0 && j < 32;
@@ -194,20 +218,33 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         mbar_expect_tx(bar, bytes);
         bulk_g2s(smem_u32(s_rows), B.bitboards + (size_t)wg0 * (size_t)(P + 3) * (size_t)BW, bytes, bar);
     }
-    if (gvalid) {  // per-game scalars, spread over the octet
+    if (gvalid) {  // per-game scalars: every lane issues all eight loads (one round trip), then the octet scatters
         StepGame &gs = s_game[sub];
-        if (ol < P) {
-            gs.tot[ol] = B.army_total[(size_t)g * P + ol];
-            gs.land[ol] = B.land[(size_t)g * P + ol];
-            gs.gcell[ol] = B.general_cell[(size_t)g * P + ol];
-        }
-        if (ol == 0) { gs.turn = B.turn[g]; gs.episode = B.episode[g]; }
-        if (ol == 1) { gs.alive = B.alive[g]; gs.done = B.done[g]; gs.winner = B.winner[g]; }
+        const size_t gp = (size_t)g * P + (size_t)min(ol, P - 1);
+        const int32_t v_tot = __ldcg(B.army_total + gp), v_land = __ldcg(B.land + gp);
+        const int32_t v_gc = __ldcg(B.general_cell + gp);
+        const int32_t v_turn = __ldcg(B.turn + g);
+        const uint32_t v_ep = __ldcg(B.episode + g), v_alive = __ldcg(B.alive + g), v_done = __ldcg(B.done + g);
+        const int32_t v_win = __ldcg(B.winner + g);
+        if (ol < P) { gs.tot[ol] = v_tot; gs.land[ol] = v_land; gs.gcell[ol] = v_gc; }
+        if (ol == 0) { gs.turn = v_turn; gs.episode = v_ep; }
+        if (ol == 1) { gs.alive = v_alive; gs.done = v_done; gs.winner = v_win; }
         if (ol == 2) { gs.flags = 0; gs.sat = 0; gs.rew_bits = 0; }
     }
     __syncthreads();  // the only CTA barrier: tables and the mbarrier init are visible
     if (nwg <= 0) return;
+    GEN_TRACE_MARK(0);  // scalars + barrier
     mbar_wait(bar, 0);
+    if (lane == 0) {
+        // The planes of the warp's games are contiguous: start them on their way from HBM to L2 now (after the
+        // small latency-critical loads above, so that those do not queue behind 9 KB of bulk traffic per warp);
+        // the rules below run while they travel and the emit pass finds them in L2.
+        const uint32_t cells = (uint32_t)nwg * (uint32_t)S;
+        l2_prefetch(B.army + (size_t)wg0 * S, 2u * cells);
+        l2_prefetch(B.owner + (size_t)wg0 * S, cells);
+        l2_prefetch(B.terrain + (size_t)wg0 * S, cells);
+    }
+    GEN_TRACE_MARK(1);  // cache rows arrived
 
     // ---------------------------------------------------------------- a12: valid-action sampler (R24)
     // As in the staged kernel: the LPP lanes (pl, 0..LPP-1) of the octet serve player pl and split the NW
@@ -619,44 +656,71 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     };
 
     // ---------------------------------------------------------------- a11: observation planes (octet)
-    // per 8-cell chunk: the state is read once from global memory (16 + 8 + 8 bytes per lane, the octet
-    // covers full 128 / 64-byte lines) and masked once per player: one 16-byte and three 8-byte streaming
-    // stores each
+    // Lane ol owns the 8-cell chunks ol, ol + 8, ...: per chunk the octet covers full 128 / 64-byte lines.
+    // Two passes, each with ALL its global loads issued before the first use (memory-level parallelism: one
+    // round trip per pass instead of one per chunk): (A) the army plane, 16 bytes per chunk; (B) owner and
+    // terrain, 8 + 8 bytes.  Every chunk is masked once per player with that player's fog byte and leaves
+    // as one 16-byte and three 8-byte streaming stores.
     auto emit_planes = [&](int lg) {
+        constexpr int EB = FIXED ? ((cS / 8 + LPG - 1) / LPG < 9 ? (cS / 8 + LPG - 1) / LPG : 9) : 4;  // chunks per batch
         const size_t gbase = (size_t)(wg0 + lg) * (size_t)S;
         const size_t obase = gbase * (size_t)P;
-        const unsigned char *ga = reinterpret_cast<const unsigned char *>(B.army + gbase) + 16 * ol;
-        const unsigned char *go = reinterpret_cast<const unsigned char *>(B.owner + gbase) + 8 * ol;
-        const unsigned char *gt = reinterpret_cast<const unsigned char *>(B.terrain + gbase) + 8 * ol;
-        unsigned char *oa = reinterpret_cast<unsigned char *>(B.obs_army + obase) + 16 * ol;
-        unsigned char *oo = reinterpret_cast<unsigned char *>(B.obs_owner + obase) + 8 * ol;
-        unsigned char *ot = reinterpret_cast<unsigned char *>(B.obs_terrain + obase) + 8 * ol;
-        unsigned char *ov = reinterpret_cast<unsigned char *>(B.obs_vis + obase) + 8 * ol;
+        const unsigned char *__restrict__ ga = reinterpret_cast<const unsigned char *>(B.army + gbase) + 16 * ol;
+        const unsigned char *__restrict__ go = reinterpret_cast<const unsigned char *>(B.owner + gbase) + 8 * ol;
+        const unsigned char *__restrict__ gt = reinterpret_cast<const unsigned char *>(B.terrain + gbase) + 8 * ol;
+        unsigned char *__restrict__ oa = reinterpret_cast<unsigned char *>(B.obs_army + obase) + 16 * ol;
+        unsigned char *__restrict__ oo = reinterpret_cast<unsigned char *>(B.obs_owner + obase) + 8 * ol;
+        unsigned char *__restrict__ ot = reinterpret_cast<unsigned char *>(B.obs_terrain + obase) + 8 * ol;
+        unsigned char *__restrict__ ov = reinterpret_cast<unsigned char *>(B.obs_vis + obase) + 8 * ol;
         const unsigned char *sv = reinterpret_cast<const unsigned char *>(vrow(0, lg)) + ol;
         const int nit = (NC8 - ol + LPG - 1) / LPG;
-#pragma unroll 3
-        for (int i = 0; i < nit; ++i) {
-            const uint4 a = __ldcg(reinterpret_cast<const uint4 *>(ga + 128 * i));
-            const uint2 o = __ldcg(reinterpret_cast<const uint2 *>(go + 64 * i));
-            const uint2 t = __ldcg(reinterpret_cast<const uint2 *>(gt + 64 * i));
+        for (int i0 = 0; i0 < nit; i0 += EB) {
+            // ---- pass A: army
+            uint4 a[EB];
 #pragma unroll
-            for (int p = 0; p < NP; ++p) {
-                if (p >= P) break;
-                const uint32_t vb = sv[4 * BW * p + 8 * i];
-                const uint32_t s0 = nib_sign(vb & 15u), s1 = nib_sign(vb >> 4);
-                const uint32_t m0 = prmt(s0, 0u, 0xBA98u), m1 = prmt(s1, 0u, 0xBA98u);
-                uint4 xa;
-                xa.x = a.x & prmt(s0, 0u, 0x9988u); xa.y = a.y & prmt(s0, 0u, 0xBBAAu);
-                xa.z = a.z & prmt(s1, 0u, 0x9988u); xa.w = a.w & prmt(s1, 0u, 0xBBAAu);
-                uint2 xo, xt, xv;
-                xo.x = (o.x & m0) | (~m0 & 0xFEFEFEFEu); xo.y = (o.y & m1) | (~m1 & 0xFEFEFEFEu);
-                xt.x = (t.x & m0) | (~m0 & 0x04040404u); xt.y = (t.y & m1) | (~m1 & 0x04040404u);
-                xv.x = m0 & 0x01010101u; xv.y = m1 & 0x01010101u;
-                const size_t po = (size_t)p * (size_t)S;
-                __stcs(reinterpret_cast<uint4 *>(oa + 2 * po + 128 * i), xa);
-                __stcs(reinterpret_cast<uint2 *>(oo + po + 64 * i), xo);
-                __stcs(reinterpret_cast<uint2 *>(ot + po + 64 * i), xt);
-                __stcs(reinterpret_cast<uint2 *>(ov + po + 64 * i), xv);
+            for (int k = 0; k < EB; ++k)
+                if (i0 + k < nit) a[k] = __ldcg(reinterpret_cast<const uint4 *>(ga + 128 * (i0 + k)));
+#pragma unroll
+            for (int k = 0; k < EB; ++k) {
+                if (i0 + k >= nit) break;
+                const int i = i0 + k;
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    if (p >= P) break;
+                    const uint32_t vb = sv[4 * BW * p + 8 * i];
+                    const uint32_t s0 = nib_sign(vb & 15u), s1 = nib_sign(vb >> 4);
+                    uint4 xa;
+                    xa.x = a[k].x & prmt(s0, 0u, 0x9988u); xa.y = a[k].y & prmt(s0, 0u, 0xBBAAu);
+                    xa.z = a[k].z & prmt(s1, 0u, 0x9988u); xa.w = a[k].w & prmt(s1, 0u, 0xBBAAu);
+                    __stcs(reinterpret_cast<uint4 *>(oa + 2 * (size_t)p * (size_t)S + 128 * i), xa);
+                }
+            }
+            // ---- pass B: owner, terrain, visibility
+            uint2 o[EB], t[EB];
+#pragma unroll
+            for (int k = 0; k < EB; ++k)
+                if (i0 + k < nit) {
+                    o[k] = __ldcg(reinterpret_cast<const uint2 *>(go + 64 * (i0 + k)));
+                    t[k] = __ldcg(reinterpret_cast<const uint2 *>(gt + 64 * (i0 + k)));
+                }
+#pragma unroll
+            for (int k = 0; k < EB; ++k) {
+                if (i0 + k >= nit) break;
+                const int i = i0 + k;
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    if (p >= P) break;
+                    const uint32_t vb = sv[4 * BW * p + 8 * i];
+                    const uint32_t m0 = prmt(nib_sign(vb & 15u), 0u, 0xBA98u), m1 = prmt(nib_sign(vb >> 4), 0u, 0xBA98u);
+                    uint2 xo, xt, xv;
+                    xo.x = (o[k].x & m0) | (~m0 & 0xFEFEFEFEu); xo.y = (o[k].y & m1) | (~m1 & 0xFEFEFEFEu);
+                    xt.x = (t[k].x & m0) | (~m0 & 0x04040404u); xt.y = (t[k].y & m1) | (~m1 & 0x04040404u);
+                    xv.x = m0 & 0x01010101u; xv.y = m1 & 0x01010101u;
+                    const size_t po = (size_t)p * (size_t)S;
+                    __stcs(reinterpret_cast<uint2 *>(oo + po + 64 * i), xo);
+                    __stcs(reinterpret_cast<uint2 *>(ot + po + 64 * i), xt);
+                    __stcs(reinterpret_cast<uint2 *>(ov + po + 64 * i), xv);
+                }
             }
         }
     };
@@ -664,7 +728,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     // ================================================================ the turn
     const uint32_t gstep = kp.global_step0;
     bool frozen = false;
+#ifdef GEN_EXP_NO_RULES
+    if (false) {
+#else
     if (gvalid) {
+#endif
         StepGame &gs = s_game[sub];
         frozen = !kp.auto_reset && gs.done != 0;  // R31
         int a = 0;
@@ -678,17 +746,22 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         }
     }
     __syncwarp();
+    GEN_TRACE_MARK(2);  // sampler
+#ifndef GEN_EXP_NO_RULES
     if (gvalid && ol == 0) {
         if (frozen) s_game[sub].flags |= SG_FROZEN;
         else play_moves(sub);
     }
+#endif
     __syncwarp();
+    GEN_TRACE_MARK(3);  // moves
     if (gvalid) {
         const uint32_t gf = s_game[sub].flags;
         if (gf & SG_GROW_TICK) grow_tick(sub);
         else if (gf & SG_GROW_EVEN) grow_structures(sub);
     }
     __syncwarp();
+    GEN_TRACE_MARK(4);  // growth
     bool want_reset = false;
     if (gvalid && ol == 0) {
         StepGame &gs = s_game[sub];
@@ -702,10 +775,15 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
             if ((rs >> (lg * LPG)) & 1u) regenerate(lg);
     }
     __syncwarp();
+    GEN_TRACE_MARK(5);  // end of turn (+ regeneration)
     // ---- a10 + a11 (R32: the state at the end of the call)
+#ifndef GEN_EXP_NO_EMIT
     if (gvalid) compute_vis(sub);
     __syncwarp();
+    GEN_TRACE_MARK(6);  // fog
     if (gvalid) emit_planes(sub);
+    GEN_TRACE_MARK(7);  // emit
+#endif
 
     // ================================================================ store: cache rows and scalars
     if (gvalid) {
@@ -721,6 +799,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         }
         if (ol == (P & 7)) { B.turn[g] = gs.turn; B.alive[g] = (uint8_t)gs.alive; }
     }
+    GEN_TRACE_MARK(8);  // store
 }
 
 }  // namespace gen

@@ -44,3 +44,12 @@ cudaError_t GEN_CAT(launch_variant_, GEN_VARIANT_ID)(const KParams &kp, int grid
 }
 
 }  // namespace gen
+
+#ifdef GEN_TRACE  // development only
+extern "C" int GEN_CAT(gen_debug_trace_, GEN_VARIANT_ID)(unsigned long long *out) {
+    cudaMemcpyFromSymbol(out, gen::g_trace, sizeof(gen::g_trace));
+    unsigned long long zero[32] = {0};
+    cudaMemcpyToSymbol(gen::g_trace, zero, sizeof(zero));
+    return 0;
+}
+#endif
