@@ -31,7 +31,7 @@ WORKLOAD = "c2_24x24"
 HBM_FALLBACK_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of one gen_step launch, by games per launch, from the
 # `ncu --set full` capture summarised in profiles/ (see profiles/README.md); None where not captured
-NCU_DRAM_BYTES_PER_LAUNCH = {}
+NCU_DRAM_BYTES_PER_LAUNCH = {16384: 104331008}       # profiles/r01_step_full_summary.txt
 
 
 def algorithmic_bytes_per_env_step(H, W, P):
@@ -197,7 +197,7 @@ def run_ours(args):
     barrier()
     launches = sum(e.launch_count for e in envs) - launches0
     total_ms = max_over_ranks(e0.elapsed_time(e1))
-    specialised = env.last_launch_specialised
+    specialised, reg_resident = env.last_launch_specialised, env.last_launch_register_resident
 
     # ---- the same with a 256 MB L2-flush write before every launch and one event pair per launch
     # (isolated launches: includes the launch latency a back-to-back stream hides)
@@ -251,7 +251,7 @@ def run_ours(args):
     launch_ms = total_ms / K
     achieved = N * bmin / (launch_ms * 1e-3) / 1e9
     traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(N)
-    kname = f"gen::k_generals<{P}, {H}, {W}, F_OBS_PLANES | F_K1>" if specialised else "gen::k_generals (generic)"
+    kname = ("gen::k_step" if reg_resident else "gen::k_generals") + (f"<{P}, {H}, {W}>" if specialised else " (generic)")
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
