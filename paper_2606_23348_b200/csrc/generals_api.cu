@@ -120,10 +120,11 @@ void layout_step(gen::KParams &k, int WPC) {
     k.smem_bytes = k.off_warp0 + (uint32_t)WPC * k.warp_bytes;
 }
 
+constexpr long kSMs = 148;  // B200
 using gen::F_RUNTIME;
 using gen::FF_ROLL_DIGEST;
 const gen::Variant kVariants[gen::N_VARIANTS] = {
-#define GEN_ROW(id, kind, np, h, w, ff, maxt, minb) {kind, np, h, w, ff, maxt, gen::launch_variant_##id},
+#define GEN_ROW(id, kind, np, h, w, ff, maxt, minb) {kind, np, h, w, ff, maxt, minb, gen::launch_variant_##id},
     GEN_VARIANTS(GEN_ROW)
 #undef GEN_ROW
 };
@@ -133,7 +134,7 @@ const gen::Variant kVariants[gen::N_VARIANTS] = {
 // (and, for the staged kernel, the exact mode) first, else the generic kernel of the smallest NP >= P.
 const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, bool step_ok) {
     const int kind = step_ok ? 1 : 0;
-    const gen::Variant *generic = nullptr;
+    const gen::Variant *generic = nullptr, *exact = nullptr;
     for (const gen::Variant &v : kVariants) {
         if (v.kind != kind) continue;
         if (v.h == 0) {
@@ -143,8 +144,14 @@ const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, boo
         if (env->force_generic || v.np != kp.P || v.h != kp.H || v.w != kp.W) continue;
         if (v.np == 2 && kp.team_size > 1) continue;
         if (kind == 0 && v.ff != (kp.flags & ~gen::F_SAMPLER)) continue;
-        return &v;
+        if (!exact) { exact = &v; continue; }
+        // the same kernel under two register budgets: the one-wave budget if only it holds the whole batch
+        // resident at once, else the roomier one
+        const long ctas = (kp.N + 2 * gen::GW - 1) / (2 * gen::GW);
+        const bool fits_v = ctas <= (long)v.min_ctas * kSMs, fits_e = ctas <= (long)exact->min_ctas * kSMs;
+        if (fits_v != fits_e ? fits_v : v.min_ctas < exact->min_ctas) exact = &v;
     }
+    if (exact) return exact;
     return generic;
 }
 

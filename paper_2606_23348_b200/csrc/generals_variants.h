@@ -26,13 +26,18 @@ constexpr uint32_t FF_ROLL_DIGEST = F_OBS_PLANES | F_DIGEST;     // gen_rollout(
     X(7, 1, 2, 24, 24, 0, 64, 14)                \
     X(8, 1, 2, 8, 8, 0, 64, 16)                  \
     X(9, 1, 4, 32, 32, 0, 64, 8)                 \
-    X(10, 1, 8, 32, 32, 0, 64, 6)
-constexpr int N_VARIANTS = 11;
+    X(10, 1, 8, 32, 32, 0, 64, 6)                \
+    X(11, 1, 2, 24, 24, 0, 64, 10)
+constexpr int N_VARIANTS = 12;
+// Variants 7 and 11 are the same kernel under two register budgets: 72 registers (14 CTAs of 8 games per SM:
+// a batch of up to 16,576 games -- BASELINE config 2's 16,384 -- is resident in ONE wave) and 96 registers (10 CTAs
+// per SM, no spills: faster per wave, the choice whenever the batch fits 10 CTAs per SM or needs several waves anyway).
 
 struct Variant {
     int kind, np, h, w;  // h == 0: any board with n_players <= np
     uint32_t ff;         // kind 0: F_RUNTIME = any mode, else the exact mode
     int max_threads;     // largest CTA this instantiation may be launched with
+    int min_ctas;        // resident CTAs per SM its register budget allows (launch bounds)
     cudaError_t (*launch)(const KParams &, int grid, int block, size_t smem, cudaStream_t);
 };
 
