@@ -289,6 +289,84 @@ def run_ours(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------ batch sweep
+def time_steps(torch, envs, K, warm, graph):
+    """K gen_step launches back to back, replica t % R at launch t; returns ms.  graph=True replays them as one
+    CUDA graph (host launch cost out of the picture: what matters at small N)."""
+    R = len(envs)
+    for t in range(warm):
+        envs[t % R].step()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    if graph:
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        with torch.cuda.graph(g, stream=side):
+            for t in range(K):
+                envs[t % R].step()
+        torch.cuda.synchronize()
+        e0.record()
+        g.replay()
+        e1.record()
+    else:
+        e0.record()
+        for t in range(K):
+            envs[t % R].step()
+        e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def run_sweep(args):
+    """BASELINE config 3 (batch sweep, per-step kernel vs fused K = 32 rollout) plus per-step rows for configs
+    4 and 5: one JSON line per row.  Not the driver's contract line; its results are copied into BASELINE.md."""
+    import torch
+    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, workloads
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, _ = measured_peak()
+    rows = [("c3_sweep", n) for n in (1024, 16384, 262144, 1048576)]
+    rows += [("c4_curriculum", 65536), ("c5a_2v2", 32768), ("c5b_ffa8", 32768)]
+    for name, N in rows:
+        cfg, _ = workloads.config(name, n_games=N)
+        P, H, W = cfg["n_players"], cfg["height"], cfg["width"]
+        bmin = algorithmic_bytes_per_env_step(H, W, P)
+        R = max(2, -(-(640 << 20) // (N * bmin)))
+        K = max(32, min(args.steps, (1 << 31) // (N * bmin) * 4))
+        envs = [GeneralsEnv(dict(cfg, game_id_base=r * N), device=dev, digest=False, actions_out=False) for r in range(R)]
+        for e in envs:
+            e.reset()
+        out = {"workload": name, "n_games": N, "n_players": P, "board": f"{H}x{W}", "replicas_in_rotation": R,
+               "steps": K, "algorithmic_bytes_per_env_step": bmin}
+        for graph in (False, True):
+            ms = time_steps(torch, envs, K, max(args.warmup, R), graph)
+            key = "step_graph" if graph else "step"
+            out[key] = {"env_steps_per_s": N * K / (ms * 1e-3), "us_per_launch": 1e3 * ms / K,
+                        "hbm_frac": N * bmin / (ms / K * 1e-3) / 1e9 / peak}
+        out["kernel"] = ("k_step" if envs[0].last_launch_register_resident else "k_generals") + \
+                        ("" if envs[0].last_launch_specialised else " (generic)")
+        del envs
+        torch.cuda.empty_cache()
+        if name == "c3_sweep":
+            renv = GeneralsEnv(cfg, device=dev, digest=True, actions_out=False)
+            renv.reset()
+            renv.rollout(32, OBS_DIGEST)
+            n_roll = max(2, K // 32)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(n_roll):
+                renv.rollout(32, OBS_DIGEST)
+            e1.record()
+            torch.cuda.synchronize()
+            out["rollout_K32_digest"] = {"env_steps_per_s": N * 32 * n_roll / (e0.elapsed_time(e1) * 1e-3),
+                                         "us_per_launch": 1e3 * e0.elapsed_time(e1) / n_roll}
+            del renv
+            torch.cuda.empty_cache()
+        print(json.dumps(out), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -298,8 +376,11 @@ def main():
     ap.add_argument("--games", type=int, default=0, help="override games per GPU (default: config 2's 16,384)")
     ap.add_argument("--replicas", type=int, default=0, help="replicas in the round-robin (default: enough for 640 MB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.sweep:
+        return run_sweep(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 

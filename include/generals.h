@@ -188,7 +188,9 @@ int gen_set_launch(gen_env *env, int32_t games_per_cta);
  * and without a digest buffer, uniform policy), each as a generic instantiation for every board up to
  * 32x32 and as instantiations compiled for the paper-sized configurations (1v1 8x8 and 24x24, 4 and 8
  * players on 32x32).  force_generic != 0: never launch a board-specialised instantiation;
- * force_staged != 0: never launch the register-resident kernel.  Results do not depend on either. */
+ * force_staged == 1: never launch the register-resident kernel; force_staged == -1: launch it
+ * whenever it can serve the call (by default games with more than 4 players stay on the staged kernel, which
+ * is faster for them).  Results do not depend on either. */
 int gen_set_generic(gen_env *env, int32_t force_generic, int32_t force_staged);
 
 /* Which instantiation the last launch of this handle used: returns its index in the library's variant

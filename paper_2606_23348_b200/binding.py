@@ -218,8 +218,9 @@ class GeneralsEnv:
         self._check(self.lib.gen_set_launch(self._env, int(games_per_cta)))
 
     def set_generic(self, force_generic=True, force_staged=False):
-        """Test hooks: never launch a board-specialised / the register-resident kernel."""
-        self._check(self.lib.gen_set_generic(self._env, 1 if force_generic else 0, 1 if force_staged else 0))
+        """Test hooks: never launch a board-specialised / the register-resident kernel (force_staged=-1:
+        launch the register-resident kernel wherever it can serve, also for more than 4 players)."""
+        self._check(self.lib.gen_set_generic(self._env, 1 if force_generic else 0, int(force_staged)))
 
     @property
     def last_launch_specialised(self):

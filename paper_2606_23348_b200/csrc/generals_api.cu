@@ -16,6 +16,7 @@ struct gen_env {
     int last_cuda_error;
     int32_t force_generic;   // 1: never pick a board-specialised kernel (tests)
     int32_t force_staged;    // 1: never pick the register-resident step kernel (tests)
+    int32_t force_step;      // 1: pick it whenever it can serve the call, also where the staged one is faster (tests)
     int32_t last_variant;    // index into GEN_VARIANTS of the last launch (-1: none yet)
 };
 
@@ -122,6 +123,7 @@ void layout_step(gen::KParams &k, int WPC) {
 
 constexpr long kSMs = 148;  // B200
 using gen::F_RUNTIME;
+using gen::F_OBS_PLANES;
 using gen::FF_ROLL_DIGEST;
 const gen::Variant kVariants[gen::N_VARIANTS] = {
 #define GEN_ROW(id, kind, np, h, w, ff, maxt, minb) {kind, np, h, w, ff, maxt, minb, gen::launch_variant_##id},
@@ -170,8 +172,10 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     kp.sample_out = sample_out;
     // gen_step proper (one turn, planes, no digest) with the bitboard cache and the uniform policy runs the
     // register-resident kernel; everything else the staged one
+    // (more than 4 players: one lane per player in the word passes and 8 x 4 half-written lines per chunk in the
+    // emit pass -- measured 2x the DRAM traffic and half the speed of the staged kernel, so those stay there)
     const bool step_ok = !env->force_staged && K == 1 && bufs->bitboards && kp.bias_thr == 0 &&
-                         (flags & ~gen::F_SAMPLER) == gen::F_OBS_PLANES;
+                         (flags & ~gen::F_SAMPLER) == gen::F_OBS_PLANES && (kp.P <= 4 || env->force_step);
     const gen::Variant *v = pick_variant(env, kp, step_ok);
     if (!v) return GEN_ERR_CONFIG;
     // warps per CTA (4 games each): 2 by default; fewer while the CTA would not fit
@@ -352,7 +356,8 @@ int gen_set_launch(gen_env *env, int32_t games_per_cta) {
 int gen_set_generic(gen_env *env, int32_t force_generic, int32_t force_staged) {
     if (!env) return GEN_ERR_NULL;
     env->force_generic = force_generic ? 1 : 0;
-    env->force_staged = force_staged ? 1 : 0;
+    env->force_staged = force_staged == 1 ? 1 : 0;
+    env->force_step = force_staged == -1 ? 1 : 0;
     return GEN_OK;
 }
 

@@ -12,6 +12,8 @@
 
 namespace gen {
 
+// variant 12: gen_step on the staged kernel at 24x24 1v1 (the biased policy R25 of config 4 scans army values,
+// which only the staged kernel holds on chip)
 constexpr uint32_t FF_ROLL_DIGEST = F_OBS_PLANES | F_DIGEST;     // gen_rollout(K, GEN_OBS_DIGEST)
 
 //  X(id, kind, NP, H, W, flags (kind 0) or 0, max threads per CTA, min CTAs per SM (kind 1))
@@ -27,8 +29,9 @@ constexpr uint32_t FF_ROLL_DIGEST = F_OBS_PLANES | F_DIGEST;     // gen_rollout(
     X(8, 1, 2, 8, 8, 0, 64, 16)                  \
     X(9, 1, 4, 32, 32, 0, 64, 8)                 \
     X(10, 1, 8, 32, 32, 0, 64, 6)                \
-    X(11, 1, 2, 24, 24, 0, 64, 10)
-constexpr int N_VARIANTS = 12;
+    X(11, 1, 2, 24, 24, 0, 64, 10)               \
+    X(12, 0, 2, 24, 24, F_OBS_PLANES, 256, 1)
+constexpr int N_VARIANTS = 13;
 // Variants 7 and 11 are the same kernel under two register budgets: 72 registers (14 CTAs of 8 games per SM:
 // a batch of up to 16,576 games -- BASELINE config 2's 16,384 -- is resident in ONE wave) and 96 registers (10 CTAs
 // per SM, no spills: faster per wave, the choice whenever the batch fits 10 CTAs per SM or needs several waves anyway).

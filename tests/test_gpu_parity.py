@@ -139,8 +139,9 @@ def test_specialised_step_kernels_match_oracle(gpu, oracle_mod, name, N, T, over
     instantiation and the staged kernel must agree too."""
     cfg, _ = workloads.config(name, n_games=N, **over)
     env = gpu.GeneralsEnv(cfg, digest=False)
+    env.set_generic(False, -1)                              # also for 8 players, where the default is the staged kernel
     gen = gpu.GeneralsEnv(cfg, digest=False)
-    gen.set_generic(True, False)
+    gen.set_generic(True, -1)
     stg = gpu.GeneralsEnv(cfg, digest=False, bitboards=False)
     o = oracle_mod.Oracle(cfg)
     for e in (env, gen, stg):
@@ -155,7 +156,7 @@ def test_specialised_step_kernels_match_oracle(gpu, oracle_mod, name, N, T, over
             compare(gen, o, digest=False, where=f"{name} generic step {t}")
             compare(stg, o, digest=False, where=f"{name} staged step {t}")
     uniform = cfg["bias_thr"] == 0                          # the biased policy (R25) runs on the staged kernel
-    assert env.last_launch_specialised == uniform and env.last_launch_register_resident == uniform
+    assert env.last_launch_specialised and env.last_launch_register_resident == uniform
     assert not gen.last_launch_specialised and gen.last_launch_register_resident == uniform
     assert not stg.last_launch_register_resident
     assert int(o.episodes_done.sum()) > 0
