@@ -495,3 +495,68 @@ def test_config2_full_size_sampled_games(gpu, oracle_mod, digest):
                               np.where(owner[:, :576] == p, army[:, :576], 0).astype(np.int64).sum(1))
     vis = env.field("obs_vis")
     assert ((owner[:, None, :] == np.arange(2)[None, :, None]) <= vis.astype(bool)).all()
+
+
+@pytest.mark.parametrize("name,N,T,roll", [
+    ("c3_sweep", 262144, 130, 32),        # config 3: steps interleaved with fused rollouts
+    ("c3_sweep", 1048576, 70, 0),
+    ("c4_curriculum", 65536, 150, 0),     # biased policy: the staged kernel
+    ("c5a_2v2", 32768, 120, 0),
+    ("c5b_ffa8", 32768, 120, 0),
+])
+def test_full_size_configs_sampled_games(gpu, oracle_mod, name, N, T, roll):
+    """BASELINE configs 3, 4, 5 at their full batch sizes, in the launch configuration bench.py --sweep times
+    (bitboard cache, no digest buffer): the oracle replays a sample of global game ids one by one (first /
+    last / strided: a game depends on its global id only, M2) and must agree on every tensor; plus properties
+    that hold at any size."""
+    import torch
+    cfg, _ = workloads.config(name, n_games=N)
+    P, HW = cfg["n_players"], cfg["height"] * cfg["width"]
+    env = gpu.GeneralsEnv(cfg, digest=False, actions_out=False)
+    env.reset()
+    plan = []                                                # the same call sequence on both sides
+    t = 0
+    while t < T:
+        if roll and t % 50 == 10:
+            env.rollout(roll, gpu.OBS_NONE)
+            plan.append(roll)
+            t += roll
+        else:
+            env.step()
+            plan.append(1)
+            t += 1
+    env.step()                                               # a state-only rollout leaves no observation: end on a step
+    plan.append(1)
+    env.torch.cuda.synchronize()
+    ids = sorted(set(list(range(12)) + list(range(N - 12, N)) + list(range(7, N, N // 23))))
+    sel = torch.tensor(ids, device=env.device)
+    fields = [f for f in STATE_FIELDS + OUT_FIELDS]
+    got = {}
+    for f in fields:
+        tns = env.tensors[f]
+        if f in OUT_FIELDS:
+            tns = tns[0]
+        got[f] = tns.index_select(0, sel).cpu().numpy()
+    for k, gid in enumerate(ids):
+        o = oracle_mod.Oracle(dict(cfg, n_games=1, game_id_base=gid))
+        o.reset()
+        for n in plan:
+            if n == 1:
+                o.step()
+            else:
+                o.rollout(n, oracle_mod.OBS_NONE)
+        for f in fields:
+            want = np.asarray(o.field(f))[0]
+            have = got[f][k]
+            if have.dtype != want.dtype:
+                have = have.view(want.dtype)
+            assert np.array_equal(have, want.reshape(have.shape)), (name, gid, f)
+    # properties that hold at any size (all games)
+    owner, army, terrain = env.tensors["owner"][:, :HW], env.tensors["army"][:, :HW], env.tensors["terrain"][:, :HW]
+    assert bool((army >= 0).all()) and bool((owner[terrain == MT] == -1).all())
+    for p in range(P):
+        mine = owner == p
+        assert torch.equal(env.tensors["land"][:, p], mine.sum(1).to(torch.int32))
+        assert torch.equal(env.tensors["army_total"][:, p].to(torch.int64), (army.to(torch.int64) * mine).sum(1))
+        assert bool((env.tensors["obs_vis"][0, :, p, :HW][mine] == 1).all())      # fog: vis contains owned (I5)
+    assert int(env.tensors["episodes_done"].sum()) >= 0
