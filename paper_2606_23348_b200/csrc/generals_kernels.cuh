@@ -195,6 +195,10 @@ __device__ __forceinline__ void l2_prefetch(const void *src, uint32_t bytes) {  
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes)
                  : "memory");
 }
+// programmatic dependent launch: let the next grid in the stream start being placed / wait until everything the
+// previous grid wrote is visible
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t ok;
     do {
@@ -458,6 +462,8 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         for (int c = tid; c < S; c += blockDim.x)
             s_key[c] = (c < HW) ? (mix64((uint64_t)(c + 1) * 0x9E3779B97F4A7C15ull) | 1ull) : 0ull;
     }
+    pdl_launch_dependents();
+    pdl_wait();
     const bool loading = !(flags & F_RESET) && nwg > 0;
     if (loading && lane == 0) {
         mbar_init(bar, 1);

@@ -212,6 +212,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         s_ncL[j] = in ? kp.notcolL[j & 31] : 0u;
         s_inb[j] = in ? kp.inb[j & 31] : 0u;
     }
+    pdl_launch_dependents();  // the next launch may be placed as CTAs of this one retire ...
+    pdl_wait();               // ... and nothing of the previous launch is read before it has completed
     if (nwg > 0 && lane == 0) {
         mbar_init(bar, 1);
         const uint32_t bytes = (uint32_t)nwg * (uint32_t)(P + 3) * (uint32_t)BW * 4u;

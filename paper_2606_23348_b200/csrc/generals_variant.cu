@@ -39,8 +39,20 @@ cudaError_t GEN_CAT(launch_variant_, GEN_VARIANT_ID)(const KParams &kp, int grid
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    kernel<<<grid, block, smem, stream>>>(kp);
-    return cudaGetLastError();
+    // Programmatic dependent launch: the CTAs of this grid may be placed while the previous grid in the stream
+    // drains; both kernels execute griddepcontrol.wait before their first global access, so the overlap is
+    // launch latency and prologue only.
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, kp);
 }
 
 }  // namespace gen
