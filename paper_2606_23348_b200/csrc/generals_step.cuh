@@ -506,7 +506,21 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
             bool changed = false;
             for (int p = 0; p < P; ++p) {
                 uint32_t m = sw & row(p, lg)[j];
+                if (m == 0) continue;
                 int inc = 0;
+                // Fast path, no load: a cell of a player whose whole army is below 32767 cannot saturate, and a cell
+                // with army >= 2 keeps its bit: +1 as a fire-and-forget reduction on the 32-bit word that holds it.
+                if (gs.tot[p] <= 32766) {
+                    uint32_t f = m & a2w;
+                    m &= ~a2w;
+                    inc = __popc(f);
+                    while (f) {
+                        const int b = __ffs(f) - 1;
+                        f &= f - 1;
+                        const int c = 32 * j + b;
+                        atomicAdd(reinterpret_cast<unsigned int *>(A + (c & ~1)), (c & 1) ? 0x10000u : 1u);
+                    }
+                }
                 while (m) {
                     const int b = __ffs(m) - 1;
                     m &= m - 1;
