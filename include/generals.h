@@ -113,7 +113,7 @@ typedef struct gen_buffers {
 } gen_buffers;
 
 /* `bitboards` caches what the rules need of the three planes as one bit per cell (bit c & 31 of word
- * c >> 5; BW = gen_sizes.bitboard_row_words = ceil(H*W / 32) rounded up to 4 words): rows 0..P-1 "owned by
+ * c >> 5; BW = gen_sizes.bitboard_row_words = ceil(H*W / 32) rounded up to 8 words, so that every row is a whole number of 32-byte sectors): rows 0..P-1 "owned by
  * player p", row P "army >= 2", row P+1 "city or general", row P+2 "mountain or off the board" (all ones
  * past H*W).  gen_reset and gen_observe build it from the planes; gen_step and gen_rollout keep it
  * current.  With it, gen_step without a digest buffer runs the register-resident per-step kernel, which

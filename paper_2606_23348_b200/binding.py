@@ -59,7 +59,7 @@ BUFFERS = [
     ("sat_events", "int32", lambda N, P, S, K: (N,)),
     ("obs_digest", "int64", lambda N, P, S, K: (N,)),         # bits of uint64
     ("actions_out", "int32", lambda N, P, S, K: (K, N, P)),
-    ("bitboards", "int32", lambda N, P, S, K: (N, P + 3, (-(-S // 32) + 3) // 4 * 4)),   # bits of uint32
+    ("bitboards", "int32", lambda N, P, S, K: (N, P + 3, (-(-S // 32) + 7) // 8 * 8)),   # bits of uint32
 ]
 
 

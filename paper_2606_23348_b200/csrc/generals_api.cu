@@ -55,7 +55,7 @@ void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
     s->obs_vis = k * N * P * S;
     s->episodes_done = N * 4; s->wins = N * P * 4; s->truncations = N * 4; s->sat_events = N * 4;
     s->obs_digest = N * 8; s->actions_out = k * N * P * 4;
-    const size_t BW = (size_t)round_up((c->height * c->width + 31) / 32, 4);
+    const size_t BW = (size_t)round_up((c->height * c->width + 31) / 32, 8);
     s->bitboard_row_words = (int32_t)BW;
     s->bitboards = N * (P + 3) * BW * 4;
 }
@@ -230,7 +230,7 @@ int gen_init(const gen_config *cfg, gen_env **out) {
     gen::KParams &k = env->base;
     k.N = cfg->n_games; k.H = cfg->height; k.W = cfg->width; k.P = cfg->n_players;
     k.HW = k.H * k.W; k.S = round_up(k.HW, 16); k.NW = (k.HW + 31) / 32; k.NC8 = k.S / 8;
-    k.NCH = 4 * k.NW; k.RW = k.NW | 1; k.M = 2 * k.P + 7; k.BW = round_up(k.NW, 4);
+    k.NCH = 4 * k.NW; k.RW = k.NW | 1; k.M = 2 * k.P + 7; k.BW = round_up(k.NW, 8);
     k.team_size = cfg->team_size;
     k.n_teams = (cfg->n_players + cfg->team_size - 1) / cfg->team_size;
     k.n_cities = cfg->n_cities; k.city_lo = cfg->city_army_lo;

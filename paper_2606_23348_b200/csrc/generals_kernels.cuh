@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     const int HW = FIXED ? cHW : kp.HW, S = FIXED ? cS : kp.S, NW = FIXED ? cNW : kp.NW;
     const int NC8 = FIXED ? cS / 8 : kp.NC8, NCH = FIXED ? 4 * cNW : kp.NCH;
     const int RW = FIXED ? (cNW | 1) : kp.RW, M = FIXED ? 2 * NP + 7 : kp.M;
-    const int BW = FIXED ? (cNW + 3) / 4 * 4 : kp.BW;
+    const int BW = FIXED ? (cNW + 7) / 8 * 8 : kp.BW;
     const int WS = (NW + LPP - 1) / LPP;  // words per sub-lane
     const uint32_t flags = (FF == F_RUNTIME) ? kp.flags : ((FF & ~F_K1) | (kp.flags & F_SAMPLER));
     const int K = (FF != F_RUNTIME && (FF & F_K1)) ? 1 : kp.K;

@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     const int H = FIXED ? CH : kp.H, W = FIXED ? CW : kp.W, P = FIXED ? NP : kp.P;
     const int HW = FIXED ? cHW : kp.HW, S = FIXED ? cS : kp.S, NW = FIXED ? cNW : kp.NW;
     const int NC8 = FIXED ? cS / 8 : kp.NC8;
-    const int BW = FIXED ? (cNW + 3) / 4 * 4 : kp.BW;
+    const int BW = FIXED ? (cNW + 7) / 8 * 8 : kp.BW;
     const int WS = (NW + LPP - 1) / LPP;
     const uint32_t flags = kp.flags;  // F_SAMPLER is the only mode bit this kernel looks at
     const gen_buffers &B = kp.b;
@@ -744,11 +744,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     // ================================================================ the turn
     const uint32_t gstep = kp.global_step0;
     bool frozen = false;
-#ifdef GEN_EXP_NO_RULES
-    if (false) {
-#else
     if (gvalid) {
-#endif
         StepGame &gs = s_game[sub];
         frozen = !kp.auto_reset && gs.done != 0;  // R31
         int a = 0;
@@ -763,12 +759,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     }
     __syncwarp();
     GEN_TRACE_MARK(2);  // sampler
-#ifndef GEN_EXP_NO_RULES
     if (gvalid && ol == 0) {
         if (frozen) s_game[sub].flags |= SG_FROZEN;
         else play_moves(sub);
     }
-#endif
     __syncwarp();
     GEN_TRACE_MARK(3);  // moves
     if (gvalid) {
@@ -792,16 +786,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     }
     __syncwarp();
     GEN_TRACE_MARK(5);  // end of turn (+ regeneration)
-    // ---- a10 + a11 (R32: the state at the end of the call)
-#ifndef GEN_EXP_NO_EMIT
-    if (gvalid) compute_vis(sub);
-    __syncwarp();
-    GEN_TRACE_MARK(6);  // fog
-    if (gvalid) emit_planes(sub);
-    GEN_TRACE_MARK(7);  // emit
-#endif
-
-    // ================================================================ store: cache rows and scalars
+    // ---- store the cache rows and scalars now: they are final, and after the emit pass the warp can retire at once
     if (gvalid) {
         const StepGame &gs = s_game[sub];
         const int nrows = (gs.flags & SG_STATIC_DIRTY) ? P + 3 : P + 1;  // own[p] + army >= 2 (+ structure, mountain)
@@ -815,6 +800,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         }
         if (ol == (P & 7)) { B.turn[g] = gs.turn; B.alive[g] = (uint8_t)gs.alive; }
     }
+    // ---- a10 + a11 (R32: the state at the end of the call)
+    if (gvalid) compute_vis(sub);
+    __syncwarp();
+    GEN_TRACE_MARK(6);  // fog
+    if (gvalid) emit_planes(sub);
+    GEN_TRACE_MARK(7);  // emit
+
     GEN_TRACE_MARK(8);  // store
 }
 

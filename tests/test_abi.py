@@ -42,7 +42,7 @@ def test_query_sizes(lib):
     assert s.army == N * S * 2 and s.owner == N * S and s.terrain == N * S
     assert s.obs_army == N * P * S * 2 and s.obs_vis == N * P * S
     assert s.reward == N * P and s.done == N and s.obs_digest == 8 * N
-    assert s.bitboard_row_words == 20 and s.bitboards == N * (P + 3) * 20 * 4       # ceil(576 / 32) = 18 -> 20
+    assert s.bitboard_row_words == 24 and s.bitboards == N * (P + 3) * 24 * 4       # ceil(576 / 32) = 18 -> 24
     assert lib.gen_query_sizes(C.byref(cfg), 32, C.byref(s)) == 0
     assert s.obs_owner == 32 * N * P * S and s.army == N * S * 2
     cfg5, _ = binding.make_config(workloads.config("c1_8x8", height=5, width=7)[0])
