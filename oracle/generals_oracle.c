@@ -70,6 +70,7 @@ typedef struct {
     uint32_t *truncations;    /* [N] */
     uint32_t *sat_events;     /* [N] */
     uint64_t *obs_digest;     /* [N] or NULL */
+    uint8_t *obs_packed;      /* [N][P][S] or NULL: owner, terrain and visibility in one byte (R33) */
 } orc_buffers;
 
 /* ------------------------------------------------------------------ Philox
@@ -244,6 +245,10 @@ static void observe(const orc_config *cfg, const orc_buffers *b, int g, size_t o
             b->obs_owner[o + c] = vis ? owner[c] : (int8_t)OWNER_FOG;
             b->obs_terrain[o + c] = vis ? terrain[c] : (int8_t)T_FOG;
             b->obs_vis[o + c] = (uint8_t)vis;
+            /* R33: the three byte planes in one byte.  Visible: bit 7 set, bits 4-5 the
+             * terrain, bits 0-3 owner + 2 (1 = neutral, 2.. = player 0..); fogged: 0. */
+            if (b->obs_packed)
+                b->obs_packed[o + c] = vis ? (uint8_t)(0x80 | (terrain[c] << 4) | (owner[c] + 2)) : (uint8_t)0;
         }
     }
 }
@@ -487,6 +492,7 @@ int32_t orc_rollout(const orc_config *cfg, const orc_buffers *b, int32_t K, uint
         orc_buffers v = *b;
         v.obs_army += (size_t)k * N * P * S; v.obs_owner += (size_t)k * N * P * S;
         v.obs_terrain += (size_t)k * N * P * S; v.obs_vis += (size_t)k * N * P * S;
+        if (v.obs_packed) v.obs_packed += (size_t)k * N * P * S;
         v.reward += (size_t)k * N * P; v.done += (size_t)k * N; v.winner += (size_t)k * N;
         if (k > 0) {                                           /* carry the frozen game's flags forward */
             memcpy(v.done, v.done - N, (size_t)N);

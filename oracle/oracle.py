@@ -43,7 +43,7 @@ _BUF_FIELDS = [
     ("army_total", np.int32), ("reward", np.int8), ("done", np.uint8), ("winner", np.int8),
     ("obs_army", np.int16), ("obs_owner", np.int8), ("obs_terrain", np.int8), ("obs_vis", np.uint8),
     ("episodes_done", np.uint32), ("wins", np.uint32), ("truncations", np.uint32),
-    ("sat_events", np.uint32), ("obs_digest", np.uint64),
+    ("sat_events", np.uint32), ("obs_digest", np.uint64), ("obs_packed", np.uint8),
 ]
 
 
@@ -122,7 +122,7 @@ class Oracle:
             "reward": (Kb, N, P), "done": (Kb, N), "winner": (Kb, N),
             "obs_army": (Kb, N, P, S), "obs_owner": (Kb, N, P, S), "obs_terrain": (Kb, N, P, S),
             "obs_vis": (Kb, N, P, S), "episodes_done": (N,), "wins": (N, P), "truncations": (N,),
-            "sat_events": (N,), "obs_digest": (N,),
+            "sat_events": (N,), "obs_digest": (N,), "obs_packed": (Kb, N, P, S),
         }
         self.bufs = OrcBuffers()
         for name, dt in _BUF_FIELDS:
@@ -138,7 +138,7 @@ class Oracle:
     def field(self, name):
         a = getattr(self, name)
         return a[0] if name in ("reward", "done", "winner", "obs_army", "obs_owner", "obs_terrain",
-                                "obs_vis") else a
+                                "obs_vis", "obs_packed") else a
 
     def reset(self):
         lib().orc_reset(C.byref(self.cfg), C.byref(self.bufs))

@@ -596,3 +596,29 @@ def test_digest_definition(oracle_mod):
         o.step()
         d = chain(d)
         assert [int(x) for x in o.obs_digest] == d
+
+
+@pytest.mark.parametrize("name,N,T,over", [
+    ("c2_24x24", 12, 120, dict(max_turns=60, spawn_dmin=4)),
+    ("c5b_ffa8", 6, 80, dict(height=12, width=12, spawn_dmin=3, n_cities=4, max_turns=50)),
+])
+def test_R33_packed_plane_decodes_to_the_three_byte_planes(oracle_mod, name, N, T, over):
+    """R33 (NEXT-4): the packed byte is visible << 7 | terrain << 4 | (owner + 2), 0 under fog.  Decoding it here,
+    independently, must give back obs_owner / obs_terrain / obs_vis on every cell of sampled play."""
+    cfg, _ = workloads.config(name, n_games=N, **over)
+    o = oracle_mod.Oracle(cfg)
+    o.reset()
+    seen_fog = seen_enemy = False
+    for t in range(T):
+        o.step()
+        b = o.field("obs_packed").astype(np.int32)
+        vis = b >> 7
+        owner = np.where(vis == 1, (b & 15) - 2, -2)
+        terrain = np.where(vis == 1, (b >> 4) & 3, 4)
+        assert np.array_equal(vis, o.field("obs_vis"))
+        assert np.array_equal(owner, o.field("obs_owner"))
+        assert np.array_equal(terrain, o.field("obs_terrain"))
+        assert ((b & 0x40) == 0).all() and (b[vis == 0] == 0).all()
+        seen_fog |= bool((vis == 0).any())
+        seen_enemy |= bool(((owner >= 0) & (owner != np.arange(o.P)[None, :, None])).any())
+    assert seen_fog and seen_enemy
