@@ -110,7 +110,13 @@ typedef struct gen_buffers {
     uint64_t *obs_digest;    /* state [N]   may be NULL for gen_reset / gen_step (no digest then) */
     int32_t *actions_out;    /* out   [K][N][P]  the actions actually applied; may be NULL */
     uint32_t *bitboards;     /* state [N][P+3][BW]  derived cache, may be NULL (see below) */
+    uint8_t *obs_packed;     /* out   [K][N][P][S]  packed observation, may be NULL (see below) */
 } gen_buffers;
+
+/* `obs_packed` (R33) selects the 3-byte-per-cell observation format: when it is non-NULL
+ * every call writes obs_army and obs_packed and does NOT write obs_owner / obs_terrain / obs_vis (which may
+ * then be NULL).  One byte per cell and player: visible -> 0x80 | terrain << 4 | (owner + 2) (owner + 2: 1 =
+ * neutral, 2.. = player 0..); fogged -> 0.  Observation traffic drops from 5 to 3 bytes per cell and player. */
 
 /* `bitboards` caches what the rules need of the three planes as one bit per cell (bit c & 31 of word
  * c >> 5; BW = gen_sizes.bitboard_row_words = ceil(H*W / 32) rounded up to 8 words, so that every row is a whole number of 32-byte sectors): rows 0..P-1 "owned by
@@ -126,7 +132,7 @@ typedef struct gen_sizes {
     int32_t alignment;       /* 16 */
     size_t army, owner, terrain, turn, episode, alive, general_cell, land, army_total;
     size_t reward, done, winner, obs_army, obs_owner, obs_terrain, obs_vis;
-    size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out, bitboards;
+    size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out, bitboards, obs_packed;
     int32_t bitboard_row_words; /* BW */
 } gen_sizes;
 

@@ -60,6 +60,7 @@ BUFFERS = [
     ("obs_digest", "int64", lambda N, P, S, K: (N,)),         # bits of uint64
     ("actions_out", "int32", lambda N, P, S, K: (K, N, P)),
     ("bitboards", "int32", lambda N, P, S, K: (N, P + 3, (-(-S // 32) + 7) // 8 * 8)),   # bits of uint32
+    ("obs_packed", "uint8", lambda N, P, S, K: (K, N, P, S)),
 ]
 
 
@@ -145,7 +146,8 @@ class GeneralsEnv:
     k_slots > 1 sizes the output buffers for rollout(K, OBS_EVERY_STEP).
     """
 
-    def __init__(self, cfg, device="cuda:0", k_slots=1, digest=True, actions_out=True, bitboards=True):
+    def __init__(self, cfg, device="cuda:0", k_slots=1, digest=True, actions_out=True, bitboards=True,
+                 packed=False):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -165,7 +167,8 @@ class GeneralsEnv:
         self.tensors = {}
         for name, dt, shape in BUFFERS:
             if ((name == "obs_digest" and not digest) or (name == "actions_out" and not actions_out)
-                    or (name == "bitboards" and not bitboards)):
+                    or (name == "bitboards" and not bitboards) or (name == "obs_packed" and not packed)
+                    or (packed and name in ("obs_owner", "obs_terrain", "obs_vis"))):
                 setattr(self.bufs, name, None)
                 continue
             t = torch.zeros(shape(self.N, self.P, self.S, self.K), dtype=getattr(torch, dt), device=self.device)
@@ -280,7 +283,8 @@ class GeneralsEnv:
         """numpy view of a buffer (unsigned where the C type is unsigned); slot 0 of [K]-strided ones."""
         import numpy as np
         t = self.tensors[name]
-        if name in ("reward", "done", "winner", "obs_army", "obs_owner", "obs_terrain", "obs_vis", "actions_out"):
+        if name in ("reward", "done", "winner", "obs_army", "obs_owner", "obs_terrain", "obs_vis", "actions_out",
+                    "obs_packed"):
             t = t[slot]
         a = t.cpu().numpy()
         if name in ("episode", "episodes_done", "wins", "truncations", "sat_events"):

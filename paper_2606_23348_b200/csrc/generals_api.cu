@@ -58,6 +58,7 @@ void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
     const size_t BW = (size_t)round_up((c->height * c->width + 31) / 32, 8);
     s->bitboard_row_words = (int32_t)BW;
     s->bitboards = N * (P + 3) * BW * 4;
+    s->obs_packed = k * N * P * S;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -70,10 +71,12 @@ int check_buffers(const gen_buffers *b, bool need_obs) {
         if (!p) return GEN_ERR_NULL;
         if (!aligned16(p)) return GEN_ERR_ALIGN;
     }
-    const void *obs[] = {b->obs_army, b->obs_owner, b->obs_terrain, b->obs_vis};
-    for (const void *p : obs) {
-        if (need_obs && !p) return GEN_ERR_NULL;
-        if (p && !aligned16(p)) return GEN_ERR_ALIGN;
+    // observation: army plus either the packed byte plane (R33) or the three byte planes
+    const void *obs[] = {b->obs_army, b->obs_owner, b->obs_terrain, b->obs_vis, b->obs_packed};
+    for (int i = 0; i < 5; ++i) {
+        const bool needed = need_obs && (i == 0 || (b->obs_packed ? i == 4 : i < 4));
+        if (needed && !obs[i]) return GEN_ERR_NULL;
+        if (obs[i] && !aligned16(obs[i])) return GEN_ERR_ALIGN;
     }
     if (b->obs_digest && !aligned16(b->obs_digest)) return GEN_ERR_ALIGN;
     if (b->actions_out && !aligned16(b->actions_out)) return GEN_ERR_ALIGN;

@@ -883,6 +883,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             unsigned char *go = reinterpret_cast<unsigned char *>(B.obs_owner + base + (size_t)p * S) + 8 * ol;
             unsigned char *gt = reinterpret_cast<unsigned char *>(B.obs_terrain + base + (size_t)p * S) + 8 * ol;
             unsigned char *gv = reinterpret_cast<unsigned char *>(B.obs_vis + base + (size_t)p * S) + 8 * ol;
+            unsigned char *gp = reinterpret_cast<unsigned char *>(B.obs_packed + base + (size_t)p * S) + 8 * ol;
 #pragma unroll 3
             for (int i = 0; i < nit; ++i) {
                 const uint4 a = *reinterpret_cast<const uint4 *>(sa + 128 * i);
@@ -894,11 +895,19 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 uint4 oa;
                 oa.x = a.x & prmt(s0, 0u, 0x9988u); oa.y = a.y & prmt(s0, 0u, 0xBBAAu);
                 oa.z = a.z & prmt(s1, 0u, 0x9988u); oa.w = a.w & prmt(s1, 0u, 0xBBAAu);
+                __stcs(reinterpret_cast<uint4 *>(ga + 128 * i), oa);
+                if (B.obs_packed) {  // R33: 0x80 | terrain << 4 | (owner + 2) under the fog mask
+                    const uint32_t qx = 0x80808080u | ((t.x << 4) & 0x30303030u) |
+                                        (((o.x & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu);
+                    const uint32_t qy = 0x80808080u | ((t.y << 4) & 0x30303030u) |
+                                        (((o.y & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu);
+                    __stcs(reinterpret_cast<uint2 *>(gp + 64 * i), make_uint2(qx & m0, qy & m1));
+                    continue;
+                }
                 uint2 oo, ot, ov;
                 oo.x = (o.x & m0) | (~m0 & 0xFEFEFEFEu); oo.y = (o.y & m1) | (~m1 & 0xFEFEFEFEu);
                 ot.x = (t.x & m0) | (~m0 & 0x04040404u); ot.y = (t.y & m1) | (~m1 & 0x04040404u);
                 ov.x = m0 & 0x01010101u; ov.y = m1 & 0x01010101u;
-                __stcs(reinterpret_cast<uint4 *>(ga + 128 * i), oa);
                 __stcs(reinterpret_cast<uint2 *>(go + 64 * i), oo);
                 __stcs(reinterpret_cast<uint2 *>(gt + 64 * i), ot);
                 __stcs(reinterpret_cast<uint2 *>(gv + 64 * i), ov);

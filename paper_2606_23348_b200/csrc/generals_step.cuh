@@ -688,6 +688,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         unsigned char *__restrict__ oo = reinterpret_cast<unsigned char *>(B.obs_owner + obase) + 8 * ol;
         unsigned char *__restrict__ ot = reinterpret_cast<unsigned char *>(B.obs_terrain + obase) + 8 * ol;
         unsigned char *__restrict__ ov = reinterpret_cast<unsigned char *>(B.obs_vis + obase) + 8 * ol;
+        unsigned char *__restrict__ op = reinterpret_cast<unsigned char *>(B.obs_packed + obase) + 8 * ol;
+        const bool packed = B.obs_packed != nullptr;
         const unsigned char *sv = reinterpret_cast<const unsigned char *>(vrow(0, lg)) + ol;
         const int nit = (NC8 - ol + LPG - 1) / LPG;
         for (int i0 = 0; i0 < nit; i0 += EB) {
@@ -711,7 +713,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
                     __stcs(reinterpret_cast<uint4 *>(oa + 2 * (size_t)p * (size_t)S + 128 * i), xa);
                 }
             }
-            // ---- pass B: owner, terrain, visibility
+            // ---- pass B: owner, terrain, visibility -- three byte planes, or one packed byte (R33)
             uint2 o[EB], t[EB];
 #pragma unroll
             for (int k = 0; k < EB; ++k)
@@ -719,6 +721,26 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
                     o[k] = __ldcg(reinterpret_cast<const uint2 *>(go + 64 * (i0 + k)));
                     t[k] = __ldcg(reinterpret_cast<const uint2 *>(gt + 64 * (i0 + k)));
                 }
+            if (packed) {
+#pragma unroll
+                for (int k = 0; k < EB; ++k) {
+                    if (i0 + k >= nit) break;
+                    const int i = i0 + k;
+                    // per byte: 0x80 | terrain << 4 | (owner + 2); owner + 2 on the low nibble cannot carry
+                    const uint32_t qx = 0x80808080u | ((t[k].x << 4) & 0x30303030u) |
+                                        (((o[k].x & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu);
+                    const uint32_t qy = 0x80808080u | ((t[k].y << 4) & 0x30303030u) |
+                                        (((o[k].y & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu);
+#pragma unroll
+                    for (int p = 0; p < NP; ++p) {
+                        if (p >= P) break;
+                        const uint32_t vb = sv[4 * BW * p + 8 * i];
+                        const uint32_t m0 = prmt(nib_sign(vb & 15u), 0u, 0xBA98u), m1 = prmt(nib_sign(vb >> 4), 0u, 0xBA98u);
+                        __stcs(reinterpret_cast<uint2 *>(op + (size_t)p * (size_t)S + 64 * i), make_uint2(qx & m0, qy & m1));
+                    }
+                }
+                continue;
+            }
 #pragma unroll
             for (int k = 0; k < EB; ++k) {
                 if (i0 + k >= nit) break;

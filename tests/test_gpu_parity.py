@@ -28,7 +28,7 @@ def compare(env, o, fields=ALL_FIELDS, digest=True, slot=0, oslot=0, where=""):
     for f in fields:
         got = env.field(f, slot)
         want = np.asarray(getattr(o, f))
-        if f in OUT_FIELDS:
+        if f in OUT_FIELDS or f == "obs_packed":
             want = want[oslot]
         if not np.array_equal(got, want.reshape(got.shape)):
             bad = np.argwhere(got != want.reshape(got.shape))
@@ -205,6 +205,55 @@ def test_specialised_rollout_kernel_matches_oracle(gpu, oracle_mod):
         o.rollout(32)
         compare(env, o, where=f"rollout {it}")
     assert env.last_launch_specialised
+
+
+# ------------------------------------------------------------------------------- packed observation (R33)
+PACKED_FIELDS = STATE_FIELDS + ["reward", "done", "winner", "obs_army", "obs_packed"]
+
+
+@pytest.mark.parametrize("name,N,T,over", [
+    ("c2_24x24", 90, 200, dict(max_turns=90)),
+    ("c5a_2v2", 30, 160, dict(max_turns=100)),
+    ("c5b_ffa8", 21, 120, dict(height=12, width=13, n_players=5, spawn_dmin=4, n_cities=4, max_turns=80)),
+])
+def test_packed_observation_matches_oracle(gpu, oracle_mod, name, N, T, over):
+    """The 3-byte-per-cell format (army + one packed byte, R33) on the register-resident kernel and on the staged
+    kernel, every step; the three byte planes are not allocated at all."""
+    cfg, _ = workloads.config(name, n_games=N, **over)
+    env = gpu.GeneralsEnv(cfg, digest=False, packed=True)
+    env.set_generic(False, -1)                              # the step kernel also for more than 4 players
+    stg = gpu.GeneralsEnv(cfg, digest=True, packed=True, bitboards=False)
+    o = oracle_mod.Oracle(cfg)
+    for e in (env, stg):
+        assert "obs_owner" not in e.tensors and "obs_vis" not in e.tensors
+        e.reset()
+    o.reset()
+    compare(env, o, fields=PACKED_FIELDS, digest=False, where="reset")
+    for t in range(T):
+        env.step()
+        stg.step()
+        o.step()
+        compare(env, o, fields=PACKED_FIELDS, digest=False, where=f"{name} packed step {t}")
+        if t % 8 == 0:
+            compare(stg, o, fields=PACKED_FIELDS, digest=True, where=f"{name} packed staged step {t}")
+    assert env.last_launch_register_resident and not stg.last_launch_register_resident
+    assert int(o.episodes_done.sum()) > 0
+
+
+def test_packed_rollout_every_step_slots(gpu, oracle_mod):
+    K = 6
+    cfg, _ = workloads.config("c2_24x24", n_games=41, max_turns=25)
+    env = gpu.GeneralsEnv(cfg, k_slots=K, packed=True)
+    o = oracle_mod.Oracle(cfg, every_step_K=K)
+    env.reset()
+    o.reset()
+    for it in range(4):
+        env.rollout(K, gpu.OBS_EVERY_STEP)
+        o.rollout(K, oracle_mod.OBS_EVERY_STEP)
+        for k in range(K):
+            compare(env, o, fields=["reward", "done", "winner", "obs_army", "obs_packed"], digest=False, slot=k, oslot=k,
+                    where=f"it {it} slot {k}")
+        compare(env, o, fields=STATE_FIELDS, where=f"it {it}")
 
 
 # ------------------------------------------------------------------------------- rollout == steps
