@@ -34,10 +34,10 @@ HBM_FALLBACK_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PE
 NCU_DRAM_BYTES_PER_LAUNCH = {16384: 104331008}       # profiles/r01_step_full_summary.txt
 
 
-def algorithmic_bytes_per_env_step(H, W, P):
-    """SURVEY 8(d) B_min: read state 4*HW, write observations 5*P*HW, O(P) scalars
-    (actions 4P, reward P, done + winner 2, scoreboard 8P, turn 4)."""
-    return 4 * H * W + 5 * P * H * W + 13 * P + 6
+def algorithmic_bytes_per_env_step(H, W, P, packed=False):
+    """SURVEY 8(d) B_min: read state 4*HW, write observations 5*P*HW (3*P*HW in the packed format, R33),
+    O(P) scalars (actions 4P, reward P, done + winner 2, scoreboard 8P, turn 4)."""
+    return 4 * H * W + (3 if packed else 5) * P * H * W + 13 * P + 6
 
 
 def measured_peak():
@@ -325,18 +325,20 @@ def run_sweep(args):
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     peak, _ = measured_peak()
-    rows = [("c3_sweep", n) for n in (1024, 16384, 262144, 1048576)]
-    rows += [("c4_curriculum", 65536), ("c5a_2v2", 32768), ("c5b_ffa8", 32768)]
-    for name, N in rows:
+    rows = [("c3_sweep", n, False) for n in (1024, 16384, 262144, 1048576)]
+    rows += [("c4_curriculum", 65536, False), ("c5a_2v2", 32768, False), ("c5b_ffa8", 32768, False)]
+    rows += [("c3_sweep", 16384, True), ("c3_sweep", 262144, True)]        # packed observation format (R33)
+    for name, N, packed in rows:
         cfg, _ = workloads.config(name, n_games=N)
         P, H, W = cfg["n_players"], cfg["height"], cfg["width"]
-        bmin = algorithmic_bytes_per_env_step(H, W, P)
+        bmin = algorithmic_bytes_per_env_step(H, W, P, packed)
         R = max(2, -(-(640 << 20) // (N * bmin)))
         K = max(32, min(args.steps, (1 << 31) // (N * bmin) * 4))
-        envs = [GeneralsEnv(dict(cfg, game_id_base=r * N), device=dev, digest=False, actions_out=False) for r in range(R)]
+        envs = [GeneralsEnv(dict(cfg, game_id_base=r * N), device=dev, digest=False, actions_out=False, packed=packed)
+                for r in range(R)]
         for e in envs:
             e.reset()
-        out = {"workload": name, "n_games": N, "n_players": P, "board": f"{H}x{W}", "replicas_in_rotation": R,
+        out = {"workload": name, "obs_format": "army + packed byte (R33)" if packed else "4 planes", "n_games": N, "n_players": P, "board": f"{H}x{W}", "replicas_in_rotation": R,
                "steps": K, "algorithmic_bytes_per_env_step": bmin}
         for graph in (False, True):
             ms = time_steps(torch, envs, K, max(args.warmup, R), graph)
@@ -347,7 +349,27 @@ def run_sweep(args):
                         ("" if envs[0].last_launch_specialised else " (generic)")
         del envs
         torch.cuda.empty_cache()
-        if name == "c3_sweep":
+        if name == "c3_sweep" and not packed and N <= 262144:
+            # fused rollout with the planes of EVERY turn written to K-strided buffers (apples to apples with gen_step)
+            Ke = 8
+            eenv = GeneralsEnv(cfg, device=dev, k_slots=Ke, digest=False, actions_out=False)
+            eenv.reset()
+            eenv.rollout(Ke, 1)
+            n_roll = max(2, K // Ke)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(n_roll):
+                eenv.rollout(Ke, 1)
+            e1.record()
+            torch.cuda.synchronize()
+            out["rollout_K8_every_step"] = {"env_steps_per_s": N * Ke * n_roll / (e0.elapsed_time(e1) * 1e-3),
+                                            "us_per_launch": 1e3 * e0.elapsed_time(e1) / n_roll,
+                                            "hbm_frac": N * Ke * (bmin - 4 * H * W * (Ke - 1) / Ke) /
+                                                        (e0.elapsed_time(e1) / n_roll * 1e-3) / 1e9 / peak}
+            del eenv
+            torch.cuda.empty_cache()
+        if name == "c3_sweep" and not packed:
             renv = GeneralsEnv(cfg, device=dev, digest=True, actions_out=False)
             renv.reset()
             renv.rollout(32, OBS_DIGEST)
