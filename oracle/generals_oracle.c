@@ -71,6 +71,7 @@ typedef struct {
     uint32_t *sat_events;     /* [N] */
     uint64_t *obs_digest;     /* [N] or NULL */
     uint8_t *obs_packed;      /* [N][P][S] or NULL: owner, terrain and visibility in one byte (R33) */
+    int32_t *score_hist;      /* [N][512][2P] or NULL: ring of the public scoreboard per turn (R34) */
 } orc_buffers;
 
 /* ------------------------------------------------------------------ Philox
@@ -218,6 +219,22 @@ static void scoreboard(const orc_config *cfg, const orc_buffers *b, int g)
     for (int p = 0; p < P; ++p) { b->land[g * P + p] = 0; b->army_total[g * P + p] = 0; }
     for (int c = 0; c < HW; ++c)
         if (owner[c] >= 0) { b->land[g * P + owner[c]] += 1; b->army_total[g * P + owner[c]] += army[c]; }
+}
+
+/* ------------------------- R34: the raw material of the paper's two temporal
+ * tokens, "a 512-step sliding window of the opponent's total army count and a matching window of their total
+ * land count".  Slot (turn mod 512) of the game's ring holds (land[p], army_total[p]) of every player as the
+ * scoreboard stands at the end of that turn (turn 0: the freshly generated board). */
+enum { HIST_LEN = 512 };
+static void record_history(const orc_config *cfg, const orc_buffers *b, int g)
+{
+    const int P = cfg->n_players;
+    if (!b->score_hist) return;
+    int32_t *slot = b->score_hist + ((size_t)g * HIST_LEN + (size_t)(b->turn[g] % HIST_LEN)) * 2 * P;
+    for (int p = 0; p < P; ++p) {
+        slot[2 * p] = b->land[g * P + p];
+        slot[2 * p + 1] = b->army_total[g * P + p];
+    }
 }
 
 /* ------------------------- a10 + a11: fog of war and the four planes (R18, R19, R32)
@@ -425,6 +442,7 @@ static void step_game(const orc_config *cfg, const orc_buffers *b, int g, const 
         generate(cfg, b, g);
         scoreboard(cfg, b, g);
     }
+    record_history(cfg, b, g);                                /* R34: the scoreboard as this call leaves it */
     /* 6. observation of the state at the end of the call (R32) */
     observe(cfg, b, g, obs_game_index);
 }
@@ -440,6 +458,7 @@ int32_t orc_reset(const orc_config *cfg, const orc_buffers *b)
         b->done[g] = 0; b->winner[g] = -1;
         b->episodes_done[g] = 0; b->truncations[g] = 0; b->sat_events[g] = 0;
         for (int p = 0; p < P; ++p) { b->reward[g * P + p] = 0; b->wins[g * P + p] = 0; }
+        record_history(cfg, b, g);
         observe(cfg, b, g, (size_t)g);
         if (b->obs_digest) b->obs_digest[g] = chain_digest(cfg, b, g, (size_t)g, 0);
     }

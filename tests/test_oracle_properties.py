@@ -622,3 +622,47 @@ def test_R33_packed_plane_decodes_to_the_three_byte_planes(oracle_mod, name, N, 
         seen_fog |= bool((vis == 0).any())
         seen_enemy |= bool(((owner >= 0) & (owner != np.arange(o.P)[None, :, None])).any())
     assert seen_fog and seen_enemy
+
+
+def test_R34_scoreboard_history_closed_form_and_wrap(oracle_mod):
+    """R34 (NEXT-2; P:L141 "512-step sliding window of the opponent's total army count and ... land count"):
+    under all-pass play the general holds 1 + t // 2 + t // 50 at turn t (closed form C1) and land stays 1, so
+    slot t mod 512 of the ring must hold exactly that, and after 600 turns slots 0..87 hold turns 512..599."""
+    cfg, _ = workloads.config("c1_8x8", n_games=3)
+    o = oracle_mod.Oracle(cfg)
+    o.reset()
+    passes = np.zeros((3, 2), dtype=np.int32)
+    for t in range(1, 601):
+        o.step(passes)
+    h = o.score_hist                                        # [N][512][2P]: (land, army) per player
+    for slot in range(512):
+        t = slot + 512 if slot + 512 <= 600 else slot
+        want_army = 1 + t // 2 + t // 50
+        assert (h[:, slot, 0::2] == 1).all() and (h[:, slot, 1::2] == want_army).all(), slot
+
+
+def test_R34_history_is_the_scoreboard_of_every_turn(oracle_mod):
+    """On sampled play with auto-reset: an independent Python log of (turn, land, army_total) after every call must
+    equal the ring on the last min(turn + 1, 512) turns of the current episode of every game."""
+    cfg, _ = workloads.config("c4_curriculum", n_games=10, height=10, width=10, spawn_dmin=3, spawn_dmax=5,
+                              n_cities=3, max_turns=90)
+    o = oracle_mod.Oracle(cfg)
+    o.reset()
+    log = [dict() for _ in range(10)]                       # per game: turn -> (land, army) of the current episode
+    ep = o.episode.copy()
+    def note():
+        for g in range(10):
+            if o.episode[g] != ep[g]:
+                log[g].clear()
+                ep[g] = o.episode[g]
+            log[g][int(o.turn[g])] = (o.land[g].copy(), o.army_total[g].copy())
+    note()
+    for _ in range(300):
+        o.step()
+        note()
+        for g in range(10):
+            for t, (land, army) in log[g].items():
+                if t > int(o.turn[g]) - 512:
+                    assert np.array_equal(o.score_hist[g, t % 512, 0::2], land)
+                    assert np.array_equal(o.score_hist[g, t % 512, 1::2], army)
+    assert int(o.episodes_done.sum()) > 5 and int(o.wins.sum()) > 0
