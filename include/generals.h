@@ -111,7 +111,14 @@ typedef struct gen_buffers {
     int32_t *actions_out;    /* out   [K][N][P]  the actions actually applied; may be NULL */
     uint32_t *bitboards;     /* state [N][P+3][BW]  derived cache, may be NULL (see below) */
     uint8_t *obs_packed;     /* out   [K][N][P][S]  packed observation, may be NULL (see below) */
+    int32_t *score_hist;     /* state [N][512][2P]  scoreboard history ring, may be NULL (see below) */
 } gen_buffers;
+
+/* `score_hist` (R34; the paper's two temporal tokens are 512-step windows of
+ * the opponent's army and land totals): when non-NULL, gen_reset and every turn of gen_step / gen_rollout store
+ * (land[p], army_total[p]) of every player, as the call leaves the scoreboard, in slot (turn mod 512) of the
+ * game's ring ([2p] = land, [2p+1] = army).  The last min(turn + 1, 512) slots belong to the current episode;
+ * older slots are leftovers.  Frozen games are not recorded. */
 
 /* `obs_packed` (R33) selects the 3-byte-per-cell observation format: when it is non-NULL
  * every call writes obs_army and obs_packed and does NOT write obs_owner / obs_terrain / obs_vis (which may
@@ -132,7 +139,7 @@ typedef struct gen_sizes {
     int32_t alignment;       /* 16 */
     size_t army, owner, terrain, turn, episode, alive, general_cell, land, army_total;
     size_t reward, done, winner, obs_army, obs_owner, obs_terrain, obs_vis;
-    size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out, bitboards, obs_packed;
+    size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out, bitboards, obs_packed, score_hist;
     int32_t bitboard_row_words; /* BW */
 } gen_sizes;
 

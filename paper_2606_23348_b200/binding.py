@@ -61,6 +61,7 @@ BUFFERS = [
     ("actions_out", "int32", lambda N, P, S, K: (K, N, P)),
     ("bitboards", "int32", lambda N, P, S, K: (N, P + 3, (-(-S // 32) + 7) // 8 * 8)),   # bits of uint32
     ("obs_packed", "uint8", lambda N, P, S, K: (K, N, P, S)),
+    ("score_hist", "int32", lambda N, P, S, K: (N, 512, 2 * P)),
 ]
 
 
@@ -147,7 +148,7 @@ class GeneralsEnv:
     """
 
     def __init__(self, cfg, device="cuda:0", k_slots=1, digest=True, actions_out=True, bitboards=True,
-                 packed=False):
+                 packed=False, history=False):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -167,7 +168,7 @@ class GeneralsEnv:
         self.tensors = {}
         for name, dt, shape in BUFFERS:
             if ((name == "obs_digest" and not digest) or (name == "actions_out" and not actions_out)
-                    or (name == "bitboards" and not bitboards) or (name == "obs_packed" and not packed)
+                    or (name == "bitboards" and not bitboards) or (name == "obs_packed" and not packed) or (name == "score_hist" and not history)
                     or (packed and name in ("obs_owner", "obs_terrain", "obs_vis"))):
                 setattr(self.bufs, name, None)
                 continue

@@ -59,6 +59,7 @@ void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
     s->bitboard_row_words = (int32_t)BW;
     s->bitboards = N * (P + 3) * BW * 4;
     s->obs_packed = k * N * P * S;
+    s->score_hist = N * 512 * 2 * P * 4;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -81,6 +82,7 @@ int check_buffers(const gen_buffers *b, bool need_obs) {
     if (b->obs_digest && !aligned16(b->obs_digest)) return GEN_ERR_ALIGN;
     if (b->actions_out && !aligned16(b->actions_out)) return GEN_ERR_ALIGN;
     if (b->bitboards && !aligned16(b->bitboards)) return GEN_ERR_ALIGN;
+    if (b->score_hist && !aligned16(b->score_hist)) return GEN_ERR_ALIGN;
     return GEN_OK;
 }
 

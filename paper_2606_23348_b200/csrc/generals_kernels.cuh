@@ -1049,6 +1049,12 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             }
         }
         __syncwarp();
+        // ---- R34: slot (turn mod 512) of the scoreboard history ring, the scoreboard as this turn leaves it
+        if (B.score_hist && gvalid && !frozen && ol < P) {
+            const GameS &gs = s_game[sub];
+            *reinterpret_cast<int2 *>(B.score_hist + (((size_t)g * 512 + (size_t)(gs.turn & 511)) * P + ol) * 2) =
+                make_int2(gs.land[ol], gs.tot[ol]);
+        }
         // ---- a10 + a11 (R32: the state at the end of the call)
         const bool planes = (flags & F_OBS_PLANES) && (every || last_step);
         if (planes || (flags & F_DIGEST)) {
@@ -1061,6 +1067,10 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
 
     if (K == 0) {  // gen_reset / gen_observe: observation of the state as it stands
         if (gvalid) {
+            if ((flags & F_RESET) && B.score_hist && ol < P) {  // R34: turn 0 of the ring
+                const GameS &gs = s_game[sub];
+                *reinterpret_cast<int2 *>(B.score_hist + (((size_t)g * 512) * P + ol) * 2) = make_int2(gs.land[ol], gs.tot[ol]);
+            }
             compute_vis(sub);
             if ((flags & F_RESET) && ol == 0) {
                 GameS &gs = s_game[sub];

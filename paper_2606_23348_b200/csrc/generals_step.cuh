@@ -819,6 +819,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         if (ol < P) {
             B.land[(size_t)g * P + ol] = gs.land[ol];
             B.army_total[(size_t)g * P + ol] = gs.tot[ol];
+            if (B.score_hist && !frozen)  // R34: slot (turn mod 512) of the scoreboard history ring
+                *reinterpret_cast<int2 *>(B.score_hist + (((size_t)g * 512 + (size_t)(gs.turn & 511)) * P + ol) * 2) =
+                    make_int2(gs.land[ol], gs.tot[ol]);
         }
         if (ol == (P & 7)) { B.turn[g] = gs.turn; B.alive[g] = (uint8_t)gs.alive; }
     }

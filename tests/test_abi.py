@@ -29,8 +29,8 @@ def test_exports_every_declared_symbol(lib):
 
 def test_struct_layouts_match_header():
     assert C.sizeof(binding.GenConfig) == 13 * 4 + 3 * 4 + 8
-    assert C.sizeof(binding.GenBuffers) == 24 * 8
-    assert C.sizeof(binding.GenSizes) == 8 + 24 * C.sizeof(C.c_size_t) + 8      # + bitboard_row_words, padding
+    assert C.sizeof(binding.GenBuffers) == 25 * 8
+    assert C.sizeof(binding.GenSizes) == 8 + 25 * C.sizeof(C.c_size_t) + 8      # + bitboard_row_words, padding
 
 
 def test_query_sizes(lib):

@@ -256,6 +256,51 @@ def test_packed_rollout_every_step_slots(gpu, oracle_mod):
         compare(env, o, fields=STATE_FIELDS, where=f"it {it}")
 
 
+# ------------------------------------------------------------------------------- scoreboard history (R34)
+@pytest.mark.parametrize("name,N,over", [
+    ("c2_24x24", 45, dict(max_turns=70, spawn_dmin=4)),
+    ("c5a_2v2", 18, dict(max_turns=60)),
+])
+def test_scoreboard_history_ring_matches_oracle(gpu, oracle_mod, name, N, over):
+    """The 512-slot ring of (land, army_total) per player and turn (R34, the raw material of the paper's temporal
+    tokens) written by the step kernel, the staged kernel and fused rollouts, across auto-resets and a ring wrap."""
+    cfg, _ = workloads.config(name, n_games=N, **over)
+    env = gpu.GeneralsEnv(cfg, digest=False, history=True)
+    stg = gpu.GeneralsEnv(cfg, digest=True, history=True, bitboards=False)
+    o = oracle_mod.Oracle(cfg)
+    for e in (env, stg):
+        e.reset()
+    o.reset()
+    fields = ["score_hist", "land", "army_total", "turn", "episode"]
+    compare(env, o, fields=fields, digest=False, where="reset")
+    for it in range(8):
+        for _ in range(20):
+            env.step()
+            stg.step()
+            o.step()
+        compare(env, o, fields=fields, digest=False, where=f"steps {it}")
+        compare(stg, o, fields=fields, digest=False, where=f"staged steps {it}")
+        for e in (env, stg):
+            e.rollout(17, gpu.OBS_NONE)
+        o.rollout(17, oracle_mod.OBS_NONE)
+        compare(env, o, fields=fields, digest=False, where=f"rollout {it}")
+        compare(stg, o, fields=fields, digest=False, where=f"staged rollout {it}")
+    assert int(o.episodes_done.sum()) > N                    # several episodes per game
+    # ring wrap: one long episode
+    cfg2, _ = workloads.config(name, n_games=5, auto_reset=0, max_turns=0, pass_thr=workloads.thr(90))
+    env2 = gpu.GeneralsEnv(cfg2, digest=False, history=True)
+    o2 = oracle_mod.Oracle(cfg2)
+    env2.reset()
+    o2.reset()
+    for _ in range(19):
+        env2.rollout(32, gpu.OBS_NONE)
+        o2.rollout(32, oracle_mod.OBS_NONE)
+    env2.step()
+    o2.step()
+    assert int(o2.turn.max()) > 512
+    compare(env2, o2, fields=fields, digest=False, where="wrap")
+
+
 # ------------------------------------------------------------------------------- rollout == steps
 @pytest.mark.parametrize("mode", ["digest", "none"])
 def test_rollout_equals_steps(gpu, oracle_mod, mode):
