@@ -597,6 +597,7 @@ def test_config2_full_size_sampled_games(gpu, oracle_mod, digest):
     ("c4_curriculum", 65536, 150, 0),     # biased policy: the staged kernel
     ("c5a_2v2", 32768, 120, 0),
     ("c5b_ffa8", 32768, 120, 0),
+    ("c4_flags", 65536, 150, 0),          # NEXT-4: all three alternative rule readings at scale (uniform policy)
 ])
 def test_full_size_configs_sampled_games(gpu, oracle_mod, name, N, T, roll):
     """BASELINE configs 3, 4, 5 at their full batch sizes, in the launch configuration bench.py --sweep times
@@ -604,7 +605,10 @@ def test_full_size_configs_sampled_games(gpu, oracle_mod, name, N, T, roll):
     last / strided: a game depends on its global id only, M2) and must agree on every tensor; plus properties
     that hold at any size."""
     import torch
-    cfg, _ = workloads.config(name, n_games=N)
+    if name == "c4_flags":                                   # short spawn distances: captures (floor halving), ticks, rotation
+        cfg, _ = workloads.config("c4_curriculum", n_games=N, rule_flags=7, bias_thr=0, spawn_dmax=8, max_turns=120)
+    else:
+        cfg, _ = workloads.config(name, n_games=N)
     P, HW = cfg["n_players"], cfg["height"] * cfg["width"]
     env = gpu.GeneralsEnv(cfg, digest=False, actions_out=False)
     env.reset()
