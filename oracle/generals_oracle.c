@@ -528,3 +528,100 @@ int32_t orc_observe(const orc_config *cfg, const orc_buffers *b)
     for (int g = 0; g < cfg->n_games; ++g) { scoreboard(cfg, b, g); observe(cfg, b, g, (size_t)g); }
     return 0;
 }
+
+/* ===================================================================== NEXT-1: the 38-channel feature tensor
+ * PAPER.md Appendix A and Table IV, 1v1 only (the table speaks of "the agent" and "the
+ * opponent").  One call per turn and game: it folds the current observation into the per-episode memory and
+ * writes, for each player p as the agent, C = 24 + 2 * 7 = 38 float maps feat[g][p][ch][S].  Readings (DESIGN.md
+ * R35): the memory is cleared when turn == 0 (a new episode always starts there); "opponent army (last observed)"
+ * is the public scoreboard; channel 9 counts every visible neutral-owned cell; channel 21 is 0 where the enemy was
+ * never seen or is visible now; deltas that reach before the episode's first frame are 0; coordinates are
+ * col / (W - 1) and row / (H - 1); stride padding cells are 0 in every channel. */
+enum { FEAT_C = 38, FEAT_HIST = 7, FEAT_RING = 8 };
+
+typedef struct {
+    uint8_t *bits;        /* [N][2][5][S]  seen, enemy_seen, generals, castles, mountains (0 / 1) */
+    int16_t *last_army;   /* [N][2][S]     enemy army last observed on the cell */
+    int32_t *last_turn;   /* [N][2][S]     turn of that observation, -1 = never */
+    int16_t *hist;        /* [N][2][2][8][S]  own_army / enemy_army frames, slot turn mod 8 */
+} orc_feat_state;
+
+#include <math.h>
+
+int32_t orc_features(const orc_config *cfg, const orc_buffers *b, const orc_feat_state *m, float *feat)
+{
+    const int H = cfg->height, W = cfg->width, P = cfg->n_players, HW = H * W, S = plane_stride(cfg);
+    if (P != 2) return -1;
+    for (int g = 0; g < cfg->n_games; ++g) {
+        const int16_t *army = b->army + (size_t)g * S;
+        const int8_t *owner = b->owner + (size_t)g * S, *terrain = b->terrain + (size_t)g * S;
+        const int t = b->turn[g];
+        for (int p = 0; p < 2; ++p) {
+            const int opp = 1 - p;
+            const size_t gp = (size_t)g * 2 + p;
+            uint8_t *bits = m->bits + gp * 5 * S;
+            int16_t *last_army = m->last_army + gp * S;
+            int32_t *last_turn = m->last_turn + gp * S;
+            int16_t *hist_own = m->hist + (gp * 2 + 0) * FEAT_RING * S, *hist_en = m->hist + (gp * 2 + 1) * FEAT_RING * S;
+            float *out = feat + gp * FEAT_C * S;
+            if (t == 0) {                                      /* new episode: forget */
+                memset(bits, 0, (size_t)5 * S);
+                memset(last_army, 0, sizeof(int16_t) * S);
+                for (int c = 0; c < S; ++c) last_turn[c] = -1;
+                memset(hist_own, 0, sizeof(int16_t) * FEAT_RING * S);
+                memset(hist_en, 0, sizeof(int16_t) * FEAT_RING * S);
+            }
+            memset(out, 0, sizeof(float) * FEAT_C * S);
+            for (int c = 0; c < HW; ++c) {
+                const int r = c / W, col = c % W;
+                int vis = 0;                                   /* own cells and their 8 neighbours */
+                for (int dr = -1; dr <= 1; ++dr)
+                    for (int dc = -1; dc <= 1; ++dc) {
+                        int rr = r + dr, cc = col + dc;
+                        if (rr >= 0 && rr < H && cc >= 0 && cc < W && owner[rr * W + cc] == p) vis = 1;
+                    }
+                const int a = army[c], o = owner[c], tr = terrain[c];
+                const int own_a = (o == p) ? a : 0;
+                const int en_vis = vis && o == opp;
+                const int en_a = en_vis ? a : 0;
+                /* fold into the memory */
+                bits[0 * S + c] |= (uint8_t)vis;
+                bits[1 * S + c] |= (uint8_t)en_vis;
+                bits[2 * S + c] |= (uint8_t)(vis && tr == T_GENERAL);
+                bits[3 * S + c] |= (uint8_t)(vis && tr == T_CITY);
+                bits[4 * S + c] |= (uint8_t)(vis && tr == T_MOUNTAIN);
+                if (en_vis) { last_army[c] = (int16_t)a; last_turn[c] = t; }
+                hist_own[(t % FEAT_RING) * S + c] = (int16_t)own_a;
+                hist_en[(t % FEAT_RING) * S + c] = (int16_t)en_a;
+                /* Table IV */
+                out[0 * S + c] = (float)(vis ? a : 0);
+                out[1 * S + c] = (float)own_a;
+                out[2 * S + c] = (float)en_a;
+                out[3 * S + c] = (float)((vis && o == OWNER_NEUTRAL) ? a : 0);
+                for (int k = 0; k < 5; ++k) out[(4 + k) * S + c] = (float)bits[k * S + c];
+                out[9 * S + c] = (float)(vis && o == OWNER_NEUTRAL);
+                out[10 * S + c] = (float)(o == p);
+                out[11 * S + c] = (float)en_vis;
+                out[12 * S + c] = (float)(!vis);
+                out[13 * S + c] = (float)(!vis && (bits[2 * S + c] | bits[3 * S + c] | bits[4 * S + c]));
+                out[14 * S + c] = (float)t;
+                out[15 * S + c] = (float)(t % 50) / 50.0f;
+                out[16 * S + c] = (float)b->land[g * 2 + p];
+                out[17 * S + c] = (float)b->army_total[g * 2 + p];
+                out[18 * S + c] = (float)b->land[g * 2 + opp];
+                out[19 * S + c] = (float)b->army_total[g * 2 + opp];
+                out[20 * S + c] = (float)last_army[c];
+                out[21 * S + c] = (last_turn[c] < 0 || en_vis) ? 0.0f : logf(1.0f + (float)(t - last_turn[c])) / 5.0f;
+                out[22 * S + c] = W > 1 ? (float)col / (float)(W - 1) : 0.0f;
+                out[23 * S + c] = H > 1 ? (float)r / (float)(H - 1) : 0.0f;
+                for (int k = 0; k < FEAT_HIST; ++k) {
+                    if (t - k - 1 < 0) continue;               /* before the first frame of the episode: 0 */
+                    const int s1 = ((t - k) % FEAT_RING) * S + c, s0 = ((t - k - 1) % FEAT_RING) * S + c;
+                    out[(24 + k) * S + c] = (float)(hist_own[s1] - hist_own[s0]);
+                    out[(31 + k) * S + c] = (float)(hist_en[s1] - hist_en[s0]);
+                }
+            }
+        }
+    }
+    return 0;
+}

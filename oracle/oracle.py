@@ -25,7 +25,7 @@ def build(force=False):
     """Compile the oracle with gcc (plain C99, -O2). Building the checker is not using it."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         subprocess.check_call(["gcc", "-std=c99", "-O2", "-Wall", "-Wextra", "-fPIC", "-shared",
-                               "-o", _LIB, _SRC])
+                               "-o", _LIB, _SRC, "-lm"])
     return _LIB
 
 
@@ -46,6 +46,10 @@ _BUF_FIELDS = [
     ("sat_events", np.uint32), ("obs_digest", np.uint64), ("obs_packed", np.uint8),
     ("score_hist", np.int32),
 ]
+
+
+class OrcFeatState(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("bits", "last_army", "last_turn", "hist")]
 
 
 class OrcBuffers(C.Structure):
@@ -73,6 +77,7 @@ def lib():
         _lib.orc_rollout.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers), C.c_int32, C.c_uint32,
                                      C.c_int32]
         _lib.orc_observe.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers)]
+        _lib.orc_features.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers), C.POINTER(OrcFeatState), C.c_void_p]
     return _lib
 
 
@@ -167,6 +172,20 @@ class Oracle:
 
     def observe(self):
         lib().orc_observe(C.byref(self.cfg), C.byref(self.bufs))
+
+    def features(self):
+        """NEXT-1: fold the current turn into the per-episode memory and return feat[N][2][38][S] (float32).
+        Call once per turn (after reset and after every step)."""
+        N, S = self.N, self.S
+        if not hasattr(self, "feat"):
+            self.feat = np.zeros((N, 2, 38, S), dtype=np.float32)
+            self._fm = dict(bits=np.zeros((N, 2, 5, S), np.uint8), last_army=np.zeros((N, 2, S), np.int16),
+                            last_turn=np.full((N, 2, S), -1, np.int32), hist=np.zeros((N, 2, 2, 8, S), np.int16))
+            self._fs = OrcFeatState(*[self._fm[k].ctypes.data for k in ("bits", "last_army", "last_turn", "hist")])
+        rc = lib().orc_features(C.byref(self.cfg), C.byref(self.bufs), C.byref(self._fs), self.feat.ctypes.data)
+        if rc != 0:
+            raise ValueError("orc_features: 1v1 only")
+        return self.feat
 
     def set_policy(self, pass_thr=None, half_thr=None, bias_thr=None):
         for k, v in (("pass_thr", pass_thr), ("half_thr", half_thr), ("bias_thr", bias_thr)):

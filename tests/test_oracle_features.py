@@ -1,0 +1,115 @@
+"""Pins of the oracle's 38-channel feature tensor (NEXT-1; App. A, Table IV; DESIGN R35).
+The paper prints no numeric example of the tensor, so the oracle is pinned by what Table IV and arithmetic fix:
+identities between channels, a closed form, and an independent history kept by the test from the oracle's OWN plain
+observation planes (obs_army / obs_owner / obs_terrain / obs_vis, themselves pinned elsewhere) -- never by re-running
+the featuriser's formulas on its own memory."""
+import numpy as np
+import pytest
+
+from paper_2606_23348_b200 import workloads
+
+
+def play(oracle_mod, cfg, T, actions=None):
+    o = oracle_mod.Oracle(cfg)
+    o.reset()
+    frames = []
+    for t in range(T + 1):
+        if t > 0:
+            o.step(actions)
+        f = o.features().copy()
+        frames.append(dict(feat=f, turn=o.turn.copy(), episode=o.episode.copy(), land=o.land.copy(),
+                           tot=o.army_total.copy(), army=o.field("obs_army").astype(np.int64).copy(),
+                           owner=o.field("obs_owner").astype(np.int64).copy(),
+                           terrain=o.field("obs_terrain").astype(np.int64).copy(),
+                           vis=o.field("obs_vis").astype(np.int64).copy()))
+    return o, frames
+
+
+def test_channel_identities_and_memory_from_an_independent_log(oracle_mod):
+    cfg, _ = workloads.config("c4_curriculum", n_games=8, height=9, width=11, spawn_dmin=3, spawn_dmax=5, n_cities=3,
+                              max_turns=70)
+    o, frames = play(oracle_mod, cfg, 150)
+    N, S, HW = 8, o.S, 99
+    me = np.arange(2)[None, :, None]
+    # the test's own memory, rebuilt from the plain observation planes
+    seen = np.zeros((N, 2, S), bool); en_seen = seen.copy(); gens = seen.copy(); cast = seen.copy(); mont = seen.copy()
+    last_army = np.zeros((N, 2, S), np.int64); last_turn = np.full((N, 2, S), -1, np.int64)
+    own_hist, en_hist = [], []
+    resets = 0
+    for fr in frames:
+        f, vis, owner, army, terrain = fr["feat"], fr["vis"] == 1, fr["owner"], fr["army"], fr["terrain"]
+        t = fr["turn"][:, None, None]
+        new = (fr["turn"] == 0)
+        resets += int(new.sum())
+        for arr in (seen, en_seen, gens, cast, mont):
+            arr[new] = False
+        last_army[new] = 0; last_turn[new] = -1
+        own = owner == me
+        enemy = vis & (owner == 1 - me)
+        neutral = vis & (owner == -1)
+        own_a, en_a = np.where(own, army, 0), np.where(enemy, army, 0)
+        # Table IV, instantaneous channels
+        assert np.array_equal(f[:, :, 0], army) and np.array_equal(f[:, :, 1], own_a) and np.array_equal(f[:, :, 2], en_a)
+        assert np.array_equal(f[:, :, 0], f[:, :, 1] + f[:, :, 2] + f[:, :, 3])           # visible army splits by owner
+        assert np.array_equal(f[:, :, 9], neutral) and np.array_equal(f[:, :, 10], own)
+        assert np.array_equal(f[:, :, 11], enemy) and np.array_equal(f[:, :, 12][:, :, :HW], ~vis[:, :, :HW])
+        assert np.array_equal((f[:, :, 9] + f[:, :, 10] + f[:, :, 11] + f[:, :, 12])[:, :, :HW], np.ones((N, 2, HW)))
+        # persistent memory
+        seen |= vis; en_seen |= enemy; gens |= vis & (terrain == 3); cast |= vis & (terrain == 2); mont |= vis & (terrain == 1)
+        for ch, arr in zip(range(4, 9), (seen, en_seen, gens, cast, mont)):
+            assert np.array_equal(f[:, :, ch], arr), ch
+        assert np.array_equal(f[:, :, 13][:, :, :HW], (~vis & (gens | cast | mont))[:, :, :HW])
+        last_army = np.where(enemy, army, last_army); last_turn = np.where(enemy, t, last_turn)
+        assert np.array_equal(f[:, :, 20], last_army)
+        age = np.where((last_turn < 0) | enemy, 0.0, np.log1p((t - last_turn).astype(np.float64)) / 5.0)
+        assert np.abs(f[:, :, 21] - age).max() < 1e-6
+        # scalars
+        b = f[:, :, :, :HW]                                                                 # broadcast over the board
+        assert (b[:, :, 14] == t).all() and np.allclose(b[:, :, 15], (t % 50) / 50.0, atol=1e-7)
+        for p in range(2):
+            assert (b[:, p, 16] == fr["land"][:, p, None]).all() and (b[:, p, 17] == fr["tot"][:, p, None]).all()
+            assert (b[:, p, 18] == fr["land"][:, 1 - p, None]).all() and (b[:, p, 19] == fr["tot"][:, 1 - p, None]).all()
+        # delta stacks against the test's own frame log (frames before the episode start count as absent)
+        own_hist.append((fr["turn"].copy(), own_a)); en_hist.append((fr["turn"].copy(), en_a))
+        for k in range(7):
+            for base, hist in ((24, own_hist), (31, en_hist)):
+                want = np.zeros((N, 2, S), np.int64)
+                if len(hist) >= k + 2:
+                    (t1, a1), (t0, a0) = hist[-1 - k], hist[-2 - k]
+                    same = (fr["turn"] - k - 1 >= 0) & (t1 == fr["turn"] - k) & (t0 == fr["turn"] - k - 1)
+                    want[same] = (a1 - a0)[same]
+                assert np.array_equal(f[:, :, base + k], want), (base, k)
+        assert (f[:, :, :, HW:] == 0).all()                                                 # stride padding
+    assert resets > 12 and en_seen.any() and gens.sum() > 16                                # captures, re-fog, memory
+
+
+def test_closed_form_under_all_pass_play(oracle_mod):
+    """All players pass: the general holds 1 + t // 2 + t // 50 (closed form C1), so own_army_delta[k] at the general
+    is the increment of that sequence, the coordinates are col / (W - 1), row / (H - 1), nothing enemy is ever seen."""
+    cfg, _ = workloads.config("c1_8x8", n_games=2)
+    o = oracle_mod.Oracle(cfg)
+    o.reset()
+    passes = np.zeros((2, 2), np.int32)
+    gen = lambda t: 1 + t // 2 + t // 50 if t >= 0 else 0
+    for t in range(0, 120):
+        if t > 0:
+            o.step(passes)
+        f = o.features()
+        for g in range(2):
+            for p in range(2):
+                c = int(o.general_cell[g, p])
+                assert f[g, p, 1, c] == gen(t) and f[g, p, 17, c] == gen(t) and f[g, p, 16, c] == 1
+                for k in range(7):
+                    want = gen(t - k) - gen(t - k - 1) if t - k - 1 >= 0 else 0
+                    assert f[g, p, 24 + k, c] == want, (t, k)
+                assert f[g, p, 2].sum() == 0 and f[g, p, 5].sum() == 0 and f[g, p, 31:38].sum() == 0
+                assert f[g, p, 22, c] == np.float32((c % 8) / 7) and f[g, p, 23, c] == np.float32((c // 8) / 7)
+                assert f[g, p, 4].sum() == f[g, p, 0, :64].size - f[g, p, 12, :64].sum()    # seen == visible: nothing moves
+
+
+def test_features_are_1v1_only(oracle_mod):
+    cfg, _ = workloads.config("c5a_2v2", n_games=1, height=10, width=10, spawn_dmin=3, n_cities=2)
+    o = oracle_mod.Oracle(cfg)
+    o.reset()
+    with pytest.raises(ValueError):
+        o.features()
