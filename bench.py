@@ -389,6 +389,79 @@ def run_sweep(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------ NEXT-1: features
+def feature_bytes_per_game(H, W):
+    """Algorithmic bytes of one gen_features call per game: per cell read the three state
+    planes (4 B) and, per player, write 38 float32 channels (152 B), write this turn's two history frames (4 B),
+    read the seven previous ones (28 B) and the memory (bits 1 B, last army 2 B, last sighting 4 B)."""
+    return H * W * (4 + 2 * (152 + 4 + 28 + 7))
+
+
+def run_features(args):
+    """gen_features alone and gen_step + gen_features per turn on BASELINE config 2 (one JSON
+    line; not the driver's contract line)."""
+    import torch
+    from paper_2606_23348_b200 import GeneralsEnv, workloads
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, peak_src = measured_peak()
+    cfg, _ = workloads.config(WORKLOAD)
+    if args.games:
+        cfg["n_games"] = args.games
+    N, H, W = cfg["n_games"], cfg["height"], cfg["width"]
+    K, Wm = args.steps, max(args.warmup, 8)
+    env = GeneralsEnv(cfg, device=dev, digest=False, actions_out=False)
+    env.reset()
+    env.features()
+    for _ in range(Wm):                       # a full delta history (7 frames) before anything is timed
+        env.step()
+        env.features()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(K):
+        env.step()
+        env.features()
+    e1.record()
+    torch.cuda.synchronize()
+    both_ms = e0.elapsed_time(e1) / K
+    # the featuriser alone: one event pair per launch (a step in between keeps the contract of one call per turn)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    for a, b in ev:
+        env.step()
+        a.record()
+        env.features()
+        b.record()
+    torch.cuda.synchronize()
+    feat_ms = statistics.mean(a.elapsed_time(b) for a, b in ev)
+    bfeat = feature_bytes_per_game(H, W)
+    achieved = N * bfeat / (feat_ms * 1e-3) / 1e9
+    line = {"workload": f"{WORKLOAD}: 1v1 {H}x{W}, {N} games, gen_step + gen_features every turn",
+            "n_games": N, "steps": K, "feature_tensor_bytes": N * 2 * 38 * env.S * 4,
+            "step_plus_features": {"env_steps_per_s": N / (both_ms * 1e-3), "us_per_turn": 1e3 * both_ms},
+            "features": {"games_per_s": N / (feat_ms * 1e-3), "us_per_launch": 1e3 * feat_ms,
+                         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                                      "frac": achieved / peak, "traffic": None, "kernel": "gen::k_features",
+                                      "peak_source": peak_src, "algorithmic_bytes_per_game": bfeat,
+                                      "units_per_launch": N}}}
+    if not args.no_cpu_baseline:
+        from oracle import oracle
+        sample, steps = 64, 100
+        o = oracle.Oracle(dict(cfg, n_games=sample))
+        o.reset()
+        o.features()
+        t_feat = 0.0
+        for _ in range(steps):
+            o.step()
+            t0 = time.perf_counter()
+            o.features()
+            t_feat += time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": sample * steps / t_feat, "unit": "games/s (orc_features alone)", "cores": 1,
+                                "kind": "oracle", "sample": f"first {sample} global game ids x {steps} turns"}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -399,10 +472,13 @@ def main():
     ap.add_argument("--replicas", type=int, default=0, help="replicas in the round-robin (default: enough for 640 MB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
+    ap.add_argument("--features", action="store_true", help="NEXT-1: gen_features alone and with gen_step (one JSON line)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.sweep:
         return run_sweep(args)
+    if args.features:
+        return run_features(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 

@@ -192,6 +192,46 @@ int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, vo
 int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
                   uint8_t *h_done, void *cuda_stream);
 
+/* ---- the 38-channel feature tensor (Appendix A, Table IV; R35) ----
+ * What the paper's policy consumes, built from the state the step leaves behind plus a per-episode memory.
+ * 1v1 only (Table IV speaks of "the agent" and "the opponent").  Channels, per player p as the agent, float32:
+ *   0 armies (visible)  1 own_army  2 enemy_army (visible)  3 neutral_army (visible)
+ *   4 seen  5 enemy_seen  6 generals  7 castles  8 mountains          (memory: ever observed, this episode)
+ *   9 neutral_cells (visible)  10 owned_cells  11 opponent_cells (visible)  12 fog_cells
+ *   13 structures_in_fog (fogged now, remembered general / castle / mountain)
+ *   14 timestep (raw turn)  15 (turn mod 50) / 50  16 own land  17 own army  18 opponent land  19 opponent army
+ *   20 last_enemy_army_seen  21 log(1 + turns since that sighting) / 5, 0 if never seen or visible now
+ *   22 col / (W - 1)  23 row / (H - 1)
+ *   24..30 own_army_delta[k], 31..37 enemy_army_delta[k]: frame(t-k) - frame(t-k-1) of channel 1 / 2, k = 0..6,
+ *          0 where t-k-1 lies before the episode's first turn.
+ * All members are DEVICE pointers, 16-byte aligned, caller-owned; sizes from gen_query_feat_sizes.  The memory
+ * members are opaque to the caller: allocate them ZEROED once (a zeroed memory is an empty one) and pass the same
+ * ones to every call. */
+typedef struct gen_feat_buffers {
+    float *feat;         /* out   [N][2][38][S]; stride padding cells are 0 */
+    uint8_t *mem_bits;   /* state [N][2][S]     bit k = channel 4 + k */
+    int16_t *last_army;  /* state [N][2][S]     channel 20 */
+    int32_t *last_seen;  /* state [N][2][S]     turn of the last enemy sighting + 1, 0 = never */
+    int16_t *hist;       /* state [N][2][8][2][S]  own_army / enemy_army frames, slot = turn mod 8 */
+} gen_feat_buffers;
+
+typedef struct gen_feat_sizes {
+    int32_t channels;     /* 38 */
+    int32_t plane_stride; /* S */
+    size_t feat, mem_bits, last_army, last_seen, hist; /* bytes */
+} gen_feat_sizes;
+
+/* Byte sizes of the gen_feat_buffers members for `cfg`.  Host-only.  GEN_ERR_CONFIG unless n_players == 2 and
+ * team_size == 1. */
+int gen_query_feat_sizes(const gen_config *cfg, gen_feat_sizes *out);
+
+/* Fold the state as it stands (after gen_reset, gen_step or gen_rollout) into each player's memory and write the
+ * feature tensor.  Call it ONCE PER TURN: the delta channels difference consecutive calls' frames, and a game whose
+ * turn counter is 0 (fresh or auto-reset, R17) starts from an empty memory.  Reads bufs->army / owner / terrain /
+ * turn / land / army_total only; no game state changes.  One kernel launch on cuda_stream.  GEN_ERR_CONFIG unless
+ * the handle is 1v1; GEN_ERR_NULL / GEN_ERR_ALIGN on a missing / misaligned pointer. */
+int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *feat, void *cuda_stream);
+
 /* Launch geometry override for tuning: games per CTA in {4, 8, 16, 32} (8 threads per game); 0 restores
  * the default (8).  Results do not depend on it. */
 int gen_set_launch(gen_env *env, int32_t games_per_cta);

@@ -15,6 +15,7 @@ RULE_TICK_PLAIN_ONLY, RULE_CAPTURE_HALF_FLOOR, RULE_ROTATE_PRIORITY = 1, 2, 4
 
 EXPORTS = ["gen_query_sizes", "gen_init", "gen_set_policy", "gen_global_step", "gen_set_global_step",
            "gen_reset", "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host",
+           "gen_query_feat_sizes", "gen_features",
            "gen_set_launch", "gen_set_generic", "gen_last_variant",
            "gen_launch_count", "gen_last_cuda_error", "gen_destroy",
            "gen_error_string", "gen_version"]
@@ -74,6 +75,25 @@ class GenSizes(C.Structure):
                 + [("bitboard_row_words", C.c_int32)])
 
 
+FEAT_CHANNELS = 38
+# gen_feat_buffers: name -> (torch dtype name, shape builder(N, S))
+FEAT_BUFFERS = [
+    ("feat", "float32", lambda N, S: (N, 2, FEAT_CHANNELS, S)),
+    ("mem_bits", "uint8", lambda N, S: (N, 2, S)),
+    ("last_army", "int16", lambda N, S: (N, 2, S)),
+    ("last_seen", "int32", lambda N, S: (N, 2, S)),
+    ("hist", "int16", lambda N, S: (N, 2, 8, 2, S)),
+]
+
+
+class GenFeatBuffers(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n, _, _ in FEAT_BUFFERS]
+
+
+class GenFeatSizes(C.Structure):
+    _fields_ = ([("channels", C.c_int32), ("plane_stride", C.c_int32)] + [(n, C.c_size_t) for n, _, _ in FEAT_BUFFERS])
+
+
 _lib = None
 
 
@@ -100,6 +120,8 @@ def load_library(path=None):
     lib.gen_observe.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p]
     lib.gen_sample.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
     lib.gen_step_host.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.gen_query_feat_sizes.argtypes = [C.POINTER(GenConfig), C.POINTER(GenFeatSizes)]
+    lib.gen_features.argtypes = [env_p, C.POINTER(GenBuffers), C.POINTER(GenFeatBuffers), C.c_void_p]
     lib.gen_set_launch.argtypes = [env_p, C.c_int32]
     lib.gen_set_generic.argtypes = [env_p, C.c_int32, C.c_int32]
     lib.gen_last_variant.argtypes = [env_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
@@ -114,7 +136,7 @@ def load_library(path=None):
     lib.gen_version.restype = C.c_char_p
     for name in ("gen_query_sizes", "gen_init", "gen_set_policy", "gen_set_global_step", "gen_reset",
                  "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host", "gen_set_launch",
-                 "gen_set_generic", "gen_last_cuda_error"):
+                 "gen_set_generic", "gen_last_cuda_error", "gen_query_feat_sizes", "gen_features"):
         getattr(lib, name).restype = C.c_int
     if path == LIB_PATH:
         _lib = lib
@@ -270,6 +292,23 @@ class GeneralsEnv:
             out = self.torch.zeros((self.N, self.P), dtype=self.torch.int32, device=self.device)
         self._check(self.lib.gen_sample(self._env, C.byref(self.bufs), C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out
+
+    def features(self, stream=None):
+        """NEXT-1 (R35): fold the current turn into each player's memory and return feat, a float32 CUDA tensor
+        [N][2][38][S].  Call once per turn (after reset and after every step).  1v1 only."""
+        if not hasattr(self, "feat_bufs"):
+            sizes = GenFeatSizes()
+            self._check(self.lib.gen_query_feat_sizes(C.byref(self.cfg), C.byref(sizes)))
+            self.feat_bufs = GenFeatBuffers()
+            self.feat_tensors = {}
+            for name, dt, shape in FEAT_BUFFERS:
+                t = self.torch.zeros(shape(self.N, self.S), dtype=getattr(self.torch, dt), device=self.device)
+                assert t.numel() * t.element_size() == getattr(sizes, name), name
+                self.feat_tensors[name] = t
+                setattr(self.feat_bufs, name, t.data_ptr() if t.numel() else 16)
+            self.feat = self.feat_tensors["feat"]
+        self._check(self.lib.gen_features(self._env, C.byref(self.bufs), C.byref(self.feat_bufs), self._stream(stream)))
+        return self.feat
 
     def step_host(self, h_actions=None, h_reward=None, h_done=None, stream=None):
         """End to end through host buffers (pinned CPU tensors); synchronises the stream."""

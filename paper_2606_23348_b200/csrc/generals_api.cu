@@ -5,6 +5,7 @@
 #include <new>
 
 #include "generals_variants.h"
+#include "generals_features.h"
 
 struct gen_env {
     gen_config cfg;
@@ -346,6 +347,47 @@ int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_action
     if (ce == cudaSuccess && h_done) ce = cudaMemcpyAsync(h_done, bufs->done, N, cudaMemcpyDeviceToHost, s);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
     if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
+    return GEN_OK;
+}
+
+int gen_query_feat_sizes(const gen_config *cfg, gen_feat_sizes *out) {
+    if (!cfg || !out) return GEN_ERR_NULL;
+    if (int e = validate(cfg)) return e;
+    if (cfg->n_players != 2 || cfg->team_size != 1) return GEN_ERR_CONFIG;
+    const size_t N = (size_t)cfg->n_games, S = (size_t)round_up(cfg->height * cfg->width, 16);
+    std::memset(out, 0, sizeof(*out));
+    out->channels = 38;
+    out->plane_stride = (int32_t)S;
+    out->feat = N * 2 * 38 * S * 4;
+    out->mem_bits = N * 2 * S;
+    out->last_army = N * 2 * S * 2;
+    out->last_seen = N * 2 * S * 4;
+    out->hist = N * 2 * 8 * 2 * S * 2;
+    return GEN_OK;
+}
+
+int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *feat, void *cuda_stream) {
+    if (!env || !bufs || !feat) return GEN_ERR_NULL;
+    if (env->cfg.n_players != 2 || env->cfg.team_size != 1) return GEN_ERR_CONFIG;
+    const void *req[] = {bufs->army, bufs->owner, bufs->terrain, bufs->turn, bufs->land, bufs->army_total,
+                         feat->feat, feat->mem_bits, feat->last_army, feat->last_seen, feat->hist};
+    for (const void *p : req) {
+        if (!p) return GEN_ERR_NULL;
+        if (!aligned16(p)) return GEN_ERR_ALIGN;
+    }
+    if (env->cfg.n_games == 0) return GEN_OK;
+    gen::FeatParams fp;
+    fp.N = env->base.N; fp.H = env->base.H; fp.W = env->base.W; fp.HW = env->base.HW; fp.S = env->base.S;
+    // 2 * S / 4 threads per game; small boards share a CTA of about 256 threads
+    const int per_game = fp.S / 2;
+    fp.G = per_game >= 256 ? 1 : 256 / per_game;
+    fp.army = bufs->army; fp.owner = bufs->owner; fp.terrain = bufs->terrain; fp.turn = bufs->turn;
+    fp.land = bufs->land; fp.army_total = bufs->army_total;
+    fp.feat = feat->feat; fp.mem_bits = feat->mem_bits; fp.last_army = feat->last_army;
+    fp.last_seen = feat->last_seen; fp.hist = feat->hist;
+    const cudaError_t e = gen::launch_features(fp, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
+    env->launches += 1;
     return GEN_OK;
 }
 

@@ -1,0 +1,26 @@
+// generals_features.h -- launch parameters of k_features (generals_features.cu), shared with generals_api.cu.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+namespace gen {
+
+struct FeatParams {
+    int N, H, W, HW, S;
+    int G;                       // games per CTA (2 * S / 4 threads each)
+    const int16_t *army;         // state planes and scalars of gen_buffers (read only)
+    const int8_t *owner;
+    const int8_t *terrain;
+    const int32_t *turn;
+    const int32_t *land;
+    const int32_t *army_total;
+    float *feat;                 // gen_feat_buffers
+    uint8_t *mem_bits;
+    int16_t *last_army;
+    int32_t *last_seen;
+    int16_t *hist;
+};
+
+cudaError_t launch_features(const FeatParams &fp, cudaStream_t stream);
+
+}  // namespace gen

@@ -27,10 +27,29 @@ def test_exports_every_declared_symbol(lib):
     assert b"sm_100a" in lib.gen_version()
 
 
+def binding_err(name):
+    return {"GEN_ERR_NULL": -1, "GEN_ERR_CONFIG": -2, "GEN_ERR_ALIGN": -3, "GEN_ERR_ARG": -4, "GEN_ERR_CUDA": -5}[name]
+
+
 def test_struct_layouts_match_header():
     assert C.sizeof(binding.GenConfig) == 13 * 4 + 3 * 4 + 8
     assert C.sizeof(binding.GenBuffers) == 25 * 8
     assert C.sizeof(binding.GenSizes) == 8 + 25 * C.sizeof(C.c_size_t) + 8      # + bitboard_row_words, padding
+    assert C.sizeof(binding.GenFeatBuffers) == 5 * 8
+    assert C.sizeof(binding.GenFeatSizes) == 8 + 5 * C.sizeof(C.c_size_t)
+
+
+def test_query_feat_sizes(lib):
+    cfg, _ = binding.make_config(workloads.config("c2_24x24")[0])
+    s = binding.GenFeatSizes()
+    assert lib.gen_query_feat_sizes(C.byref(cfg), C.byref(s)) == 0
+    N, S = 16384, 576
+    assert s.channels == 38 and s.plane_stride == S
+    assert s.feat == N * 2 * 38 * S * 4 and s.mem_bits == N * 2 * S and s.last_army == N * 2 * S * 2
+    assert s.last_seen == N * 2 * S * 4 and s.hist == N * 2 * 8 * 2 * S * 2
+    cfg4, _ = binding.make_config(workloads.config("c5a_2v2")[0])
+    assert lib.gen_query_feat_sizes(C.byref(cfg4), C.byref(s)) == binding_err("GEN_ERR_CONFIG")
+    assert lib.gen_query_feat_sizes(None, C.byref(s)) == binding_err("GEN_ERR_NULL")
 
 
 def test_query_sizes(lib):

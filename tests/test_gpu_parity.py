@@ -658,3 +658,110 @@ def test_full_size_configs_sampled_games(gpu, oracle_mod, name, N, T, roll):
         assert torch.equal(env.tensors["army_total"][:, p].to(torch.int64), (army.to(torch.int64) * mine).sum(1))
         assert bool((env.tensors["obs_vis"][0, :, p, :HW][mine] == 1).all())      # fog: vis contains owned (I5)
     assert int(env.tensors["episodes_done"].sum()) >= 0
+
+
+# ------------------------------------------------------------------------------- NEXT-1: 38-channel features (R35)
+def compare_features(env, o, where=""):
+    """Exact on every channel but 21 (integers and exactly rounded fp32 quotients); channel 21 = log(1 + dt) / 5
+    within 1e-6 (logf is not bit-reproducible between libm and CUDA; DESIGN R35)."""
+    got = env.features()
+    want = o.features()
+    env.torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    assert got.shape == want.shape and got.dtype == np.float32
+    for ch in range(38):
+        g, w = got[:, :, ch], want[:, :, ch]
+        if ch == 21:
+            assert np.allclose(g, w, rtol=0, atol=1e-6), f"{where}: channel 21 off by {np.abs(g - w).max()}"
+            assert np.array_equal(g == 0, w == 0), f"{where}: channel 21 zero pattern"
+        elif not np.array_equal(g, w):
+            bad = np.argwhere(g != w)
+            raise AssertionError(f"{where}: channel {ch} differs at {bad[:5].tolist()} got {g[tuple(bad[0])]} "
+                                 f"want {w[tuple(bad[0])]}")
+
+
+@pytest.mark.parametrize("name,N,T,over", [
+    ("c1_8x8", 64, 200, dict(auto_reset=1, max_turns=45)),                     # 8 games per CTA
+    ("c1_8x8", 13, 120, dict(auto_reset=0)),                                   # frozen games, ragged last CTA
+    ("c2_24x24", 37, 220, dict(max_turns=90, spawn_dmin=4)),                   # the paper-sized board
+    ("c4_curriculum", 21, 160, dict(height=5, width=7, spawn_dmin=3, spawn_dmax=5, n_cities=2, max_turns=50)),
+    ("c4_curriculum", 19, 160, dict(height=9, width=11, spawn_dmin=3, spawn_dmax=5, n_cities=3, max_turns=70)),
+    ("c2_24x24", 5, 90, dict(height=32, width=32, max_turns=60, spawn_dmin=3)),  # largest board
+    ("c2_24x24", 9, 60, dict(height=1, width=17, n_cities=1, spawn_dmin=2, max_turns=40)),   # one row
+])
+def test_features_match_oracle_every_turn(gpu, oracle_mod, name, N, T, over):
+    """gen_features after reset and after every step against orc_features on the same play: every channel of Table
+    IV, the memory across auto-resets (R17), ring wrap of the delta history, stride padding, quads that straddle
+    rows (W not a multiple of 4) and ragged CTAs."""
+    cfg, _ = workloads.config(name, n_games=N, **over)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    # the memory buffers of a fresh binding are zero; poison them to show turn 0 starts from an empty memory
+    env.reset()
+    o.reset()
+    env.features()
+    for k in ("mem_bits", "last_army", "last_seen", "hist"):
+        env.feat_tensors[k].fill_(0x55 if k != "last_seen" else 7)
+    env.feat_tensors["feat"].fill_(float("nan"))
+    compare_features(env, o, where="reset")
+    for t in range(T):
+        env.step()
+        o.step()
+        compare_features(env, o, where=f"step {t}")
+    compare(env, o, where="state untouched by gen_features")
+    if cfg["auto_reset"]:
+        assert int(o.episodes_done.sum()) > 0
+
+
+def test_features_staged_kernel_and_errors(gpu, oracle_mod):
+    """gen_features reads only the state planes and scalars, so it does not matter which kernel stepped the game
+    (here the staged one: no bitboard cache).  Multi-player handles are refused."""
+    cfg, _ = workloads.config("c2_24x24", n_games=11, max_turns=64, spawn_dmin=4)
+    env = gpu.GeneralsEnv(cfg, bitboards=False)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+    compare_features(env, o, where="reset")
+    for it in range(80):
+        env.step()
+        o.step()
+        compare_features(env, o, where=f"it {it}")
+    cfg4, _ = workloads.config("c5a_2v2", n_games=3)
+    env4 = gpu.GeneralsEnv(cfg4)
+    env4.reset()
+    with pytest.raises(gpu.GenError):
+        env4.features()
+
+
+def test_features_full_size_sampled_games(gpu, oracle_mod):
+    """BASELINE config 2 at its full batch (16,384 games) in the launch configuration bench.py --features times:
+    gen_step + gen_features every turn; the oracle replays a sample of global game ids one by one (M2)."""
+    import torch
+    N, T = 16384, 70
+    cfg, _ = workloads.config("c2_24x24", n_games=N, max_turns=50)
+    env = gpu.GeneralsEnv(cfg, digest=False, actions_out=False)
+    env.reset()
+    env.features()
+    for _ in range(T):
+        env.step()
+        feat = env.features()
+    env.torch.cuda.synchronize()
+    ids = sorted(set(list(range(6)) + list(range(N - 6, N)) + list(range(5, N, N // 11))))
+    got = feat.index_select(0, torch.tensor(ids, device=env.device)).cpu().numpy()
+    for k, gid in enumerate(ids):
+        o = oracle_mod.Oracle(dict(cfg, n_games=1, game_id_base=gid))
+        o.reset()
+        o.features()
+        for _ in range(T):
+            o.step()
+            want = o.features()
+        for ch in range(38):
+            if ch == 21:
+                assert np.allclose(got[k, :, ch], want[0, :, ch], rtol=0, atol=1e-6), (gid, ch)
+            else:
+                assert np.array_equal(got[k, :, ch], want[0, :, ch]), (gid, ch)
+    # properties at any size: the four cell classes partition the board; visible army splits by owner
+    HW = 576
+    f = feat[:, :, :, :HW]
+    assert bool(((f[:, :, 9] + f[:, :, 10] + f[:, :, 11] + f[:, :, 12]) == 1).all())
+    assert bool((f[:, :, 0] == f[:, :, 1] + f[:, :, 2] + f[:, :, 3]).all())
+    assert bool((f[:, :, 14] == env.tensors["turn"].float()[:, None, None]).all())
