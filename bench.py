@@ -32,6 +32,7 @@ HBM_FALLBACK_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PE
 # dram__bytes_read.sum + dram__bytes_write.sum of one gen_step launch, by games per launch, from the
 # `ncu --set full` capture summarised in profiles/ (see profiles/README.md); None where not captured
 NCU_DRAM_BYTES_PER_LAUNCH = {16384: 104331008}       # profiles/r01_step_full_summary.txt
+NCU_FEAT_DRAM_BYTES_PER_LAUNCH = {16384: 3601662088}  # profiles/r01_features_full_summary.txt (k_features)
 
 
 def algorithmic_bytes_per_env_step(H, W, P, packed=False):
@@ -441,7 +442,8 @@ def run_features(args):
             "step_plus_features": {"env_steps_per_s": N / (both_ms * 1e-3), "us_per_turn": 1e3 * both_ms},
             "features": {"games_per_s": N / (feat_ms * 1e-3), "us_per_launch": 1e3 * feat_ms,
                          "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                                      "frac": achieved / peak, "traffic": None, "kernel": "gen::k_features",
+                                      "frac": achieved / peak, "traffic": NCU_FEAT_DRAM_BYTES_PER_LAUNCH.get(N),
+                                      "kernel": "gen::k_features",
                                       "peak_source": peak_src, "algorithmic_bytes_per_game": bfeat,
                                       "units_per_launch": N}}}
     if not args.no_cpu_baseline:

@@ -381,6 +381,7 @@ int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *
     // 2 * S / 4 threads per game; small boards share a CTA of about 256 threads
     const int per_game = fp.S / 2;
     fp.G = per_game >= 256 ? 1 : 256 / per_game;
+    fp.force_generic = env->force_generic;
     fp.army = bufs->army; fp.owner = bufs->owner; fp.terrain = bufs->terrain; fp.turn = bufs->turn;
     fp.land = bufs->land; fp.army_total = bufs->army_total;
     fp.feat = feat->feat; fp.mem_bits = feat->mem_bits; fp.last_army = feat->last_army;

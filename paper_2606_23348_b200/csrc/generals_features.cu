@@ -3,8 +3,11 @@
 // planes (4 B per cell), the per-player memory (<= 35 B per cell and player) and writes 38 float planes per player
 // (152 B per cell and player).  Nothing here is a contraction; the work per cell is a handful of selects, so the
 // design is all about the store stream: one thread owns four consecutive cells of one player's view and issues 38
-// 16-byte streaming stores, a warp covers 512 contiguous bytes of each plane; a few CTAs of 288 threads per SM keep
-// hundreds of KB of stores in flight per SM, far beyond what the HBM latency-bandwidth product asks for.
+// 16-byte streaming stores, a warp covers 512 contiguous bytes of each plane, three CTAs of 288 threads per SM
+// keep hundreds of KB of stores in flight.  To stay off the issue and conversion pipes the kernel is compiled for
+// the paper-sized boards (no integer division, channel offsets as store immediates), army values become floats by
+// a byte permute and one add (no I2F), flags by a select, and the two coordinate planes come from a table built
+// once per CTA.
 //
 // Visibility (own cells and their 8 neighbours) is rebuilt from the owner plane, independent of which
 // observation format the step kernel was asked for: owner bytes -> one row word per player and row in shared
@@ -26,154 +29,215 @@ __device__ __forceinline__ void st4(float *p, float a, float b, float c, float d
     __stcs(reinterpret_cast<float4 *>(p), make_float4(a, b, c, d));
 }
 
-__device__ __forceinline__ void unpack4(uint2 v, int (&o)[4]) {  // four int16 in 8 bytes
-    o[0] = (int16_t)(v.x & 0xffffu); o[1] = (int16_t)(v.x >> 16);
-    o[2] = (int16_t)(v.y & 0xffffu); o[3] = (int16_t)(v.y >> 16);
+// a non-negative int16 (army counts, R21) as a float without a conversion instruction: drop its 16 bits into the
+// mantissa of 2^23 and subtract 2^23 (exact)
+__device__ __forceinline__ float lo16f(uint32_t v) {
+    return __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7610)) - 8388608.0f;
 }
-
-__device__ __forceinline__ uint2 pack4(const int (&v)[4]) {
-    return make_uint2((uint32_t)(v[0] & 0xffff) | ((uint32_t)(v[1] & 0xffff) << 16),
-                      (uint32_t)(v[2] & 0xffff) | ((uint32_t)(v[3] & 0xffff) << 16));
+__device__ __forceinline__ float hi16f(uint32_t v) {
+    return __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7632)) - 8388608.0f;
 }
+__device__ __forceinline__ void unpack4f(uint2 v, float (&o)[4]) {
+    o[0] = lo16f(v.x); o[1] = hi16f(v.x); o[2] = lo16f(v.y); o[3] = hi16f(v.y);
+}
+__device__ __forceinline__ uint32_t pack2(uint32_t lo, uint32_t hi) { return (lo & 0xffffu) | (hi << 16); }
 
 }  // namespace
 
 // grid = ceil(N / G) CTAs; a CTA serves G games with 2 * Q threads each (Q = S / 4 quads per plane).
-// dynamic shared memory: [G][S] owner bytes | [G][2][H + 2] own-row words (rows 0 and H + 1 stay zero)
-__global__ void __launch_bounds__(512) k_features(const FeatParams fp) {
+// dynamic shared memory: [G][S] owner bytes | [G][2][H + 2] own-row words (rows 0 and H + 1 stay zero) |
+// 32 + 32 coordinate floats.  TH, TW: the board this instantiation is compiled for (0 = any board).
+template <int TH, int TW, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_features(const FeatParams fp) {
     extern __shared__ __align__(16) unsigned char smem[];
-    const int S = fp.S, Q = S >> 2, H = fp.H, W = fp.W, HW = fp.HW, G = fp.G;
+    const int H = TH ? TH : fp.H, W = TW ? TW : fp.W, HW = H * W;
+    const int S = TH ? (TH * TW + 15) / 16 * 16 : fp.S, Q = S >> 2, G = fp.G;
+    constexpr bool kRowQuads = TW != 0 && TW % 4 == 0;              // a quad never straddles two rows
+    constexpr bool kAllValid = TH != 0 && (TH * TW) % 16 == 0;      // no stride padding
     int8_t *s_owner = reinterpret_cast<int8_t *>(smem);
     uint32_t *s_rows = reinterpret_cast<uint32_t *>(smem + (size_t)G * S);
+    float *s_cx = reinterpret_cast<float *>(s_rows + G * 2 * (H + 2));
+    float *s_cy = s_cx + 32;
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int g0 = blockIdx.x * G;
     const int ng = min(G, fp.N - g0);
 
-    // phase 0: owner planes of this CTA's games -> shared memory (16-byte loads; S is a multiple of 16)
-    {
-        const int4 *src = reinterpret_cast<const int4 *>(fp.owner + (size_t)g0 * S);
-        int4 *dst = reinterpret_cast<int4 *>(s_owner);
-        for (int i = tid; i < ng * (S >> 4); i += nthr) dst[i] = __ldg(src + i);
-        for (int i = tid; i < G * 2 * (H + 2); i += nthr) s_rows[i] = 0u;
-    }
-    __syncthreads();
-    // phase 1: one thread per (game, player, row) packs "owned by p" into a row word
-    for (int i = tid; i < ng * 2 * H; i += nthr) {
-        const int gl = i / (2 * H), rem = i - gl * 2 * H, p = rem / H, r = rem - p * H;
-        const int8_t *row = s_owner + gl * S + r * W;
-        uint32_t w = 0;
-        for (int c = 0; c < W; ++c) w |= (uint32_t)(row[c] == p) << c;
-        s_rows[(gl * 2 + p) * (H + 2) + r + 1] = w;
-    }
-    __syncthreads();
-
-    // phase 2: one thread per (game, player, quad)
+    // this thread's (game, player, quad); its global loads are issued before the shared-memory phases
     const int per_game = 2 * Q;
     const int gl = tid / per_game;
-    if (gl >= ng) return;
+    const bool active = gl < ng;
     const int rem = tid - gl * per_game, p = rem / Q, q = rem - p * Q;
     const int g = g0 + gl, opp = 1 - p;
     const size_t gp = (size_t)g * 2 + p;
     const int c0 = 4 * q;
 
-    const int t = __ldg(fp.turn + g);
-    const int2 land2 = __ldg(reinterpret_cast<const int2 *>(fp.land) + g);
-    const int2 tot2 = __ldg(reinterpret_cast<const int2 *>(fp.army_total) + g);
-
-    int army[4], own[4], terr[4];
-    unpack4(__ldg(reinterpret_cast<const uint2 *>(fp.army + (size_t)g * S + c0)), army);
-    {
-        const uint32_t o4 = *reinterpret_cast<const uint32_t *>(s_owner + gl * S + c0);
-        const uint32_t t4 = __ldg(reinterpret_cast<const uint32_t *>(fp.terrain + (size_t)g * S + c0));
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            own[j] = (int8_t)((o4 >> (8 * j)) & 0xffu);
-            terr[j] = (int)((t4 >> (8 * j)) & 0xffu);
-        }
-    }
-
-    // the per-episode memory; a game at turn 0 starts from an empty one (R35), whatever the buffer holds
+    int t = 0;
+    int2 land2 = make_int2(0, 0), tot2 = make_int2(0, 0);
+    uint2 army2 = make_uint2(0u, 0u);
+    uint32_t terr4 = 0, bits4 = 0;
+    uint2 last2 = make_uint2(0u, 0u);
+    int4 seen4 = make_int4(0, 0, 0, 0);                        // turn of the last sighting + 1, 0 = never
+    uint2 hown[FEAT_HIST], hen[FEAT_HIST];                     // frames t-1 .. t-7 (0 before the first frame)
     uint8_t *mb = fp.mem_bits + gp * S + c0;
     int16_t *la = fp.last_army + gp * S + c0;
     int32_t *ls = fp.last_seen + gp * S + c0;
-    int16_t *hist = fp.hist + gp * FEAT_RING * 2 * S + c0;   // [slot][kind][S]
-    uint32_t bits4 = 0;
-    int last_a[4] = {0, 0, 0, 0};
-    int4 seen4 = make_int4(0, 0, 0, 0);                       // turn of the last sighting + 1, 0 = never
-    if (t > 0) {
-        bits4 = *reinterpret_cast<const uint32_t *>(mb);
-        unpack4(*reinterpret_cast<const uint2 *>(la), last_a);
-        seen4 = *reinterpret_cast<const int4 *>(ls);
-    }
-    // frames t-1 .. t-7 of own_army / enemy_army (0 before the episode's first frame)
-    uint2 hown[FEAT_HIST], hen[FEAT_HIST];
+    int16_t *hist = fp.hist + gp * FEAT_RING * 2 * S + c0;     // [slot][kind][S]
 #pragma unroll
-    for (int k = 0; k < FEAT_HIST; ++k) {
-        hown[k] = make_uint2(0u, 0u);
-        hen[k] = make_uint2(0u, 0u);
-        if (t - k - 1 >= 0) {
-            const int slot = (t - k - 1) & (FEAT_RING - 1);
-            hown[k] = *reinterpret_cast<const uint2 *>(hist + (size_t)(slot * 2 + 0) * S);
-            hen[k] = *reinterpret_cast<const uint2 *>(hist + (size_t)(slot * 2 + 1) * S);
+    for (int k = 0; k < FEAT_HIST; ++k) hown[k] = hen[k] = make_uint2(0u, 0u);
+    if (active) {
+        t = __ldg(fp.turn + g);
+        land2 = __ldg(reinterpret_cast<const int2 *>(fp.land) + g);
+        tot2 = __ldg(reinterpret_cast<const int2 *>(fp.army_total) + g);
+        army2 = __ldg(reinterpret_cast<const uint2 *>(fp.army + (size_t)g * S + c0));
+        terr4 = __ldg(reinterpret_cast<const uint32_t *>(fp.terrain + (size_t)g * S + c0));
+        // the per-episode memory; a game at turn 0 starts from an empty one (R35), whatever the buffer holds
+        if (t > 0) {
+            bits4 = *reinterpret_cast<const uint32_t *>(mb);
+            last2 = *reinterpret_cast<const uint2 *>(la);
+            seen4 = *reinterpret_cast<const int4 *>(ls);
+        }
+#pragma unroll
+        for (int k = 0; k < FEAT_HIST; ++k) {
+            if (t - k - 1 >= 0) {
+                const int slot = (t - k - 1) & (FEAT_RING - 1);
+                hown[k] = *reinterpret_cast<const uint2 *>(hist + (size_t)(slot * 2 + 0) * S);
+                hen[k] = *reinterpret_cast<const uint2 *>(hist + (size_t)(slot * 2 + 1) * S);
+            }
         }
     }
 
-    // per-cell quantities
+    // phase 0: owner planes of this CTA's games -> shared memory (16-byte loads; S is a multiple of 16);
+    // coordinate tables col / (W - 1), row / (H - 1) (R35), one IEEE division per entry and CTA
+    {
+        const int4 *src = reinterpret_cast<const int4 *>(fp.owner + (size_t)g0 * S);
+        int4 *dst = reinterpret_cast<int4 *>(s_owner);
+        for (int i = tid; i < ng * (S >> 4); i += nthr) dst[i] = __ldg(src + i);
+        for (int i = tid; i < G * 2 * (H + 2); i += nthr) s_rows[i] = 0u;
+        if (tid < 32) s_cx[tid] = W > 1 ? __fdiv_rn((float)tid, (float)(W - 1)) : 0.0f;
+        else if (tid < 64) s_cy[tid - 32] = H > 1 ? __fdiv_rn((float)(tid - 32), (float)(H - 1)) : 0.0f;
+    }
+    __syncthreads();
+    // phase 1: one thread per (game, player, row) packs "owned by p" into a row word
+    for (int i = tid; i < ng * 2 * H; i += nthr) {
+        const int gi = i / (2 * H), ri = i - gi * 2 * H, pi = ri / H, r = ri - pi * H;
+        const int8_t *row = s_owner + gi * S + r * W;
+        uint32_t w = 0;
+        if (kRowQuads) {          // four cells per word: byte-wise compare, then gather the four flags
+#pragma unroll
+            for (int c4 = 0; c4 < TW / 4; ++c4) {
+                const uint32_t x = reinterpret_cast<const uint32_t *>(row)[c4];
+                const uint32_t m = __vcmpeq4(x, pi ? 0x01010101u : 0u) & 0x01010101u;
+                w |= ((m * 0x01020408u) >> 24) << (4 * c4);
+            }
+        } else {
+            for (int c = 0; c < W; ++c) w |= (uint32_t)(row[c] == pi) << c;
+        }
+        s_rows[(gi * 2 + pi) * (H + 2) + r + 1] = w;
+    }
+    __syncthreads();
+    if (!active) return;
+
+    // phase 2: per-cell quantities of the quad
+    const uint32_t own4 = *reinterpret_cast<const uint32_t *>(s_owner + gl * S + c0);
     const uint32_t *rows = s_rows + (gl * 2 + p) * (H + 2);
-    int vis[4], valid[4], colv[4], rowv[4], own_a[4], en_a[4], en_vis[4];
+    bool valid[4], vis[4], mine[4], en[4], neu[4];
+    int rowj[4], colj[4];
+    if (kRowQuads) {
+        const bool ok = kAllValid || c0 < HW;
+        const int r = ok ? c0 / W : 0, col0 = ok ? c0 - r * W : 0;
+        uint32_t v = rows[r] | rows[r + 1] | rows[r + 2];
+        v |= (v << 1) | (v >> 1);
+        v = ok ? v >> col0 : 0u;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { valid[j] = ok; vis[j] = (v >> j) & 1u; rowj[j] = r; colj[j] = col0 + j; }
+    } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int c = c0 + j;
+            valid[j] = c < HW;
+            const int r = valid[j] ? c / W : 0, col = valid[j] ? c - r * W : 0;
+            uint32_t v = rows[r] | rows[r + 1] | rows[r + 2];
+            v |= (v << 1) | (v >> 1);
+            vis[j] = valid[j] && ((v >> col) & 1u);
+            rowj[j] = r; colj[j] = col;
+        }
+    }
+    const uint32_t a16[4] = {army2.x & 0xffffu, army2.x >> 16, army2.y & 0xffffu, army2.y >> 16};
+    uint32_t l16[4] = {last2.x & 0xffffu, last2.x >> 16, last2.y & 0xffffu, last2.y >> 16};
     int seen[4] = {seen4.x, seen4.y, seen4.z, seen4.w};
+    uint32_t own_f[4], en_f[4];                                  // this turn's history frames
     uint32_t newbits4 = bits4;
     bool any_en = false;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        const int c = c0 + j;
-        valid[j] = c < HW;
-        const int r = valid[j] ? c / W : 0, col = valid[j] ? c - r * W : 0;
-        rowv[j] = r; colv[j] = col;
-        uint32_t v = rows[r] | rows[r + 1] | rows[r + 2];
-        v |= (v << 1) | (v >> 1);
-        vis[j] = valid[j] ? (int)((v >> col) & 1u) : 0;
-        own_a[j] = (valid[j] && own[j] == p) ? army[j] : 0;
-        en_vis[j] = vis[j] && own[j] == opp;
-        en_a[j] = en_vis[j] ? army[j] : 0;
-        uint32_t b = (uint32_t)vis[j] | ((uint32_t)en_vis[j] << 1);
-        if (vis[j]) b |= (terr[j] == 3 ? 4u : 0u) | (terr[j] == 2 ? 8u : 0u) | (terr[j] == 1 ? 16u : 0u);
+        const int o = (int8_t)((own4 >> (8 * j)) & 0xffu);
+        const uint32_t tr = (terr4 >> (8 * j)) & 0xffu;
+        mine[j] = valid[j] && o == p;
+        en[j] = vis[j] && o == opp;
+        neu[j] = vis[j] && o == -1;
+        uint32_t b = (uint32_t)vis[j] | ((uint32_t)en[j] << 1);
+        if (vis[j]) b |= (tr == 3u ? 4u : 0u) | (tr == 2u ? 8u : 0u) | (tr == 1u ? 16u : 0u);
         newbits4 |= b << (8 * j);
-        if (en_vis[j]) { last_a[j] = army[j]; seen[j] = t + 1; any_en = true; }
+        if (en[j]) { l16[j] = a16[j]; seen[j] = t + 1; any_en = true; }
+        own_f[j] = mine[j] ? a16[j] : 0u;
+        en_f[j] = en[j] ? a16[j] : 0u;
     }
+    const uint2 newlast2 = make_uint2(pack2(l16[0], l16[1]), pack2(l16[2], l16[3]));
     // fold into the memory (stores only where something changed)
     if (newbits4 != bits4 || t == 0) *reinterpret_cast<uint32_t *>(mb) = newbits4;
     if (any_en || t == 0) {
-        *reinterpret_cast<uint2 *>(la) = pack4(last_a);
+        *reinterpret_cast<uint2 *>(la) = newlast2;
         *reinterpret_cast<int4 *>(ls) = make_int4(seen[0], seen[1], seen[2], seen[3]);
     }
     {
         const int slot = t & (FEAT_RING - 1);
-        *reinterpret_cast<uint2 *>(hist + (size_t)(slot * 2 + 0) * S) = pack4(own_a);
-        *reinterpret_cast<uint2 *>(hist + (size_t)(slot * 2 + 1) * S) = pack4(en_a);
+        *reinterpret_cast<uint2 *>(hist + (size_t)(slot * 2 + 0) * S) =
+            make_uint2(pack2(own_f[0], own_f[1]), pack2(own_f[2], own_f[3]));
+        *reinterpret_cast<uint2 *>(hist + (size_t)(slot * 2 + 1) * S) =
+            make_uint2(pack2(en_f[0], en_f[1]), pack2(en_f[2], en_f[3]));
     }
 
-    // Table IV, channel by channel
+    // Table IV, channel by channel.  EMIT(ch, expr): expr is a float in terms of j; padding cells are 0.
     float *out = fp.feat + gp * FEAT_C * S + c0;
-    float f[4];
-#define EMIT(ch, expr)                                                     \
-    {                                                                      \
-        _Pragma("unroll") for (int j = 0; j < 4; ++j) f[j] = valid[j] ? (float)(expr) : 0.0f; \
-        st4(out + (size_t)(ch) * S, f[0], f[1], f[2], f[3]);               \
+    float f[4], fa[4];
+    unpack4f(army2, fa);
+#define EMIT(ch, expr)                                                                                  \
+    {                                                                                                   \
+        _Pragma("unroll") for (int j = 0; j < 4; ++j) f[j] = (kAllValid || valid[j]) ? (expr) : 0.0f;  \
+        st4(out + (size_t)(ch) * S, f[0], f[1], f[2], f[3]);                                            \
     }
-    EMIT(0, vis[j] ? army[j] : 0)
-    EMIT(1, own_a[j])
-    EMIT(2, en_a[j])
-    EMIT(3, (vis[j] && own[j] == -1) ? army[j] : 0)
-#pragma unroll
-    for (int k = 0; k < 5; ++k) EMIT(4 + k, (newbits4 >> (8 * j + k)) & 1u)
-    EMIT(9, vis[j] && own[j] == -1)
-    EMIT(10, own[j] == p)
-    EMIT(11, en_vis[j])
-    EMIT(12, !vis[j])
-    EMIT(13, !vis[j] && ((newbits4 >> (8 * j)) & 0x1cu) != 0u)
+    // deltas first (the 28 registers of history frames retire early): frame(t-k) - frame(t-k-1), 0 when t-k-1 < 0;
+    // frames are exact small integers in fp32, so the float difference is exact
     {
-        const float ft = (float)t, tick = (float)(t % 50) / 50.0f;
+        float cur_o[4], cur_e[4], prev[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { cur_o[j] = mine[j] ? fa[j] : 0.0f; cur_e[j] = en[j] ? fa[j] : 0.0f; }
+#pragma unroll
+        for (int k = 0; k < FEAT_HIST; ++k) {
+            const bool have = t - k - 1 >= 0;
+            unpack4f(hown[k], prev);
+            EMIT(24 + k, have ? cur_o[j] - prev[j] : 0.0f)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) cur_o[j] = prev[j];
+            unpack4f(hen[k], prev);
+            EMIT(31 + k, have ? cur_e[j] - prev[j] : 0.0f)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) cur_e[j] = prev[j];
+        }
+    }
+    EMIT(0, vis[j] ? fa[j] : 0.0f)
+    EMIT(1, mine[j] ? fa[j] : 0.0f)
+    EMIT(2, en[j] ? fa[j] : 0.0f)
+    EMIT(3, neu[j] ? fa[j] : 0.0f)
+#pragma unroll
+    for (int k = 0; k < 5; ++k) EMIT(4 + k, ((newbits4 >> (8 * j + k)) & 1u) ? 1.0f : 0.0f)
+    EMIT(9, neu[j] ? 1.0f : 0.0f)
+    EMIT(10, mine[j] ? 1.0f : 0.0f)
+    EMIT(11, en[j] ? 1.0f : 0.0f)
+    EMIT(12, vis[j] ? 0.0f : 1.0f)
+    EMIT(13, (!vis[j] && ((newbits4 >> (8 * j)) & 0x1cu) != 0u) ? 1.0f : 0.0f)
+    {
+        const float ft = (float)t, tick = __fdiv_rn((float)(t % 50), 50.0f);
         const float l_me = (float)(p ? land2.y : land2.x), a_me = (float)(p ? tot2.y : tot2.x);
         const float l_op = (float)(p ? land2.x : land2.y), a_op = (float)(p ? tot2.x : tot2.y);
         EMIT(14, ft)
@@ -183,41 +247,47 @@ __global__ void __launch_bounds__(512) k_features(const FeatParams fp) {
         EMIT(18, l_op)
         EMIT(19, a_op)
     }
-    EMIT(20, last_a[j])
-    EMIT(21, (seen[j] == 0 || en_vis[j]) ? 0.0f : logf(1.0f + (float)(t - (seen[j] - 1))) / 5.0f)
     {
-        const float wx = (float)(W - 1), hy = (float)(H - 1);
-        EMIT(22, W > 1 ? (float)colv[j] / wx : 0.0f)
-        EMIT(23, H > 1 ? (float)rowv[j] / hy : 0.0f)
-    }
-    // deltas: frame(t-k) - frame(t-k-1), 0 when t-k-1 < 0
-    {
-        int cur_o[4], cur_e[4], prev[4];
+        float fl[4], age[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+        unpack4f(newlast2, fl);
+        EMIT(20, fl[j])
+        // log(1 + turns since the last sighting) / 5; 0 where the enemy was never seen or is visible now (R35).
+        // Most quads have no remembered enemy cell: the transcendental path is skipped for them.
+        bool need = false;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) { cur_o[j] = own_a[j]; cur_e[j] = en_a[j]; }
+        for (int j = 0; j < 4; ++j) need |= seen[j] != 0 && !en[j];
+        if (need) {
 #pragma unroll
-        for (int k = 0; k < FEAT_HIST; ++k) {
-            const bool have = t - k - 1 >= 0;
-            unpack4(hown[k], prev);
-            EMIT(24 + k, have ? cur_o[j] - prev[j] : 0)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) cur_o[j] = prev[j];
-            unpack4(hen[k], prev);
-            EMIT(31 + k, have ? cur_e[j] - prev[j] : 0)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) cur_e[j] = prev[j];
+            for (int j = 0; j < 4; ++j)
+                if (seen[j] != 0 && !en[j]) age[j] = __fdiv_rn(logf(1.0f + (float)(t - (seen[j] - 1))), 5.0f);
         }
+        EMIT(21, age[j])
     }
+    EMIT(22, s_cx[colj[j]])
+    EMIT(23, s_cy[rowj[j]])
 #undef EMIT
 }
 
+namespace {
+
+template <int TH, int TW, int MAXT, int MINB>
+cudaError_t launch_one(const FeatParams &fp, int threads, cudaStream_t stream) {
+    const size_t smem = (size_t)fp.G * fp.S + (size_t)fp.G * 2 * (fp.H + 2) * 4 + 64 * 4;
+    const int grid = (fp.N + fp.G - 1) / fp.G;
+    k_features<TH, TW, MAXT, MINB><<<grid, threads, smem, stream>>>(fp);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// Board-specialised instantiations for the paper-sized 1v1 boards (BASELINE configs 1 and 2-4), else the generic one.
 cudaError_t launch_features(const FeatParams &fp, cudaStream_t stream) {
     const int per_game = 2 * (fp.S >> 2);
     const int threads = (fp.G * per_game + 31) / 32 * 32;
-    const size_t smem = (size_t)fp.G * fp.S + (size_t)fp.G * 2 * (fp.H + 2) * 4;
-    const int grid = (fp.N + fp.G - 1) / fp.G;
-    k_features<<<grid, threads, smem, stream>>>(fp);
-    return cudaGetLastError();
+    if (threads < 64) return cudaErrorInvalidConfiguration;   // the coordinate tables need two warps
+    if (!fp.force_generic && fp.H == 24 && fp.W == 24 && threads <= 288) return launch_one<24, 24, 288, 3>(fp, threads, stream);
+    if (!fp.force_generic && fp.H == 8 && fp.W == 8 && threads <= 256) return launch_one<8, 8, 256, 4>(fp, threads, stream);
+    return launch_one<0, 0, 512, 2>(fp, threads, stream);
 }
 
 }  // namespace gen

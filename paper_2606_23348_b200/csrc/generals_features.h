@@ -8,6 +8,7 @@ namespace gen {
 struct FeatParams {
     int N, H, W, HW, S;
     int G;                       // games per CTA (2 * S / 4 threads each)
+    int force_generic;           // never launch a board-specialised instantiation (tests)
     const int16_t *army;         // state planes and scalars of gen_buffers (read only)
     const int8_t *owner;
     const int8_t *terrain;

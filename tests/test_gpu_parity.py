@@ -714,9 +714,11 @@ def test_features_match_oracle_every_turn(gpu, oracle_mod, name, N, T, over):
 
 def test_features_staged_kernel_and_errors(gpu, oracle_mod):
     """gen_features reads only the state planes and scalars, so it does not matter which kernel stepped the game
-    (here the staged one: no bitboard cache).  Multi-player handles are refused."""
+    (here the staged one: no bitboard cache), nor whether k_features was compiled for the board (here: not).
+    Multi-player handles are refused."""
     cfg, _ = workloads.config("c2_24x24", n_games=11, max_turns=64, spawn_dmin=4)
     env = gpu.GeneralsEnv(cfg, bitboards=False)
+    env.set_generic(True, True)                              # the generic k_features instantiation on a 24x24 board
     o = oracle_mod.Oracle(cfg)
     env.reset()
     o.reset()
