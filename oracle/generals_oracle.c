@@ -19,6 +19,9 @@
  *   step rules      : hand-worked examples W1..W11, closed forms C1..C3,
  *                     invariants I1..I7, brute force B1/B2, metamorphic M1/M2
  *   generator       : statistical + constraint checks, brute-force candidate lists
+ *   official maps   : (R36) constraints of P:L79 re-checked with an independent shortest-path routine, Manhattan
+ *                     closed form, tiny boards by hand (tests/test_oracle_mapgen.py)
+ *   feature tensor  : (R35) channel identities, closed form, an independent memory log (test_oracle_features.py)
  *   sampler         : brute force "valid set == set of board-changing actions"
  * Parity unpinned BY THE PAPER (fixed by decree in DESIGN.md, the paper prints no
  * value that decides them): R6 move order, R11 rounding of the transferred half,
@@ -45,6 +48,10 @@ typedef struct {
     uint32_t rule_flags, game_id_base, mountain_thr;
     uint32_t pass_thr, half_thr, bias_thr, pad_;
     uint64_t seed;
+    int32_t map_mode;         /* 0 = synthetic generator (R30), 1 = official generator (R36) */
+    int32_t n_cities_max;     /* R36: castle count uniform in [n_cities, n_cities_max]; 0 = exactly n_cities */
+    int32_t play_min;         /* R36: playable area h x w uniform in [play_min..H] x [play_min..W]; 0 = H x W */
+    int32_t castle_radius;    /* R36: each general has a castle within this many steps (6); 0 = none */
 } orc_config;
 
 /* all arrays host memory, game-major; S = plane stride = round_up(H*W, 16) */
@@ -139,8 +146,10 @@ static int iabs(int x) { return x < 0 ? -x : x; }
  * P:L79 gives only the distribution; the algorithm is reading R30, on the
  * synthetic recipe of BASELINE.json (Bernoulli mountains, fixed city count,
  * Manhattan spawn distance, R29). */
+static void generate_official(const orc_config *cfg, const orc_buffers *b, int g);
 static void generate(const orc_config *cfg, const orc_buffers *b, int g)
 {
+    if (cfg->map_mode == 1) { generate_official(cfg, b, g); return; }
     const int H = cfg->height, W = cfg->width, P = cfg->n_players, HW = H * W, S = plane_stride(cfg);
     const uint32_t gid = cfg->game_id_base + (uint32_t)g, ep = b->episode[g];
     int16_t *army = b->army + (size_t)g * S;
@@ -208,6 +217,125 @@ static void generate(const orc_config *cfg, const orc_buffers *b, int g)
     free(list);
     b->turn[g] = 0;
     b->alive[g] = (uint8_t)((1u << P) - 1u);
+}
+
+/* ------------------------------------------------------------ NEXT-3: the official generator (R36)
+ * "fills a random 20% of cells with mountains and places 9-11 neutral castles, each pre-loaded with 40-50
+ * neutral units.  The two generals are placed at least 17 steps apart, and each player is guaranteed at least one
+ * neutral castle within radius 6 of their general"; the distance is the BFS distance; "cells
+ * outside the playable area are padded with mountain tokens".  The paper gives the constraints, not the
+ * procedure; reading R36 is rejection sampling over whole maps, 1v1 only.  Attempt a = 0..15, every
+ * draw of attempt a carries a in the counter's player byte:
+ *   (0) one draw fixes the playable size h x w, the spawn window [lo, hi] (in steps) and the castle count;
+ *   (1) cells outside the playable rectangle (top-left anchored) are MOUNTAIN; inside, Bernoulli(mountain_thr)
+ *       with the same word assignment as R30; on the last attempt the playable area has no mountains;
+ *   (2) general 0 uniform over the PLAIN cells (row-major list); none => next attempt;
+ *   (3) dist0 = BFS steps from general 0 over non-mountain cells (4-neighbourhood);
+ *   (4) general 1 uniform over the PLAIN cells with lo <= dist0 <= hi; none => next attempt (last attempt: widen
+ *       the window by one on each side until some cell qualifies, as R30 does);
+ *   (5) castle 0 uniform over PLAIN cells with dist0 <= radius, castle 1 over PLAIN cells with dist1 <= radius
+ *       (BFS from general 1); none => next attempt (last attempt: over all PLAIN cells); castles 2.. uniform over
+ *       the remaining PLAIN cells; garrison lo + mulhi32(u, span) as R14.  radius 0: every castle uniform.
+ * Unreachable cells have no distance and never qualify, so an accepted map always connects the two generals. */
+enum { MAP_ATTEMPTS = 16, DIST_NONE = 1 << 20 };
+
+static void bfs_steps(const int8_t *terrain, int H, int W, int src, int *dist, int *queue)
+{
+    for (int c = 0; c < H * W; ++c) dist[c] = DIST_NONE;
+    int head = 0, tail = 0;
+    dist[src] = 0; queue[tail++] = src;
+    while (head < tail) {
+        const int c = queue[head++], r = c / W, col = c % W;
+        const int nb[4] = { r > 0 ? c - W : -1, r < H - 1 ? c + W : -1, col > 0 ? c - 1 : -1, col < W - 1 ? c + 1 : -1 };
+        for (int k = 0; k < 4; ++k) {
+            const int n = nb[k];
+            if (n < 0 || terrain[n] == T_MOUNTAIN || dist[n] != DIST_NONE) continue;
+            dist[n] = dist[c] + 1; queue[tail++] = n;
+        }
+    }
+}
+
+static void generate_official(const orc_config *cfg, const orc_buffers *b, int g)
+{
+    const int H = cfg->height, W = cfg->width, HW = H * W, S = plane_stride(cfg);
+    const uint32_t gid = cfg->game_id_base + (uint32_t)g, ep = b->episode[g];
+    int16_t *army = b->army + (size_t)g * S;
+    int8_t *owner = b->owner + (size_t)g * S, *terrain = b->terrain + (size_t)g * S;
+    int16_t *gen = b->general_cell + (size_t)g * 2;
+    int *list = (int *)malloc(sizeof(int) * (size_t)HW * 4);
+    int *dist0 = list + HW, *dist1 = list + 2 * HW, *queue = list + 3 * HW;
+    uint32_t w[4];
+
+    for (uint32_t a = 0; a < MAP_ATTEMPTS; ++a) {
+        const int last = (a == MAP_ATTEMPTS - 1);
+        /* (0) sizes of this attempt */
+        draw(cfg, gid, DOM_SPAWN, 0, ep, a, w);
+        int h = H, wd = W;
+        if (cfg->play_min > 0) {
+            const int hmin = cfg->play_min < H ? cfg->play_min : H, wmin = cfg->play_min < W ? cfg->play_min : W;
+            h = hmin + (int)mulhi32(w[0], (uint32_t)(H - hmin + 1));
+            wd = wmin + (int)mulhi32(w[1], (uint32_t)(W - wmin + 1));
+        }
+        int lo = cfg->spawn_dmin, hi = cfg->spawn_dmax > 0 ? cfg->spawn_dmax : DIST_NONE - 1;
+        if (cfg->spawn_exact)
+            lo = hi = cfg->spawn_dmin + (int)mulhi32(w[2], (uint32_t)(cfg->spawn_dmax - cfg->spawn_dmin + 1));
+        int n_castles = cfg->n_cities;
+        if (cfg->n_cities_max > cfg->n_cities)
+            n_castles += (int)mulhi32(w[3], (uint32_t)(cfg->n_cities_max - cfg->n_cities + 1));
+        /* (1) terrain */
+        for (int c = 0; c < S; ++c) { army[c] = 0; owner[c] = OWNER_NEUTRAL; terrain[c] = T_MOUNTAIN; }
+        for (int c = 0; c < HW; ++c) {
+            if (c / W >= h || c % W >= wd) continue;
+            uint32_t m[4];
+            draw(cfg, gid, DOM_MOUNTAIN, (uint32_t)(c >> 2), ep, a, m);
+            terrain[c] = (!last && m[c & 3] < cfg->mountain_thr) ? T_MOUNTAIN : T_PLAIN;
+        }
+        /* (2) general 0 */
+        draw(cfg, gid, DOM_SPAWN, 1, ep, a, w);
+        int n = 0;
+        for (int c = 0; c < HW; ++c) if (terrain[c] == T_PLAIN) list[n++] = c;
+        if (n == 0) continue;
+        const int g0 = list[mulhi32(w[0], (uint32_t)n)];
+        /* (3), (4) general 1 at lo..hi steps */
+        bfs_steps(terrain, H, W, g0, dist0, queue);
+        for (;;) {
+            n = 0;
+            for (int c = 0; c < HW; ++c)
+                if (terrain[c] == T_PLAIN && c != g0 && dist0[c] >= lo && dist0[c] <= hi) list[n++] = c;
+            if (n > 0 || !last) break;
+            if (lo == 0 && hi >= HW) break;                 /* a one-cell playable area: nothing to place */
+            if (lo > 0) lo -= 1;
+            hi += 1;
+        }
+        if (n == 0) continue;
+        const int g1 = list[mulhi32(w[1], (uint32_t)n)];
+        bfs_steps(terrain, H, W, g1, dist1, queue);
+        terrain[g0] = T_GENERAL; owner[g0] = 0; army[g0] = 1;       /* R13 */
+        terrain[g1] = T_GENERAL; owner[g1] = 1; army[g1] = 1;
+        /* (5) castles */
+        int ok = 1;
+        for (int k = 0; k < n_castles; ++k) {
+            const int *near = (cfg->castle_radius > 0 && k < 2) ? (k == 0 ? dist0 : dist1) : NULL;
+            n = 0;
+            if (near)
+                for (int c = 0; c < HW; ++c) if (terrain[c] == T_PLAIN && near[c] <= cfg->castle_radius) list[n++] = c;
+            if (near && n == 0 && !last) { ok = 0; break; }
+            if (n == 0)
+                for (int c = 0; c < HW; ++c) if (terrain[c] == T_PLAIN) list[n++] = c;
+            if (n == 0) break;
+            draw(cfg, gid, DOM_CITY, (uint32_t)k, ep, a, w);
+            const int cell = list[mulhi32(w[0], (uint32_t)n)];
+            terrain[cell] = T_CITY;
+            army[cell] = (int16_t)(cfg->city_army_lo +
+                                   (int)mulhi32(w[1], (uint32_t)(cfg->city_army_hi - cfg->city_army_lo + 1)));
+        }
+        if (!ok) continue;
+        gen[0] = (int16_t)g0; gen[1] = (int16_t)g1;
+        break;
+    }
+    free(list);
+    b->turn[g] = 0;
+    b->alive[g] = 3;
 }
 
 /* ------------------------------------------------- a7: scoreboard (R23) */

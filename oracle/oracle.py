@@ -34,7 +34,8 @@ class OrcConfig(C.Structure):
         "n_games", "height", "width", "n_players", "team_size", "n_cities", "city_army_lo",
         "city_army_hi", "spawn_dmin", "spawn_dmax", "spawn_exact", "max_turns", "auto_reset")] + [
         (n, C.c_uint32) for n in ("rule_flags", "game_id_base", "mountain_thr", "pass_thr", "half_thr",
-                                  "bias_thr", "pad_")] + [("seed", C.c_uint64)]
+                                  "bias_thr", "pad_")] + [("seed", C.c_uint64)] + [
+        (n, C.c_int32) for n in ("map_mode", "n_cities_max", "play_min", "castle_radius")]
 
 
 _BUF_FIELDS = [
