@@ -75,6 +75,14 @@ typedef struct gen_config {
     uint32_t game_id_base; /* global game id = game_id_base + g keys every random draw */
     uint32_t mountain_thr; /* P(mountain) = mountain_thr / 2^32 per non-general cell */
     uint64_t seed;         /* Philox4x32-10 key */
+    /* the official map generator (R36).  All zero = the synthetic
+     * generator of R30 (BASELINE configs 1-5). */
+    int32_t map_mode;      /* 0 synthetic (R30); 1 official: spawn distance in BFS steps, connected generals, castle
+                              guarantee, optional mountain-padded playable area.  1v1 only */
+    int32_t n_cities_max;  /* map_mode 1: castle count uniform in [n_cities, n_cities_max] (9-11); 0 = n_cities */
+    int32_t play_min;      /* map_mode 1: playable area h x w uniform in [play_min, H] x [play_min, W], top-left
+                              anchored, the rest mountains; 0 = the full board */
+    int32_t castle_radius; /* map_mode 1: each general has a castle within this many steps (6); 0 = no guarantee */
 } gen_config;
 
 /* probabilities as uint32 thresholds floor(p * 2^32): no float enters the hot path (R24, R25) */

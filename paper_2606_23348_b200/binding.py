@@ -29,7 +29,8 @@ class GenConfig(C.Structure):
     _fields_ = [(n, C.c_int32) for n in (
         "n_games", "height", "width", "n_players", "team_size", "n_cities", "city_army_lo",
         "city_army_hi", "spawn_dmin", "spawn_dmax", "spawn_exact", "max_turns", "auto_reset")] + [
-        (n, C.c_uint32) for n in ("rule_flags", "game_id_base", "mountain_thr")] + [("seed", C.c_uint64)]
+        (n, C.c_uint32) for n in ("rule_flags", "game_id_base", "mountain_thr")] + [("seed", C.c_uint64)] + [
+        (n, C.c_int32) for n in ("map_mode", "n_cities_max", "play_min", "castle_radius")]
 
 
 class GenPolicy(C.Structure):

@@ -39,6 +39,17 @@ int validate(const gen_config *c) {
     if (c->max_turns < 0) return GEN_ERR_CONFIG;
     if (c->rule_flags & ~7u) return GEN_ERR_CONFIG;
     if ((uint64_t)c->game_id_base + (uint64_t)c->n_games > 0x100000000ull) return GEN_ERR_CONFIG;
+    if (c->map_mode != 0 && c->map_mode != 1) return GEN_ERR_CONFIG;
+    if (c->map_mode == 0 && (c->n_cities_max || c->play_min || c->castle_radius)) return GEN_ERR_CONFIG;
+    if (c->map_mode == 1) {                                    // the official generator (R36): 1v1
+        if (c->n_players != 2 || c->team_size != 1) return GEN_ERR_CONFIG;
+        if (c->n_cities_max != 0 && c->n_cities_max < c->n_cities) return GEN_ERR_CONFIG;
+        if (c->n_cities_max > c->height * c->width) return GEN_ERR_CONFIG;
+        if (c->play_min < 0 || c->castle_radius < 0) return GEN_ERR_CONFIG;
+        const int hmin = c->play_min > 0 && c->play_min < c->height ? c->play_min : c->height;
+        const int wmin = c->play_min > 0 && c->play_min < c->width ? c->play_min : c->width;
+        if (hmin * wmin < 2) return GEN_ERR_CONFIG;            // two generals need two cells
+    }
     return GEN_OK;
 }
 
@@ -243,6 +254,8 @@ int gen_init(const gen_config *cfg, gen_env **out) {
     k.city_span = cfg->city_army_hi - cfg->city_army_lo + 1;
     k.dmin = cfg->spawn_dmin; k.dmax = cfg->spawn_dmax; k.spawn_exact = cfg->spawn_exact;
     k.max_turns = cfg->max_turns; k.auto_reset = cfg->auto_reset;
+    k.map_mode = cfg->map_mode; k.n_cities_max = cfg->n_cities_max; k.play_min = cfg->play_min;
+    k.castle_radius = cfg->castle_radius;
     k.rule_flags = cfg->rule_flags; k.gid_base = cfg->game_id_base; k.mountain_thr = cfg->mountain_thr;
     k.key0 = (uint32_t)(cfg->seed & 0xffffffffu); k.key1 = (uint32_t)(cfg->seed >> 32);
     // row = (cell * recipW) >> 16 must equal cell / W for every cell of the largest board

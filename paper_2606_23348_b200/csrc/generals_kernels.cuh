@@ -79,6 +79,7 @@ struct KParams {
     int32_t team_size, n_teams;
     int32_t n_cities, city_lo, city_span;
     int32_t dmin, dmax, spawn_exact, max_turns, auto_reset;
+    int32_t map_mode, n_cities_max, play_min, castle_radius;  // R36 (official generator)
     uint32_t rule_flags, gid_base, mountain_thr, key0, key1;
     uint32_t pass_thr, half_thr, bias_thr;
     uint32_t global_step0, flags, recipW;
@@ -207,6 +208,148 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     } while (!ok);
 }
 
+// ------------------------------------------------------------------------------------------------
+// NEXT-3: the official map generator (R36), one warp per game, 1v1.
+// The board is held as ROW WORDS while it is built: lane r owns row r, bit c = column c (H, W <= 32).  Steps
+// between cells (the paper's BFS distance) come from a frontier expansion on those words: one level = two
+// shifts, two shuffles (the rows above and below) and a mask with the passable cells.
+__device__ __forceinline__ uint32_t rows_count(uint32_t word) { return __reduce_add_sync(FULL, __popc(word)); }
+
+// cell index of the k-th set bit, row-major, of a board held one row word per lane
+__device__ __forceinline__ int rows_select(uint32_t word, uint32_t k, uint32_t lane, int W) {
+    const uint32_t cnt = __popc(word);
+    uint32_t incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(FULL, incl, o);
+        if (lane >= (uint32_t)o) incl += v;
+    }
+    const uint32_t b = __ballot_sync(FULL, k < incl);
+    const int j = __ffs(b) - 1;
+    const uint32_t excl_j = __shfl_sync(FULL, incl - cnt, j);
+    const uint32_t wj = __shfl_sync(FULL, word, j);
+    return j * W + nth_bit(wj, k - excl_j);
+}
+
+// V_i = the cells within t_i steps of (src_r, src_c) over `pass` (t_i < 0: the empty set); stops at the largest
+// threshold or when the frontier dies (then every later threshold sees the whole reachable set)
+static __device__ __noinline__ void rows_bfs(uint32_t pass, int src_r, int src_c, uint32_t lane, int t0, int t1, int t2,
+                                      uint32_t &V0, uint32_t &V1, uint32_t &V2) {
+    uint32_t V = ((int)lane == src_r) ? 1u << src_c : 0u, F = V;
+    V0 = V1 = V2 = 0u;
+    const int tmax = max(t0, max(t1, t2));
+    for (int L = 0;; ++L) {
+        if (L == t0) V0 = V;
+        if (L == t1) V1 = V;
+        if (L == t2) V2 = V;
+        if (L >= tmax) break;
+        uint32_t up = __shfl_up_sync(FULL, F, 1), dn = __shfl_down_sync(FULL, F, 1);
+        if (lane == 0) up = 0u;
+        if (lane == 31) dn = 0u;
+        const uint32_t N = ((F << 1) | (F >> 1) | up | dn) & pass & ~V;
+        if (!__any_sync(FULL, N != 0u)) {
+            if (t0 > L) V0 = V;
+            if (t1 > L) V1 = V;
+            if (t2 > L) V2 = V;
+            break;
+        }
+        V |= N;
+        F = N;
+    }
+}
+
+static __device__ __noinline__ void generate_official(const KParams &kp, uint32_t lane, uint32_t gid, uint32_t episode,
+                                               int16_t *A, int8_t *O, int8_t *Tr, int16_t *gcell_out) {
+    const int H = kp.H, W = kp.W, HW = kp.HW, S = kp.S;
+    constexpr int kAttempts = 16, kFar = (1 << 20) - 1;
+    uint32_t w[4];
+    for (uint32_t a = 0; a < (uint32_t)kAttempts; ++a) {
+        const bool last = a == (uint32_t)kAttempts - 1;
+        __syncwarp();
+        // (0) sizes of this attempt
+        philox(0u, gid, episode, (DOM_SPAWN << 24) | a, kp.key0, kp.key1, w);
+        int h = H, wd = W;
+        if (kp.play_min > 0) {
+            const int hmin = min(kp.play_min, H), wmin = min(kp.play_min, W);
+            h = hmin + (int)mulhi32(w[0], (uint32_t)(H - hmin + 1));
+            wd = wmin + (int)mulhi32(w[1], (uint32_t)(W - wmin + 1));
+        }
+        int lo = kp.dmin, hi = kp.dmax > 0 ? kp.dmax : kFar;
+        if (kp.spawn_exact) lo = hi = kp.dmin + (int)mulhi32(w[2], (uint32_t)(kp.dmax - kp.dmin + 1));
+        int n_castles = kp.n_cities;
+        if (kp.n_cities_max > kp.n_cities) n_castles += (int)mulhi32(w[3], (uint32_t)(kp.n_cities_max - kp.n_cities + 1));
+        // (1) terrain: mountains outside the playable rectangle, Bernoulli inside (none on the last attempt)
+        for (int q = (int)lane; q < S / 4; q += 32) {
+            philox((uint32_t)q, gid, episode, (DOM_MOUNTAIN << 24) | a, kp.key0, kp.key1, w);
+            uint32_t tw = 0;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const int c = 4 * q + b, r = (int)(((uint32_t)c * kp.recipW) >> 16), col = c - r * W;
+                const bool playable = c < HW && r < h && col < wd;
+                tw |= (!playable || (!last && w[b] < kp.mountain_thr)) ? (uint32_t)T_MOUNTAIN << (8 * b) : 0u;
+            }
+            reinterpret_cast<uint32_t *>(Tr)[q] = tw;
+            reinterpret_cast<uint32_t *>(O)[q] = 0xFFFFFFFFu;
+            reinterpret_cast<uint32_t *>(A)[2 * q] = 0;
+            reinterpret_cast<uint32_t *>(A)[2 * q + 1] = 0;
+        }
+        __syncwarp();
+        uint32_t plain = 0;                                     // lane r: the PLAIN cells of row r
+        if ((int)lane < H)
+            for (int col = 0; col < W; ++col) plain |= (uint32_t)(Tr[(int)lane * W + col] == T_PLAIN) << col;
+        const uint32_t pass = plain;                            // non-mountain cells: castles do not block
+        // (2) general 0
+        philox(1u, gid, episode, (DOM_SPAWN << 24) | a, kp.key0, kp.key1, w);
+        const uint32_t u_g1 = w[1];
+        uint32_t n = rows_count(plain);
+        if (n == 0) continue;
+        const int g0 = rows_select(plain, mulhi32(w[0], n), lane, W);
+        const int r0 = (int)(((uint32_t)g0 * kp.recipW) >> 16), c0 = g0 - r0 * W;
+        if ((int)lane == r0) plain &= ~(1u << c0);
+        // (3), (4) general 1 at lo..hi steps
+        uint32_t cand, Vlo, Vhi, Vnear0, Vnear1, unused;
+        for (;;) {
+            rows_bfs(pass, r0, c0, lane, lo - 1, hi, kp.castle_radius, Vlo, Vhi, Vnear0);
+            cand = plain & Vhi & ~Vlo;
+            n = rows_count(cand);
+            if (n > 0 || !last) break;
+            if (lo == 0 && hi >= HW) break;
+            if (lo > 0) lo -= 1;
+            hi += 1;
+        }
+        if (n == 0) continue;
+        const int g1 = rows_select(cand, mulhi32(u_g1, n), lane, W);
+        const int r1 = (int)(((uint32_t)g1 * kp.recipW) >> 16), c1 = g1 - r1 * W;
+        if ((int)lane == r1) plain &= ~(1u << c1);
+        rows_bfs(pass, r1, c1, lane, kp.castle_radius, -1, -1, Vnear1, unused, unused);
+        // (5) castles: the first near general 0, the second near general 1, the rest anywhere
+        bool ok = true;
+        for (int k = 0; k < n_castles; ++k) {
+            const bool near = kp.castle_radius > 0 && k < 2;
+            uint32_t set = near ? plain & (k == 0 ? Vnear0 : Vnear1) : 0u;
+            n = near ? rows_count(set) : 0u;
+            if (near && n == 0 && !last) { ok = false; break; }
+            if (n == 0) { set = plain; n = rows_count(set); }
+            if (n == 0) break;
+            philox((uint32_t)k, gid, episode, (DOM_CITY << 24) | a, kp.key0, kp.key1, w);
+            const int cell = rows_select(set, mulhi32(w[0], n), lane, W);
+            const int rc = (int)(((uint32_t)cell * kp.recipW) >> 16);
+            if ((int)lane == rc) plain &= ~(1u << (cell - rc * W));
+            if (lane == 0) {
+                Tr[cell] = (int8_t)T_CITY;
+                A[cell] = (int16_t)(kp.city_lo + (int)mulhi32(w[1], (uint32_t)kp.city_span));
+            }
+        }
+        if (!ok) continue;
+        if (lane == 0) {
+            Tr[g0] = (int8_t)T_GENERAL; O[g0] = 0; A[g0] = 1; gcell_out[0] = (int16_t)g0;
+            Tr[g1] = (int8_t)T_GENERAL; O[g1] = 1; A[g1] = 1; gcell_out[1] = (int16_t)g1;
+        }
+        break;
+    }
+    __syncwarp();
+}
+
 // ================================================================================================
 // Template arguments: NP = bound of the player loops (register arrays).  CH x CW > 0 = the board size is a
 // compile-time constant and P == NP exactly (the paper-sized configs: strides, word counts and the row
@@ -278,6 +421,17 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         const int gg = wg0 + lg;
         const uint32_t gid = kp.gid_base + (uint32_t)gg, episode = gs.episode;
         __syncwarp();
+        if (kp.map_mode == 1) {                                  // the official generator (R36)
+            generate_official(kp, lane, gid, episode, A, O, Tr, B.general_cell + (size_t)gg * P);
+            if (lane == 0) {
+                gs.turn = 0;
+                gs.alive = allp;
+                gs.flags |= GF_TERRAIN_DIRTY | GF_ALL_DIRTY;
+                for (int p = 0; p < P; ++p) { gs.tot[p] = 1; gs.land[p] = 1; }
+            }
+            __syncwarp();
+            return;
+        }
         for (int i = lane; i < S / 4; i += 32) {
             reinterpret_cast<uint32_t *>(O)[i] = 0xFFFFFFFFu;
             reinterpret_cast<uint32_t *>(A)[2 * i] = 0;

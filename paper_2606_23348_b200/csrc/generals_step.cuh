@@ -65,6 +65,10 @@ __device__ __noinline__ void generate_board(const KParams &kp, uint32_t lane, ui
                                             int16_t *A, int8_t *O, int8_t *Tr, int16_t *gcell_out) {
     const int P = kp.P, HW = kp.HW, S = kp.S, NW = kp.NW, W = kp.W;
     __syncwarp();
+    if (kp.map_mode == 1) {                                      // the official generator (R36)
+        generate_official(kp, lane, gid, episode, A, O, Tr, gcell_out);
+        return;
+    }
     for (int i = lane; i < S / 4; i += 32) {
         reinterpret_cast<uint32_t *>(O)[i] = 0xFFFFFFFFu;
         reinterpret_cast<uint32_t *>(A)[2 * i] = 0;

@@ -41,6 +41,12 @@ CONFIGS = {
     "c5b_ffa8": (dict(_BASE, n_games=32768, height=32, width=32, n_players=8, team_size=1,
                       mountain_thr=thr(20), n_cities=16, spawn_dmin=10, pass_thr=0, auto_reset=1,
                       max_turns=1000), 2000),
+    # NEXT-3 (R36): the official generator on the paper's own parameters: up to 23x23, 20 % mountains, 9-11
+    # castles of 40-50, generals >= 17 BFS steps apart, a castle within 6 steps of each general, playable area
+    # from 18x18 up, padded with mountains
+    "official_23x23": (dict(_BASE, n_games=16384, height=23, width=23, n_players=2, mountain_thr=thr(20),
+                            n_cities=9, n_cities_max=11, spawn_dmin=17, pass_thr=thr(5), auto_reset=1, max_turns=1000,
+                            map_mode=1, play_min=18, castle_radius=6), 2000),
 }
 
 

@@ -32,7 +32,7 @@ def binding_err(name):
 
 
 def test_struct_layouts_match_header():
-    assert C.sizeof(binding.GenConfig) == 13 * 4 + 3 * 4 + 8
+    assert C.sizeof(binding.GenConfig) == 13 * 4 + 3 * 4 + 8 + 4 * 4
     assert C.sizeof(binding.GenBuffers) == 25 * 8
     assert C.sizeof(binding.GenSizes) == 8 + 25 * C.sizeof(C.c_size_t) + 8      # + bitboard_row_words, padding
     assert C.sizeof(binding.GenFeatBuffers) == 5 * 8
@@ -73,7 +73,9 @@ def test_query_sizes(lib):
                                  dict(n_players=9), dict(team_size=0), dict(team_size=3),
                                  dict(city_army_lo=60), dict(n_cities=-1), dict(spawn_exact=1, spawn_dmax=0),
                                  dict(spawn_dmax=2), dict(rule_flags=64), dict(max_turns=-5),
-                                 dict(n_games=-1), dict(city_army_hi=40000)])
+                                 dict(n_games=-1), dict(city_army_hi=40000), dict(map_mode=2), dict(play_min=3),
+                                 dict(map_mode=1, n_players=4), dict(map_mode=1, n_cities=10, n_cities_max=9),
+                                 dict(map_mode=1, height=1, width=8, play_min=1)])
 def test_bad_config_is_rejected(lib, bad):
     cfg, _ = binding.make_config(workloads.config("c1_8x8", **bad)[0])
     env = C.c_void_p()

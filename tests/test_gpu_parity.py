@@ -767,3 +767,71 @@ def test_features_full_size_sampled_games(gpu, oracle_mod):
     assert bool(((f[:, :, 9] + f[:, :, 10] + f[:, :, 11] + f[:, :, 12]) == 1).all())
     assert bool((f[:, :, 0] == f[:, :, 1] + f[:, :, 2] + f[:, :, 3]).all())
     assert bool((f[:, :, 14] == env.tensors["turn"].float()[:, None, None]).all())
+
+
+# ------------------------------------------------------------------------------- NEXT-3: official map generator (R36)
+@pytest.mark.parametrize("N,T,over,staged", [
+    (96, 60, dict(max_turns=25), False),                                         # the paper's parameters, frequent resets
+    (96, 60, dict(max_turns=25), True),                                          # the staged kernel's generator call
+    (64, 40, dict(play_min=0, spawn_dmin=3, spawn_dmax=20, spawn_exact=1, max_turns=15), False),   # curriculum in BFS steps
+    (50, 30, dict(mountain_thr=workloads.thr(45), spawn_dmin=12, max_turns=10), False),  # many rejected attempts
+    (40, 30, dict(height=9, width=13, play_min=5, spawn_dmin=6, n_cities=2, n_cities_max=4, castle_radius=2, max_turns=10), False),
+    (40, 20, dict(height=32, width=32, play_min=20, spawn_dmin=25, n_cities=12, n_cities_max=16, max_turns=8), False),
+    (30, 20, dict(height=1, width=5, play_min=0, mountain_thr=0, spawn_dmin=4, n_cities=1, n_cities_max=0, castle_radius=1, max_turns=6), False),
+    (30, 20, dict(height=4, width=4, play_min=0, spawn_dmin=9, n_cities=3, n_cities_max=0, castle_radius=0, max_turns=6), False),   # infeasible window: the last attempt widens it
+])
+def test_official_maps_match_oracle(gpu, oracle_mod, N, T, over, staged):
+    """The warp-level generator (row-word BFS) against the oracle's queue BFS: gen_reset and every auto-reset
+    regeneration inside gen_step (both kernels) and inside fused rollouts produce the same boards bit for bit."""
+    cfg, _ = workloads.config("official_23x23", n_games=N, **over)
+    env = gpu.GeneralsEnv(cfg, bitboards=not staged)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+    compare(env, o, where="reset")
+    for t in range(T):
+        env.step()
+        o.step()
+        compare(env, o, where=f"step {t}")
+    env.rollout(24, gpu.OBS_DIGEST)
+    o.rollout(24, oracle_mod.OBS_DIGEST)
+    compare(env, o, where="rollout")
+    assert int(o.episode.min()) >= 2                           # every game was regenerated at least twice
+
+
+def test_official_maps_full_size_sampled_games(gpu, oracle_mod):
+    """16,384 official 23x23 maps (the batch bench.py --sweep times): sampled global ids replayed by the oracle,
+    constraints of P:L79 checked on ALL maps with torch ops (castle count and garrison, two generals, padding)."""
+    import torch
+    N, T = 16384, 40
+    cfg, _ = workloads.config("official_23x23", n_games=N, max_turns=30)
+    env = gpu.GeneralsEnv(cfg, digest=False, actions_out=False)
+    env.reset()
+    terrain0 = env.tensors["terrain"].clone()
+    army0 = env.tensors["army"].clone()
+    for _ in range(T):
+        env.step()
+    env.torch.cuda.synchronize()
+    n_castles = (terrain0 == CT).sum(1)
+    assert int(n_castles.min()) >= 9 and int(n_castles.max()) <= 11
+    assert bool(((terrain0 == GN).sum(1) == 2).all())
+    garrison = army0[terrain0 == CT]
+    assert int(garrison.min()) >= 40 and int(garrison.max()) <= 50
+    dens = (terrain0[:, :529] == MT).float().mean().item()
+    assert 0.2 < dens < 0.45                                    # 20 % inside the playable area plus the padding
+    ids = sorted(set(list(range(8)) + list(range(N - 8, N)) + list(range(3, N, N // 17))))
+    sel = torch.tensor(ids, device=env.device)
+    fields = STATE_FIELDS + OUT_FIELDS
+    got = {f: (env.tensors[f][0] if f in OUT_FIELDS else env.tensors[f]).index_select(0, sel).cpu().numpy() for f in fields}
+    for k, gid in enumerate(ids):
+        o = oracle_mod.Oracle(dict(cfg, n_games=1, game_id_base=gid))
+        o.reset()
+        assert np.array_equal(terrain0[gid].cpu().numpy(), o.terrain[0]), gid
+        for _ in range(T):
+            o.step()
+        for f in fields:
+            want = np.asarray(o.field(f))[0]
+            have = got[f][k]
+            if have.dtype != want.dtype:
+                have = have.view(want.dtype)
+            assert np.array_equal(have, want.reshape(have.shape)), (gid, f)
