@@ -329,7 +329,10 @@ def run_sweep(args):
     rows = [("c3_sweep", n, False) for n in (1024, 16384, 262144, 1048576)]
     rows += [("c4_curriculum", 65536, False), ("c5a_2v2", 32768, False), ("c5b_ffa8", 32768, False)]
     rows += [("c3_sweep", 16384, True), ("c3_sweep", 262144, True)]        # packed observation format (R33)
+    rows += [("official_23x23", 16384, False), ("official_23x23", 262144, False)]   # official maps (R36, NEXT-3)
     for name, N, packed in rows:
+        if args.rows and args.rows not in name:
+            continue
         cfg, _ = workloads.config(name, n_games=N)
         P, H, W = cfg["n_players"], cfg["height"], cfg["width"]
         bmin = algorithmic_bytes_per_env_step(H, W, P, packed)
@@ -339,7 +342,14 @@ def run_sweep(args):
                 for r in range(R)]
         for e in envs:
             e.reset()
-        out = {"workload": name, "obs_format": "army + packed byte (R33)" if packed else "4 planes", "n_games": N, "n_players": P, "board": f"{H}x{W}", "replicas_in_rotation": R,
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        envs[0].reset()                                     # board generation for all N games + first observation
+        e1.record()
+        torch.cuda.synchronize()
+        reset_ms = e0.elapsed_time(e1)
+        out = {"workload": name, "reset_us": 1e3 * reset_ms, "maps_per_s": N / (reset_ms * 1e-3), "obs_format": "army + packed byte (R33)" if packed else "4 planes", "n_games": N, "n_players": P, "board": f"{H}x{W}", "replicas_in_rotation": R,
                "steps": K, "algorithmic_bytes_per_env_step": bmin}
         for graph in (False, True):
             ms = time_steps(torch, envs, K, max(args.warmup, R), graph)
@@ -474,6 +484,7 @@ def main():
     ap.add_argument("--replicas", type=int, default=0, help="replicas in the round-robin (default: enough for 640 MB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
+    ap.add_argument("--rows", default="", help="with --sweep: only the rows whose workload name contains this")
     ap.add_argument("--features", action="store_true", help="NEXT-1: gen_features alone and with gen_step (one JSON line)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -30,8 +30,12 @@ constexpr uint32_t FF_ROLL_DIGEST = F_OBS_PLANES | F_DIGEST;     // gen_rollout(
     X(9, 1, 4, 32, 32, 0, 64, 8)                 \
     X(10, 1, 8, 32, 32, 0, 64, 6)                \
     X(11, 1, 2, 24, 24, 0, 64, 10)               \
-    X(12, 0, 2, 24, 24, F_OBS_PLANES, 256, 1)
-constexpr int N_VARIANTS = 13;
+    X(12, 0, 2, 24, 24, F_OBS_PLANES, 256, 1)    \
+    X(13, 1, 2, 23, 23, 0, 64, 14)               \
+    X(14, 1, 2, 23, 23, 0, 64, 10)
+constexpr int N_VARIANTS = 15;
+// Variants 13 and 14: the paper's own board ("up to 23x23"; workload official_23x23, R36) under the same two
+// register budgets as 7 and 11.
 // Variants 7 and 11 are the same kernel under two register budgets: 72 registers (14 CTAs of 8 games per SM:
 // a batch of up to 16,576 games -- BASELINE config 2's 16,384 -- is resident in ONE wave) and 96 registers (10 CTAs
 // per SM, no spills: faster per wave, the choice whenever the batch fits 10 CTAs per SM or needs several waves anyway).
