@@ -120,7 +120,19 @@ typedef struct gen_buffers {
     uint32_t *bitboards;     /* state [N][P+3][BW]  derived cache, may be NULL (see below) */
     uint8_t *obs_packed;     /* out   [K][N][P][S]  packed observation, may be NULL (see below) */
     int32_t *score_hist;     /* state [N][512][2P]  scoreboard history ring, may be NULL (see below) */
+    uint32_t *step_epoch;    /* state [ceil(N/4)]  launch chaining of gen_step, may be NULL (see below) */
 } gen_buffers;
+
+/* `step_epoch` lets consecutive gen_step launches of one handle overlap.  Without it a launch starts working only
+ * when the whole previous grid in the stream has completed (griddepcontrol.wait); the batch then moves through the
+ * kernel's phases in lock-step and HBM idles while the rules run.  With it, every warp of the register-resident
+ * per-step kernel records the handle's launch counter for its 4 games when it is done, and the same warp of the next
+ * launch waits for exactly that record instead of for the grid: games are independent, so a launch
+ * depends on the previous one only game by game.  Launches then stream through the GPU like the waves of one
+ * large launch.  Ordering against everything else is unchanged: kernels that are not gen_step launches of this
+ * handle never start before a gen_step grid has completed, the first gen_step after any other call of the handle
+ * (reset, rollout, observe, a staged-kernel step) waits for the grid, and so does every launch recorded into a CUDA
+ * graph.  One handle per buffer set.  Results do not depend on it. */
 
 /* `score_hist` (R34; the paper's two temporal tokens are 512-step windows of
  * the opponent's army and land totals): when non-NULL, gen_reset and every turn of gen_step / gen_rollout store
@@ -148,6 +160,7 @@ typedef struct gen_sizes {
     size_t army, owner, terrain, turn, episode, alive, general_cell, land, army_total;
     size_t reward, done, winner, obs_army, obs_owner, obs_terrain, obs_vis;
     size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out, bitboards, obs_packed, score_hist;
+    size_t step_epoch;
     int32_t bitboard_row_words; /* BW */
 } gen_sizes;
 
@@ -253,6 +266,10 @@ int gen_set_launch(gen_env *env, int32_t games_per_cta);
  * whenever it can serve the call (by default games with more than 4 players stay on the staged kernel, which
  * is faster for them).  Results do not depend on either. */
 int gen_set_generic(gen_env *env, int32_t force_generic, int32_t force_staged);
+
+/* Launch chaining through gen_buffers.step_epoch (see there): enabled != 0 (default) / 0 = every gen_step waits for
+ * the whole previous grid even when step_epoch is given.  Results do not depend on it. */
+int gen_set_chaining(gen_env *env, int32_t enabled);
 
 /* Which instantiation the last launch of this handle used: returns its index in the library's variant
  * table (-1 before the first launch); if non-NULL, *board_specialised is set to 1 when that kernel was

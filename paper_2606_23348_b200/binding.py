@@ -16,7 +16,7 @@ RULE_TICK_PLAIN_ONLY, RULE_CAPTURE_HALF_FLOOR, RULE_ROTATE_PRIORITY = 1, 2, 4
 EXPORTS = ["gen_query_sizes", "gen_init", "gen_set_policy", "gen_global_step", "gen_set_global_step",
            "gen_reset", "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host",
            "gen_query_feat_sizes", "gen_features",
-           "gen_set_launch", "gen_set_generic", "gen_last_variant",
+           "gen_set_launch", "gen_set_generic", "gen_set_chaining", "gen_last_variant",
            "gen_launch_count", "gen_last_cuda_error", "gen_destroy",
            "gen_error_string", "gen_version"]
 
@@ -64,6 +64,7 @@ BUFFERS = [
     ("bitboards", "int32", lambda N, P, S, K: (N, P + 3, (-(-S // 32) + 7) // 8 * 8)),   # bits of uint32
     ("obs_packed", "uint8", lambda N, P, S, K: (K, N, P, S)),
     ("score_hist", "int32", lambda N, P, S, K: (N, 512, 2 * P)),
+    ("step_epoch", "int32", lambda N, P, S, K: ((N + 3) // 4,)),                         # bits of uint32
 ]
 
 
@@ -125,6 +126,7 @@ def load_library(path=None):
     lib.gen_features.argtypes = [env_p, C.POINTER(GenBuffers), C.POINTER(GenFeatBuffers), C.c_void_p]
     lib.gen_set_launch.argtypes = [env_p, C.c_int32]
     lib.gen_set_generic.argtypes = [env_p, C.c_int32, C.c_int32]
+    lib.gen_set_chaining.argtypes = [env_p, C.c_int32]
     lib.gen_last_variant.argtypes = [env_p, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     lib.gen_last_variant.restype = C.c_int32
     lib.gen_launch_count.argtypes = [env_p]
@@ -137,7 +139,7 @@ def load_library(path=None):
     lib.gen_version.restype = C.c_char_p
     for name in ("gen_query_sizes", "gen_init", "gen_set_policy", "gen_set_global_step", "gen_reset",
                  "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host", "gen_set_launch",
-                 "gen_set_generic", "gen_last_cuda_error", "gen_query_feat_sizes", "gen_features"):
+                 "gen_set_generic", "gen_set_chaining", "gen_last_cuda_error", "gen_query_feat_sizes", "gen_features"):
         getattr(lib, name).restype = C.c_int
     if path == LIB_PATH:
         _lib = lib
@@ -171,7 +173,7 @@ class GeneralsEnv:
     """
 
     def __init__(self, cfg, device="cuda:0", k_slots=1, digest=True, actions_out=True, bitboards=True,
-                 packed=False, history=False):
+                 packed=False, history=False, chain=True):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -191,7 +193,7 @@ class GeneralsEnv:
         self.tensors = {}
         for name, dt, shape in BUFFERS:
             if ((name == "obs_digest" and not digest) or (name == "actions_out" and not actions_out)
-                    or (name == "bitboards" and not bitboards) or (name == "obs_packed" and not packed) or (name == "score_hist" and not history)
+                    or (name == "bitboards" and not bitboards) or (name == "obs_packed" and not packed) or (name == "score_hist" and not history) or (name == "step_epoch" and not chain)
                     or (packed and name in ("obs_owner", "obs_terrain", "obs_vis"))):
                 setattr(self.bufs, name, None)
                 continue
@@ -248,6 +250,10 @@ class GeneralsEnv:
         """Test hooks: never launch a board-specialised / the register-resident kernel (force_staged=-1:
         launch the register-resident kernel wherever it can serve, also for more than 4 players)."""
         self._check(self.lib.gen_set_generic(self._env, 1 if force_generic else 0, int(force_staged)))
+
+    def set_chaining(self, enabled=True):
+        """Launch chaining through step_epoch (see include/generals.h); off = every step waits for the whole grid."""
+        self._check(self.lib.gen_set_chaining(self._env, 1 if enabled else 0))
 
     @property
     def last_launch_specialised(self):

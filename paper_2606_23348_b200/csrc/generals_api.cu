@@ -19,6 +19,9 @@ struct gen_env {
     int32_t force_staged;    // 1: never pick the register-resident step kernel (tests)
     int32_t force_step;      // 1: pick it whenever it can serve the call, also where the staged one is faster (tests)
     int32_t last_variant;    // index into GEN_VARIANTS of the last launch (-1: none yet)
+    uint32_t epoch;          // launch counter of the chained gen_step launches (gen_buffers.step_epoch)
+    const uint32_t *chain_buf;  // non-NULL: the last launch of this handle was a k_step that recorded `epoch` there
+    int32_t no_chain;        // tests: never chain
 };
 
 namespace {
@@ -72,6 +75,7 @@ void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
     s->bitboards = N * (P + 3) * BW * 4;
     s->obs_packed = k * N * P * S;
     s->score_hist = N * 512 * 2 * P * 4;
+    s->step_epoch = (N + 3) / 4 * 4;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -95,6 +99,7 @@ int check_buffers(const gen_buffers *b, bool need_obs) {
     if (b->actions_out && !aligned16(b->actions_out)) return GEN_ERR_ALIGN;
     if (b->bitboards && !aligned16(b->bitboards)) return GEN_ERR_ALIGN;
     if (b->score_hist && !aligned16(b->score_hist)) return GEN_ERR_ALIGN;
+    if (b->step_epoch && !aligned16(b->step_epoch)) return GEN_ERR_ALIGN;
     return GEN_OK;
 }
 
@@ -152,7 +157,7 @@ const gen::Variant kVariants[gen::N_VARIANTS] = {
 // be used (gen_step with the bitboard cache, no digest, uniform policy).  Within a kind: the exact board
 // (and, for the staged kernel, the exact mode) first, else the generic kernel of the smallest NP >= P.
 const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, bool step_ok) {
-    const int kind = step_ok ? 1 : 0;
+    const int kind = (step_ok ? 1 : 0) + (kp.map_mode == 1 ? 2 : 0);
     const gen::Variant *generic = nullptr, *exact = nullptr;
     for (const gen::Variant &v : kVariants) {
         if (v.kind != kind) continue;
@@ -162,7 +167,7 @@ const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, boo
         }
         if (env->force_generic || v.np != kp.P || v.h != kp.H || v.w != kp.W) continue;
         if (v.np == 2 && kp.team_size > 1) continue;
-        if (kind == 0 && v.ff != (kp.flags & ~gen::F_SAMPLER)) continue;
+        if ((kind & 1) == 0 && v.ff != (kp.flags & ~gen::F_SAMPLER)) continue;
         if (!exact) { exact = &v; continue; }
         // the same kernel under two register budgets: the one-wave budget if only it holds the whole batch
         // resident at once, else the roomier one
@@ -199,16 +204,36 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     int WPC = env->games_per_cta ? env->games_per_cta / gen::GW : 2;
     while (32 * WPC > v->max_threads) WPC >>= 1;
     const bool digest = (flags & gen::F_DIGEST) != 0;
-    if (v->kind == 1) layout_step(kp, WPC); else layout(kp, WPC, digest);
+    if (v->kind & 1) layout_step(kp, WPC); else layout(kp, WPC, digest);
     while (WPC > 1 && kp.smem_bytes > kMaxSmem) {
         WPC >>= 1;
-        if (v->kind == 1) layout_step(kp, WPC); else layout(kp, WPC, digest);
+        if (v->kind & 1) layout_step(kp, WPC); else layout(kp, WPC, digest);
     }
     if (kp.smem_bytes > kMaxSmem) return GEN_ERR_CONFIG;
     const int per_cta = gen::GW * kp.WPC;
     const int grid = (kp.N + per_cta - 1) / per_cta;
+    // launch chaining (gen_buffers.step_epoch): a k_step launch waits warp by warp for the previous k_step launch of
+    // this handle instead of for the whole grid -- unless that previous launch was something else, or this launch is
+    // being recorded into a graph (the counter would be replayed)
+    kp.chain = 0;
+    kp.epoch = 0;
+    bool record = false;
+    // (measured on config 2's boards: chained launches sustain 290 / 490 / 620-660 M env steps/s at 2,048 / 4,096 /
+    // 8,192-131,072 games against 118 / 227 / 420-653 M with the grid-wide wait; beyond ~8 waves the waves of one
+    // launch mix the phases by themselves and the record's release costs 1-2 %, so those launches do not chain)
+    if ((v->kind & 1) && bufs->step_epoch && !env->no_chain && grid <= 8 * 14 * (int)kSMs) {
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(static_cast<cudaStream_t>(stream), &cap) != cudaSuccess) { (void)cudaGetLastError(); cap = cudaStreamCaptureStatusActive; }
+        if (cap == cudaStreamCaptureStatusNone) {
+            record = true;
+            kp.chain = env->chain_buf == bufs->step_epoch ? 1 : 0;
+            kp.epoch = env->epoch + 1;
+        }
+    }
     cudaError_t e = v->launch(kp, grid, 32 * kp.WPC, kp.smem_bytes, static_cast<cudaStream_t>(stream));
-    if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
+    if (e != cudaSuccess) { env->last_cuda_error = (int)e; env->chain_buf = nullptr; return GEN_ERR_CUDA; }
+    env->chain_buf = record ? bufs->step_epoch : nullptr;
+    if (record) env->epoch += 1;
     env->launches += 1;
     env->last_variant = (int32_t)(v - kVariants);
     return GEN_OK;
@@ -422,10 +447,17 @@ int gen_set_generic(gen_env *env, int32_t force_generic, int32_t force_staged) {
     return GEN_OK;
 }
 
+int gen_set_chaining(gen_env *env, int32_t enabled) {
+    if (!env) return GEN_ERR_NULL;
+    env->no_chain = enabled ? 0 : 1;
+    env->chain_buf = nullptr;
+    return GEN_OK;
+}
+
 int32_t gen_last_variant(const gen_env *env, int32_t *board_specialised, int32_t *register_resident) {
     if (!env || env->last_variant < 0) return -1;
     if (board_specialised) *board_specialised = kVariants[env->last_variant].h > 0 ? 1 : 0;
-    if (register_resident) *register_resident = kVariants[env->last_variant].kind == 1 ? 1 : 0;
+    if (register_resident) *register_resident = (kVariants[env->last_variant].kind & 1) ? 1 : 0;
     return env->last_variant;
 }
 

@@ -84,6 +84,8 @@ struct KParams {
     uint32_t pass_thr, half_thr, bias_thr;
     uint32_t global_step0, flags, recipW;
     int32_t K, WPC;  // turns per launch; warps per CTA
+    uint32_t epoch;  // k_step: this launch's number in gen_buffers.step_epoch (0: do not record)
+    int32_t chain;   // k_step: wait per warp for record epoch - 1 instead of for the previous grid
     // shared memory: [tables | digest keys | warp 0 | warp 1 | ...]; w_* are offsets inside a warp's slice
     uint32_t off_key, off_warp0, warp_bytes, w_owner, w_terr, w_mask, w_game, w_bar, w_scratch, smem_bytes;
     unsigned long long key_sum;  // sum of the digest keys of cells 0..HW-1
@@ -350,13 +352,107 @@ static __device__ __noinline__ void generate_official(const KParams &kp, uint32_
     __syncwarp();
 }
 
+// ------------------------------------------------------------------------------------------------
+// a1: board generator (R13, R14, R29, R30), one warp per game, planes in shared memory (S cells each).
+// Writes general_cell[p] through gcell_out.  Used by the per-step kernel (a call, not inlined: generation is rare
+// and must not tax the register allocation of the turn); the staged kernel carries the same procedure inline.
+template <int NP, bool OFFICIAL>
+__device__ __noinline__ void generate_board(const KParams &kp, uint32_t lane, uint32_t gid, uint32_t episode,
+                                            int16_t *A, int8_t *O, int8_t *Tr, int16_t *gcell_out) {
+    const int P = kp.P, HW = kp.HW, S = kp.S, NW = kp.NW, W = kp.W;
+    __syncwarp();
+    if constexpr (OFFICIAL) {                                    // the official generator (R36)
+        generate_official(kp, lane, gid, episode, A, O, Tr, gcell_out);
+        return;
+    }
+    for (int i = lane; i < S / 4; i += 32) {
+        reinterpret_cast<uint32_t *>(O)[i] = 0xFFFFFFFFu;
+        reinterpret_cast<uint32_t *>(A)[2 * i] = 0;
+        reinterpret_cast<uint32_t *>(A)[2 * i + 1] = 0;
+    }
+    uint32_t w[4];
+    int lo = kp.dmin, hi = kp.dmax > 0 ? kp.dmax : 64;
+    if (kp.spawn_exact) {
+        philox(0, gid, episode, DOM_SPAWN << 24, kp.key0, kp.key1, w);
+        lo = hi = kp.dmin + (int)mulhi32(w[1], (uint32_t)(kp.dmax - kp.dmin + 1));
+    }
+    for (int q = lane; q < S / 4; q += 32) {
+        philox((uint32_t)q, gid, episode, DOM_MOUNTAIN << 24, kp.key0, kp.key1, w);
+        uint32_t tw = 0;
+#pragma unroll
+        for (int b = 0; b < 4; ++b)
+            tw |= (w[b] < kp.mountain_thr || 4 * q + b >= HW) ? (uint32_t)T_MOUNTAIN << (8 * b) : 0u;
+        reinterpret_cast<uint32_t *>(Tr)[q] = tw;
+    }
+    __syncwarp();
+    int gr[NP], gc[NP];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) { gr[p] = 0; gc[p] = 0; }
+    for (int p = 0; p < P; ++p) {
+        philox((uint32_t)p, gid, episode, DOM_SPAWN << 24, kp.key0, kp.key1, w);
+        int cell;
+        if (p == 0) {
+            cell = (int)mulhi32(w[0], (uint32_t)HW);
+        } else {
+            int l = lo, h = hi;
+            uint32_t cand, n;
+            for (;;) {
+                cand = 0;
+                for (int j = 0; j < NW; ++j) {
+                    const int c = 32 * j + (int)lane;
+                    const int r = (int)(((uint32_t)c * kp.recipW) >> 16), col = c - r * W;
+                    int mind = 1 << 20;
+#pragma unroll
+                    for (int q = 0; q < NP; ++q)
+                        if (q < p) mind = min(mind, abs(r - gr[q]) + abs(col - gc[q]));
+                    const uint32_t bal = __ballot_sync(FULL, c < HW && mind >= l && mind <= h && mind > 0);
+                    if ((int)lane == j) cand = bal;
+                }
+                n = __reduce_add_sync(FULL, __popc(cand));
+                if (n > 0) break;
+                if (l > 0) l -= 1;
+                h += 1;
+            }
+            cell = select_kth(cand, mulhi32(w[0], n), lane);
+        }
+        const int r = (int)(((uint32_t)cell * kp.recipW) >> 16);
+#pragma unroll
+        for (int q = 0; q < NP; ++q)
+            if (q == p) { gr[q] = r; gc[q] = cell - r * W; }
+        if (lane == 0) {
+            Tr[cell] = (int8_t)T_GENERAL;
+            O[cell] = (int8_t)p;
+            A[cell] = 1;
+            gcell_out[p] = (int16_t)cell;
+        }
+    }
+    __syncwarp();
+    uint32_t plain = 0;
+    for (int j = 0; j < NW; ++j) {
+        const int c = 32 * j + (int)lane;
+        const uint32_t bal = __ballot_sync(FULL, c < HW && Tr[c] == T_PLAIN);
+        if ((int)lane == j) plain = bal;
+    }
+    uint32_t n = __reduce_add_sync(FULL, __popc(plain));
+    for (int k = 0; k < kp.n_cities && n > 0; ++k, --n) {
+        philox((uint32_t)k, gid, episode, DOM_CITY << 24, kp.key0, kp.key1, w);
+        const int cell = select_kth(plain, mulhi32(w[0], n), lane);
+        if ((int)lane == (cell >> 5)) plain &= ~(1u << (cell & 31));
+        if (lane == 0) {
+            Tr[cell] = (int8_t)T_CITY;
+            A[cell] = (int16_t)(kp.city_lo + (int)mulhi32(w[1], (uint32_t)kp.city_span));
+        }
+    }
+    __syncwarp();
+}
+
 // ================================================================================================
 // Template arguments: NP = bound of the player loops (register arrays).  CH x CW > 0 = the board size is a
 // compile-time constant and P == NP exactly (the paper-sized configs: strides, word counts and the row
 // division fold into immediates and the cell loops unroll); 0 = any board up to 32 x 32, read from KParams.
 // FF = the mode flags as a compile-time constant (dead modes drop out of the instruction stream), or
 // F_RUNTIME.  With FF fixed, F_SAMPLER alone stays a runtime choice.
-template <int NP, int CH, int CW, uint32_t FF>
+template <int NP, int CH, int CW, uint32_t FF, bool OFFICIAL>
 __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParams kp) {
     constexpr bool FIXED = CH > 0;
     constexpr int LPP = LPG / NP;  // lanes serving one (game, player) pair in the word passes
@@ -421,7 +517,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         const int gg = wg0 + lg;
         const uint32_t gid = kp.gid_base + (uint32_t)gg, episode = gs.episode;
         __syncwarp();
-        if (kp.map_mode == 1) {                                  // the official generator (R36)
+        if constexpr (OFFICIAL) {                                // R36, in the instantiations compiled for it
             generate_official(kp, lane, gid, episode, A, O, Tr, B.general_cell + (size_t)gg * P);
             if (lane == 0) {
                 gs.turn = 0;

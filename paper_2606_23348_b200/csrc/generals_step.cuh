@@ -57,103 +57,10 @@ enum : uint32_t {
     SG_STATIC_DIRTY = 1u << 4,  // structure / mountain rows changed (regenerated): write them back too
 };
 
-// ------------------------------------------------------------------------------------------------
-// a1: board generator (R13, R14, R29, R30), one warp per game, planes in shared memory (S cells each).
-// Writes general_cell[p] through gcell_out.  The same procedure as the generator of the staged kernel.
-template <int NP>
-__device__ __noinline__ void generate_board(const KParams &kp, uint32_t lane, uint32_t gid, uint32_t episode,
-                                            int16_t *A, int8_t *O, int8_t *Tr, int16_t *gcell_out) {
-    const int P = kp.P, HW = kp.HW, S = kp.S, NW = kp.NW, W = kp.W;
-    __syncwarp();
-    if (kp.map_mode == 1) {                                      // the official generator (R36)
-        generate_official(kp, lane, gid, episode, A, O, Tr, gcell_out);
-        return;
-    }
-    for (int i = lane; i < S / 4; i += 32) {
-        reinterpret_cast<uint32_t *>(O)[i] = 0xFFFFFFFFu;
-        reinterpret_cast<uint32_t *>(A)[2 * i] = 0;
-        reinterpret_cast<uint32_t *>(A)[2 * i + 1] = 0;
-    }
-    uint32_t w[4];
-    int lo = kp.dmin, hi = kp.dmax > 0 ? kp.dmax : 64;
-    if (kp.spawn_exact) {
-        philox(0, gid, episode, DOM_SPAWN << 24, kp.key0, kp.key1, w);
-        lo = hi = kp.dmin + (int)mulhi32(w[1], (uint32_t)(kp.dmax - kp.dmin + 1));
-    }
-    for (int q = lane; q < S / 4; q += 32) {
-        philox((uint32_t)q, gid, episode, DOM_MOUNTAIN << 24, kp.key0, kp.key1, w);
-        uint32_t tw = 0;
-#pragma unroll
-        for (int b = 0; b < 4; ++b)
-            tw |= (w[b] < kp.mountain_thr || 4 * q + b >= HW) ? (uint32_t)T_MOUNTAIN << (8 * b) : 0u;
-        reinterpret_cast<uint32_t *>(Tr)[q] = tw;
-    }
-    __syncwarp();
-    int gr[NP], gc[NP];
-#pragma unroll
-    for (int p = 0; p < NP; ++p) { gr[p] = 0; gc[p] = 0; }
-    for (int p = 0; p < P; ++p) {
-        philox((uint32_t)p, gid, episode, DOM_SPAWN << 24, kp.key0, kp.key1, w);
-        int cell;
-        if (p == 0) {
-            cell = (int)mulhi32(w[0], (uint32_t)HW);
-        } else {
-            int l = lo, h = hi;
-            uint32_t cand, n;
-            for (;;) {
-                cand = 0;
-                for (int j = 0; j < NW; ++j) {
-                    const int c = 32 * j + (int)lane;
-                    const int r = (int)(((uint32_t)c * kp.recipW) >> 16), col = c - r * W;
-                    int mind = 1 << 20;
-#pragma unroll
-                    for (int q = 0; q < NP; ++q)
-                        if (q < p) mind = min(mind, abs(r - gr[q]) + abs(col - gc[q]));
-                    const uint32_t bal = __ballot_sync(FULL, c < HW && mind >= l && mind <= h && mind > 0);
-                    if ((int)lane == j) cand = bal;
-                }
-                n = __reduce_add_sync(FULL, __popc(cand));
-                if (n > 0) break;
-                if (l > 0) l -= 1;
-                h += 1;
-            }
-            cell = select_kth(cand, mulhi32(w[0], n), lane);
-        }
-        const int r = (int)(((uint32_t)cell * kp.recipW) >> 16);
-#pragma unroll
-        for (int q = 0; q < NP; ++q)
-            if (q == p) { gr[q] = r; gc[q] = cell - r * W; }
-        if (lane == 0) {
-            Tr[cell] = (int8_t)T_GENERAL;
-            O[cell] = (int8_t)p;
-            A[cell] = 1;
-            gcell_out[p] = (int16_t)cell;
-        }
-    }
-    __syncwarp();
-    uint32_t plain = 0;
-    for (int j = 0; j < NW; ++j) {
-        const int c = 32 * j + (int)lane;
-        const uint32_t bal = __ballot_sync(FULL, c < HW && Tr[c] == T_PLAIN);
-        if ((int)lane == j) plain = bal;
-    }
-    uint32_t n = __reduce_add_sync(FULL, __popc(plain));
-    for (int k = 0; k < kp.n_cities && n > 0; ++k, --n) {
-        philox((uint32_t)k, gid, episode, DOM_CITY << 24, kp.key0, kp.key1, w);
-        const int cell = select_kth(plain, mulhi32(w[0], n), lane);
-        if ((int)lane == (cell >> 5)) plain &= ~(1u << (cell & 31));
-        if (lane == 0) {
-            Tr[cell] = (int8_t)T_CITY;
-            A[cell] = (int16_t)(kp.city_lo + (int)mulhi32(w[1], (uint32_t)kp.city_span));
-        }
-    }
-    __syncwarp();
-}
-
 // ================================================================================================
 // NP = bound of the player loops; CH x CW > 0: board size fixed at compile time and P == NP; MAXT / MINB:
 // launch bounds (threads per CTA, resident CTAs per SM the register allocation must allow).
-template <int NP, int CH, int CW, int MAXT, int MINB>
+template <int NP, int CH, int CW, int MAXT, int MINB, bool OFFICIAL>
 __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KParams kp) {
     constexpr bool FIXED = CH > 0;
     constexpr int LPP = LPG / NP;
@@ -217,7 +124,26 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         s_inb[j] = in ? kp.inb[j & 31] : 0u;
     }
     pdl_launch_dependents();  // the next launch may be placed as CTAs of this one retire ...
-    pdl_wait();               // ... and nothing of the previous launch is read before it has completed
+    // ... and nothing of the previous launch is read before it has completed: the whole grid, or -- chained launches
+    // (gen_buffers.step_epoch) -- the one warp of it that owned this warp's games.  A record that does not arrive
+    // (a foreign writer of the buffer) ends in the grid-wide wait, which is always sufficient.
+    if (kp.chain && nwg > 0) {
+        const uint32_t *rec = B.step_epoch + (wg0 >> 2);
+        uint32_t seen = 0;
+        int spins = 0;
+        if (lane == 0) {
+            for (;;) {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(rec) : "memory");
+                if (seen == kp.epoch - 1u || ++spins > (1 << 16)) break;
+                __nanosleep(100);
+            }
+            asm volatile("fence.proxy.async.global;" ::: "memory");  // the cache rows are read by the async proxy (TMA)
+        }
+        seen = __shfl_sync(FULL, seen, 0);
+        if (seen != kp.epoch - 1u) pdl_wait();
+    } else {
+        pdl_wait();
+    }
     if (nwg > 0 && lane == 0) {
         mbar_init(bar, 1);
         const uint32_t bytes = (uint32_t)nwg * (uint32_t)(P + 3) * (uint32_t)BW * 4u;
@@ -600,7 +526,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         const int gg = wg0 + lg;
         int16_t *sA = reinterpret_cast<int16_t *>(s_scratch);
         int8_t *sO = reinterpret_cast<int8_t *>(s_scratch + 2 * S), *sT = reinterpret_cast<int8_t *>(s_scratch + 3 * S);
-        generate_board<NP>(kp, lane, kp.gid_base + (uint32_t)gg, gs.episode, sA, sO, sT,
+        generate_board<NP, OFFICIAL>(kp, lane, kp.gid_base + (uint32_t)gg, gs.episode, sA, sO, sT,
                            B.general_cell + (size_t)gg * P);
         const int rb = 4 * BW;  // row stride in bytes
         unsigned char *rows = row8(0, lg);
@@ -835,6 +761,16 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     GEN_TRACE_MARK(6);  // fog
     if (gvalid) emit_planes(sub);
     GEN_TRACE_MARK(7);  // emit
+    if (kp.epoch) {  // everything this warp wrote for its games is ordered before the record the next launch waits for
+        __syncwarp();
+        if (lane == 0) {  // release at gpu scope: cumulative over the lanes' stores ordered by the __syncwarp above
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(B.step_epoch + (wg0 >> 2)), "r"(kp.epoch) : "memory");
+            // A chained grid did not wait for its predecessor on the way in, so one of its warps does on the way
+            // out: this grid cannot complete before the previous one has, and whatever follows in the stream (a
+            // kernel that is not ours, a staged-kernel call) sees completed grids in stream order by construction.
+            if (kp.chain && blockIdx.x == 0 && wic == 0) pdl_wait();
+        }
+    }
 
     GEN_TRACE_MARK(8);  // store
 }

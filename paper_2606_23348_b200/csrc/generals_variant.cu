@@ -20,10 +20,16 @@ GEN_VARIANTS(GEN_DEFINE)
 
 template <typename S, int KIND> struct KernelOf;
 template <typename S> struct KernelOf<S, 0> {
-    static constexpr auto fn = k_generals<S::NP, S::H, S::W, S::FF>;
+    static constexpr auto fn = k_generals<S::NP, S::H, S::W, S::FF, false>;
 };
 template <typename S> struct KernelOf<S, 1> {
-    static constexpr auto fn = k_step<S::NP, S::H, S::W, S::MAXT, S::MINB>;
+    static constexpr auto fn = k_step<S::NP, S::H, S::W, S::MAXT, S::MINB, false>;
+};
+template <typename S> struct KernelOf<S, 2> {   // kinds 2 / 3: the same kernels with the official generator (R36)
+    static constexpr auto fn = k_generals<S::NP, S::H, S::W, S::FF, true>;
+};
+template <typename S> struct KernelOf<S, 3> {
+    static constexpr auto fn = k_step<S::NP, S::H, S::W, S::MAXT, S::MINB, true>;
 };
 
 #define GEN_CAT_(a, b) a##b

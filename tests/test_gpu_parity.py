@@ -835,3 +835,79 @@ def test_official_maps_full_size_sampled_games(gpu, oracle_mod):
             if have.dtype != want.dtype:
                 have = have.view(want.dtype)
             assert np.array_equal(have, want.reshape(have.shape)), (gid, f)
+
+
+# ------------------------------------------------------------------------------- launch chaining (step_epoch)
+def test_chained_launches_keep_stream_order(gpu, oracle_mod):
+    """gen_step launches of one handle chain warp by warp through gen_buffers.step_epoch instead of waiting for the
+    whole previous grid.  Adversarial interleaving: a large batch A and a tiny batch B stepped alternately on one
+    stream (B's grid is done long before A's), with a foreign kernel (a torch copy of A's outputs) or a staged-kernel
+    call on A right behind B's launch.  Every snapshot must equal the unchained run's."""
+    import torch
+    cfgA, _ = workloads.config("c2_24x24", n_games=16384, max_turns=40)
+    cfgB, _ = workloads.config("c2_24x24", n_games=4, game_id_base=1 << 20)
+    A = gpu.GeneralsEnv(cfgA, digest=False, actions_out=False)
+    B = gpu.GeneralsEnv(cfgB, digest=False, actions_out=False)
+    R = gpu.GeneralsEnv(cfgA, digest=False, actions_out=False)         # reference: every launch waits for the grid
+    R.set_chaining(False)
+    for e in (A, B, R):
+        e.reset()
+    names = ["obs_army", "obs_owner", "obs_vis", "army", "owner", "land", "reward", "done", "turn"]
+    snaps, refs = [], []
+    for t in range(60):
+        A.step()
+        A.step()
+        B.step()
+        snaps.append([A.tensors[n].clone() for n in names])             # a kernel that is not ours, behind B's launch
+        R.step()
+        R.step()
+        torch.cuda.synchronize()
+        refs.append([R.tensors[n].clone() for n in names])
+        if t % 20 == 19:                                                 # a staged-kernel call on A behind B's launch
+            A.step()
+            B.step()
+            A.rollout(3, gpu.OBS_NONE)
+            A.step()
+            R.step()
+            R.rollout(3, gpu.OBS_NONE)
+            R.step()
+    torch.cuda.synchronize()
+    for t, (s, r) in enumerate(zip(snaps, refs)):
+        for n, a, b in zip(names, s, r):
+            assert torch.equal(a, b), (t, n)
+    for n in names:
+        assert torch.equal(A.tensors[n], R.tensors[n]), n
+    assert A.last_launch_register_resident
+
+
+def test_chaining_under_graph_capture_and_replay(gpu, oracle_mod):
+    """Launches recorded into a CUDA graph never chain (the launch counter would be replayed): a graph of five steps
+    replayed once, with chained eager steps before and after it, stays bit-exact with the oracle; replaying it again
+    (same counters: not a valid trajectory, only a liveness check) does not hang."""
+    import torch
+    cfg, _ = workloads.config("c2_24x24", n_games=300, max_turns=40, spawn_dmin=5)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    o = oracle_mod.Oracle(cfg, digest=False)
+    env.reset()
+    o.reset()
+    for _ in range(3):
+        env.step()
+        o.step()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    with torch.cuda.graph(g, stream=side):
+        for _ in range(5):
+            env.step()
+    torch.cuda.synchronize()
+    assert env.global_step == 8
+    g.replay()
+    for _ in range(4):
+        env.step()
+    for _ in range(9):
+        o.step()
+    compare(env, o, digest=False, where="graph + eager")
+    g.replay()
+    g.replay()
+    env.step()
+    torch.cuda.synchronize()
