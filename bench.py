@@ -31,7 +31,7 @@ WORKLOAD = "c2_24x24"
 HBM_FALLBACK_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of one gen_step launch, by games per launch, from the
 # `ncu --set full` capture summarised in profiles/ (see profiles/README.md); None where not captured
-NCU_DRAM_BYTES_PER_LAUNCH = {16384: 104331008}       # profiles/r01_step_full_summary.txt
+NCU_DRAM_BYTES_PER_LAUNCH = {16384: 99168512}        # profiles/r01_step_full_chained_summary.txt
 NCU_FEAT_DRAM_BYTES_PER_LAUNCH = {16384: 3601662088}  # profiles/r01_features_full_summary.txt (k_features)
 
 
