@@ -753,3 +753,24 @@ int32_t orc_features(const orc_config *cfg, const orc_buffers *b, const orc_feat
     }
     return 0;
 }
+
+/* The same tensor in bfloat16 ("half that in bf16"; DESIGN R37): every fp32 value of orc_features
+ * rounded to the nearest bfloat16, ties to even (all values are finite), returned as the 16 bit patterns.  Army counts
+ * above 256 are not exact in bfloat16; that is the format's resolution, not a tolerance of the method. */
+static uint16_t bf16_rne(float f)
+{
+    uint32_t u;
+    memcpy(&u, &f, sizeof u);
+    u += 0x7FFFu + ((u >> 16) & 1u);
+    return (uint16_t)(u >> 16);
+}
+
+int32_t orc_features_bf16(const orc_config *cfg, const orc_buffers *b, const orc_feat_state *m, float *scratch,
+                          uint16_t *feat16)
+{
+    const int32_t rc = orc_features(cfg, b, m, scratch);
+    if (rc != 0) return rc;
+    const size_t n = (size_t)cfg->n_games * 2 * FEAT_C * (size_t)plane_stride(cfg);
+    for (size_t i = 0; i < n; ++i) feat16[i] = bf16_rne(scratch[i]);
+    return 0;
+}

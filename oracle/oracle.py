@@ -79,6 +79,8 @@ def lib():
                                      C.c_int32]
         _lib.orc_observe.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers)]
         _lib.orc_features.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers), C.POINTER(OrcFeatState), C.c_void_p]
+        _lib.orc_features_bf16.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers), C.POINTER(OrcFeatState),
+                                           C.c_void_p, C.c_void_p]
     return _lib
 
 
@@ -174,19 +176,25 @@ class Oracle:
     def observe(self):
         lib().orc_observe(C.byref(self.cfg), C.byref(self.bufs))
 
-    def features(self):
-        """NEXT-1: fold the current turn into the per-episode memory and return feat[N][2][38][S] (float32).
-        Call once per turn (after reset and after every step)."""
+    def features(self, bf16=False):
+        """NEXT-1: fold the current turn into the per-episode memory and return feat[N][2][38][S] (float32; with
+        bf16=True the bfloat16 bit patterns as uint16, R37).  Call once per turn (after reset and after every step)."""
         N, S = self.N, self.S
         if not hasattr(self, "feat"):
             self.feat = np.zeros((N, 2, 38, S), dtype=np.float32)
             self._fm = dict(bits=np.zeros((N, 2, 5, S), np.uint8), last_army=np.zeros((N, 2, S), np.int16),
                             last_turn=np.full((N, 2, S), -1, np.int32), hist=np.zeros((N, 2, 2, 8, S), np.int16))
             self._fs = OrcFeatState(*[self._fm[k].ctypes.data for k in ("bits", "last_army", "last_turn", "hist")])
-        rc = lib().orc_features(C.byref(self.cfg), C.byref(self.bufs), C.byref(self._fs), self.feat.ctypes.data)
+        if bf16:
+            if not hasattr(self, "feat16"):
+                self.feat16 = np.zeros((N, 2, 38, S), dtype=np.uint16)
+            rc = lib().orc_features_bf16(C.byref(self.cfg), C.byref(self.bufs), C.byref(self._fs),
+                                         self.feat.ctypes.data, self.feat16.ctypes.data)
+        else:
+            rc = lib().orc_features(C.byref(self.cfg), C.byref(self.bufs), C.byref(self._fs), self.feat.ctypes.data)
         if rc != 0:
             raise ValueError("orc_features: 1v1 only")
-        return self.feat
+        return self.feat16 if bf16 else self.feat
 
     def set_policy(self, pass_thr=None, half_thr=None, bias_thr=None):
         for k, v in (("pass_thr", pass_thr), ("half_thr", half_thr), ("bias_thr", bias_thr)):

@@ -113,3 +113,29 @@ def test_features_are_1v1_only(oracle_mod):
     o.reset()
     with pytest.raises(ValueError):
         o.features()
+
+
+def test_bf16_output_is_the_fp32_tensor_rounded_to_nearest_even(oracle_mod):
+    """R37: the bfloat16 variant is the fp32 tensor rounded once, ties to even.  Pinned against torch's own
+    float32 -> bfloat16 conversion (a library routine, not the oracle's bit trick) on real play, and on hand-picked
+    ties: 257 = 0x4380_8000 is halfway between 256 and 258 -> 256 (even mantissa); 259 -> 260; 32767 -> 32768."""
+    import torch
+    cfg, _ = workloads.config("c4_curriculum", n_games=6, height=9, width=11, spawn_dmin=3, spawn_dmax=5, n_cities=3,
+                              max_turns=70)
+    o = oracle_mod.Oracle(cfg)
+    o.reset()
+    for t in range(120):
+        if t:
+            o.step()
+        if t % 10 == 0:                     # make large armies appear: bf16 cannot hold them exactly
+            big = np.minimum(o.army[:, :99].astype(np.int32) * 7 + 250, 30000).astype(np.int16)
+            o.army[:, :99] = np.where(o.owner[:, :99] >= 0, big, o.army[:, :99])
+            o.observe()
+        f16 = o.features(bf16=True).copy()
+        f32 = o.feat.copy()
+        want = torch.from_numpy(f32).to(torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+        assert np.array_equal(f16, want)
+    assert (f32 > 256).any()
+    for val, bits in ((257.0, 0x4380), (259.0, 0x4382), (32767.0, 0x4700), (1.0, 0x3F80), (0.0, 0)):
+        got = torch.tensor([val], dtype=torch.float32).to(torch.bfloat16).view(torch.int16).item() & 0xFFFF
+        assert got == bits
