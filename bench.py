@@ -401,11 +401,11 @@ def run_sweep(args):
 
 
 # ------------------------------------------------------------------------------------------ NEXT-1: features
-def feature_bytes_per_game(H, W):
+def feature_bytes_per_game(H, W, bf16=False):
     """Algorithmic bytes of one gen_features call per game: per cell read the three state
-    planes (4 B) and, per player, write 38 float32 channels (152 B), write this turn's two history frames (4 B),
-    read the seven previous ones (28 B) and the memory (bits 1 B, last army 2 B, last sighting 4 B)."""
-    return H * W * (4 + 2 * (152 + 4 + 28 + 7))
+    planes (4 B) and, per player, write 38 float32 channels (152 B; 76 B as bfloat16, R37), write this turn's two
+    history frames (4 B), read the seven previous ones (28 B) and the memory (bits 1 B, last army 2 B, last sighting 4 B)."""
+    return H * W * (4 + 2 * ((76 if bf16 else 152) + 4 + 28 + 7))
 
 
 def run_features(args):
@@ -421,9 +421,10 @@ def run_features(args):
         cfg["n_games"] = args.games
     N, H, W = cfg["n_games"], cfg["height"], cfg["width"]
     K, Wm = args.steps, max(args.warmup, 8)
+    bf16 = args.bf16
     env = GeneralsEnv(cfg, device=dev, digest=False, actions_out=False)
     env.reset()
-    env.features()
+    env.features(bf16=bf16)
     for _ in range(Wm):                       # a full delta history (7 frames) before anything is timed
         env.step()
         env.features()
@@ -445,14 +446,15 @@ def run_features(args):
         b.record()
     torch.cuda.synchronize()
     feat_ms = statistics.mean(a.elapsed_time(b) for a, b in ev)
-    bfeat = feature_bytes_per_game(H, W)
+    bfeat = feature_bytes_per_game(H, W, bf16)
     achieved = N * bfeat / (feat_ms * 1e-3) / 1e9
     line = {"workload": f"{WORKLOAD}: 1v1 {H}x{W}, {N} games, gen_step + gen_features every turn",
-            "n_games": N, "steps": K, "feature_tensor_bytes": N * 2 * 38 * env.S * 4,
+            "n_games": N, "steps": K, "dtype": "bf16 (R37)" if bf16 else "f32",
+            "feature_tensor_bytes": N * 2 * 38 * env.S * (2 if bf16 else 4),
             "step_plus_features": {"env_steps_per_s": N / (both_ms * 1e-3), "us_per_turn": 1e3 * both_ms},
             "features": {"games_per_s": N / (feat_ms * 1e-3), "us_per_launch": 1e3 * feat_ms,
                          "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                                      "frac": achieved / peak, "traffic": NCU_FEAT_DRAM_BYTES_PER_LAUNCH.get(N),
+                                      "frac": achieved / peak, "traffic": None if bf16 else NCU_FEAT_DRAM_BYTES_PER_LAUNCH.get(N),
                                       "kernel": "gen::k_features",
                                       "peak_source": peak_src, "algorithmic_bytes_per_game": bfeat,
                                       "units_per_launch": N}}}
@@ -485,6 +487,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
     ap.add_argument("--rows", default="", help="with --sweep: only the rows whose workload name contains this")
+    ap.add_argument("--bf16", action="store_true", help="with --features: the bfloat16 feature tensor (R37)")
     ap.add_argument("--features", action="store_true", help="NEXT-1: gen_features alone and with gen_step (one JSON line)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

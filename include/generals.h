@@ -234,12 +234,14 @@ typedef struct gen_feat_buffers {
     int16_t *last_army;  /* state [N][2][S]     channel 20 */
     int32_t *last_seen;  /* state [N][2][S]     turn of the last enemy sighting + 1, 0 = never */
     int16_t *hist;       /* state [N][2][8][2][S]  own_army / enemy_army frames, slot = turn mod 8 */
+    uint16_t *feat_bf16; /* out   [N][2][38][S] bfloat16 bit patterns (R37); when non-NULL it is written INSTEAD of
+                            feat (which may then be NULL): every fp32 value rounded once, ties to even */
 } gen_feat_buffers;
 
 typedef struct gen_feat_sizes {
     int32_t channels;     /* 38 */
     int32_t plane_stride; /* S */
-    size_t feat, mem_bits, last_army, last_seen, hist; /* bytes */
+    size_t feat, mem_bits, last_army, last_seen, hist, feat_bf16; /* bytes */
 } gen_feat_sizes;
 
 /* Byte sizes of the gen_feat_buffers members for `cfg`.  Host-only.  GEN_ERR_CONFIG unless n_players == 2 and

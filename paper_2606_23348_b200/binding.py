@@ -85,6 +85,7 @@ FEAT_BUFFERS = [
     ("last_army", "int16", lambda N, S: (N, 2, S)),
     ("last_seen", "int32", lambda N, S: (N, 2, S)),
     ("hist", "int16", lambda N, S: (N, 2, 8, 2, S)),
+    ("feat_bf16", "bfloat16", lambda N, S: (N, 2, FEAT_CHANNELS, S)),
 ]
 
 
@@ -300,20 +301,24 @@ class GeneralsEnv:
         self._check(self.lib.gen_sample(self._env, C.byref(self.bufs), C.c_void_p(out.data_ptr()), self._stream(stream)))
         return out
 
-    def features(self, stream=None):
+    def features(self, stream=None, bf16=False):
         """NEXT-1 (R35): fold the current turn into each player's memory and return feat, a float32 CUDA tensor
-        [N][2][38][S].  Call once per turn (after reset and after every step).  1v1 only."""
+        [N][2][38][S] (bf16=True: a bfloat16 tensor, R37; the choice is made at the first call).  Call once per turn
+        (after reset and after every step).  1v1 only."""
         if not hasattr(self, "feat_bufs"):
             sizes = GenFeatSizes()
             self._check(self.lib.gen_query_feat_sizes(C.byref(self.cfg), C.byref(sizes)))
             self.feat_bufs = GenFeatBuffers()
             self.feat_tensors = {}
             for name, dt, shape in FEAT_BUFFERS:
+                if name == ("feat" if bf16 else "feat_bf16"):
+                    setattr(self.feat_bufs, name, None)
+                    continue
                 t = self.torch.zeros(shape(self.N, self.S), dtype=getattr(self.torch, dt), device=self.device)
                 assert t.numel() * t.element_size() == getattr(sizes, name), name
                 self.feat_tensors[name] = t
                 setattr(self.feat_bufs, name, t.data_ptr() if t.numel() else 16)
-            self.feat = self.feat_tensors["feat"]
+            self.feat = self.feat_tensors["feat_bf16" if bf16 else "feat"]
         self._check(self.lib.gen_features(self._env, C.byref(self.bufs), C.byref(self.feat_bufs), self._stream(stream)))
         return self.feat
 

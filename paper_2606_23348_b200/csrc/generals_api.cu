@@ -401,14 +401,17 @@ int gen_query_feat_sizes(const gen_config *cfg, gen_feat_sizes *out) {
     out->last_army = N * 2 * S * 2;
     out->last_seen = N * 2 * S * 4;
     out->hist = N * 2 * 8 * 2 * S * 2;
+    out->feat_bf16 = N * 2 * 38 * S * 2;
     return GEN_OK;
 }
 
 int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *feat, void *cuda_stream) {
     if (!env || !bufs || !feat) return GEN_ERR_NULL;
     if (env->cfg.n_players != 2 || env->cfg.team_size != 1) return GEN_ERR_CONFIG;
+    const void *out = feat->feat_bf16 ? (const void *)feat->feat_bf16 : (const void *)feat->feat;
+    if (feat->feat && !aligned16(feat->feat)) return GEN_ERR_ALIGN;
     const void *req[] = {bufs->army, bufs->owner, bufs->terrain, bufs->turn, bufs->land, bufs->army_total,
-                         feat->feat, feat->mem_bits, feat->last_army, feat->last_seen, feat->hist};
+                         out, feat->mem_bits, feat->last_army, feat->last_seen, feat->hist};
     for (const void *p : req) {
         if (!p) return GEN_ERR_NULL;
         if (!aligned16(p)) return GEN_ERR_ALIGN;
@@ -422,7 +425,7 @@ int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *
     fp.force_generic = env->force_generic;
     fp.army = bufs->army; fp.owner = bufs->owner; fp.terrain = bufs->terrain; fp.turn = bufs->turn;
     fp.land = bufs->land; fp.army_total = bufs->army_total;
-    fp.feat = feat->feat; fp.mem_bits = feat->mem_bits; fp.last_army = feat->last_army;
+    fp.feat = const_cast<void *>(out); fp.bf16 = feat->feat_bf16 ? 1 : 0; fp.mem_bits = feat->mem_bits; fp.last_army = feat->last_army;
     fp.last_seen = feat->last_seen; fp.hist = feat->hist;
     const cudaError_t e = gen::launch_features(fp, static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }

@@ -12,6 +12,7 @@
 // Visibility (own cells and their 8 neighbours) is rebuilt from the owner plane, independent of which
 // observation format the step kernel was asked for: owner bytes -> one row word per player and row in shared
 // memory -> (up | mid | down) dilated by one bit each way.
+#include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <cstdint>
 
@@ -27,6 +28,12 @@ constexpr int FEAT_RING = 8;
 
 __device__ __forceinline__ void st4(float *p, float a, float b, float c, float d) {
     __stcs(reinterpret_cast<float4 *>(p), make_float4(a, b, c, d));
+}
+// the bfloat16 variant (R37): each fp32 value rounded once, ties to even; four cells = one 8-byte store
+__device__ __forceinline__ void st4(__nv_bfloat16 *p, float a, float b, float c, float d) {
+    const __nv_bfloat162 lo = __floats2bfloat162_rn(a, b), hi = __floats2bfloat162_rn(c, d);
+    __stcs(reinterpret_cast<uint2 *>(p), make_uint2(*reinterpret_cast<const uint32_t *>(&lo),
+                                                     *reinterpret_cast<const uint32_t *>(&hi)));
 }
 
 // a non-negative int16 (army counts, R21) as a float without a conversion instruction: drop its 16 bits into the
@@ -46,8 +53,9 @@ __device__ __forceinline__ uint32_t pack2(uint32_t lo, uint32_t hi) { return (lo
 
 // grid = ceil(N / G) CTAs; a CTA serves G games with 2 * Q threads each (Q = S / 4 quads per plane).
 // dynamic shared memory: [G][S] owner bytes | [G][2][H + 2] own-row words (rows 0 and H + 1 stay zero) |
-// 32 + 32 coordinate floats.  TH, TW: the board this instantiation is compiled for (0 = any board).
-template <int TH, int TW, int MAXT, int MINB>
+// 32 + 32 coordinate floats.  TH, TW: the board this instantiation is compiled for (0 = any board); OUT: float or
+// __nv_bfloat16 (R37).
+template <int TH, int TW, int MAXT, int MINB, typename OUT>
 __global__ void __launch_bounds__(MAXT, MINB) k_features(const FeatParams fp) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int H = TH ? TH : fp.H, W = TW ? TW : fp.W, HW = H * W;
@@ -198,7 +206,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_features(const FeatParams fp) {
     }
 
     // Table IV, channel by channel.  EMIT(ch, expr): expr is a float in terms of j; padding cells are 0.
-    float *out = fp.feat + gp * FEAT_C * S + c0;
+    OUT *out = reinterpret_cast<OUT *>(fp.feat) + gp * FEAT_C * S + c0;
     float f[4], fa[4];
     unpack4f(army2, fa);
 #define EMIT(ch, expr)                                                                                  \
@@ -274,7 +282,8 @@ template <int TH, int TW, int MAXT, int MINB>
 cudaError_t launch_one(const FeatParams &fp, int threads, cudaStream_t stream) {
     const size_t smem = (size_t)fp.G * fp.S + (size_t)fp.G * 2 * (fp.H + 2) * 4 + 64 * 4;
     const int grid = (fp.N + fp.G - 1) / fp.G;
-    k_features<TH, TW, MAXT, MINB><<<grid, threads, smem, stream>>>(fp);
+    if (fp.bf16) k_features<TH, TW, MAXT, MINB, __nv_bfloat16><<<grid, threads, smem, stream>>>(fp);
+    else k_features<TH, TW, MAXT, MINB, float><<<grid, threads, smem, stream>>>(fp);
     return cudaGetLastError();
 }
 

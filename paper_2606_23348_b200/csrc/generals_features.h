@@ -15,7 +15,8 @@ struct FeatParams {
     const int32_t *turn;
     const int32_t *land;
     const int32_t *army_total;
-    float *feat;                 // gen_feat_buffers
+    int bf16;                    // feat points at bfloat16 (R37) instead of float
+    void *feat;                  // gen_feat_buffers: feat or feat_bf16
     uint8_t *mem_bits;
     int16_t *last_army;
     int32_t *last_seen;

@@ -35,8 +35,8 @@ def test_struct_layouts_match_header():
     assert C.sizeof(binding.GenConfig) == 13 * 4 + 3 * 4 + 8 + 4 * 4
     assert C.sizeof(binding.GenBuffers) == 26 * 8
     assert C.sizeof(binding.GenSizes) == 8 + 26 * C.sizeof(C.c_size_t) + 8      # + bitboard_row_words, padding
-    assert C.sizeof(binding.GenFeatBuffers) == 5 * 8
-    assert C.sizeof(binding.GenFeatSizes) == 8 + 5 * C.sizeof(C.c_size_t)
+    assert C.sizeof(binding.GenFeatBuffers) == 6 * 8
+    assert C.sizeof(binding.GenFeatSizes) == 8 + 6 * C.sizeof(C.c_size_t)
 
 
 def test_query_feat_sizes(lib):
@@ -46,7 +46,7 @@ def test_query_feat_sizes(lib):
     N, S = 16384, 576
     assert s.channels == 38 and s.plane_stride == S
     assert s.feat == N * 2 * 38 * S * 4 and s.mem_bits == N * 2 * S and s.last_army == N * 2 * S * 2
-    assert s.last_seen == N * 2 * S * 4 and s.hist == N * 2 * 8 * 2 * S * 2
+    assert s.last_seen == N * 2 * S * 4 and s.hist == N * 2 * 8 * 2 * S * 2 and s.feat_bf16 == N * 2 * 38 * S * 2
     cfg4, _ = binding.make_config(workloads.config("c5a_2v2")[0])
     assert lib.gen_query_feat_sizes(C.byref(cfg4), C.byref(s)) == binding_err("GEN_ERR_CONFIG")
     assert lib.gen_query_feat_sizes(None, C.byref(s)) == binding_err("GEN_ERR_NULL")
