@@ -181,14 +181,14 @@ def run_ours(args):
 
     # ---- device-resident leg: K gen_step launches back to back, replica t % R at step t; one CUDA event pair
     # on the launching (torch current) stream around the timed region
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()                                       # sampling spans warm-up and every timed leg below
     for e in envs:
         e.reset()
     for t in range(Wm):
         envs[t % R].step()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    clocks = ClockSampler(local)
-    if rank == 0:
-        clocks.start()
     launches0 = sum(e.launch_count for e in envs)
     barrier()
     e0.record()
@@ -226,6 +226,14 @@ def run_ours(args):
     e1.record()
     barrier()
     roll_ms = max_over_ranks(e0.elapsed_time(e1))
+    # The timed regions above last a few milliseconds, nvidia-smi samples every 100 ms: keep the same launches going
+    # (untimed) until the sampler has seen the GPU under this load at least three times.
+    if rank == 0:
+        t_end = time.perf_counter() + 1.5
+        while len(clocks.lines) < 3 and time.perf_counter() < t_end:
+            for t in range(64):
+                envs[t % R].step()
+            torch.cuda.synchronize()
     clock_info = clocks.stop() if rank == 0 else None
 
     # ---- end-to-end leg: host actions in (pinned), gen_step_host, host reward + done out, every step
