@@ -120,19 +120,22 @@ typedef struct gen_buffers {
     uint32_t *bitboards;     /* state [N][P+3][BW]  derived cache, may be NULL (see below) */
     uint8_t *obs_packed;     /* out   [K][N][P][S]  packed observation, may be NULL (see below) */
     int32_t *score_hist;     /* state [N][512][2P]  scoreboard history ring, may be NULL (see below) */
-    uint32_t *step_epoch;    /* state [ceil(N/4)]  launch chaining of gen_step, may be NULL (see below) */
+    uint32_t *step_epoch;    /* state [2][ceil(N/4)]  launch chaining of gen_step, may be NULL (see below); zeroed once */
 } gen_buffers;
 
 /* `step_epoch` lets consecutive gen_step launches of one handle overlap.  Without it a launch starts working only
  * when the whole previous grid in the stream has completed (griddepcontrol.wait); the batch then moves through the
  * kernel's phases in lock-step and HBM idles while the rules run.  With it, every warp of the register-resident
- * per-step kernel records the handle's launch counter for its 4 games when it is done, and the same warp of the next
- * launch waits for exactly that record instead of for the grid: games are independent, so a launch
- * depends on the previous one only game by game.  Launches then stream through the GPU like the waves of one
- * large launch.  Ordering against everything else is unchanged: kernels that are not gen_step launches of this
- * handle never start before a gen_step grid has completed, the first gen_step after any other call of the handle
- * (reset, rollout, observe, a staged-kernel step) waits for the grid, and so does every launch recorded into a CUDA
- * graph.  One handle per buffer set.  Results do not depend on it. */
+ * per-step kernel takes a ticket for its group of 4 games when it starts (start[group]++: the number of earlier
+ * launches on the group) and records done[group] = ticket + 1 when everything it wrote is visible; a warp begins its
+ * work when done[group] equals its ticket instead of waiting for the grid: games are independent, so
+ * a launch depends on the previous one only game by game.  Launches then stream through the GPU like the waves of
+ * one large launch.  The counters live on the device, so eager launches, CUDA-graph replays and other handles'
+ * launches in between need no bookkeeping.  Ordering against everything else is unchanged: kernels that are not
+ * gen_step launches never start before a gen_step grid has completed, one warp of every chained grid waits for the
+ * previous grid before it exits (grids complete in stream order), and the first gen_step after any other call on the
+ * handle (reset, rollout, observe, a staged-kernel step) waits for the whole grid.  Allocate it zeroed, once; one
+ * handle per buffer set.  Results do not depend on it. */
 
 /* `score_hist` (R34; the paper's two temporal tokens are 512-step windows of
  * the opponent's army and land totals): when non-NULL, gen_reset and every turn of gen_step / gen_rollout store

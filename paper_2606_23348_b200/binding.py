@@ -64,7 +64,7 @@ BUFFERS = [
     ("bitboards", "int32", lambda N, P, S, K: (N, P + 3, (-(-S // 32) + 7) // 8 * 8)),   # bits of uint32
     ("obs_packed", "uint8", lambda N, P, S, K: (K, N, P, S)),
     ("score_hist", "int32", lambda N, P, S, K: (N, 512, 2 * P)),
-    ("step_epoch", "int32", lambda N, P, S, K: ((N + 3) // 4,)),                         # bits of uint32
+    ("step_epoch", "int32", lambda N, P, S, K: (2, (N + 3) // 4)),                      # bits of uint32
 ]
 
 

@@ -19,8 +19,7 @@ struct gen_env {
     int32_t force_staged;    // 1: never pick the register-resident step kernel (tests)
     int32_t force_step;      // 1: pick it whenever it can serve the call, also where the staged one is faster (tests)
     int32_t last_variant;    // index into GEN_VARIANTS of the last launch (-1: none yet)
-    uint32_t epoch;          // launch counter of the chained gen_step launches (gen_buffers.step_epoch)
-    const uint32_t *chain_buf;  // non-NULL: the last launch of this handle was a k_step that recorded `epoch` there
+    const uint32_t *chain_buf;  // non-NULL: the last launch of this handle was a k_step that kept records there
     int32_t no_chain;        // tests: never chain
 };
 
@@ -75,7 +74,7 @@ void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
     s->bitboards = N * (P + 3) * BW * 4;
     s->obs_packed = k * N * P * S;
     s->score_hist = N * 512 * 2 * P * 4;
-    s->step_epoch = (N + 3) / 4 * 4;
+    s->step_epoch = (N + 3) / 4 * 8;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -212,28 +211,17 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     if (kp.smem_bytes > kMaxSmem) return GEN_ERR_CONFIG;
     const int per_cta = gen::GW * kp.WPC;
     const int grid = (kp.N + per_cta - 1) / per_cta;
-    // launch chaining (gen_buffers.step_epoch): a k_step launch waits warp by warp for the previous k_step launch of
-    // this handle instead of for the whole grid -- unless that previous launch was something else, or this launch is
-    // being recorded into a graph (the counter would be replayed)
-    kp.chain = 0;
-    kp.epoch = 0;
-    bool record = false;
+    // launch chaining (gen_buffers.step_epoch): a k_step launch waits warp by warp for the earlier k_step launches on
+    // the same games instead of for the whole previous grid -- unless the previous call on this handle was something
+    // else (a staged-kernel launch triggers its dependents early too and keeps no records)
     // (measured on config 2's boards: chained launches sustain 290 / 490 / 620-660 M env steps/s at 2,048 / 4,096 /
     // 8,192-131,072 games against 118 / 227 / 420-653 M with the grid-wide wait; beyond ~8 waves the waves of one
-    // launch mix the phases by themselves and the record's release costs 1-2 %, so those launches do not chain)
-    if ((v->kind & 1) && bufs->step_epoch && !env->no_chain && grid <= 8 * 14 * (int)kSMs) {
-        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(static_cast<cudaStream_t>(stream), &cap) != cudaSuccess) { (void)cudaGetLastError(); cap = cudaStreamCaptureStatusActive; }
-        if (cap == cudaStreamCaptureStatusNone) {
-            record = true;
-            kp.chain = env->chain_buf == bufs->step_epoch ? 1 : 0;
-            kp.epoch = env->epoch + 1;
-        }
-    }
+    // launch mix the phases by themselves and the record's release costs 1-2 %, so those launches keep no records)
+    kp.count = ((v->kind & 1) && bufs->step_epoch && !env->no_chain && grid <= 8 * 14 * (int)kSMs) ? 1 : 0;
+    kp.chain = (kp.count && env->chain_buf == bufs->step_epoch) ? 1 : 0;
     cudaError_t e = v->launch(kp, grid, 32 * kp.WPC, kp.smem_bytes, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) { env->last_cuda_error = (int)e; env->chain_buf = nullptr; return GEN_ERR_CUDA; }
-    env->chain_buf = record ? bufs->step_epoch : nullptr;
-    if (record) env->epoch += 1;
+    env->chain_buf = kp.count ? bufs->step_epoch : nullptr;
     env->launches += 1;
     env->last_variant = (int32_t)(v - kVariants);
     return GEN_OK;

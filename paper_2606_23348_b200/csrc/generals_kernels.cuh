@@ -84,8 +84,8 @@ struct KParams {
     uint32_t pass_thr, half_thr, bias_thr;
     uint32_t global_step0, flags, recipW;
     int32_t K, WPC;  // turns per launch; warps per CTA
-    uint32_t epoch;  // k_step: this launch's number in gen_buffers.step_epoch (0: do not record)
-    int32_t chain;   // k_step: wait per warp for record epoch - 1 instead of for the previous grid
+    int32_t count;   // k_step: take a ticket per group of 4 games in gen_buffers.step_epoch and record completion
+    int32_t chain;   // k_step: wait per warp for the earlier tickets of its group instead of for the previous grid
     // shared memory: [tables | digest keys | warp 0 | warp 1 | ...]; w_* are offsets inside a warp's slice
     uint32_t off_key, off_warp0, warp_bytes, w_owner, w_terr, w_mask, w_game, w_bar, w_scratch, smem_bytes;
     unsigned long long key_sum;  // sum of the digest keys of cells 0..HW-1

@@ -123,24 +123,36 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         s_ncL[j] = in ? kp.notcolL[j & 31] : 0u;
         s_inb[j] = in ? kp.inb[j & 31] : 0u;
     }
+    // Launch chaining (gen_buffers.step_epoch = start[NG] | done[NG], one pair per group of 4 games).  Every warp
+    // takes a ticket for its group: the number of earlier launches that started on it.  The trigger below comes after
+    // the tickets of this CTA have been taken (their values have arrived), and the CTAs of the next launch are placed
+    // only after every CTA of this one has triggered, so tickets are handed out in launch order without any host
+    // counter (graph replays and eager launches mix freely).
+    uint32_t ticket = 0;
+    const int NG = (kp.N + 3) >> 2;
+    if (kp.count) {
+        if (lane == 0 && nwg > 0) ticket = atomicAdd(B.step_epoch + (wg0 >> 2), 1u);
+        ticket = __shfl_sync(FULL, ticket, 0);
+        __syncthreads();
+    }
     pdl_launch_dependents();  // the next launch may be placed as CTAs of this one retire ...
     // ... and nothing of the previous launch is read before it has completed: the whole grid, or -- chained launches
-    // (gen_buffers.step_epoch) -- the one warp of it that owned this warp's games.  A record that does not arrive
+    // -- the warps of earlier launches that owned this warp's games: done == ticket.  A record that does not arrive
     // (a foreign writer of the buffer) ends in the grid-wide wait, which is always sufficient.
     if (kp.chain && nwg > 0) {
-        const uint32_t *rec = B.step_epoch + (wg0 >> 2);
+        const uint32_t *rec = B.step_epoch + NG + (wg0 >> 2);
         uint32_t seen = 0;
         int spins = 0;
         if (lane == 0) {
             for (;;) {
                 asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(rec) : "memory");
-                if (seen == kp.epoch - 1u || ++spins > (1 << 16)) break;
+                if (seen == ticket || ++spins > (1 << 16)) break;
                 __nanosleep(100);
             }
             asm volatile("fence.proxy.async.global;" ::: "memory");  // the cache rows are read by the async proxy (TMA)
         }
         seen = __shfl_sync(FULL, seen, 0);
-        if (seen != kp.epoch - 1u) pdl_wait();
+        if (seen != ticket) pdl_wait();
     } else {
         pdl_wait();
     }
@@ -761,10 +773,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     GEN_TRACE_MARK(6);  // fog
     if (gvalid) emit_planes(sub);
     GEN_TRACE_MARK(7);  // emit
-    if (kp.epoch) {  // everything this warp wrote for its games is ordered before the record the next launch waits for
+    if (kp.count) {  // everything this warp wrote for its games is ordered before the record the next launch waits for
         __syncwarp();
         if (lane == 0) {  // release at gpu scope: cumulative over the lanes' stores ordered by the __syncwarp above
-            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(B.step_epoch + (wg0 >> 2)), "r"(kp.epoch) : "memory");
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(B.step_epoch + NG + (wg0 >> 2)), "r"(ticket + 1u) : "memory");
             // A chained grid did not wait for its predecessor on the way in, so one of its warps does on the way
             // out: this grid cannot complete before the previous one has, and whatever follows in the stream (a
             // kernel that is not ours, a staged-kernel call) sees completed grids in stream order by construction.

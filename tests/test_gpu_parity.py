@@ -881,36 +881,55 @@ def test_chained_launches_keep_stream_order(gpu, oracle_mod):
 
 
 def test_chaining_under_graph_capture_and_replay(gpu, oracle_mod):
-    """Launches recorded into a CUDA graph never chain (the launch counter would be replayed): a graph of five steps
-    replayed once, with chained eager steps before and after it, stays bit-exact with the oracle; replaying it again
-    (same counters: not a valid trajectory, only a liveness check) does not hang."""
+    """The tickets of launch chaining live on the device, so launches recorded into a CUDA graph chain as well and
+    replays mix freely with eager launches: a graph of five steps replayed once between eager steps stays bit-exact
+    with the oracle; further replays (same sampler counters: not a valid trajectory, but deterministic) and eager steps
+    give the same tensors with chaining on and off."""
     import torch
-    cfg, _ = workloads.config("c2_24x24", n_games=300, max_turns=40, spawn_dmin=5)
-    env = gpu.GeneralsEnv(cfg, digest=False)
-    o = oracle_mod.Oracle(cfg, digest=False)
-    env.reset()
-    o.reset()
-    for _ in range(3):
-        env.step()
-        o.step()
-    torch.cuda.synchronize()
-    g = torch.cuda.CUDAGraph()
-    side = torch.cuda.Stream()
-    with torch.cuda.graph(g, stream=side):
-        for _ in range(5):
+    cfg, _ = workloads.config("c2_24x24", n_games=3000, max_turns=40, spawn_dmin=5)
+
+    def run(chain):
+        env = gpu.GeneralsEnv(cfg, digest=False)
+        env.set_chaining(chain)
+        env.reset()
+        for _ in range(3):
             env.step()
-    torch.cuda.synchronize()
-    assert env.global_step == 8
-    g.replay()
-    for _ in range(4):
-        env.step()
-    for _ in range(9):
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(5):
+                env.step()
+        torch.cuda.synchronize()
+        assert env.global_step == 8
+        g.replay()
+        for _ in range(4):
+            env.step()
+        torch.cuda.synchronize()
+        mid = {k: v.clone() for k, v in env.tensors.items() if k != "step_epoch"}
+        for _ in range(3):
+            g.replay()
+            g.replay()
+            env.step()
+            env.step()
+        torch.cuda.synchronize()
+        return env, mid, {k: v.clone() for k, v in env.tensors.items() if k != "step_epoch"}
+
+    env, mid, end = run(True)
+    o = oracle_mod.Oracle(cfg, digest=False)
+    o.reset()
+    for _ in range(12):
         o.step()
-    compare(env, o, digest=False, where="graph + eager")
-    g.replay()
-    g.replay()
-    env.step()
-    torch.cuda.synchronize()
+    for f in STATE_FIELDS + OUT_FIELDS:
+        t = mid[f][0] if f in OUT_FIELDS else mid[f]
+        got = t.cpu().numpy()
+        want = np.asarray(o.field(f))
+        if got.dtype != want.dtype:
+            got = got.view(want.dtype)
+        assert np.array_equal(got, want.reshape(got.shape)), f
+    _, mid2, end2 = run(False)
+    for k in end:
+        assert torch.equal(end[k], end2[k]) and torch.equal(mid[k], mid2[k]), k
 
 
 @pytest.mark.parametrize("name,N,T,over", [
