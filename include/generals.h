@@ -210,9 +210,12 @@ int gen_observe(gen_env *env, const gen_buffers *bufs, void *cuda_stream);
 int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, void *cuda_stream);
 
 /* End-to-end convenience: HOST actions in (int32 [N][P], may be NULL = sampler), HOST results out
- * (reward int8 [N][P], done uint8 [N]; either may be NULL).  Copies host->device into
- * bufs->actions_out (must be non-NULL when h_actions is given), runs gen_step, copies device->host,
- * all on cuda_stream, and synchronises that stream before returning.  Use pinned host memory. */
+ * (reward int8 [N][P], done uint8 [N]; either may be NULL); runs gen_step on cuda_stream and synchronises that stream
+ * before returning.  Pinned (page-locked or registered) host buffers are used in place: the step kernel reads the
+ * actions through their device alias and one small kernel writes reward + done into the host arrays -- no
+ * copy-engine transfers.  Pageable buffers go through cudaMemcpyAsync (actions via bufs->actions_out, which must
+ * then be non-NULL; it must be non-NULL whenever h_actions is given).  Whether a buffer is pinned is looked up when
+ * the pointer passed differs from the previous call's; do not unregister a buffer between calls and keep passing it. */
 int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
                   uint8_t *h_done, void *cuda_stream);
 

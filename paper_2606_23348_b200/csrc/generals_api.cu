@@ -21,6 +21,8 @@ struct gen_env {
     int32_t last_variant;    // index into GEN_VARIANTS of the last launch (-1: none yet)
     const uint32_t *chain_buf;  // non-NULL: the last launch of this handle was a k_step that kept records there
     int32_t no_chain;        // tests: never chain
+    const void *hp_key[3];   // gen_step_host: the host pointers last looked up (actions, reward, done) ...
+    void *hp_dev[3];         // ... and their device aliases (nullptr: pageable memory)
 };
 
 namespace {
@@ -227,6 +229,36 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     return GEN_OK;
 }
 
+// gen_step_host with pinned host buffers: one kernel carries reward [N][P] and done [N] to the mapped host memory
+// (two byte ranges, 16-byte vectors where the alignment allows) instead of two copy-engine transfers.
+__global__ void k_mirror(const unsigned char *__restrict__ src0, unsigned char *__restrict__ dst0, size_t n0,
+                         const unsigned char *__restrict__ src1, unsigned char *__restrict__ dst1, size_t n1) {
+    const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nthr = (size_t)gridDim.x * blockDim.x;
+    for (int r = 0; r < 2; ++r) {
+        const unsigned char *src = r ? src1 : src0;
+        unsigned char *dst = r ? dst1 : dst0;
+        const size_t n = r ? n1 : n0;
+        if (!dst || !n) continue;
+        if ((((uintptr_t)src | (uintptr_t)dst) & 15u) == 0) {
+            const size_t nv = n / 16;
+            for (size_t i = tid; i < nv; i += nthr)
+                reinterpret_cast<uint4 *>(dst)[i] = reinterpret_cast<const uint4 *>(src)[i];
+            for (size_t i = nv * 16 + tid; i < n; i += nthr) dst[i] = src[i];
+        } else {
+            for (size_t i = tid; i < n; i += nthr) dst[i] = src[i];
+        }
+    }
+}
+
+// device alias of a host pointer that the GPU can access directly (pinned / registered memory), else nullptr
+void *mapped_alias(const void *h) {
+    if (!h) return nullptr;
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, h) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+    if (at.type != cudaMemoryTypeHost) return nullptr;
+    return at.devicePointer;
+}
+
 uint64_t host_mix64(uint64_t z) {  // splitmix64 finaliser: the digest keys of R28
     z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ull;
     z ^= z >> 27; z *= 0x94D049BB133111EBull;
@@ -365,12 +397,40 @@ int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_action
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     const size_t N = (size_t)env->cfg.n_games, P = (size_t)env->cfg.n_players;
     cudaError_t ce = cudaSuccess;
-    if (h_actions) ce = cudaMemcpyAsync(bufs->actions_out, h_actions, N * P * 4, cudaMemcpyHostToDevice, s);
-    if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
-    const int e = gen_step(env, bufs, h_actions ? bufs->actions_out : nullptr, cuda_stream);
+    // Pinned host buffers are used in place: the step kernel reads the actions through their device alias and one
+    // small kernel writes reward + done into the host arrays (no copy-engine transfers).  Pageable buffers take the
+    // cudaMemcpyAsync route.  The alias lookups are cached per handle (same buffers every step in an RL loop).
+    if (h_actions != env->hp_key[0] || h_reward != env->hp_key[1] || h_done != env->hp_key[2]) {
+        env->hp_key[0] = h_actions; env->hp_key[1] = h_reward; env->hp_key[2] = h_done;
+        env->hp_dev[0] = mapped_alias(h_actions);
+        env->hp_dev[1] = mapped_alias(h_reward);
+        env->hp_dev[2] = mapped_alias(h_done);
+    }
+    const int32_t *d_act = nullptr;
+    if (h_actions) {
+        if (env->hp_dev[0] && aligned16(env->hp_dev[0])) {
+            d_act = static_cast<const int32_t *>(env->hp_dev[0]);
+        } else {
+            ce = cudaMemcpyAsync(bufs->actions_out, h_actions, N * P * 4, cudaMemcpyHostToDevice, s);
+            if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
+            d_act = bufs->actions_out;
+        }
+    }
+    const int e = gen_step(env, bufs, d_act, cuda_stream);
     if (e != GEN_OK) return e;
-    if (h_reward) ce = cudaMemcpyAsync(h_reward, bufs->reward, N * P, cudaMemcpyDeviceToHost, s);
-    if (ce == cudaSuccess && h_done) ce = cudaMemcpyAsync(h_done, bufs->done, N, cudaMemcpyDeviceToHost, s);
+    const bool mirror = N > 0 && (!h_reward || env->hp_dev[1]) && (!h_done || env->hp_dev[2]) && (h_reward || h_done);
+    if (mirror) {
+        const size_t bytes = N * P + N;
+        const int threads = 256, blocks = (int)((bytes / 16 + threads) / threads < 296 ? (bytes / 16 + threads) / threads : 296);
+        k_mirror<<<blocks, threads, 0, s>>>(reinterpret_cast<const unsigned char *>(bufs->reward),
+                                            static_cast<unsigned char *>(env->hp_dev[1]), h_reward ? N * P : 0,
+                                            bufs->done, static_cast<unsigned char *>(env->hp_dev[2]), h_done ? N : 0);
+        ce = cudaGetLastError();
+        if (ce == cudaSuccess) env->launches += 1;
+    } else {
+        if (h_reward) ce = cudaMemcpyAsync(h_reward, bufs->reward, N * P, cudaMemcpyDeviceToHost, s);
+        if (ce == cudaSuccess && h_done) ce = cudaMemcpyAsync(h_done, bufs->done, N, cudaMemcpyDeviceToHost, s);
+    }
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
     if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
     return GEN_OK;

@@ -535,22 +535,39 @@ def test_keep_episode_reset(gpu, oracle_mod):
     assert env.field("episode").tolist() == list(range(16))
 
 
-def test_step_host_end_to_end(gpu, oracle_mod):
+@pytest.mark.parametrize("pinned,N", [(True, 32), (False, 32), (True, 37), (True, 3000)])
+def test_step_host_end_to_end(gpu, oracle_mod, pinned, N):
+    """gen_step_host: pinned host buffers are used in place (the step kernel reads the actions through their device
+    alias, one small kernel writes reward + done into the host arrays); pageable buffers take the memcpy route; odd
+    sizes exercise the unaligned tails.  Mixed: pinned actions with pageable results and the other way round."""
     import torch
-    cfg, _ = workloads.config("c1_8x8", n_games=32)
+    cfg, _ = workloads.config("c1_8x8", n_games=N, auto_reset=1, max_turns=30)
     env, o = make_pair(gpu, oracle_mod, cfg)
     env.reset()
     o.reset()
-    h_a = torch.zeros((32, 2), dtype=torch.int32).pin_memory()
-    h_r = torch.zeros((32, 2), dtype=torch.int8).pin_memory()
-    h_d = torch.zeros((32,), dtype=torch.uint8).pin_memory()
-    for t in range(40):
+    mk = (lambda t: t.pin_memory()) if pinned else (lambda t: t)
+    h_a = mk(torch.zeros((N, 2), dtype=torch.int32))
+    h_r = mk(torch.zeros((N, 2), dtype=torch.int8))
+    h_d = mk(torch.zeros((N,), dtype=torch.uint8))
+    h_r2 = torch.zeros((N, 2), dtype=torch.int8)                 # pageable
+    h_a2 = torch.zeros((N, 2), dtype=torch.int32).pin_memory()  # pinned
+    for t in range(60):
         a = o.sample()
+        if t % 3 == 2:                                           # mixed kinds of memory in one call
+            h_a2.copy_(torch.from_numpy(a))
+            env.step_host(h_a2, h_r2, h_d)
+            o.step(a)
+            assert np.array_equal(h_r2.numpy(), o.reward[0]) and np.array_equal(h_d.numpy(), o.done[0])
+            continue
         h_a.copy_(torch.from_numpy(a))
         env.step_host(h_a, h_r, h_d)
         o.step(a)
         assert np.array_equal(h_r.numpy(), o.reward[0]) and np.array_equal(h_d.numpy(), o.done[0])
+    env.step_host(None, None, h_d)                               # sampler, done only
+    o.step()
+    assert np.array_equal(h_d.numpy(), o.done[0])
     compare(env, o, where="step_host")
+    assert int(o.episodes_done.sum()) > 0
 
 
 # ------------------------------------------------------------------------------- full-size sampled check
