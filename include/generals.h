@@ -267,7 +267,7 @@ int gen_set_launch(gen_env *env, int32_t games_per_cta);
 
 /* Kernel selection overrides for tests.  The library holds two kernels: the STAGED one (planes resident in
  * shared memory; serves every call) and the REGISTER-RESIDENT per-step one (gen_step with bufs->bitboards
- * and without a digest buffer, uniform policy), each as a generic instantiation for every board up to
+ * and without a digest buffer), each as a generic instantiation for every board up to
  * 32x32 and as instantiations compiled for the paper-sized configurations (1v1 8x8 and 24x24, 4 and 8
  * players on 32x32).  force_generic != 0: never launch a board-specialised instantiation;
  * force_staged == 1: never launch the register-resident kernel; force_staged == -1: launch it

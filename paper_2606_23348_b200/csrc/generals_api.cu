@@ -155,7 +155,7 @@ const gen::Variant kVariants[gen::N_VARIANTS] = {
 };
 
 // The most specialised instantiation that serves this launch.  step_ok: the register-resident kernel may
-// be used (gen_step with the bitboard cache, no digest, uniform policy).  Within a kind: the exact board
+// be used (gen_step with the bitboard cache, no digest).  Within a kind: the exact board
 // (and, for the staged kernel, the exact mode) first, else the generic kernel of the smallest NP >= P.
 const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, bool step_ok) {
     const int kind = (step_ok ? 1 : 0) + (kp.map_mode == 1 ? 2 : 0);
@@ -193,11 +193,11 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     kp.b = *bufs;
     kp.actions = actions;
     kp.sample_out = sample_out;
-    // gen_step proper (one turn, planes, no digest) with the bitboard cache and the uniform policy runs the
-    // register-resident kernel; everything else the staged one
+    // gen_step proper (one turn, planes, no digest) with the bitboard cache runs the register-resident kernel;
+    // everything else the staged one
     // (more than 4 players: one lane per player in the word passes and 8 x 4 half-written lines per chunk in the
     // emit pass -- measured 2x the DRAM traffic and half the speed of the staged kernel, so those stay there)
-    const bool step_ok = !env->force_staged && K == 1 && bufs->bitboards && kp.bias_thr == 0 &&
+    const bool step_ok = !env->force_staged && K == 1 && bufs->bitboards &&
                          (flags & ~gen::F_SAMPLER) == gen::F_OBS_PLANES && (kp.P <= 4 || env->force_step);
     const gen::Variant *v = pick_variant(env, kp, step_ok);
     if (!v) return GEN_ERR_CONFIG;

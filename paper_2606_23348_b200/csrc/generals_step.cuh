@@ -15,8 +15,8 @@
 // Same thread mapping as generals_kernels.cuh: a warp owns 4 consecutive games, an octet of 8 lanes one
 // game; word passes split the octet by player; lane 0 of the octet runs the serial rules.  Same rules
 // text (section IV, readings R1..R32 of DESIGN.md); parity with the oracle is bit-exact.
-// Not served here (the host falls back to the staged kernel): observation digest, K > 1, the biased
-// policy (R25), gen_reset / gen_observe / gen_sample.
+// Not served here (the host falls back to the staged kernel): observation digest, K > 1, gen_reset /
+// gen_observe / gen_sample.
 #pragma once
 #include "generals_kernels.cuh"
 
@@ -227,7 +227,51 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         const uint32_t total = n0 + n1 + n2 + n3;
         const int half = (w[2] < kp.half_thr) ? 1 : 0;
         int action = 0;
-        const bool decided = (w[0] < kp.pass_thr) || total == 0;
+        bool decided = (w[0] < kp.pass_thr) || total == 0;
+        if (kp.bias_thr) {  // uniform branch: the biased policy of config 4 (R25)
+            // largest owned stack, ties -> lowest cell index: max of (army + 1) << 10 | (1023 - cell).  The army
+            // plane stays in HBM / L2 in this kernel: every lane reads the 8-cell vectors of its words that hold an
+            // owned cell (four independent 16-byte loads per word), compares in registers, the player's lanes reduce.
+            const int16_t *Ag = B.army + (size_t)(wg0 + lg) * S;
+            uint32_t best = 0;
+            for (int j = js; j < je; ++j) {
+                const uint32_t m = own[j] & s_inb[j];
+                uint4 v[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    v[q] = ((m >> (8 * q)) & 0xFFu) ? __ldcg(reinterpret_cast<const uint4 *>(Ag + 32 * j + 8 * q))
+                                                    : make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t mb = (m >> (8 * q)) & 0xFFu;
+                    if (!mb) continue;
+                    const uint32_t a[4] = {v[q].x, v[q].y, v[q].z, v[q].w};
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const uint32_t army = (a[e >> 1] >> (16 * (e & 1))) & 0xFFFFu;
+                        const int c = 32 * j + 8 * q + e;
+                        if ((mb >> e) & 1u) best = max(best, ((army + 1u) << 10) | (uint32_t)(1023 - c));
+                    }
+                }
+            }
+#pragma unroll
+            for (int o = LPP / 2; o >= 1; o >>= 1) best = max(best, __shfl_xor_sync(gmask, best, o));
+            if (!decided && w[3] < kp.bias_thr && best) {
+                const int bc = 1023 - (int)(best & 1023u), jb = bc >> 5, bb = bc & 31;
+                const uint32_t fp = freew(mtn, jb - 1), fc = freew(mtn, jb), fn = freew(mtn, jb + 1);
+                const uint32_t src = (own[jb] & a2[jb]) >> bb;
+                const uint32_t okw[4] = {__funnelshift_lc(fp, fc, W), __funnelshift_rc(fc, fn, W),
+                                         __funnelshift_l(fp, fc, 1) & s_nc0[jb], __funnelshift_r(fc, fn, 1) & s_ncL[jb]};
+                uint32_t vb = 0;
+#pragma unroll
+                for (int dd = 0; dd < 4; ++dd) vb |= ((src & (okw[dd] >> bb)) & 1u) << dd;
+                if (vb) {
+                    const int dd = nth_bit(vb, mulhi32(w[1], (uint32_t)__popc(vb)));
+                    action = bc * 9 + 1 + 2 * dd + half;
+                    decided = true;
+                }
+            }
+        }
         uint32_t idx = mulhi32(w[1], total);
         int d = 0;
         uint32_t cnt = ln01 & 0xFFFFu;

@@ -5,7 +5,7 @@
 //           every call (reset, observe, sample, step, K-step rollout, digest).
 //   kind 2 / 3: kind 0 / 1 with the official map generator (see the end of the table).
 //   kind 1: the REGISTER-RESIDENT per-step kernel k_step (generals_step.cuh): gen_step when the caller
-//           provides the bitboard cache and no digest buffer, uniform policy.
+//           provides the bitboard cache and no digest buffer.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -13,8 +13,7 @@
 
 namespace gen {
 
-// variant 12: gen_step on the staged kernel at 24x24 1v1 (the biased policy R25 of config 4 scans army values,
-// which only the staged kernel holds on chip)
+// variant 12: gen_step on the staged kernel at 24x24 1v1 (callers without the bitboard cache)
 constexpr uint32_t FF_ROLL_DIGEST = F_OBS_PLANES | F_DIGEST;     // gen_rollout(K, GEN_OBS_DIGEST)
 
 //  X(id, kind, NP, H, W, flags (kind 0) or 0, max threads per CTA, min CTAs per SM (kind 1))

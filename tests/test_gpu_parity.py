@@ -155,9 +155,8 @@ def test_specialised_step_kernels_match_oracle(gpu, oracle_mod, name, N, T, over
         if t % 16 == 0:
             compare(gen, o, digest=False, where=f"{name} generic step {t}")
             compare(stg, o, digest=False, where=f"{name} staged step {t}")
-    uniform = cfg["bias_thr"] == 0                          # the biased policy (R25) runs on the staged kernel
-    assert env.last_launch_specialised and env.last_launch_register_resident == uniform
-    assert not gen.last_launch_specialised and gen.last_launch_register_resident == uniform
+    assert env.last_launch_specialised and env.last_launch_register_resident      # also under the biased policy (R25)
+    assert not gen.last_launch_specialised and gen.last_launch_register_resident
     assert not stg.last_launch_register_resident
     assert int(o.episodes_done.sum()) > 0
 
@@ -611,7 +610,7 @@ def test_config2_full_size_sampled_games(gpu, oracle_mod, digest):
 @pytest.mark.parametrize("name,N,T,roll", [
     ("c3_sweep", 262144, 130, 32),        # config 3: steps interleaved with fused rollouts
     ("c3_sweep", 1048576, 70, 0),
-    ("c4_curriculum", 65536, 150, 0),     # biased policy: the staged kernel
+    ("c4_curriculum", 65536, 150, 0),     # biased policy (R25): the step kernel scans the army plane for the largest stack
     ("c5a_2v2", 32768, 120, 0),
     ("c5b_ffa8", 32768, 120, 0),
     ("c4_flags", 65536, 150, 0),          # NEXT-4: all three alternative rule readings at scale (uniform policy)
