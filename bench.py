@@ -31,7 +31,7 @@ WORKLOAD = "c2_24x24"
 HBM_FALLBACK_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum of one gen_step launch, by games per launch, from the
 # `ncu --set full` capture summarised in profiles/ (see profiles/README.md); None where not captured
-NCU_DRAM_BYTES_PER_LAUNCH = {16384: 99168512}        # profiles/r01_step_full_chained_summary.txt
+NCU_DRAM_BYTES_PER_LAUNCH = {16384: 99745536}        # profiles/r01_step_full_chained_summary.txt
 NCU_FEAT_DRAM_BYTES_PER_LAUNCH = {16384: 3601662088}  # profiles/r01_features_full_summary.txt (k_features)
 
 
@@ -282,7 +282,7 @@ def run_ours(args):
                      "isolated_launch_us": 1e3 * iso_ms,
                      "isolated_note": "median of single launches, each after a 256 MB L2-flush write, own event pair"},
         "e2e": {"value": world * N * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": N * P * 4,
-                "d2h_bytes_per_step": N * P + N, "api": "gen_step_host (pinned host actions in, reward + done out)",
+                "d2h_bytes_per_step": N * P + N, "api": "gen_step_host (pinned host actions read in place, reward + done written to pinned host arrays, stream synchronised every step)",
                 "done_checksum": checksum},
         "rollout": {"value": world * N * 32 * n_roll / (roll_ms * 1e-3), "unit": UNIT, "K": 32, "launches": n_roll,
                     "obs": "digest every turn, planes of the last turn", "bound": "alu"},
