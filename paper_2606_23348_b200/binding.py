@@ -207,6 +207,7 @@ class GeneralsEnv:
             for name, _, _ in BUFFERS:                     # any aligned non-NULL value passes validation
                 if name in self.tensors:
                     setattr(self.bufs, name, 16)
+        self._bufs_ref = C.byref(self.bufs)
         self.set_policy(**pol)
 
     # ------------------------------------------------------------------ plumbing
@@ -217,8 +218,12 @@ class GeneralsEnv:
             raise GenError(f"generals: {msg} (code {code}, cuda error {cuda})")
 
     def _stream(self, stream=None):
-        s = stream if stream is not None else self.torch.cuda.current_stream(self.device)
-        return C.c_void_p(s.cuda_stream)
+        if stream is not None:
+            return C.c_void_p(stream.cuda_stream)
+        raw = getattr(self.torch._C, "_cuda_getCurrentRawStream", None)      # the current stream, without the wrapper
+        if raw is not None:
+            return C.c_void_p(raw(self.device.index if self.device.index is not None else self.torch.cuda.current_device()))
+        return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
 
     def close(self):
         if getattr(self, "_env", None):
@@ -285,7 +290,9 @@ class GeneralsEnv:
             assert actions.is_cuda and actions.dtype == self.torch.int32 and actions.is_contiguous()
             assert actions.numel() == self.N * self.P
             ptr = C.c_void_p(actions.data_ptr())
-        self._check(self.lib.gen_step(self._env, C.byref(self.bufs), ptr, self._stream(stream)))
+        code = self.lib.gen_step(self._env, self._bufs_ref, ptr, self._stream(stream))
+        if code != 0:
+            self._check(code)
 
     def rollout(self, K, obs_mode=OBS_DIGEST, stream=None):
         if obs_mode == OBS_EVERY_STEP and K > self.K:
