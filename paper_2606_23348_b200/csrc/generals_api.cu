@@ -206,6 +206,18 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     while (32 * WPC > v->max_threads) WPC >>= 1;
     const bool digest = (flags & gen::F_DIGEST) != 0;
     if (v->kind & 1) layout_step(kp, WPC); else layout(kp, WPC, digest);
+    // staged kernel, default geometry: big boards with many players are limited by shared memory (7.4 KB per game at
+    // 32x32 with 8 players); one warp per CTA then packs more games onto an SM (FFA-8: 28 instead of 24, +9 %)
+    if (!(v->kind & 1) && !env->games_per_cta && WPC == 2) {
+        auto resident = [&](int w) {
+            layout(kp, w, digest);
+            const long ctas = 232448L / ((long)kp.smem_bytes + 1024L);
+            return (ctas < 32 ? ctas : 32) * gen::GW * w;
+        };
+        const long r2 = resident(2), r1 = resident(1);
+        if (r1 > r2) WPC = 1;
+        layout(kp, WPC, digest);
+    }
     while (WPC > 1 && kp.smem_bytes > kMaxSmem) {
         WPC >>= 1;
         if (v->kind & 1) layout_step(kp, WPC); else layout(kp, WPC, digest);
