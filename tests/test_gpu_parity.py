@@ -748,6 +748,11 @@ def test_features_staged_kernel_and_errors(gpu, oracle_mod):
     env4.reset()
     with pytest.raises(gpu.GenError):
         env4.features()
+    cfg0, _ = workloads.config("c2_24x24", n_games=0)          # an empty batch is served without a launch
+    env0 = gpu.GeneralsEnv(cfg0)
+    env0.reset()
+    n0 = env0.launch_count
+    assert env0.features().shape == (0, 2, 38, 576) and env0.launch_count == n0
 
 
 def test_features_full_size_sampled_games(gpu, oracle_mod):
