@@ -114,7 +114,8 @@ void layout(gen::KParams &k, int WPC, bool digest) {
     k.WPC = WPC;
     const uint32_t GW = (uint32_t)gen::GW, S = (uint32_t)k.S;
     k.off_key = 416;  // three tables of 34 words (zero guards at both ends), 16-byte aligned
-    k.off_warp0 = align_up(k.off_key + (digest ? 8u * S : 0u), 128);
+    (void)digest;     // the digest keys are a global table (generals_kernels.cuh), no shared memory
+    k.off_warp0 = align_up(k.off_key, 128);
     uint32_t off = 2 * GW * S;
     k.w_owner = off; off += GW * S;
     k.w_terr = off; off += GW * S;

@@ -31,6 +31,10 @@
 
 #include "generals.h"
 
+// `if constexpr (OFFICIAL) { ...; return; }` leaves the synthetic generator behind it unreachable in the official
+// instantiations: that is the intent, not a finding
+#pragma nv_diag_suppress 128
+
 namespace gen {
 
 constexpr uint32_t FULL = 0xffffffffu;
@@ -123,6 +127,23 @@ __device__ __forceinline__ uint64_t mix64(uint64_t z) {  // splitmix64 finaliser
 }
 
 __device__ __forceinline__ uint32_t mulhi32(uint32_t u, uint32_t n) { return __umulhi(u, n); }
+
+// Digest keys (R28): key(c) = the (c + 1)-th output of splitmix64(seed 0), forced odd.  They do not depend on the
+// board, so they are a compile-time table in global memory, read through the read-only path (8 KB, L1-resident)
+// instead of a per-CTA copy in shared memory (which cost the fused rollout one resident CTA per SM).
+struct DigestKeys { unsigned long long k[1024]; };
+constexpr DigestKeys make_digest_keys() {
+    DigestKeys t{};
+    for (int c = 0; c < 1024; ++c) {
+        unsigned long long z = (unsigned long long)(c + 1) * 0x9E3779B97F4A7C15ull;
+        z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ull;
+        z ^= z >> 27; z *= 0x94D049BB133111EBull;
+        z ^= z >> 31;
+        t.k[c] = z | 1ull;
+    }
+    return t;
+}
+static __device__ const DigestKeys g_digest_keys = make_digest_keys();
 
 __device__ __forceinline__ int nth_bit(uint32_t w, uint32_t r) {  // position of the r-th (0-based) set bit
     int pos = 0;
@@ -483,7 +504,6 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     // CTA-wide tables, index j + 1 for bitboard word j (entries 0 and 33 are zero guards): column masks,
     // in-bounds mask; digest keys
     uint32_t *s_nc0 = reinterpret_cast<uint32_t *>(smem) + 1, *s_ncL = s_nc0 + 34, *s_inb = s_nc0 + 68;
-    uint64_t *s_key = reinterpret_cast<uint64_t *>(smem + kp.off_key);
     // this warp's slice
     unsigned char *wb = smem + kp.off_warp0 + (size_t)wic * kp.warp_bytes;
     int16_t *s_army = reinterpret_cast<int16_t *>(wb);
@@ -707,10 +727,6 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         s_nc0[j] = in ? kp.notcol0[j & 31] : 0u;
         s_ncL[j] = in ? kp.notcolL[j & 31] : 0u;
         s_inb[j] = in ? kp.inb[j & 31] : 0u;
-    }
-    if (flags & F_DIGEST) {
-        for (int c = tid; c < S; c += blockDim.x)
-            s_key[c] = (c < HW) ? (mix64((uint64_t)(c + 1) * 0x9E3779B97F4A7C15ull) | 1ull) : 0ull;
     }
     pdl_launch_dependents();
     pdl_wait();
@@ -1186,11 +1202,18 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 const uint32_t otx = (((o.x & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu) | (t.x << 4);
                 const uint32_t oty = (((o.y & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu) | (t.y << 4);
                 const uint32_t aw[4] = {a.x, a.y, a.z, a.w};
+                // the eight keys of the chunk: four 16-byte loads (cells past the board are never visible)
+                unsigned long long key[8];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const ulonglong2 kk = __ldg(reinterpret_cast<const ulonglong2 *>(g_digest_keys.k + 8 * ch) + i);
+                    key[2 * i] = kk.x; key[2 * i + 1] = kk.y;
+                }
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
                     const uint32_t half = (i & 1) ? (aw[i >> 1] >> 16) : (aw[i >> 1] & 0xFFFFu);
                     const uint32_t ob = (((i < 4) ? otx : oty) >> (8 * (i & 3))) & 0xFFu;
-                    const uint64_t xk = (uint64_t)(half | (ob << 16) | 0xC00000u) * s_key[8 * ch + i];
+                    const uint64_t xk = (uint64_t)(half | (ob << 16) | 0xC00000u) * key[i];
 #pragma unroll
                     for (int p = 0; p < NP; ++p)
                         if (p < P && ((vb[p] >> i) & 1u)) h[p] += xk;
