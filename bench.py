@@ -200,6 +200,18 @@ def run_ours(args):
     total_ms = max_over_ranks(e0.elapsed_time(e1))
     specialised, reg_resident = env.last_launch_specialised, env.last_launch_register_resident
 
+    # ---- one environment stepped K times back to back (an RL loop with a device-side policy: launch t+1 depends on
+    # launch t game by game; the 132 MB working set of one batch is partly L2-resident, so this is NOT the roofline leg)
+    for t in range(Wm):
+        env.step()
+    barrier()
+    e0.record()
+    for t in range(K):
+        env.step()
+    e1.record()
+    barrier()
+    same_ms = max_over_ranks(e0.elapsed_time(e1))
+
     # ---- the same with a 256 MB L2-flush write before every launch and one event pair per launch
     # (isolated launches: includes the launch latency a back-to-back stream hides)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -284,6 +296,9 @@ def run_ours(args):
         "e2e": {"value": world * N * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": N * P * 4,
                 "d2h_bytes_per_step": N * P + N, "api": "gen_step_host (pinned host actions read in place, reward + done written to pinned host arrays, stream synchronised every step)",
                 "done_checksum": checksum},
+        "same_env": {"value": world * N * K / (same_ms * 1e-3), "unit": UNIT, "us_per_launch": 1e3 * same_ms / K,
+                     "note": "one environment stepped K times back to back (true game-by-game dependency between "
+                             "launches; working set partly L2-resident: not a roofline figure)"},
         "rollout": {"value": world * N * 32 * n_roll / (roll_ms * 1e-3), "unit": UNIT, "K": 32, "launches": n_roll,
                     "obs": "digest every turn, planes of the last turn", "bound": "alu"},
     }
