@@ -439,7 +439,8 @@ def run_features(args):
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     peak, peak_src = measured_peak()
-    cfg, _ = workloads.config(WORKLOAD)
+    wl = args.workload or WORKLOAD
+    cfg, _ = workloads.config(wl)
     if args.games:
         cfg["n_games"] = args.games
     N, H, W = cfg["n_games"], cfg["height"], cfg["width"]
@@ -471,7 +472,7 @@ def run_features(args):
     feat_ms = statistics.mean(a.elapsed_time(b) for a, b in ev)
     bfeat = feature_bytes_per_game(H, W, bf16)
     achieved = N * bfeat / (feat_ms * 1e-3) / 1e9
-    line = {"workload": f"{WORKLOAD}: 1v1 {H}x{W}, {N} games, gen_step + gen_features every turn",
+    line = {"workload": f"{wl}: 1v1 {H}x{W}, {N} games, gen_step + gen_features every turn",
             "n_games": N, "steps": K, "dtype": "bf16 (R37)" if bf16 else "f32",
             "feature_tensor_bytes": N * 2 * 38 * env.S * (2 if bf16 else 4),
             "step_plus_features": {"env_steps_per_s": N / (both_ms * 1e-3), "us_per_turn": 1e3 * both_ms},
@@ -510,6 +511,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
     ap.add_argument("--rows", default="", help="with --sweep: only the rows whose workload name contains this")
+    ap.add_argument("--workload", default="", help="with --features: workload name (default c2_24x24)")
     ap.add_argument("--bf16", action="store_true", help="with --features: the bfloat16 feature tensor (R37)")
     ap.add_argument("--features", action="store_true", help="NEXT-1: gen_features alone and with gen_step (one JSON line)")
     args = ap.parse_args()

@@ -289,12 +289,14 @@ cudaError_t launch_one(const FeatParams &fp, int threads, cudaStream_t stream) {
 
 }  // namespace
 
-// Board-specialised instantiations for the paper-sized 1v1 boards (BASELINE configs 1 and 2-4), else the generic one.
+// Board-specialised instantiations for the paper-sized 1v1 boards (BASELINE configs 1 and 2-4, the paper's own 23x23),
+// else the generic one.
 cudaError_t launch_features(const FeatParams &fp, cudaStream_t stream) {
     const int per_game = 2 * (fp.S >> 2);
     const int threads = (fp.G * per_game + 31) / 32 * 32;
     if (threads < 64) return cudaErrorInvalidConfiguration;   // the coordinate tables need two warps
     if (!fp.force_generic && fp.H == 24 && fp.W == 24 && threads <= 288) return launch_one<24, 24, 288, 3>(fp, threads, stream);
+    if (!fp.force_generic && fp.H == 23 && fp.W == 23 && threads <= 288) return launch_one<23, 23, 288, 3>(fp, threads, stream);
     if (!fp.force_generic && fp.H == 8 && fp.W == 8 && threads <= 256) return launch_one<8, 8, 256, 4>(fp, threads, stream);
     return launch_one<0, 0, 512, 2>(fp, threads, stream);
 }
