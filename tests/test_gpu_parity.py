@@ -607,6 +607,50 @@ def test_config2_full_size_sampled_games(gpu, oracle_mod, digest):
     assert ((owner[:, None, :] == np.arange(2)[None, :, None]) <= vis.astype(bool)).all()
 
 
+@pytest.mark.parametrize("name,n_ids,history", [
+    ("c2_24x24", 64, True),          # 16,384 games x 2,000 steps
+    ("c3_sweep", 32, False),         # 262,144 games x 1,000 steps
+    ("c4_curriculum", 24, False),    # 65,536 games x 4,000 steps, biased policy
+    ("c5a_2v2", 16, False),          # 32,768 games x 2,000 steps, 2v2 on 32x32
+    ("c5b_ffa8", 10, False),         # 32,768 games x 2,000 steps, 8-player free-for-all
+])
+def test_configs_full_length(gpu, oracle_mod, name, n_ids, history):
+    """BASELINE configs 2-5 in full -- every game of the batch stepped for the config's whole length with auto-reset,
+    in the launch configuration bench.py times (bitboard cache, no digest, chained launches where they apply).  The
+    oracle replays a sample of global game ids over all turns: state, observation and accumulators (episodes
+    finished, wins, truncations, saturations) must agree at the end; for config 2 the scoreboard history ring (R34)
+    pins the last 512 turns of the trajectory on the way."""
+    cfg, T = workloads.config(name)
+    N = cfg["n_games"]
+    env = gpu.GeneralsEnv(cfg, digest=False, actions_out=False, history=history)
+    env.reset()
+    for _ in range(T):
+        env.step()
+    env.torch.cuda.synchronize()
+    assert env.global_step == T
+    stride = max(1, N // max(1, n_ids - 4))
+    ids = sorted(set([0, 1, N - 2, N - 1] + list(range(stride // 2, N, stride))))
+    fields = STATE_FIELDS + OUT_FIELDS + (["score_hist"] if history else [])
+    import torch
+    sel = torch.tensor(ids, device=env.device)
+    got = {}
+    for f in fields:
+        t = env.tensors[f][0] if f in OUT_FIELDS else env.tensors[f]
+        got[f] = t.index_select(0, sel).cpu().numpy()
+    for k, gid in enumerate(ids):
+        o = oracle_mod.Oracle(dict(cfg, n_games=1, game_id_base=gid))
+        o.reset()
+        for _ in range(T):
+            o.step()
+        for f in fields:
+            want = np.asarray(o.field(f))[0] if f != "score_hist" else np.asarray(o.score_hist)[0]
+            have = got[f][k]
+            if have.dtype != want.dtype:
+                have = have.view(want.dtype)
+            assert np.array_equal(have, want.reshape(have.shape)), (name, gid, f)
+    assert int(env.tensors["episodes_done"].sum()) > 0
+
+
 @pytest.mark.parametrize("name,N,T,roll", [
     ("c3_sweep", 262144, 130, 32),        # config 3: steps interleaved with fused rollouts
     ("c3_sweep", 1048576, 70, 0),
