@@ -110,6 +110,23 @@ def oracle_throughput(cfg, sample_games, steps, warmup):
     return sample_games * steps / dt, dt
 
 
+def _oracle_worker(job):
+    cfg, base, games, steps = job
+    v, dt = oracle_throughput(dict(cfg, game_id_base=base), games, steps, 3)
+    return games * steps, dt
+
+
+def oracle_throughput_all_cores(cfg, games_per_core, steps):
+    """one oracle process per host core over disjoint game-id ranges (the oracle itself stays
+    single-threaded); aggregate env steps/s = all steps / the slowest process's time."""
+    import multiprocessing as mp
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    jobs = [(cfg, c * games_per_core, games_per_core, steps) for c in range(cores)]
+    with mp.get_context("spawn").Pool(cores) as pool:
+        out = pool.map(_oracle_worker, jobs)
+    return sum(n for n, _ in out) / max(dt for _, dt in out), cores
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -307,6 +324,13 @@ def run_ours(args):
         v, _ = oracle_throughput(dict(cfg, game_id_base=0), sample, steps, 5)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"first {sample} global game ids x {steps} turns of {WORKLOAD}, single thread"}
+        try:
+            va, cores = oracle_throughput_all_cores(dict(cfg), 64, 300)
+            line["cpu_baseline_all_cores"] = {"value": va, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                              "sample": f"one single-threaded oracle process per host core, 64 games x "
+                                                        f"300 turns of {WORKLOAD} each, disjoint global game ids"}
+        except Exception as exc:                                   # a baseline, never a reason to lose the line
+            line["cpu_baseline_all_cores"] = {"value": None, "error": repr(exc)}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
