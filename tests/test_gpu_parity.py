@@ -1035,3 +1035,24 @@ def test_features_bf16_match_oracle(gpu, oracle_mod, name, N, T, over):
             else:
                 assert np.array_equal(g[:, :, ch], want[:, :, ch]), f"turn {t}: channel {ch}"
     assert (o.feat > 256).any()
+
+
+def test_chaining_survives_geometry_changes(gpu, oracle_mod):
+    """Tickets are per group of 4 games, not per CTA: changing the CTA size between chained launches (gen_set_launch),
+    switching chaining off and on, and a batch that is not a multiple of the CTA size keep the trajectory bit-exact."""
+    cfg, _ = workloads.config("c2_24x24", n_games=1021, max_turns=60, spawn_dmin=5)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    o = oracle_mod.Oracle(cfg, digest=False)
+    env.reset()
+    o.reset()
+    for t in range(90):
+        if t % 7 == 3:
+            env.set_launch((4, 8, 16, 0)[(t // 7) % 4])
+        if t % 11 == 5:
+            env.set_chaining(t % 2 == 0)
+        env.step()
+        o.step()
+        if t % 10 == 9:
+            compare(env, o, digest=False, where=f"step {t}")
+    compare(env, o, digest=False, where="end")
