@@ -171,11 +171,11 @@ const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, boo
         if (v.np == 2 && kp.team_size > 1) continue;
         if ((kind & 1) == 0 && v.ff != (kp.flags & ~gen::F_SAMPLER)) continue;
         if (!exact) { exact = &v; continue; }
-        // the same kernel under several register budgets (resident CTAs per SM): 14 if that holds the whole batch
-        // resident in one wave, 12 while the launches of a multi-wave batch still chain (launch()), else 10; the
-        // closest budget on offer wins, the roomier one on a tie
+        // the same kernel under several register budgets (resident CTAs per SM): 14 if only that holds the whole
+        // batch resident in one wave, 12 for smaller batches and while the launches of a multi-wave batch still chain
+        // (launch()), else 10; the closest budget on offer wins, the roomier one on a tie
         const long ctas = (kp.N + 2 * gen::GW - 1) / (2 * gen::GW);
-        const int want = ctas <= 14 * kSMs ? 14 : (ctas <= 8 * 14 * kSMs ? 12 : 10);
+        const int want = ctas <= 12 * kSMs ? 12 : ctas <= 14 * kSMs ? 14 : ctas <= 8 * 14 * kSMs ? 12 : 10;
         const int dv = v.min_ctas > want ? v.min_ctas - want : want - v.min_ctas;
         const int de = exact->min_ctas > want ? exact->min_ctas - want : want - exact->min_ctas;
         if (dv < de || (dv == de && v.min_ctas < exact->min_ctas)) exact = &v;
