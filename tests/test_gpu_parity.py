@@ -1041,7 +1041,6 @@ def test_chaining_survives_geometry_changes(gpu, oracle_mod):
     """Tickets are per group of 4 games, not per CTA: changing the CTA size between chained launches (gen_set_launch),
     switching chaining off and on, and a batch that is not a multiple of the CTA size keep the trajectory bit-exact."""
     cfg, _ = workloads.config("c2_24x24", n_games=1021, max_turns=60, spawn_dmin=5)
-    env, o = make_pair(gpu, oracle_mod, cfg)
     env = gpu.GeneralsEnv(cfg, digest=False)
     o = oracle_mod.Oracle(cfg, digest=False)
     env.reset()
