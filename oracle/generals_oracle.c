@@ -21,7 +21,8 @@
  *   generator       : statistical + constraint checks, brute-force candidate lists
  *   official maps   : (R36) constraints of P:L79 re-checked with an independent shortest-path routine, Manhattan
  *                     closed form, tiny boards by hand (tests/test_oracle_mapgen.py)
- *   feature tensor  : (R35) channel identities, closed form, an independent memory log (test_oracle_features.py)
+ *   feature tensor  : (R35) hand-worked example W12 (tests/golden/features_worked_example.txt), channel identities,
+ *                     closed form, an independent memory log (test_oracle_features.py); bfloat16 (R37): torch's conversion
  *   sampler         : brute force "valid set == set of board-changing actions"
  * Parity unpinned BY THE PAPER (fixed by decree in DESIGN.md, the paper prints no
  * value that decides them): R6 move order, R11 rounding of the transferred half,

@@ -1055,3 +1055,37 @@ def test_chaining_survives_geometry_changes(gpu, oracle_mod):
         if t % 10 == 9:
             compare(env, o, digest=False, where=f"step {t}")
     compare(env, o, digest=False, where="end")
+
+
+def test_features_hand_worked_example_W12_on_gpu(gpu, oracle_mod):
+    """The hand-worked feature example of tests/golden/features_worked_example.txt replayed through gen_step (explicit
+    actions) and gen_features: the CUDA path against the values written out by hand, not against the oracle."""
+    import os
+    import torch
+    from helpers import hand_board
+    o = hand_board(oracle_mod, 2, 3, 2, {(0, 0): (GN, 0, 5), (0, 1): (PL, 0, 3), (0, 2): (MT, -1, 0),
+                                         (1, 0): (CT, -1, 42), (1, 2): (GN, 1, 7)}, turn=0)
+    env = gpu.GeneralsEnv(dict(n_games=1, height=2, width=3, n_players=2, team_size=1), digest=False)
+    put_board(env, o)
+    moves = [None, (act(0, 1, 3, DOWN), 0), (0, act(1, 2, 3, LEFT)), (0, act(1, 1, 3, UP))]
+    frames = []
+    for mv in moves:
+        if mv is not None:
+            env.step(torch.tensor([mv], dtype=torch.int32, device=env.device))
+        frames.append(env.features().cpu().numpy().copy())
+    want = {}
+    path = os.path.join(os.path.dirname(__file__), "golden", "features_worked_example.txt")
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        tok = line.split()
+        want.setdefault((int(tok[0]), int(tok[1])), {})[int(tok[2])] = np.array([float(x) for x in tok[3:]], np.float32)
+    for (fr, p), chans in want.items():
+        for ch in range(38):
+            got = frames[fr][0, p, ch, :6]
+            exp = chans.get(ch, np.zeros(6, np.float32))
+            if ch == 21:
+                assert np.allclose(got, exp, atol=1e-6), (fr, p, ch, got)
+            else:
+                assert np.array_equal(got, exp), (fr, p, ch, got, exp)
+        assert not frames[fr][0, p, :, 6:].any()

@@ -139,3 +139,37 @@ def test_bf16_output_is_the_fp32_tensor_rounded_to_nearest_even(oracle_mod):
     for val, bits in ((257.0, 0x4380), (259.0, 0x4382), (32767.0, 0x4700), (1.0, 0x3F80), (0.0, 0)):
         got = torch.tensor([val], dtype=torch.float32).to(torch.bfloat16).view(torch.int16).item() & 0xFFFF
         assert got == bits
+
+
+def test_hand_worked_example_W12(oracle_mod):
+    """tests/golden/features_worked_example.txt: four turns on a 2 x 3 board, every channel of three (turn, player)
+    views written out by hand from Table IV (values, memory, fog, age, scoreboard, coordinates, both delta stacks)."""
+    import os
+    from helpers import hand_board, act, DOWN, LEFT, UP
+    PL, MT, CT, GN = 0, 1, 2, 3
+    o = hand_board(oracle_mod, 2, 3, 2, {(0, 0): (GN, 0, 5), (0, 1): (PL, 0, 3), (0, 2): (MT, -1, 0),
+                                         (1, 0): (CT, -1, 42), (1, 2): (GN, 1, 7)}, turn=0)
+    moves = [None, (act(0, 1, 3, DOWN), 0), (0, act(1, 2, 3, LEFT)), (0, act(1, 1, 3, UP))]
+    frames = []
+    for mv in moves:
+        if mv is not None:
+            o.step(np.array([mv], dtype=np.int32))
+        frames.append(o.features().copy())
+    assert int(o.turn[0]) == 3
+    want = {}
+    path = os.path.join(os.path.dirname(__file__), "golden", "features_worked_example.txt")
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        tok = line.split()
+        want.setdefault((int(tok[0]), int(tok[1])), {})[int(tok[2])] = np.array([float(x) for x in tok[3:]], np.float32)
+    assert sorted(want) == [(0, 1), (1, 1), (3, 0)]
+    for (fr, p), chans in want.items():
+        for ch in range(38):
+            got = frames[fr][0, p, ch, :6]
+            exp = chans.get(ch, np.zeros(6, np.float32))
+            if ch == 21:
+                assert np.allclose(got, exp, atol=1e-6), (fr, p, ch, got)
+            else:
+                assert np.array_equal(got, exp), (fr, p, ch, got, exp)
+        assert not frames[fr][0, p, :, 6:].any()                 # stride padding is zero
