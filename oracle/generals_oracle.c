@@ -80,6 +80,7 @@ typedef struct {
     uint64_t *obs_digest;     /* [N] or NULL */
     uint8_t *obs_packed;      /* [N][P][S] or NULL: owner, terrain and visibility in one byte (R33) */
     int32_t *score_hist;      /* [N][512][2P] or NULL: ring of the public scoreboard per turn (R34) */
+    int8_t *play_size;        /* [N][2] or NULL: playable rows, columns of the current map (R36; R35 padded border) */
 } orc_buffers;
 
 /* ------------------------------------------------------------------ Philox
@@ -216,6 +217,7 @@ static void generate(const orc_config *cfg, const orc_buffers *b, int g)
                                (int)mulhi32(w[1], (uint32_t)(cfg->city_army_hi - cfg->city_army_lo + 1)));
     }
     free(list);
+    if (b->play_size) { b->play_size[2 * g] = (int8_t)H; b->play_size[2 * g + 1] = (int8_t)W; }
     b->turn[g] = 0;
     b->alive[g] = (uint8_t)((1u << P) - 1u);
 }
@@ -332,6 +334,7 @@ static void generate_official(const orc_config *cfg, const orc_buffers *b, int g
         }
         if (!ok) continue;
         gen[0] = (int16_t)g0; gen[1] = (int16_t)g1;
+        if (b->play_size) { b->play_size[2 * g] = (int8_t)h; b->play_size[2 * g + 1] = (int8_t)wd; }
         break;
     }
     free(list);
@@ -665,7 +668,8 @@ int32_t orc_observe(const orc_config *cfg, const orc_buffers *b)
  * R35): the memory is cleared when turn == 0 (a new episode always starts there); "opponent army (last observed)"
  * is the public scoreboard; channel 9 counts every visible neutral-owned cell; channel 21 is 0 where the enemy was
  * never seen or is visible now; deltas that reach before the episode's first frame are 0; coordinates are
- * col / (W - 1) and row / (H - 1); stride padding cells are 0 in every channel. */
+ * col / (W - 1) and row / (H - 1); stride padding cells are 0 in every channel; the padded border of a smaller
+ * playable area (play_size) is a known mountain from turn 0. */
 enum { FEAT_C = 38, FEAT_HIST = 7, FEAT_RING = 8 };
 
 typedef struct {
@@ -701,8 +705,15 @@ int32_t orc_features(const orc_config *cfg, const orc_buffers *b, const orc_feat
                 memset(hist_en, 0, sizeof(int16_t) * FEAT_RING * S);
             }
             memset(out, 0, sizeof(float) * FEAT_C * S);
+            /* Table IV ch 8 "visible mountains U known padded border", ch 13 "... or unseen padded border": with a
+             * playable area smaller than the board (R36) the cells outside it are mountains the agent knows of
+             * from the first turn */
+            /* (0 = not recorded, e.g. a board written by hand: the full board) */
+            const int ph = (b->play_size && b->play_size[2 * g] > 0) ? b->play_size[2 * g] : H;
+            const int pw = (b->play_size && b->play_size[2 * g + 1] > 0) ? b->play_size[2 * g + 1] : W;
             for (int c = 0; c < HW; ++c) {
                 const int r = c / W, col = c % W;
+                if (r >= ph || col >= pw) bits[4 * S + c] = 1;
                 int vis = 0;                                   /* own cells and their 8 neighbours */
                 for (int dr = -1; dr <= 1; ++dr)
                     for (int dc = -1; dc <= 1; ++dc) {

@@ -173,3 +173,54 @@ def test_hand_worked_example_W12(oracle_mod):
             else:
                 assert np.array_equal(got, exp), (fr, p, ch, got, exp)
         assert not frames[fr][0, p, :, 6:].any()                 # stride padding is zero
+
+
+def test_padded_border_is_a_known_mountain(oracle_mod):
+    """Table IV ch 8 "visible mountains U known padded border" and ch 13 "... or unseen padded border" on official
+    maps with a playable area smaller than the board (R36): from turn 0 on, every cell outside the playable
+    rectangle is in the mountain memory whether or not it has been seen; in fog it counts as a known structure.  The
+    border is re-derived here from the terrain plane (all-mountain suffix rows / columns agree with play_size), the
+    rest of ch 8 / ch 13 from the plain observation planes."""
+    cfg, _ = workloads.config("official_23x23", n_games=12, max_turns=40, spawn_dmin=6)
+    o = oracle_mod.Oracle(cfg)
+    o.reset()
+    H = W = 23
+    HW = H * W
+    seen_mtn = np.zeros((12, 2, HW), bool)
+    seen_str = np.zeros((12, 2, HW), bool)
+    saw_small = False
+    for t in range(90):
+        if t:
+            o.step()
+        f = o.features().copy()
+        new = o.turn == 0
+        seen_mtn[new] = False
+        seen_str[new] = False
+        ph, pw = o.play_size[:, 0].astype(int), o.play_size[:, 1].astype(int)
+        rr, cc = np.divmod(np.arange(HW), W)
+        border = (rr[None, :] >= ph[:, None]) | (cc[None, :] >= pw[:, None])           # [N][HW]
+        terr = o.terrain[:, :HW]
+        assert (terr[border] == 1).all()                                                # the padding is mountains
+        assert ((ph >= 18) & (ph <= 23) & (pw >= 18) & (pw <= 23)).all()
+        saw_small |= bool(border.any())
+        vis = o.field("obs_vis")[:, :, :HW] == 1
+        ot = o.field("obs_terrain")[:, :, :HW]
+        seen_mtn |= vis & (ot == 1)
+        seen_str |= vis & ((ot == 2) | (ot == 3))
+        want8 = seen_mtn | border[:, None, :]
+        assert np.array_equal(f[:, :, 8, :HW] == 1, want8)
+        want13 = ~vis & (want8 | seen_str)
+        assert np.array_equal(f[:, :, 13, :HW] == 1, want13)
+        # a border cell that has never been seen is already known at turn 0
+        if t == 0:
+            unseen_border = border[:, None, :] & ~vis
+            assert unseen_border.any() and (f[:, :, 13, :HW][unseen_border] == 1).all()
+    assert saw_small and int(o.episodes_done.sum()) > 0
+    # full boards: no border, ch 8 is the seen mountains only (the synthetic generator reports H x W)
+    cfg2, _ = workloads.config("c2_24x24", n_games=3)
+    o2 = oracle_mod.Oracle(cfg2)
+    o2.reset()
+    assert (o2.play_size == 24).all()
+    f2 = o2.features()
+    vis2 = o2.field("obs_vis")[:, :, :576] == 1
+    assert np.array_equal(f2[:, :, 8, :576] == 1, vis2 & (o2.field("obs_terrain")[:, :, :576] == 1))
