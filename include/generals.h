@@ -121,6 +121,9 @@ typedef struct gen_buffers {
     uint8_t *obs_packed;     /* out   [K][N][P][S]  packed observation, may be NULL (see below) */
     int32_t *score_hist;     /* state [N][512][2P]  scoreboard history ring, may be NULL (see below) */
     uint32_t *step_epoch;    /* state [2][ceil(N/4)]  launch chaining of gen_step, may be NULL (see below); zeroed once */
+    int8_t *play_size;       /* state [N][2]  playable rows, columns of the current map, may be NULL: written by the
+                                generators (H, W unless map_mode 1 with play_min, R36); gen_features reads it for Table
+                                IV's "known padded border" (0 = not recorded = the full board) */
 } gen_buffers;
 
 /* `step_epoch` lets consecutive gen_step launches of one handle overlap.  Without it a launch starts working only
@@ -163,7 +166,7 @@ typedef struct gen_sizes {
     size_t army, owner, terrain, turn, episode, alive, general_cell, land, army_total;
     size_t reward, done, winner, obs_army, obs_owner, obs_terrain, obs_vis;
     size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out, bitboards, obs_packed, score_hist;
-    size_t step_epoch;
+    size_t step_epoch, play_size;
     int32_t bitboard_row_words; /* BW */
 } gen_sizes;
 

@@ -65,6 +65,7 @@ BUFFERS = [
     ("obs_packed", "uint8", lambda N, P, S, K: (K, N, P, S)),
     ("score_hist", "int32", lambda N, P, S, K: (N, 512, 2 * P)),
     ("step_epoch", "int32", lambda N, P, S, K: (2, (N + 3) // 4)),                      # bits of uint32
+    ("play_size", "int8", lambda N, P, S, K: (N, 2)),
 ]
 
 

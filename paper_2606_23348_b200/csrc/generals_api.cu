@@ -77,6 +77,7 @@ void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
     s->obs_packed = k * N * P * S;
     s->score_hist = N * 512 * 2 * P * 4;
     s->step_epoch = (N + 3) / 4 * 8;
+    s->play_size = N * 2;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -101,6 +102,7 @@ int check_buffers(const gen_buffers *b, bool need_obs) {
     if (b->bitboards && !aligned16(b->bitboards)) return GEN_ERR_ALIGN;
     if (b->score_hist && !aligned16(b->score_hist)) return GEN_ERR_ALIGN;
     if (b->step_epoch && !aligned16(b->step_epoch)) return GEN_ERR_ALIGN;
+    if (b->play_size && !aligned16(b->play_size)) return GEN_ERR_ALIGN;
     return GEN_OK;
 }
 
@@ -488,7 +490,7 @@ int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *
     fp.G = per_game >= 256 ? 1 : 256 / per_game;
     fp.force_generic = env->force_generic;
     fp.army = bufs->army; fp.owner = bufs->owner; fp.terrain = bufs->terrain; fp.turn = bufs->turn;
-    fp.land = bufs->land; fp.army_total = bufs->army_total;
+    fp.land = bufs->land; fp.army_total = bufs->army_total; fp.play_size = bufs->play_size;
     fp.feat = const_cast<void *>(out); fp.bf16 = feat->feat_bf16 ? 1 : 0; fp.mem_bits = feat->mem_bits; fp.last_army = feat->last_army;
     fp.last_seen = feat->last_seen; fp.hist = feat->hist;
     const cudaError_t e = gen::launch_features(fp, static_cast<cudaStream_t>(cuda_stream));

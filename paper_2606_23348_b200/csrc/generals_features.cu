@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_features(const FeatParams fp) {
     const size_t gp = (size_t)g * 2 + p;
     const int c0 = 4 * q;
 
-    int t = 0;
+    int t = 0, ph = H, pw = W;                               // playable rows / columns (R36): the rest is a known border
     int2 land2 = make_int2(0, 0), tot2 = make_int2(0, 0);
     uint2 army2 = make_uint2(0u, 0u);
     uint32_t terr4 = 0, bits4 = 0;
@@ -94,6 +94,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_features(const FeatParams fp) {
     for (int k = 0; k < FEAT_HIST; ++k) hown[k] = hen[k] = make_uint2(0u, 0u);
     if (active) {
         t = __ldg(fp.turn + g);
+        if (fp.play_size) {
+            const int v = (int)__ldg(reinterpret_cast<const uint16_t *>(fp.play_size) + g);
+            const int vh = (int8_t)(v & 0xff), vw = (int8_t)(v >> 8);
+            if (vh > 0) ph = vh;                             // 0 = not recorded (a board written by hand): the full board
+            if (vw > 0) pw = vw;
+        }
         land2 = __ldg(reinterpret_cast<const int2 *>(fp.land) + g);
         tot2 = __ldg(reinterpret_cast<const int2 *>(fp.army_total) + g);
         army2 = __ldg(reinterpret_cast<const uint2 *>(fp.army + (size_t)g * S + c0));
@@ -185,6 +191,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_features(const FeatParams fp) {
         neu[j] = vis[j] && o == -1;
         uint32_t b = (uint32_t)vis[j] | ((uint32_t)en[j] << 1);
         if (vis[j]) b |= (tr == 3u ? 4u : 0u) | (tr == 2u ? 8u : 0u) | (tr == 1u ? 16u : 0u);
+        if (valid[j] && (rowj[j] >= ph || colj[j] >= pw)) b |= 16u;   // Table IV ch 8: "U known padded border"
         newbits4 |= b << (8 * j);
         if (en[j]) { l16[j] = a16[j]; seen[j] = t + 1; any_en = true; }
         own_f[j] = mine[j] ? a16[j] : 0u;

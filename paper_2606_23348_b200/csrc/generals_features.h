@@ -15,6 +15,7 @@ struct FeatParams {
     const int32_t *turn;
     const int32_t *land;
     const int32_t *army_total;
+    const int8_t *play_size;     // [N][2] playable rows, columns (or NULL / 0: the full board)
     int bf16;                    // feat points at bfloat16 (R37) instead of float
     void *feat;                  // gen_feat_buffers: feat or feat_bf16
     uint8_t *mem_bits;

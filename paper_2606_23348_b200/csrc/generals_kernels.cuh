@@ -282,7 +282,8 @@ static __device__ __noinline__ void rows_bfs(uint32_t pass, int src_r, int src_c
 }
 
 static __device__ __noinline__ void generate_official(const KParams &kp, uint32_t lane, uint32_t gid, uint32_t episode,
-                                               int16_t *A, int8_t *O, int8_t *Tr, int16_t *gcell_out) {
+                                               int16_t *A, int8_t *O, int8_t *Tr, int16_t *gcell_out,
+                                               int8_t *psize_out) {
     const int H = kp.H, W = kp.W, HW = kp.HW, S = kp.S;
     constexpr int kAttempts = 16, kFar = (1 << 20) - 1;
     uint32_t w[4];
@@ -367,6 +368,7 @@ static __device__ __noinline__ void generate_official(const KParams &kp, uint32_
         if (lane == 0) {
             Tr[g0] = (int8_t)T_GENERAL; O[g0] = 0; A[g0] = 1; gcell_out[0] = (int16_t)g0;
             Tr[g1] = (int8_t)T_GENERAL; O[g1] = 1; A[g1] = 1; gcell_out[1] = (int16_t)g1;
+            if (psize_out) { psize_out[0] = (int8_t)h; psize_out[1] = (int8_t)wd; }
         }
         break;
     }
@@ -379,11 +381,12 @@ static __device__ __noinline__ void generate_official(const KParams &kp, uint32_
 // and must not tax the register allocation of the turn); the staged kernel carries the same procedure inline.
 template <int NP, bool OFFICIAL>
 __device__ __noinline__ void generate_board(const KParams &kp, uint32_t lane, uint32_t gid, uint32_t episode,
-                                            int16_t *A, int8_t *O, int8_t *Tr, int16_t *gcell_out) {
+                                            int16_t *A, int8_t *O, int8_t *Tr, int16_t *gcell_out, int8_t *psize_out) {
     const int P = kp.P, HW = kp.HW, S = kp.S, NW = kp.NW, W = kp.W;
     __syncwarp();
+    if (!OFFICIAL && psize_out && lane == 0) { psize_out[0] = (int8_t)kp.H; psize_out[1] = (int8_t)kp.W; }
     if constexpr (OFFICIAL) {                                    // the official generator (R36)
-        generate_official(kp, lane, gid, episode, A, O, Tr, gcell_out);
+        generate_official(kp, lane, gid, episode, A, O, Tr, gcell_out, psize_out);
         return;
     }
     for (int i = lane; i < S / 4; i += 32) {
@@ -538,7 +541,8 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         const uint32_t gid = kp.gid_base + (uint32_t)gg, episode = gs.episode;
         __syncwarp();
         if constexpr (OFFICIAL) {                                // R36, in the instantiations compiled for it
-            generate_official(kp, lane, gid, episode, A, O, Tr, B.general_cell + (size_t)gg * P);
+            generate_official(kp, lane, gid, episode, A, O, Tr, B.general_cell + (size_t)gg * P,
+                              B.play_size ? B.play_size + 2 * (size_t)gg : nullptr);
             if (lane == 0) {
                 gs.turn = 0;
                 gs.alive = allp;
@@ -548,6 +552,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             __syncwarp();
             return;
         }
+        if (B.play_size && lane == 0) { B.play_size[2 * (size_t)gg] = (int8_t)H; B.play_size[2 * (size_t)gg + 1] = (int8_t)W; }
         for (int i = lane; i < S / 4; i += 32) {
             reinterpret_cast<uint32_t *>(O)[i] = 0xFFFFFFFFu;
             reinterpret_cast<uint32_t *>(A)[2 * i] = 0;

@@ -583,7 +583,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         int16_t *sA = reinterpret_cast<int16_t *>(s_scratch);
         int8_t *sO = reinterpret_cast<int8_t *>(s_scratch + 2 * S), *sT = reinterpret_cast<int8_t *>(s_scratch + 3 * S);
         generate_board<NP, OFFICIAL>(kp, lane, kp.gid_base + (uint32_t)gg, gs.episode, sA, sO, sT,
-                           B.general_cell + (size_t)gg * P);
+                                     B.general_cell + (size_t)gg * P,
+                                     B.play_size ? B.play_size + 2 * (size_t)gg : nullptr);
         const int rb = 4 * BW;  // row stride in bytes
         unsigned char *rows = row8(0, lg);
         for (int ch = (int)lane; ch < rb; ch += 32) {

@@ -854,10 +854,12 @@ def test_official_maps_match_oracle(gpu, oracle_mod, N, T, over, staged):
     env.reset()
     o.reset()
     compare(env, o, where="reset")
+    compare_features(env, o, where="reset")                     # Table IV's known padded border (ch 8, ch 13)
     for t in range(T):
         env.step()
         o.step()
         compare(env, o, where=f"step {t}")
+        compare_features(env, o, where=f"step {t}")
     env.rollout(24, gpu.OBS_DIGEST)
     o.rollout(24, oracle_mod.OBS_DIGEST)
     compare(env, o, where="rollout")
