@@ -662,9 +662,9 @@ int32_t orc_observe(const orc_config *cfg, const orc_buffers *b)
 }
 
 /* ===================================================================== NEXT-1: the 38-channel feature tensor
- * PAPER.md Appendix A and Table IV, 1v1 only (the table speaks of "the agent" and "the
- * opponent").  One call per turn and game: it folds the current observation into the per-episode memory and
- * writes, for each player p as the agent, C = 24 + 2 * 7 = 38 float maps feat[g][p][ch][S].  Readings (DESIGN.md
+ * PAPER.md Appendix A and Table IV.  One call per turn and game: it folds the current
+ * observation into the per-episode memory and writes, for each player p as the agent, C = 24 + 2 * 7 = 38 float
+ * maps feat[g][p][ch][S] (more than two players: reading R38 below).  Readings (DESIGN.md
  * R35): the memory is cleared when turn == 0 (a new episode always starts there); "opponent army (last observed)"
  * is the public scoreboard; channel 9 counts every visible neutral-owned cell; channel 21 is 0 where the enemy was
  * never seen or is visible now; deltas that reach before the episode's first frame are 0; coordinates are
@@ -673,10 +673,10 @@ int32_t orc_observe(const orc_config *cfg, const orc_buffers *b)
 enum { FEAT_C = 38, FEAT_HIST = 7, FEAT_RING = 8 };
 
 typedef struct {
-    uint8_t *bits;        /* [N][2][5][S]  seen, enemy_seen, generals, castles, mountains (0 / 1) */
-    int16_t *last_army;   /* [N][2][S]     enemy army last observed on the cell */
-    int32_t *last_turn;   /* [N][2][S]     turn of that observation, -1 = never */
-    int16_t *hist;        /* [N][2][2][8][S]  own_army / enemy_army frames, slot turn mod 8 */
+    uint8_t *bits;        /* [N][P][5][S]  seen, enemy_seen, generals, castles, mountains (0 / 1) */
+    int16_t *last_army;   /* [N][P][S]     enemy army last observed on the cell */
+    int32_t *last_turn;   /* [N][P][S]     turn of that observation, -1 = never */
+    int16_t *hist;        /* [N][P][2][8][S]  own_army / enemy_army frames, slot turn mod 8 */
 } orc_feat_state;
 
 #include <math.h>
@@ -684,14 +684,20 @@ typedef struct {
 int32_t orc_features(const orc_config *cfg, const orc_buffers *b, const orc_feat_state *m, float *feat)
 {
     const int H = cfg->height, W = cfg->width, P = cfg->n_players, HW = H * W, S = plane_stride(cfg);
-    if (P != 2) return -1;
+    /* More than two players (R38; "the same observation ... interface for the 1v1, 2v2, and free-for-all
+     * formats"): "the agent" is player p, "the opponent" is every player who is not on p's team; visibility is the
+     * team's (R19); an ally's cells are visible but neither own, enemy nor neutral; the opponent's scoreboard
+     * entries (ch 18, 19) are the sums over all enemies.  With two players this is Table IV verbatim. */
     for (int g = 0; g < cfg->n_games; ++g) {
         const int16_t *army = b->army + (size_t)g * S;
         const int8_t *owner = b->owner + (size_t)g * S, *terrain = b->terrain + (size_t)g * S;
         const int t = b->turn[g];
-        for (int p = 0; p < 2; ++p) {
-            const int opp = 1 - p;
-            const size_t gp = (size_t)g * 2 + p;
+        for (int p = 0; p < P; ++p) {
+            const int team = team_of(cfg, p);
+            int opp_land = 0, opp_army = 0;
+            for (int q = 0; q < P; ++q)
+                if (team_of(cfg, q) != team) { opp_land += b->land[g * P + q]; opp_army += b->army_total[g * P + q]; }
+            const size_t gp = (size_t)g * P + p;
             uint8_t *bits = m->bits + gp * 5 * S;
             int16_t *last_army = m->last_army + gp * S;
             int32_t *last_turn = m->last_turn + gp * S;
@@ -718,11 +724,12 @@ int32_t orc_features(const orc_config *cfg, const orc_buffers *b, const orc_feat
                 for (int dr = -1; dr <= 1; ++dr)
                     for (int dc = -1; dc <= 1; ++dc) {
                         int rr = r + dr, cc = col + dc;
-                        if (rr >= 0 && rr < H && cc >= 0 && cc < W && owner[rr * W + cc] == p) vis = 1;
+                        if (rr >= 0 && rr < H && cc >= 0 && cc < W && owner[rr * W + cc] >= 0 &&
+                            team_of(cfg, owner[rr * W + cc]) == team) vis = 1;
                     }
                 const int a = army[c], o = owner[c], tr = terrain[c];
                 const int own_a = (o == p) ? a : 0;
-                const int en_vis = vis && o == opp;
+                const int en_vis = vis && o >= 0 && team_of(cfg, o) != team;
                 const int en_a = en_vis ? a : 0;
                 /* fold into the memory */
                 bits[0 * S + c] |= (uint8_t)vis;
@@ -746,10 +753,10 @@ int32_t orc_features(const orc_config *cfg, const orc_buffers *b, const orc_feat
                 out[13 * S + c] = (float)(!vis && (bits[2 * S + c] | bits[3 * S + c] | bits[4 * S + c]));
                 out[14 * S + c] = (float)t;
                 out[15 * S + c] = (float)(t % 50) / 50.0f;
-                out[16 * S + c] = (float)b->land[g * 2 + p];
-                out[17 * S + c] = (float)b->army_total[g * 2 + p];
-                out[18 * S + c] = (float)b->land[g * 2 + opp];
-                out[19 * S + c] = (float)b->army_total[g * 2 + opp];
+                out[16 * S + c] = (float)b->land[g * P + p];
+                out[17 * S + c] = (float)b->army_total[g * P + p];
+                out[18 * S + c] = (float)opp_land;
+                out[19 * S + c] = (float)opp_army;
                 out[20 * S + c] = (float)last_army[c];
                 out[21 * S + c] = (last_turn[c] < 0 || en_vis) ? 0.0f : logf(1.0f + (float)(t - last_turn[c])) / 5.0f;
                 out[22 * S + c] = W > 1 ? (float)col / (float)(W - 1) : 0.0f;
@@ -782,7 +789,7 @@ int32_t orc_features_bf16(const orc_config *cfg, const orc_buffers *b, const orc
 {
     const int32_t rc = orc_features(cfg, b, m, scratch);
     if (rc != 0) return rc;
-    const size_t n = (size_t)cfg->n_games * 2 * FEAT_C * (size_t)plane_stride(cfg);
+    const size_t n = (size_t)cfg->n_games * (size_t)cfg->n_players * FEAT_C * (size_t)plane_stride(cfg);
     for (size_t i = 0; i < n; ++i) feat16[i] = bf16_rne(scratch[i]);
     return 0;
 }

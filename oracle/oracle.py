@@ -179,21 +179,21 @@ class Oracle:
     def features(self, bf16=False):
         """NEXT-1: fold the current turn into the per-episode memory and return feat[N][2][38][S] (float32; with
         bf16=True the bfloat16 bit patterns as uint16, R37).  Call once per turn (after reset and after every step)."""
-        N, S = self.N, self.S
+        N, S, P = self.N, self.S, self.P
         if not hasattr(self, "feat"):
-            self.feat = np.zeros((N, 2, 38, S), dtype=np.float32)
-            self._fm = dict(bits=np.zeros((N, 2, 5, S), np.uint8), last_army=np.zeros((N, 2, S), np.int16),
-                            last_turn=np.full((N, 2, S), -1, np.int32), hist=np.zeros((N, 2, 2, 8, S), np.int16))
+            self.feat = np.zeros((N, P, 38, S), dtype=np.float32)
+            self._fm = dict(bits=np.zeros((N, P, 5, S), np.uint8), last_army=np.zeros((N, P, S), np.int16),
+                            last_turn=np.full((N, P, S), -1, np.int32), hist=np.zeros((N, P, 2, 8, S), np.int16))
             self._fs = OrcFeatState(*[self._fm[k].ctypes.data for k in ("bits", "last_army", "last_turn", "hist")])
         if bf16:
             if not hasattr(self, "feat16"):
-                self.feat16 = np.zeros((N, 2, 38, S), dtype=np.uint16)
+                self.feat16 = np.zeros((N, P, 38, S), dtype=np.uint16)
             rc = lib().orc_features_bf16(C.byref(self.cfg), C.byref(self.bufs), C.byref(self._fs),
                                          self.feat.ctypes.data, self.feat16.ctypes.data)
         else:
             rc = lib().orc_features(C.byref(self.cfg), C.byref(self.bufs), C.byref(self._fs), self.feat.ctypes.data)
         if rc != 0:
-            raise ValueError("orc_features: 1v1 only")
+            raise ValueError("orc_features failed")
         return self.feat16 if bf16 else self.feat
 
     def set_policy(self, pass_thr=None, half_thr=None, bias_thr=None):

@@ -107,12 +107,58 @@ def test_closed_form_under_all_pass_play(oracle_mod):
                 assert f[g, p, 4].sum() == f[g, p, 0, :64].size - f[g, p, 12, :64].sum()    # seen == visible: nothing moves
 
 
-def test_features_are_1v1_only(oracle_mod):
-    cfg, _ = workloads.config("c5a_2v2", n_games=1, height=10, width=10, spawn_dmin=3, n_cities=2)
+@pytest.mark.parametrize("name,P,team_size", [("c5a_2v2", 4, 2), ("c5b_ffa8", 8, 1), ("c5b_ffa8", 3, 1)])
+def test_multi_player_features_from_the_plain_observation(oracle_mod, name, P, team_size):
+    """R38 (the same observation interface in 1v1, 2v2 and free-for-all): agent = player p, opponent = every
+    player off p's team, visibility = the team's.  Pinned against the oracle's plain observation planes (which carry
+    the team visibility of P:L83 / R19 and are pinned elsewhere) and the public scoreboard: instantaneous channels,
+    the memory rebuilt by the test, the enemy-sum scoreboard entries; the four cell classes now leave out exactly the
+    visible cells of allies."""
+    cfg, _ = workloads.config(name, n_games=6, height=12, width=13, n_players=P, team_size=team_size, spawn_dmin=3,
+                              n_cities=4, max_turns=60)
     o = oracle_mod.Oracle(cfg)
     o.reset()
-    with pytest.raises(ValueError):
-        o.features()
+    N, S, HW = 6, o.S, 12 * 13
+    me = np.arange(P)[None, :, None]
+    team = np.arange(P) // team_size
+    enemy_of = team[:, None] != team[None, :]                          # [agent][other]
+    seen = np.zeros((N, P, S), bool); en_seen = seen.copy(); last_army = np.zeros((N, P, S), np.int64)
+    last_turn = np.full((N, P, S), -1, np.int64)
+    allies_seen = False
+    for t in range(140):
+        if t:
+            o.step()
+        f = o.features().copy()
+        assert f.shape == (N, P, 38, S)
+        new = o.turn == 0
+        seen[new] = False; en_seen[new] = False; last_army[new] = 0; last_turn[new] = -1
+        vis = o.field("obs_vis").astype(bool)
+        owner = o.field("obs_owner").astype(np.int64)
+        army = o.field("obs_army").astype(np.int64)
+        own = owner == me
+        is_player = owner >= 0
+        enemy = vis & is_player & enemy_of[np.arange(P)[None, :, None], np.clip(owner, 0, P - 1)]
+        ally = vis & is_player & ~own & ~enemy
+        allies_seen |= bool(ally.any())
+        neutral = vis & (owner == -1)
+        assert np.array_equal(f[:, :, 0], army) and np.array_equal(f[:, :, 1], np.where(own, army, 0))
+        assert np.array_equal(f[:, :, 2], np.where(enemy, army, 0)) and np.array_equal(f[:, :, 3], np.where(neutral, army, 0))
+        assert np.array_equal(f[:, :, 9], neutral) and np.array_equal(f[:, :, 10], own) and np.array_equal(f[:, :, 11], enemy)
+        assert np.array_equal(f[:, :, 12][:, :, :HW], ~vis[:, :, :HW])
+        assert np.array_equal((f[:, :, 9] + f[:, :, 10] + f[:, :, 11] + f[:, :, 12])[:, :, :HW], 1 - ally[:, :, :HW])
+        seen |= vis; en_seen |= enemy
+        last_army = np.where(enemy, army, last_army); last_turn = np.where(enemy, o.turn[:, None, None], last_turn)
+        assert np.array_equal(f[:, :, 4], seen) and np.array_equal(f[:, :, 5], en_seen)
+        assert np.array_equal(f[:, :, 20], last_army)
+        age = np.where((last_turn < 0) | enemy, 0.0, np.log1p((o.turn[:, None, None] - last_turn).clip(0)) / 5.0)
+        assert np.allclose(f[:, :, 21], age, atol=1e-6)
+        land, tot = o.land.astype(np.int64), o.army_total.astype(np.int64)
+        for p in range(P):
+            assert (f[:, p, 16, :HW] == land[:, p, None]).all() and (f[:, p, 17, :HW] == tot[:, p, None]).all()
+            assert (f[:, p, 18, :HW] == land[:, enemy_of[p]].sum(1)[:, None]).all()
+            assert (f[:, p, 19, :HW] == tot[:, enemy_of[p]].sum(1)[:, None]).all()
+    assert allies_seen == (team_size > 1)
+    assert int(o.episodes_done.sum()) > 0
 
 
 def test_bf16_output_is_the_fp32_tensor_rounded_to_nearest_even(oracle_mod):
