@@ -448,11 +448,11 @@ def run_sweep(args):
 
 
 # ------------------------------------------------------------------------------------------ NEXT-1: features
-def feature_bytes_per_game(H, W, bf16=False):
+def feature_bytes_per_game(H, W, bf16=False, P=2):
     """Algorithmic bytes of one gen_features call per game: per cell read the three state
     planes (4 B) and, per player, write 38 float32 channels (152 B; 76 B as bfloat16, R37), write this turn's two
     history frames (4 B), read the seven previous ones (28 B) and the memory (bits 1 B, last army 2 B, last sighting 4 B)."""
-    return H * W * (4 + 2 * ((76 if bf16 else 152) + 4 + 28 + 7))
+    return H * W * (4 + P * ((76 if bf16 else 152) + 4 + 28 + 7))
 
 
 def run_features(args):
@@ -494,16 +494,16 @@ def run_features(args):
         b.record()
     torch.cuda.synchronize()
     feat_ms = statistics.mean(a.elapsed_time(b) for a, b in ev)
-    bfeat = feature_bytes_per_game(H, W, bf16)
+    bfeat = feature_bytes_per_game(H, W, bf16, cfg["n_players"])
     achieved = N * bfeat / (feat_ms * 1e-3) / 1e9
-    line = {"workload": f"{wl}: 1v1 {H}x{W}, {N} games, gen_step + gen_features every turn",
+    line = {"workload": f"{wl}: {cfg['n_players']} players {H}x{W}, {N} games, gen_step + gen_features every turn",
             "n_games": N, "steps": K, "dtype": "bf16 (R37)" if bf16 else "f32",
-            "feature_tensor_bytes": N * 2 * 38 * env.S * (2 if bf16 else 4),
+            "feature_tensor_bytes": N * cfg["n_players"] * 38 * env.S * (2 if bf16 else 4),
             "step_plus_features": {"env_steps_per_s": N / (both_ms * 1e-3), "us_per_turn": 1e3 * both_ms},
             "features": {"games_per_s": N / (feat_ms * 1e-3), "us_per_launch": 1e3 * feat_ms,
                          "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                                       "frac": achieved / peak, "traffic": None if bf16 else NCU_FEAT_DRAM_BYTES_PER_LAUNCH.get(N),
-                                      "kernel": "gen::k_features",
+                                      "kernel": "gen::k_features" if cfg["n_players"] == 2 else "gen::k_features_mp",
                                       "peak_source": peak_src, "algorithmic_bytes_per_game": bfeat,
                                       "units_per_launch": N}}}
     if not args.no_cpu_baseline:

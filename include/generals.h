@@ -224,7 +224,9 @@ int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_action
 
 /* ---- the 38-channel feature tensor (Appendix A, Table IV; R35) ----
  * What the paper's policy consumes, built from the state the step leaves behind plus a per-episode memory.
- * 1v1 only (Table IV speaks of "the agent" and "the opponent").  Channels, per player p as the agent, float32:
+ * Table IV speaks of "the agent" and "the opponent"; with more than two players (the same observation
+ * interface in 1v1, 2v2 and free-for-all; R38) the opponent is every player off the agent's team, visibility is the
+ * team's and channels 18 / 19 sum the enemies' scoreboard entries.  Channels, per player p as the agent, float32:
  *   0 armies (visible)  1 own_army  2 enemy_army (visible)  3 neutral_army (visible)
  *   4 seen  5 enemy_seen  6 generals  7 castles  8 mountains          (memory: ever observed, this episode)
  *   9 neutral_cells (visible)  10 owned_cells  11 opponent_cells (visible)  12 fog_cells
@@ -238,12 +240,12 @@ int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_action
  * members are opaque to the caller: allocate them ZEROED once (a zeroed memory is an empty one) and pass the same
  * ones to every call. */
 typedef struct gen_feat_buffers {
-    float *feat;         /* out   [N][2][38][S]; stride padding cells are 0 */
-    uint8_t *mem_bits;   /* state [N][2][S]     bit k = channel 4 + k */
-    int16_t *last_army;  /* state [N][2][S]     channel 20 */
-    int32_t *last_seen;  /* state [N][2][S]     turn of the last enemy sighting + 1, 0 = never */
-    int16_t *hist;       /* state [N][2][8][2][S]  own_army / enemy_army frames, slot = turn mod 8 */
-    uint16_t *feat_bf16; /* out   [N][2][38][S] bfloat16 bit patterns (R37); when non-NULL it is written INSTEAD of
+    float *feat;         /* out   [N][P][38][S]; stride padding cells are 0 */
+    uint8_t *mem_bits;   /* state [N][P][S]     bit k = channel 4 + k */
+    int16_t *last_army;  /* state [N][P][S]     channel 20 */
+    int32_t *last_seen;  /* state [N][P][S]     turn of the last enemy sighting + 1, 0 = never */
+    int16_t *hist;       /* state [N][P][8][2][S]  own_army / enemy_army frames, slot = turn mod 8 */
+    uint16_t *feat_bf16; /* out   [N][P][38][S] bfloat16 bit patterns (R37); when non-NULL it is written INSTEAD of
                             feat (which may then be NULL): every fp32 value rounded once, ties to even */
 } gen_feat_buffers;
 
@@ -253,15 +255,14 @@ typedef struct gen_feat_sizes {
     size_t feat, mem_bits, last_army, last_seen, hist, feat_bf16; /* bytes */
 } gen_feat_sizes;
 
-/* Byte sizes of the gen_feat_buffers members for `cfg`.  Host-only.  GEN_ERR_CONFIG unless n_players == 2 and
- * team_size == 1. */
+/* Byte sizes of the gen_feat_buffers members for `cfg`.  Host-only. */
 int gen_query_feat_sizes(const gen_config *cfg, gen_feat_sizes *out);
 
 /* Fold the state as it stands (after gen_reset, gen_step or gen_rollout) into each player's memory and write the
  * feature tensor.  Call it ONCE PER TURN: the delta channels difference consecutive calls' frames, and a game whose
  * turn counter is 0 (fresh or auto-reset, R17) starts from an empty memory.  Reads bufs->army / owner / terrain /
- * turn / land / army_total only; no game state changes.  One kernel launch on cuda_stream.  GEN_ERR_CONFIG unless
- * the handle is 1v1; GEN_ERR_NULL / GEN_ERR_ALIGN on a missing / misaligned pointer. */
+ * turn / land / army_total (and play_size if given) only; no game state changes.  One kernel launch on cuda_stream.
+ * GEN_ERR_NULL / GEN_ERR_ALIGN on a missing / misaligned pointer. */
 int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *feat, void *cuda_stream);
 
 /* Launch geometry override for tuning: games per CTA in {4, 8, 16, 32} (8 threads per game); 0 restores

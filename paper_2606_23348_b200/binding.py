@@ -79,14 +79,14 @@ class GenSizes(C.Structure):
 
 
 FEAT_CHANNELS = 38
-# gen_feat_buffers: name -> (torch dtype name, shape builder(N, S))
+# gen_feat_buffers: name -> (torch dtype name, shape builder(N, P, S))
 FEAT_BUFFERS = [
-    ("feat", "float32", lambda N, S: (N, 2, FEAT_CHANNELS, S)),
-    ("mem_bits", "uint8", lambda N, S: (N, 2, S)),
-    ("last_army", "int16", lambda N, S: (N, 2, S)),
-    ("last_seen", "int32", lambda N, S: (N, 2, S)),
-    ("hist", "int16", lambda N, S: (N, 2, 8, 2, S)),
-    ("feat_bf16", "bfloat16", lambda N, S: (N, 2, FEAT_CHANNELS, S)),
+    ("feat", "float32", lambda N, P, S: (N, P, FEAT_CHANNELS, S)),
+    ("mem_bits", "uint8", lambda N, P, S: (N, P, S)),
+    ("last_army", "int16", lambda N, P, S: (N, P, S)),
+    ("last_seen", "int32", lambda N, P, S: (N, P, S)),
+    ("hist", "int16", lambda N, P, S: (N, P, 8, 2, S)),
+    ("feat_bf16", "bfloat16", lambda N, P, S: (N, P, FEAT_CHANNELS, S)),
 ]
 
 
@@ -311,8 +311,8 @@ class GeneralsEnv:
 
     def features(self, stream=None, bf16=False):
         """NEXT-1 (R35): fold the current turn into each player's memory and return feat, a float32 CUDA tensor
-        [N][2][38][S] (bf16=True: a bfloat16 tensor, R37; the choice is made at the first call).  Call once per turn
-        (after reset and after every step).  1v1 only."""
+        [N][P][38][S] (bf16=True: a bfloat16 tensor, R37; the choice is made at the first call).  Call once per turn
+        (after reset and after every step).  More than two players: reading R38."""
         if not hasattr(self, "feat_bufs"):
             sizes = GenFeatSizes()
             self._check(self.lib.gen_query_feat_sizes(C.byref(self.cfg), C.byref(sizes)))
@@ -322,7 +322,7 @@ class GeneralsEnv:
                 if name == ("feat" if bf16 else "feat_bf16"):
                     setattr(self.feat_bufs, name, None)
                     continue
-                t = self.torch.zeros(shape(self.N, self.S), dtype=getattr(self.torch, dt), device=self.device)
+                t = self.torch.zeros(shape(self.N, self.P, self.S), dtype=getattr(self.torch, dt), device=self.device)
                 assert t.numel() * t.element_size() == getattr(sizes, name), name
                 self.feat_tensors[name] = t
                 setattr(self.feat_bufs, name, t.data_ptr() if t.numel() else 16)

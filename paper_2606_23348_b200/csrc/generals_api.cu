@@ -457,23 +457,22 @@ int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_action
 int gen_query_feat_sizes(const gen_config *cfg, gen_feat_sizes *out) {
     if (!cfg || !out) return GEN_ERR_NULL;
     if (int e = validate(cfg)) return e;
-    if (cfg->n_players != 2 || cfg->team_size != 1) return GEN_ERR_CONFIG;
     const size_t N = (size_t)cfg->n_games, S = (size_t)round_up(cfg->height * cfg->width, 16);
+    const size_t P = (size_t)cfg->n_players;
     std::memset(out, 0, sizeof(*out));
     out->channels = 38;
     out->plane_stride = (int32_t)S;
-    out->feat = N * 2 * 38 * S * 4;
-    out->mem_bits = N * 2 * S;
-    out->last_army = N * 2 * S * 2;
-    out->last_seen = N * 2 * S * 4;
-    out->hist = N * 2 * 8 * 2 * S * 2;
-    out->feat_bf16 = N * 2 * 38 * S * 2;
+    out->feat = N * P * 38 * S * 4;
+    out->mem_bits = N * P * S;
+    out->last_army = N * P * S * 2;
+    out->last_seen = N * P * S * 4;
+    out->hist = N * P * 8 * 2 * S * 2;
+    out->feat_bf16 = N * P * 38 * S * 2;
     return GEN_OK;
 }
 
 int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *feat, void *cuda_stream) {
     if (!env || !bufs || !feat) return GEN_ERR_NULL;
-    if (env->cfg.n_players != 2 || env->cfg.team_size != 1) return GEN_ERR_CONFIG;
     const void *out = feat->feat_bf16 ? (const void *)feat->feat_bf16 : (const void *)feat->feat;
     if (feat->feat && !aligned16(feat->feat)) return GEN_ERR_ALIGN;
     const void *req[] = {bufs->army, bufs->owner, bufs->terrain, bufs->turn, bufs->land, bufs->army_total,
@@ -485,6 +484,7 @@ int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *
     if (env->cfg.n_games == 0) return GEN_OK;
     gen::FeatParams fp;
     fp.N = env->base.N; fp.H = env->base.H; fp.W = env->base.W; fp.HW = env->base.HW; fp.S = env->base.S;
+    fp.P = env->base.P; fp.team_size = env->base.team_size;
     // 2 * S / 4 threads per game; small boards share a CTA of about 256 threads
     const int per_game = fp.S / 2;
     fp.G = per_game >= 256 ? 1 : 256 / per_game;

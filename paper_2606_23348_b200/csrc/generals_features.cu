@@ -283,6 +283,200 @@ __global__ void __launch_bounds__(MAXT, MINB) k_features(const FeatParams fp) {
 #undef EMIT
 }
 
+// ------------------------------------------------------------------------------------------------
+// More than two players (R38; the same observation interface in 1v1, 2v2 and free-for-all), any board.  "The
+// opponent" is every player off the agent's team, visibility is the team's, the opponent's scoreboard entries are
+// sums over the enemies.  One CTA per game; its threads loop over the P * Q (player, quad) items.  The per-item work
+// is the 1v1 kernel's (kept apart so that the tuned 1v1 path stays exactly what it is); the team test replaces the
+// "owner == 1 - p" compare.  dynamic shared memory: [S] owner bytes | [teams][H + 2] row words of the team's cells |
+// 32 + 32 coordinate floats | 8 + 8 scoreboard ints.
+template <typename OUT>
+__global__ void __launch_bounds__(256, 2) k_features_mp(const FeatParams fp) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int S = fp.S, Q = S >> 2, H = fp.H, W = fp.W, HW = fp.HW, P = fp.P, ts = fp.team_size;
+    const int NT = (P + ts - 1) / ts;
+    int8_t *s_owner = reinterpret_cast<int8_t *>(smem);
+    uint32_t *s_rows = reinterpret_cast<uint32_t *>(smem + S);
+    float *s_cx = reinterpret_cast<float *>(s_rows + NT * (H + 2));
+    float *s_cy = s_cx + 32;
+    int *s_land = reinterpret_cast<int *>(s_cy + 32), *s_tot = s_land + 8;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int g = blockIdx.x;
+    {
+        const int4 *src = reinterpret_cast<const int4 *>(fp.owner + (size_t)g * S);
+        int4 *dst = reinterpret_cast<int4 *>(s_owner);
+        for (int i = tid; i < (S >> 4); i += nthr) dst[i] = __ldg(src + i);
+        for (int i = tid; i < NT * (H + 2); i += nthr) s_rows[i] = 0u;
+        if (tid < 32) s_cx[tid] = W > 1 ? __fdiv_rn((float)tid, (float)(W - 1)) : 0.0f;
+        else if (tid < 64) s_cy[tid - 32] = H > 1 ? __fdiv_rn((float)(tid - 32), (float)(H - 1)) : 0.0f;
+        else if (tid < 64 + P) {
+            s_land[tid - 64] = __ldg(fp.land + (size_t)g * P + (tid - 64));
+            s_tot[tid - 64] = __ldg(fp.army_total + (size_t)g * P + (tid - 64));
+        }
+    }
+    __syncthreads();
+    for (int i = tid; i < NT * H; i += nthr) {      // one thread per (team, row): the cells of the team's members
+        const int T = i / H, r = i - T * H;
+        const int8_t *row = s_owner + r * W;
+        uint32_t w = 0;
+        for (int c = 0; c < W; ++c) {
+            const int o = row[c];
+            w |= (uint32_t)(o >= 0 && o / ts == T) << c;
+        }
+        s_rows[T * (H + 2) + r + 1] = w;
+    }
+    __syncthreads();
+
+    const int t = __ldg(fp.turn + g);
+    int ph = H, pw = W;
+    if (fp.play_size) {
+        const int v = (int)__ldg(reinterpret_cast<const uint16_t *>(fp.play_size) + g);
+        const int vh = (int8_t)(v & 0xff), vw = (int8_t)(v >> 8);
+        if (vh > 0) ph = vh;
+        if (vw > 0) pw = vw;
+    }
+    for (int item = tid; item < P * Q; item += nthr) {
+        const int p = item / Q, q = item - p * Q, team = p / ts, c0 = 4 * q;
+        const size_t gp = (size_t)g * P + p;
+        const uint2 army2 = __ldg(reinterpret_cast<const uint2 *>(fp.army + (size_t)g * S + c0));
+        const uint32_t terr4 = __ldg(reinterpret_cast<const uint32_t *>(fp.terrain + (size_t)g * S + c0));
+        const uint32_t own4 = *reinterpret_cast<const uint32_t *>(s_owner + c0);
+        uint8_t *mb = fp.mem_bits + gp * S + c0;
+        int16_t *la = fp.last_army + gp * S + c0;
+        int32_t *ls = fp.last_seen + gp * S + c0;
+        int16_t *hist = fp.hist + gp * FEAT_RING * 2 * S + c0;
+        uint32_t bits4 = 0;
+        uint2 last2 = make_uint2(0u, 0u);
+        int4 seen4 = make_int4(0, 0, 0, 0);
+        if (t > 0) {
+            bits4 = *reinterpret_cast<const uint32_t *>(mb);
+            last2 = *reinterpret_cast<const uint2 *>(la);
+            seen4 = *reinterpret_cast<const int4 *>(ls);
+        }
+        uint2 hown[FEAT_HIST], hen[FEAT_HIST];
+#pragma unroll
+        for (int k = 0; k < FEAT_HIST; ++k) {
+            hown[k] = hen[k] = make_uint2(0u, 0u);
+            if (t - k - 1 >= 0) {
+                const int slot = (t - k - 1) & (FEAT_RING - 1);
+                hown[k] = *reinterpret_cast<const uint2 *>(hist + (size_t)(slot * 2 + 0) * S);
+                hen[k] = *reinterpret_cast<const uint2 *>(hist + (size_t)(slot * 2 + 1) * S);
+            }
+        }
+        int l_op_i = 0, a_op_i = 0;
+        for (int e = 0; e < P; ++e)
+            if (e / ts != team) { l_op_i += s_land[e]; a_op_i += s_tot[e]; }
+
+        const uint32_t *rows = s_rows + team * (H + 2);
+        bool valid[4], vis[4], mine[4], en[4], neu[4];
+        int rowj[4], colj[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int c = c0 + j;
+            valid[j] = c < HW;
+            const int r = valid[j] ? c / W : 0, col = valid[j] ? c - r * W : 0;
+            uint32_t v = rows[r] | rows[r + 1] | rows[r + 2];
+            v |= (v << 1) | (v >> 1);
+            vis[j] = valid[j] && ((v >> col) & 1u);
+            rowj[j] = r; colj[j] = col;
+        }
+        const uint32_t a16[4] = {army2.x & 0xffffu, army2.x >> 16, army2.y & 0xffffu, army2.y >> 16};
+        uint32_t l16[4] = {last2.x & 0xffffu, last2.x >> 16, last2.y & 0xffffu, last2.y >> 16};
+        int seen[4] = {seen4.x, seen4.y, seen4.z, seen4.w};
+        uint32_t own_f[4], en_f[4];
+        uint32_t newbits4 = bits4;
+        bool any_en = false;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int o = (int8_t)((own4 >> (8 * j)) & 0xffu);
+            const uint32_t tr = (terr4 >> (8 * j)) & 0xffu;
+            mine[j] = valid[j] && o == p;
+            en[j] = vis[j] && o >= 0 && o / ts != team;
+            neu[j] = vis[j] && o == -1;
+            uint32_t b = (uint32_t)vis[j] | ((uint32_t)en[j] << 1);
+            if (vis[j]) b |= (tr == 3u ? 4u : 0u) | (tr == 2u ? 8u : 0u) | (tr == 1u ? 16u : 0u);
+            if (valid[j] && (rowj[j] >= ph || colj[j] >= pw)) b |= 16u;
+            newbits4 |= b << (8 * j);
+            if (en[j]) { l16[j] = a16[j]; seen[j] = t + 1; any_en = true; }
+            own_f[j] = mine[j] ? a16[j] : 0u;
+            en_f[j] = en[j] ? a16[j] : 0u;
+        }
+        const uint2 newlast2 = make_uint2(pack2(l16[0], l16[1]), pack2(l16[2], l16[3]));
+        if (newbits4 != bits4 || t == 0) *reinterpret_cast<uint32_t *>(mb) = newbits4;
+        if (any_en || t == 0) {
+            *reinterpret_cast<uint2 *>(la) = newlast2;
+            *reinterpret_cast<int4 *>(ls) = make_int4(seen[0], seen[1], seen[2], seen[3]);
+        }
+        {
+            const int slot = t & (FEAT_RING - 1);
+            *reinterpret_cast<uint2 *>(hist + (size_t)(slot * 2 + 0) * S) =
+                make_uint2(pack2(own_f[0], own_f[1]), pack2(own_f[2], own_f[3]));
+            *reinterpret_cast<uint2 *>(hist + (size_t)(slot * 2 + 1) * S) =
+                make_uint2(pack2(en_f[0], en_f[1]), pack2(en_f[2], en_f[3]));
+        }
+
+        OUT *out = reinterpret_cast<OUT *>(fp.feat) + gp * FEAT_C * S + c0;
+        float f[4], fa[4];
+        unpack4f(army2, fa);
+#define EMIT(ch, expr)                                                                     \
+    {                                                                                      \
+        _Pragma("unroll") for (int j = 0; j < 4; ++j) f[j] = valid[j] ? (expr) : 0.0f;    \
+        st4(out + (size_t)(ch) * S, f[0], f[1], f[2], f[3]);                               \
+    }
+        {
+            float cur_o[4], cur_e[4], prev[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { cur_o[j] = mine[j] ? fa[j] : 0.0f; cur_e[j] = en[j] ? fa[j] : 0.0f; }
+#pragma unroll
+            for (int k = 0; k < FEAT_HIST; ++k) {
+                const bool have = t - k - 1 >= 0;
+                unpack4f(hown[k], prev);
+                EMIT(24 + k, have ? cur_o[j] - prev[j] : 0.0f)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) cur_o[j] = prev[j];
+                unpack4f(hen[k], prev);
+                EMIT(31 + k, have ? cur_e[j] - prev[j] : 0.0f)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) cur_e[j] = prev[j];
+            }
+        }
+        EMIT(0, vis[j] ? fa[j] : 0.0f)
+        EMIT(1, mine[j] ? fa[j] : 0.0f)
+        EMIT(2, en[j] ? fa[j] : 0.0f)
+        EMIT(3, neu[j] ? fa[j] : 0.0f)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) EMIT(4 + k, ((newbits4 >> (8 * j + k)) & 1u) ? 1.0f : 0.0f)
+        EMIT(9, neu[j] ? 1.0f : 0.0f)
+        EMIT(10, mine[j] ? 1.0f : 0.0f)
+        EMIT(11, en[j] ? 1.0f : 0.0f)
+        EMIT(12, vis[j] ? 0.0f : 1.0f)
+        EMIT(13, (!vis[j] && ((newbits4 >> (8 * j)) & 0x1cu) != 0u) ? 1.0f : 0.0f)
+        {
+            const float ft = (float)t, tick = __fdiv_rn((float)(t % 50), 50.0f);
+            const float l_me = (float)s_land[p], a_me = (float)s_tot[p];
+            const float l_op = (float)l_op_i, a_op = (float)a_op_i;
+            EMIT(14, ft)
+            EMIT(15, tick)
+            EMIT(16, l_me)
+            EMIT(17, a_me)
+            EMIT(18, l_op)
+            EMIT(19, a_op)
+        }
+        {
+            float fl[4], age[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+            unpack4f(newlast2, fl);
+            EMIT(20, fl[j])
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (seen[j] != 0 && !en[j]) age[j] = __fdiv_rn(logf(1.0f + (float)(t - (seen[j] - 1))), 5.0f);
+            EMIT(21, age[j])
+        }
+        EMIT(22, s_cx[colj[j]])
+        EMIT(23, s_cy[rowj[j]])
+#undef EMIT
+    }
+}
+
 namespace {
 
 template <int TH, int TW, int MAXT, int MINB>
@@ -299,6 +493,13 @@ cudaError_t launch_one(const FeatParams &fp, int threads, cudaStream_t stream) {
 // Board-specialised instantiations for the paper-sized 1v1 boards (BASELINE configs 1 and 2-4, the paper's own 23x23),
 // else the generic one.
 cudaError_t launch_features(const FeatParams &fp, cudaStream_t stream) {
+    if (fp.P != 2 || fp.team_size != 1) {          // R38: the multi-player kernel, one CTA per game
+        const int NT = (fp.P + fp.team_size - 1) / fp.team_size;
+        const size_t smem = (size_t)fp.S + (size_t)NT * (fp.H + 2) * 4 + 64 * 4 + 16 * 4;
+        if (fp.bf16) k_features_mp<__nv_bfloat16><<<fp.N, 256, smem, stream>>>(fp);
+        else k_features_mp<float><<<fp.N, 256, smem, stream>>>(fp);
+        return cudaGetLastError();
+    }
     const int per_game = 2 * (fp.S >> 2);
     const int threads = (fp.G * per_game + 31) / 32 * 32;
     if (threads < 64) return cudaErrorInvalidConfiguration;   // the coordinate tables need two warps

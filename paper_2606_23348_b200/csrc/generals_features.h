@@ -7,6 +7,7 @@ namespace gen {
 
 struct FeatParams {
     int N, H, W, HW, S;
+    int P, team_size;            // players, team size (1v1: 2, 1: the tuned kernel; else R38's)
     int G;                       // games per CTA (2 * S / 4 threads each)
     int force_generic;           // never launch a board-specialised instantiation (tests)
     const int16_t *army;         // state planes and scalars of gen_buffers (read only)

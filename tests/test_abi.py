@@ -47,8 +47,9 @@ def test_query_feat_sizes(lib):
     assert s.channels == 38 and s.plane_stride == S
     assert s.feat == N * 2 * 38 * S * 4 and s.mem_bits == N * 2 * S and s.last_army == N * 2 * S * 2
     assert s.last_seen == N * 2 * S * 4 and s.hist == N * 2 * 8 * 2 * S * 2 and s.feat_bf16 == N * 2 * 38 * S * 2
-    cfg4, _ = binding.make_config(workloads.config("c5a_2v2")[0])
-    assert lib.gen_query_feat_sizes(C.byref(cfg4), C.byref(s)) == binding_err("GEN_ERR_CONFIG")
+    cfg4, _ = binding.make_config(workloads.config("c5a_2v2")[0])          # R38: P players, 32x32
+    assert lib.gen_query_feat_sizes(C.byref(cfg4), C.byref(s)) == 0
+    assert s.feat == 32768 * 4 * 38 * 1024 * 4 and s.hist == 32768 * 4 * 8 * 2 * 1024 * 2
     assert lib.gen_query_feat_sizes(None, C.byref(s)) == binding_err("GEN_ERR_NULL")
 
 

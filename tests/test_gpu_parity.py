@@ -787,11 +787,6 @@ def test_features_staged_kernel_and_errors(gpu, oracle_mod):
         env.step()
         o.step()
         compare_features(env, o, where=f"it {it}")
-    cfg4, _ = workloads.config("c5a_2v2", n_games=3)
-    env4 = gpu.GeneralsEnv(cfg4)
-    env4.reset()
-    with pytest.raises(gpu.GenError):
-        env4.features()
     cfg0, _ = workloads.config("c2_24x24", n_games=0)          # an empty batch is served without a launch
     env0 = gpu.GeneralsEnv(cfg0)
     env0.reset()
@@ -1091,3 +1086,38 @@ def test_features_hand_worked_example_W12_on_gpu(gpu, oracle_mod):
             else:
                 assert np.array_equal(got, exp), (fr, p, ch, got, exp)
         assert not frames[fr][0, p, :, 6:].any()
+
+
+@pytest.mark.parametrize("name,N,T,over,bf16", [
+    ("c5a_2v2", 9, 120, dict(max_turns=60), False),                                   # 2v2 on 32x32: team visibility
+    ("c5b_ffa8", 5, 100, dict(max_turns=60), False),                                  # 8 players: 2,048 items per game
+    ("c5b_ffa8", 7, 120, dict(n_players=3, height=7, width=9, n_cities=2, spawn_dmin=3, max_turns=40), False),
+    ("c5a_2v2", 6, 80, dict(height=12, width=13, n_cities=3, spawn_dmin=3, max_turns=40), True),
+])
+def test_multi_player_features_match_oracle(gpu, oracle_mod, name, N, T, over, bf16):
+    """R38: the feature tensor with more than two players (k_features_mp) against the oracle, every channel every
+    turn: team visibility, any enemy as "the opponent", enemy sums on the scoreboard channels."""
+    import torch
+    cfg, _ = workloads.config(name, n_games=N, **over)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    for t in range(T + 1):
+        if t:
+            env.step()
+            o.step()
+        if not bf16:
+            compare_features(env, o, where=f"turn {t}")
+            continue
+        got = env.features(bf16=True)
+        want = o.features(bf16=True)
+        torch.cuda.synchronize()
+        gb = got.view(torch.int16).cpu().numpy().view(np.uint16)
+        for ch in range(38):
+            if ch == 21:
+                gf = got[:, :, ch].float().cpu().numpy()
+                wf = torch.from_numpy(want[:, :, ch].view(np.int16)).view(torch.bfloat16).float().numpy()
+                assert np.abs(gf - wf).max() <= 2.0 ** -7
+            else:
+                assert np.array_equal(gb[:, :, ch], want[:, :, ch]), (t, ch)
+    assert int(o.episodes_done.sum()) > 0
