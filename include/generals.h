@@ -182,6 +182,11 @@ int gen_init(const gen_config *cfg, gen_env **out);
 /* Set the built-in sampler's thresholds (a12; R24, R25). */
 int gen_set_policy(gen_env *env, const gen_policy *policy);
 
+/* The spawn-distance curriculum ("we cap the maximum spawn distance ... and gradually raise it over training";
+ * P:L118 lists it among the environment's functions): change the spawn window of the boards generated from now on
+ * (gen_reset and every auto-reset) without a new handle.  Same meaning and checks as the gen_config fields. */
+int gen_set_spawn(gen_env *env, int32_t spawn_dmin, int32_t spawn_dmax, int32_t spawn_exact);
+
 /* Count of steps since gen_reset: the Philox counter word of the action stream. */
 uint32_t gen_global_step(const gen_env *env);
 int gen_set_global_step(gen_env *env, uint32_t step);

@@ -13,7 +13,7 @@ OBS_DIGEST, OBS_EVERY_STEP, OBS_NONE = 0, 1, 2
 GEN_KEEP_EPISODE = 1
 RULE_TICK_PLAIN_ONLY, RULE_CAPTURE_HALF_FLOOR, RULE_ROTATE_PRIORITY = 1, 2, 4
 
-EXPORTS = ["gen_query_sizes", "gen_init", "gen_set_policy", "gen_global_step", "gen_set_global_step",
+EXPORTS = ["gen_query_sizes", "gen_init", "gen_set_policy", "gen_set_spawn", "gen_global_step", "gen_set_global_step",
            "gen_reset", "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host",
            "gen_query_feat_sizes", "gen_features",
            "gen_set_launch", "gen_set_generic", "gen_set_chaining", "gen_last_variant",
@@ -115,6 +115,8 @@ def load_library(path=None):
     lib.gen_query_sizes.argtypes = [C.POINTER(GenConfig), C.c_int32, C.POINTER(GenSizes)]
     lib.gen_init.argtypes = [C.POINTER(GenConfig), C.POINTER(env_p)]
     lib.gen_set_policy.argtypes = [env_p, C.POINTER(GenPolicy)]
+    lib.gen_set_spawn.argtypes = [env_p, C.c_int32, C.c_int32, C.c_int32]
+    lib.gen_set_spawn.restype = C.c_int
     lib.gen_global_step.argtypes = [env_p]
     lib.gen_global_step.restype = C.c_uint32
     lib.gen_set_global_step.argtypes = [env_p, C.c_uint32]
@@ -241,6 +243,11 @@ class GeneralsEnv:
     def set_policy(self, pass_thr=0, half_thr=1 << 31, bias_thr=0):
         p = GenPolicy(int(pass_thr), int(half_thr), int(bias_thr))
         self._check(self.lib.gen_set_policy(self._env, C.byref(p)))
+
+    def set_spawn(self, spawn_dmin, spawn_dmax=0, spawn_exact=0):
+        """The spawn-distance curriculum: the window of the boards generated from now on."""
+        self._check(self.lib.gen_set_spawn(self._env, int(spawn_dmin), int(spawn_dmax), int(spawn_exact)))
+        self.cfg.spawn_dmin, self.cfg.spawn_dmax, self.cfg.spawn_exact = int(spawn_dmin), int(spawn_dmax), int(spawn_exact)
 
     @property
     def global_step(self):

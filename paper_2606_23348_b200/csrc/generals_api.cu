@@ -348,6 +348,16 @@ int gen_set_policy(gen_env *env, const gen_policy *policy) {
     return GEN_OK;
 }
 
+int gen_set_spawn(gen_env *env, int32_t spawn_dmin, int32_t spawn_dmax, int32_t spawn_exact) {
+    if (!env) return GEN_ERR_NULL;
+    gen_config c = env->cfg;
+    c.spawn_dmin = spawn_dmin; c.spawn_dmax = spawn_dmax; c.spawn_exact = spawn_exact ? 1 : 0;
+    if (int e = validate(&c)) return e;
+    env->cfg = c;
+    env->base.dmin = c.spawn_dmin; env->base.dmax = c.spawn_dmax; env->base.spawn_exact = c.spawn_exact;
+    return GEN_OK;
+}
+
 uint32_t gen_global_step(const gen_env *env) { return env ? env->global_step : 0u; }
 
 int gen_set_global_step(gen_env *env, uint32_t step) {

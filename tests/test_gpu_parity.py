@@ -1121,3 +1121,31 @@ def test_multi_player_features_match_oracle(gpu, oracle_mod, name, N, T, over, b
             else:
                 assert np.array_equal(gb[:, :, ch], want[:, :, ch]), (t, ch)
     assert int(o.episodes_done.sum()) > 0
+
+
+@pytest.mark.parametrize("name,over", [("c4_curriculum", dict()), ("official_23x23", dict(play_min=0))])
+def test_spawn_curriculum_raised_over_time(gpu, oracle_mod, name, over):
+    """the cap on the spawn distance starts small and is raised over training.  gen_set_spawn changes the window
+    of the boards generated from then on (auto-resets included) on the same handle; the oracle follows by changing the
+    same three config fields; boards stay bit-exact and the generals' distance tracks the window."""
+    cfg, _ = workloads.config(name, n_games=48, max_turns=12, spawn_dmin=3, spawn_dmax=4, spawn_exact=0, **over)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    W = cfg["width"]
+    for stage, (lo, hi) in enumerate([(3, 4), (3, 8), (6, 14), (17, 0)]):
+        env.set_spawn(lo, hi, 0)
+        o.cfg.spawn_dmin, o.cfg.spawn_dmax, o.cfg.spawn_exact = lo, hi, 0
+        for t in range(13):                                      # every game is truncated and regenerated once
+            env.step()
+            o.step()
+        compare(env, o, where=f"stage {stage}")
+        gc = o.general_cell.astype(int)
+        d = np.abs(gc[:, 0] // W - gc[:, 1] // W) + np.abs(gc[:, 0] % W - gc[:, 1] % W)
+        assert (o.turn <= 4).all()                               # every board on the table was drawn in this stage
+        if name == "c4_curriculum":                              # Manhattan window (R29)
+            assert d.min() >= lo and (hi == 0 or d.max() <= hi)
+        else:                                                    # BFS steps >= Manhattan distance (R36)
+            assert hi == 0 or d.max() <= hi
+    with pytest.raises(gpu.GenError):
+        env.set_spawn(5, 3, 0)
