@@ -428,12 +428,9 @@ int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_action
     // Pinned host buffers are used in place: the step kernel reads the actions through their device alias and one
     // small kernel writes reward + done into the host arrays (no copy-engine transfers).  Pageable buffers take the
     // cudaMemcpyAsync route.  The alias lookups are cached per handle (same buffers every step in an RL loop).
-    if (h_actions != env->hp_key[0] || h_reward != env->hp_key[1] || h_done != env->hp_key[2]) {
-        env->hp_key[0] = h_actions; env->hp_key[1] = h_reward; env->hp_key[2] = h_done;
-        env->hp_dev[0] = mapped_alias(h_actions);
-        env->hp_dev[1] = mapped_alias(h_reward);
-        env->hp_dev[2] = mapped_alias(h_done);
-    }
+    const void *const hp[3] = {h_actions, h_reward, h_done};
+    for (int i = 0; i < 3; ++i)
+        if (hp[i] != env->hp_key[i]) { env->hp_key[i] = hp[i]; env->hp_dev[i] = mapped_alias(hp[i]); }
     const int32_t *d_act = nullptr;
     if (h_actions) {
         if (env->hp_dev[0] && aligned16(env->hp_dev[0])) {
