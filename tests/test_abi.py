@@ -104,6 +104,12 @@ def test_init_argument_errors_without_gpu(lib):
     assert lib.gen_set_launch(env, 3) == -4 and lib.gen_set_launch(env, 4) == 0
     assert lib.gen_launch_count(env) == 0
     assert lib.gen_set_global_step(env, 41) == 0 and lib.gen_global_step(env) == 41
+    assert lib.gen_set_spawn(env, 3, 6, 0) == 0 and lib.gen_set_spawn(env, 6, 3, 0) == -2   # dmax < dmin
+    assert lib.gen_set_spawn(env, 3, 0, 1) == -2 and lib.gen_set_spawn(None, 3, 0, 0) == -1  # exact needs dmax
+    assert lib.gen_set_chaining(env, 0) == 0 and lib.gen_set_chaining(None, 1) == -1
+    fb = binding.GenFeatBuffers()                                     # all NULL
+    assert lib.gen_features(env, C.byref(bufs), C.byref(fb), None) == -1
+    assert lib.gen_features(env, C.byref(bufs), None, None) == -1
     for code in (0, -1, -2, -3, -4, -5, -99):
         assert lib.gen_error_string(code)
     lib.gen_destroy(env)
