@@ -108,6 +108,8 @@ def test_init_argument_errors_without_gpu(lib):
     assert lib.gen_set_spawn(env, 3, 0, 1) == -2 and lib.gen_set_spawn(None, 3, 0, 0) == -1  # exact needs dmax
     assert lib.gen_set_chaining(env, 0) == 0 and lib.gen_set_chaining(None, 1) == -1
     fb = binding.GenFeatBuffers()                                     # all NULL
+    assert lib.gen_features(env, C.byref(bufs), C.byref(fb), None) == -3   # owner is still misaligned
+    bufs.owner = 0x1000
     assert lib.gen_features(env, C.byref(bufs), C.byref(fb), None) == -1
     assert lib.gen_features(env, C.byref(bufs), None, None) == -1
     for code in (0, -1, -2, -3, -4, -5, -99):
