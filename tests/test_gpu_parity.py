@@ -1149,3 +1149,65 @@ def test_spawn_curriculum_raised_over_time(gpu, oracle_mod, name, over):
             assert hi == 0 or d.max() <= hi
     with pytest.raises(gpu.GenError):
         env.set_spawn(5, 3, 0)
+
+
+def test_random_configurations_fuzz(gpu, oracle_mod):
+    """Seeded differential fuzz: 90 random configurations (board 2..32 x 2..32, 2..8 players, team sizes, rule flags,
+    both generators, policies, truncation, packed observation, history ring, kernel choice), each stepped for 40 turns
+    with an explicit-action turn and a fused rollout mixed in, every tensor compared with the oracle every few turns,
+    the feature tensor on the way."""
+    import torch
+    rng = np.random.default_rng(20260623)
+    done_eps = 0
+    for case in range(90):
+        P = int(rng.choice([2, 2, 2, 3, 4, 4, 6, 8]))
+        H, W = int(rng.integers(2, 33)), int(rng.integers(2, 33))
+        if H * W < 4 * P:
+            H, W = max(H, 6), max(W, 6)
+        team_size = int(rng.choice([t for t in (1, 2, 4) if t <= P and (t == 1 or P % t == 0) and P // t >= 2] or [1]))
+        official = P == 2 and rng.random() < 0.35 and H >= 4 and W >= 4
+        cfg = dict(n_games=int(rng.integers(1, 40)), height=H, width=W, n_players=P, team_size=team_size,
+                   n_cities=int(rng.integers(0, max(1, H * W // 12) + 1)), city_army_lo=int(rng.integers(0, 30)),
+                   city_army_hi=int(rng.integers(30, 60)), spawn_dmin=int(rng.integers(0, max(1, (H + W) // 3) + 1)),
+                   spawn_dmax=0, spawn_exact=0, max_turns=int(rng.choice([0, 7, 20])), auto_reset=int(rng.integers(0, 2)),
+                   rule_flags=int(rng.integers(0, 8)), game_id_base=int(rng.integers(0, 1 << 30)),
+                   mountain_thr=workloads.thr(int(rng.integers(0, 45))), seed=int(rng.integers(0, 1 << 62)),
+                   pass_thr=workloads.thr(int(rng.integers(0, 30))), half_thr=workloads.thr(int(rng.integers(0, 101))),
+                   bias_thr=workloads.thr(int(rng.choice([0, 0, 50, 100]))))
+        if official:
+            cfg.update(map_mode=1, n_cities_max=cfg["n_cities"] + int(rng.integers(0, 3)),
+                       play_min=int(rng.choice([0, min(H, W, 3), min(H, W)])), castle_radius=int(rng.integers(0, 7)))
+        packed, history = bool(rng.random() < 0.3), bool(rng.random() < 0.3)
+        staged = bool(rng.random() < 0.3)
+        env = gpu.GeneralsEnv(cfg, packed=packed, history=history, bitboards=not staged, digest=bool(rng.random() < 0.5))
+        o = oracle_mod.Oracle(cfg, digest="obs_digest" in env.tensors)
+        env.reset()
+        o.reset()
+        fields = ([f for f in ALL_FIELDS if f in env.tensors] + (["obs_packed"] if packed else [])
+                  + (["score_hist"] if history else []))
+        where = f"case {case}: {cfg}"
+        dg = "obs_digest" in env.tensors
+        compare(env, o, fields=fields, digest=dg, where=where + " reset")
+        feats = case % 3 == 0                                     # the feature tensor every turn (R35, R38)
+        if feats:
+            compare_features(env, o, where=where + " reset")
+        for t in range(40):
+            if t == 13:
+                a = workloads.random_actions(rng, cfg["n_games"], P, H, W)
+                env.step(torch.from_numpy(a).to(env.device))
+                o.step(a)
+            elif t == 27 and not feats:                               # (one gen_features call per turn: no rollouts then)
+                env.rollout(3, gpu.OBS_DIGEST if dg else gpu.OBS_NONE)
+                o.rollout(3, oracle_mod.OBS_DIGEST if dg else oracle_mod.OBS_NONE)
+                if not dg:                                        # a state-only rollout leaves no observation
+                    env.step()
+                    o.step()
+            else:
+                env.step()
+                o.step()
+            if feats:
+                compare_features(env, o, where=where + f" t={t}")
+            if t % 9 == 8 or t == 39:
+                compare(env, o, fields=fields, digest=dg, where=where + f" t={t}")
+        done_eps += int(o.episodes_done.sum())
+    assert done_eps > 0
