@@ -131,7 +131,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    from paper_2606_23348_b200 import workloads
+    import workloads
     cfg, _ = workloads.config(WORKLOAD)
     sample = 256
     steps = min(args.steps, 400)
@@ -155,7 +155,8 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, replicas, workloads
+    import workloads
+    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -369,7 +370,8 @@ def run_sweep(args):
     """BASELINE config 3 (batch sweep, per-step kernel vs fused K = 32 rollout) plus per-step rows for configs
     4 and 5: one JSON line per row.  Not the driver's contract line; its results are copied into BASELINE.md."""
     import torch
-    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, workloads
+    import workloads
+    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     peak, _ = measured_peak()
@@ -459,7 +461,8 @@ def run_features(args):
     """gen_features alone and gen_step + gen_features per turn on BASELINE config 2 (one JSON
     line; not the driver's contract line)."""
     import torch
-    from paper_2606_23348_b200 import GeneralsEnv, workloads
+    import workloads
+    from paper_2606_23348_b200 import GeneralsEnv
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     peak, peak_src = measured_peak()

@@ -137,8 +137,12 @@ typedef struct gen_buffers {
  * launches in between need no bookkeeping.  Ordering against everything else is unchanged: kernels that are not
  * gen_step launches never start before a gen_step grid has completed, one warp of every chained grid waits for the
  * previous grid before it exits (grids complete in stream order), and the first gen_step after any other call on the
- * handle (reset, rollout, observe, a staged-kernel step) waits for the whole grid.  Allocate it zeroed, once; one
- * handle per buffer set.  Results do not depend on it. */
+ * handle (reset, rollout, observe, a staged-kernel step) waits for the whole grid.  A chained launch is therefore
+ * ordered on entry ONLY against earlier gen_step launches on the same games of the same buffer set: it consumes
+ * nothing else.  A gen_step with explicit `d_actions` (produced by whatever ran before it in the stream: a policy
+ * kernel, another handle's gen_step) is never chained -- it waits for its whole stream predecessor before its first
+ * global access -- and two handles must not share any buffer.  Allocate it zeroed, once; one handle per buffer
+ * set.  Results do not depend on it. */
 
 /* `score_hist` (R34; the paper's two temporal tokens are 512-step windows of
  * the opponent's army and land totals): when non-NULL, gen_reset and every turn of gen_step / gen_rollout store

@@ -238,7 +238,9 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     // 8,192-131,072 games against 118 / 227 / 420-653 M with the grid-wide wait; beyond ~8 waves the waves of one
     // launch mix the phases by themselves and the record's release costs 1-2 %, so those launches keep no records)
     kp.count = ((v->kind & 1) && bufs->step_epoch && !env->no_chain && grid <= 8 * 14 * (int)kSMs) ? 1 : 0;
-    kp.chain = (kp.count && env->chain_buf == bufs->step_epoch) ? 1 : 0;
+    // A chained launch skips the grid-wide wait, so it may consume nothing a foreign kernel produced: with explicit
+    // actions (written by whatever ran before this call) the launch always waits for its stream predecessor.
+    kp.chain = (kp.count && env->chain_buf == bufs->step_epoch && !actions) ? 1 : 0;
     cudaError_t e = v->launch(kp, grid, 32 * kp.WPC, kp.smem_bytes, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) { env->last_cuda_error = (int)e; env->chain_buf = nullptr; return GEN_ERR_CUDA; }
     env->chain_buf = kp.count ? bufs->step_epoch : nullptr;

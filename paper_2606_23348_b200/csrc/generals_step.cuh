@@ -22,21 +22,18 @@
 
 namespace gen {
 
-#ifdef GEN_TRACE  // development only: mean time per phase and warp (globaltimer), read by gen_debug_trace_<id>
-static __device__ unsigned long long g_trace[32];
+#ifdef GEN_TRACE  // development only: per-warp timeline (globaltimer at each mark), read by gen_debug_trace_<id>
+constexpr int TRACE_MARKS = 16, TRACE_WARPS = 8192;
+static __device__ unsigned long long g_trace[TRACE_WARPS * TRACE_MARKS];
 __device__ __forceinline__ unsigned long long gtimer() {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
-#define GEN_TRACE_MARK(k)                                                            \
-    do {                                                                             \
-        __syncwarp();                                                                \
-        if (lane == 0) {                                                             \
-            const unsigned long long t_ = gtimer();                                  \
-            atomicAdd(&g_trace[k], t_ - t_prev);                                     \
-            t_prev = t_;                                                             \
-        }                                                                            \
+#define GEN_TRACE_MARK(k)                                                                         \
+    do {                                                                                          \
+        __syncwarp();                                                                             \
+        if (lane == 0 && trace_w < TRACE_WARPS) g_trace[trace_w * TRACE_MARKS + (k) + 1] = gtimer(); \
     } while (0)
 #else
 #define GEN_TRACE_MARK(k)
@@ -113,8 +110,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
 
     // ================================================================ prologue
 #ifdef GEN_TRACE
-    unsigned long long t_prev = gtimer();
-    if (lane == 0) atomicAdd(&g_trace[31], 1ull);
+    const int trace_w = blockIdx.x * kp.WPC + wic;
+    if (lane == 0 && trace_w < TRACE_WARPS) g_trace[trace_w * TRACE_MARKS] = gtimer();
 #endif
     for (int t = tid; t < 34; t += blockDim.x) {
         const int j = t - 1;

@@ -1,5 +1,7 @@
 // generals_variant.cu -- one kernel instantiation per translation unit: compile with -DGEN_VARIANT_ID=n
 // (n indexes GEN_VARIANTS of generals_variants.h).
+#include <atomic>
+
 #include "generals_variants.h"
 
 #ifndef GEN_VARIANT_ID
@@ -39,11 +41,15 @@ cudaError_t GEN_CAT(launch_variant_, GEN_VARIANT_ID)(const KParams &kp, int grid
                                                      cudaStream_t stream) {
     using S = Sel<GEN_VARIANT_ID>;
     auto kernel = KernelOf<S, S::KIND>::fn;
-    static bool attr_set = false;
-    if (!attr_set) {
+    // the opt-in for more than 48 KB of dynamic shared memory is per device: one flag per device ordinal
+    static std::atomic<unsigned long long> attr_set{0};
+    int dev = 0;
+    if (cudaError_t e = cudaGetDevice(&dev); e != cudaSuccess) return e;
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (dev >= 64 || !(attr_set.load(std::memory_order_acquire) & bit)) {
         cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_set.fetch_or(bit, std::memory_order_release);
     }
     // Programmatic dependent launch: the CTAs of this grid may be placed while the previous grid in the stream
     // drains; both kernels execute griddepcontrol.wait before their first global access, so the overlap is
@@ -64,10 +70,11 @@ cudaError_t GEN_CAT(launch_variant_, GEN_VARIANT_ID)(const KParams &kp, int grid
 }  // namespace gen
 
 #ifdef GEN_TRACE  // development only
-extern "C" int GEN_CAT(gen_debug_trace_, GEN_VARIANT_ID)(unsigned long long *out) {
-    cudaMemcpyFromSymbol(out, gen::g_trace, sizeof(gen::g_trace));
-    unsigned long long zero[32] = {0};
-    cudaMemcpyToSymbol(gen::g_trace, zero, sizeof(zero));
+extern "C" int GEN_CAT(gen_debug_trace_, GEN_VARIANT_ID)(unsigned long long *out, int n) {
+    cudaMemcpyFromSymbol(out, gen::g_trace, sizeof(unsigned long long) * (size_t)n);
+    void *p = nullptr;
+    cudaGetSymbolAddress(&p, gen::g_trace);
+    cudaMemset(p, 0, sizeof(gen::g_trace));
     return 0;
 }
 #endif

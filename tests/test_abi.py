@@ -6,7 +6,8 @@ import re
 
 import pytest
 
-from paper_2606_23348_b200 import binding, build, workloads
+import workloads
+from paper_2606_23348_b200 import binding, build
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 

@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 
 from helpers import DOWN, LEFT, OUT_FIELDS, PASS, RIGHT, STATE_FIELDS, UP, act
-from paper_2606_23348_b200 import workloads
+import workloads
 
 pytestmark = pytest.mark.gpu
 

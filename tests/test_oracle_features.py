@@ -6,7 +6,7 @@ the featuriser's formulas on its own memory."""
 import numpy as np
 import pytest
 
-from paper_2606_23348_b200 import workloads
+import workloads
 
 
 def play(oracle_mod, cfg, T, actions=None):

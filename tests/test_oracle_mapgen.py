@@ -8,7 +8,7 @@ import pytest
 from scipy.sparse import coo_matrix
 from scipy.sparse.csgraph import shortest_path
 
-from paper_2606_23348_b200 import workloads
+import workloads
 
 PL, MT, CT, GN = 0, 1, 2, 3
 OFFICIAL = dict(map_mode=1, height=23, width=23, n_cities=9, n_cities_max=11, spawn_dmin=17, castle_radius=6,

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from helpers import DOWN, LEFT, PASS, RIGHT, UP, act, cell, hand_board
-from paper_2606_23348_b200 import workloads
+import workloads
 
 PL, MT, CT, GN = 0, 1, 2, 3
 M64 = (1 << 64) - 1

@@ -10,7 +10,8 @@ import pytest
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2606_23348_b200 import replicas, workloads
+import workloads
+from paper_2606_23348_b200 import replicas
 
 FIELDS = ["army", "owner", "terrain", "turn", "episode", "alive", "land", "army_total", "obs_digest",
           "episodes_done", "wins"]
