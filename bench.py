@@ -29,9 +29,7 @@ METRIC = "env steps/sec (1v1, all games) on 1 B200; % of HBM or int-issue roofli
 UNIT = "env_steps/s"
 WORKLOAD = "c2_24x24"
 HBM_FALLBACK_GBS = 6650.0          # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
-# dram__bytes_read.sum + dram__bytes_write.sum of one gen_step launch, by games per launch, from the
-# `ncu --set full` capture summarised in profiles/ (see profiles/README.md); None where not captured
-NCU_DRAM_BYTES_PER_LAUNCH = {16384: 99745536}        # profiles/r01_step_full_chained_summary.txt
+# dram bytes of one k_features launch (ncu --set full), by games per launch; see profiles/r01_features_full_summary.txt
 NCU_FEAT_DRAM_BYTES_PER_LAUNCH = {16384: 3601662088}  # profiles/r01_features_full_summary.txt (k_features)
 
 
@@ -152,6 +150,16 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------ our arm
+MIN_REGION_MS, MIN_REPS, MAX_REPS = 50.0, 5, 60
+# warp-instructions per env step of the fused rollout kernel (gen_rollout(32, GEN_OBS_DIGEST), 24x24 1v1):
+# smsp__inst_executed.sum / (N * K) of the ncu capture summarised in the file named beside it
+ROLLOUT_INST_PER_ENV_STEP = 720.7
+ROLLOUT_INST_SOURCE = "profiles/r01_rollout_full_summary.txt"
+ISSUE_PEAK = 148 * 4 * 1.965e9      # warp-instructions/s: 148 SMs x 4 schedulers x 1 per clock x 1.965 GHz
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of k_step at N = 262,144 (ncu --set full), by games per launch
+NCU_DRAM_BYTES_PER_LAUNCH_LARGE = {262144: (2354906856, "profiles/r01_step_full_262k_summary.txt")}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -173,13 +181,8 @@ def run_ours(args):
         cfg["n_games"] = args.games
     N, P, H, W = cfg["n_games"], cfg["n_players"], cfg["height"], cfg["width"]
     bmin = algorithmic_bytes_per_env_step(H, W, P)
-    # Replicas of the batch, stepped round-robin, so that every launch finds its inputs in HBM and not in
-    # the 126 MB L2: between two steps of the same replica the others move (R - 1) * N * bmin bytes.
-    R = args.replicas or max(2, -(-(640 << 20) // (N * bmin)))
     K, Wm = args.steps, args.warmup
-    envs = [GeneralsEnv(dict(cfg, game_id_base=(rank * R + r) * N), device=dev, digest=False, actions_out=(r == 0))
-            for r in range(R)]
-    env = envs[0]
+    peak, peak_src = measured_peak()
 
     def barrier():
         if world > 1:
@@ -189,6 +192,43 @@ def run_ours(args):
     def max_over_ranks(x):
         return replicas.max_over_ranks(x, dist if world > 1 else None, dev)
 
+    def event():
+        return torch.cuda.Event(enable_timing=True)
+
+    def timed(launch_k, k):
+        """Repetitions of exactly k calls of launch_k's body under one CUDA event pair each (barrier + synchronize on
+        both sides, max over ranks), repeated at least MIN_REPS times and until the repetitions add up to
+        MIN_REGION_MS: SURVEY 8(d) 'best and median of 5'.  Returns the list of ms per repetition."""
+        reps = []
+        while len(reps) < MIN_REPS or (sum(reps) < MIN_REGION_MS and len(reps) < MAX_REPS):
+            e0, e1 = event(), event()
+            barrier()
+            e0.record()
+            launch_k(k)
+            e1.record()
+            barrier()
+            reps.append(max_over_ranks(e0.elapsed_time(e1)))
+        return reps
+
+    def summary(reps, k, n_games):
+        med, best = statistics.median(reps), min(reps)
+        return {"value": world * n_games * k / (med * 1e-3), "best": world * n_games * k / (best * 1e-3), "unit": UNIT,
+                "us_per_launch": 1e3 * med / k, "best_us_per_launch": 1e3 * best / k, "repetitions": len(reps),
+                "launches_per_repetition": k}
+
+    def make_replicas(cfg_r, n_games, count, actions_out_first=False):
+        out = []
+        for r in range(count):
+            c = replicas.weak_replica_config(dict(cfg_r, n_games=n_games, game_id_base=0), rank * count + r)
+            out.append(GeneralsEnv(c, device=dev, digest=False, actions_out=(actions_out_first and r == 0)))
+        return out
+
+    # Replicas of the batch, stepped round-robin, so that every launch finds its inputs in HBM and not in
+    # the 126 MB L2: between two steps of the same replica the others move (R - 1) * N * bmin bytes.
+    R = args.replicas or max(2, -(-(640 << 20) // (N * bmin)))
+    envs = make_replicas(cfg, N, R, actions_out_first=True)
+    env = envs[0]
+
     # ---- record the action stream of warm-up + timed steps for the end-to-end leg (device sampler -> host)
     env.reset()
     h_actions = torch.empty((Wm + K, N, P), dtype=torch.int32).pin_memory()
@@ -197,43 +237,43 @@ def run_ours(args):
         h_actions[t].copy_(env.tensors["actions_out"][0], non_blocking=True)
     torch.cuda.synchronize()
 
-    # ---- device-resident leg: K gen_step launches back to back, replica t % R at step t; one CUDA event pair
-    # on the launching (torch current) stream around the timed region
     clocks = ClockSampler(local)
     if rank == 0:
         clocks.start()                                       # sampling spans warm-up and every timed leg below
+
+    # ---- headline: K gen_step launches back to back, replica t % R at step t
     for e in envs:
         e.reset()
-    for t in range(Wm):
+    for t in range(max(Wm, 2 * R)):                          # every replica stepped at least twice before timing
         envs[t % R].step()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    counter = [0]
+
+    def rotate(k):
+        t0 = counter[0]
+        for t in range(t0, t0 + k):
+            envs[t % R].step()
+        counter[0] = t0 + k
+
     launches0 = sum(e.launch_count for e in envs)
-    barrier()
-    e0.record()
-    for t in range(Wm, Wm + K):
-        envs[t % R].step()
-    e1.record()
-    barrier()
-    launches = sum(e.launch_count for e in envs) - launches0
-    total_ms = max_over_ranks(e0.elapsed_time(e1))
+    reps = timed(rotate, K)
+    launches = (sum(e.launch_count for e in envs) - launches0) // len(reps)
+    head = summary(reps, K, N)
+    total_ms = statistics.median(reps)
     specialised, reg_resident = env.last_launch_specialised, env.last_launch_register_resident
 
-    # ---- one environment stepped K times back to back (an RL loop with a device-side policy: launch t+1 depends on
-    # launch t game by game; the 132 MB working set of one batch is partly L2-resident, so this is NOT the roofline leg)
-    for t in range(Wm):
-        env.step()
-    barrier()
-    e0.record()
-    for t in range(K):
-        env.step()
-    e1.record()
-    barrier()
-    same_ms = max_over_ranks(e0.elapsed_time(e1))
+    # ---- one environment stepped K times back to back (launch t+1 depends on launch t game by game; the 132 MB
+    # working set of one batch is partly L2-resident, so this is NOT the roofline leg)
+    def same(k):
+        for _ in range(k):
+            env.step()
 
-    # ---- the same with a 256 MB L2-flush write before every launch and one event pair per launch
-    # (isolated launches: includes the launch latency a back-to-back stream hides)
+    same(Wm)
+    same_env = summary(timed(same, K), K, N)
+
+    # ---- isolated launches: a 256 MB L2-flush write before every launch and one event pair per launch (includes
+    # the launch latency a back-to-back stream hides); what a loop with other kernels between the steps gets
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(min(K, 50))]
+    ev = [(event(), event()) for _ in range(60)]
     barrier()
     for a, b in ev:
         flush.fill_(1)
@@ -241,30 +281,62 @@ def run_ours(args):
         env.step()
         b.record()
     barrier()
-    iso_ms = statistics.median(a.elapsed_time(b) for a, b in ev)
+    iso = sorted(a.elapsed_time(b) for a, b in ev)
+    iso_med, iso_best = max_over_ranks(statistics.median(iso)), max_over_ranks(iso[0])
     del flush
 
+    # ---- interleaved: a foreign kernel of about 10 us (the policy stand-in: a 24 MB fill) between two steps of ONE
+    # environment -- launches cannot chain across it; cost of a step = pair - foreign alone
+    foreign = torch.empty(24 << 20, dtype=torch.uint8, device=dev)
+
+    def only_foreign(k):
+        for _ in range(k):
+            foreign.fill_(3)
+
+    def pair(k):
+        for _ in range(k):
+            foreign.fill_(3)
+            env.step()
+
+    pair(Wm)
+    f_reps, p_reps = timed(only_foreign, K), timed(pair, K)
+    f_us, p_us = 1e3 * statistics.median(f_reps) / K, 1e3 * statistics.median(p_reps) / K
+    del foreign
+
+    # ---- gen_step + gen_features (bfloat16 feature tensor, R37) every turn: the featuriser between two steps
+    fenv = envs[1]
+    fenv.reset()
+    fenv.features(bf16=True)
+
+    def only_features(k):
+        for _ in range(k):
+            fenv.features()
+
+    def step_features(k):
+        for _ in range(k):
+            fenv.step()
+            fenv.features()
+
+    step_features(max(Wm, 8))
+    sf_reps = timed(step_features, max(8, K // 4))
+    of_reps = timed(only_features, max(8, K // 4))     # same turn folded again: same traffic, memory unchanged
+    sf_us, of_us = 1e3 * statistics.median(sf_reps) / max(8, K // 4), 1e3 * statistics.median(of_reps) / max(8, K // 4)
+    del fenv.feat_tensors, fenv.feat
+    del fenv.feat_bufs
+
     # ---- fused rollout leg (K_r = 32 turns per launch, observation digest chained every turn)
-    renv = GeneralsEnv(cfg, device=dev, digest=True, actions_out=False)
+    renv = GeneralsEnv(replicas.weak_replica_config(cfg, rank), device=dev, digest=True, actions_out=False)
     renv.reset()
     renv.rollout(32, OBS_DIGEST)
-    n_roll = max(1, K // 32)
-    barrier()
-    e0.record()
-    for _ in range(n_roll):
-        renv.rollout(32, OBS_DIGEST)
-    e1.record()
-    barrier()
-    roll_ms = max_over_ranks(e0.elapsed_time(e1))
-    # The timed regions above last a few milliseconds, nvidia-smi samples every 100 ms: keep the same launches going
-    # (untimed) until the sampler has seen the GPU under this load at least three times.
-    if rank == 0:
-        t_end = time.perf_counter() + 1.5
-        while len(clocks.lines) < 3 and time.perf_counter() < t_end:
-            for t in range(64):
-                envs[t % R].step()
-            torch.cuda.synchronize()
-    clock_info = clocks.stop() if rank == 0 else None
+    n_roll = max(2, K // 32)
+
+    def roll(k):
+        for _ in range(k):
+            renv.rollout(32, OBS_DIGEST)
+
+    roll_reps = timed(roll, n_roll)
+    roll_value = world * N * 32 * n_roll / (statistics.median(roll_reps) * 1e-3)
+    del renv
 
     # ---- end-to-end leg: host actions in (pinned), gen_step_host, host reward + done out, every step
     env.reset()
@@ -272,27 +344,60 @@ def run_ours(args):
     h_done = torch.zeros((N,), dtype=torch.uint8).pin_memory()
     for t in range(Wm):
         env.step_host(h_actions[t], h_reward, h_done)
-    barrier()
-    t0 = time.perf_counter()
-    for t in range(Wm, Wm + K):
-        env.step_host(h_actions[t], h_reward, h_done)
-    torch.cuda.synchronize()
-    e2e_s = max_over_ranks(time.perf_counter() - t0)
+    e2e_reps = []
+    for _ in range(MIN_REPS):
+        env.reset()
+        for t in range(Wm):
+            env.step_host(h_actions[t], h_reward, h_done)
+        barrier()
+        t0 = time.perf_counter()
+        for t in range(Wm, Wm + K):
+            env.step_host(h_actions[t], h_reward, h_done)
+        torch.cuda.synchronize()
+        e2e_reps.append(max_over_ranks(time.perf_counter() - t0))
+    e2e_s = statistics.median(e2e_reps)
     checksum = int(h_done.sum())
+
+    # ---- large batch ("quote the fraction from N >= 262,144"): the same kernel where one launch is
+    # 22 waves and the batch (2.1 GB of state + observations per replica) is far larger than L2
+    large = None
+    if not args.no_large and not args.games:
+        del envs, env, fenv
+        torch.cuda.empty_cache()
+        NL = 262144
+        lenvs = make_replicas(cfg, NL, 2)
+        for e in lenvs:
+            e.reset()
+        lc = [0]
+
+        def lrot(k):
+            for t in range(lc[0], lc[0] + k):
+                lenvs[t % 2].step()
+            lc[0] += k
+
+        lrot(6)
+        KL = max(8, min(K, 20))
+        l_reps = timed(lrot, KL)
+        large = summary(l_reps, KL, NL)
+        del lenvs
+        torch.cuda.empty_cache()
+
+    # The timed regions above last tens of milliseconds each, nvidia-smi samples every 100 ms: the sampler has seen the
+    # GPU under this load several times by now.
+    clock_info = clocks.stop() if rank == 0 else None
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    peak, peak_src = measured_peak()
-    value = world * N * K / (total_ms * 1e-3)
     launch_ms = total_ms / K
     achieved = N * bmin / (launch_ms * 1e-3) / 1e9
-    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(N)
     kname = ("gen::k_step" if reg_resident else "gen::k_generals") + (f"<{P}, {H}, {W}>" if specialised else " (generic)")
+    iso_ach = N * bmin / (iso_med * 1e-3) / 1e9
+    step_us_inter = p_us - f_us
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int16", "data": "synthetic",
         "config": {"workload": f"{WORKLOAD}: 1v1 24x24, {N} games/GPU, auto-reset, max_turns 1000, device Philox "
@@ -302,29 +407,71 @@ def run_ours(args):
                          f"{N * bmin / 1e6:.0f} MB of algorithmic traffic between two steps of one replica; L2 is "
                          "126 MB); K launches back to back, one CUDA event pair around them",
                    "replicas_in_rotation": R,
+                   "timing": f"value = median of {len(reps)} repetitions of exactly {K} launches (one event pair each, "
+                             f"barrier + synchronize on both sides; repeated until >= {MIN_REGION_MS:.0f} ms in total); "
+                             "best repetition in value_best",
                    "parallelism": f"replicas x{world}, disjoint game-id ranges, no collective"},
+        "value_best": head["best"], "repetitions": len(reps),
         "clocks": clock_info,
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "kernel": kname + " (gen_step)", "peak_source": peak_src,
+                     "traffic": None,
+                     "traffic_note": "not captured per run; one serialised cold launch under ncu leaves part of its stores "
+                                     "in L2 and undercounts -- the usable traffic ratio is roofline_large's",
+                     "kernel": kname + " (gen_step)", "peak_source": peak_src,
                      "algorithmic_bytes_per_env_step": bmin, "units_per_launch": N,
-                     "avg_launch_us": 1e3 * launch_ms,
-                     "isolated_launch_us": 1e3 * iso_ms,
-                     "isolated_note": "median of single launches, each after a 256 MB L2-flush write, own event pair"},
+                     "avg_launch_us": 1e3 * launch_ms, "best_launch_us": head["best_us_per_launch"],
+                     "isolated_launch_us": 1e3 * iso_med},
+        "roofline_isolated": {"bound": "hbm", "achieved": iso_ach, "peak": peak, "unit": "GB/s", "frac": iso_ach / peak,
+                              "launch_us": 1e3 * iso_med, "best_launch_us": 1e3 * iso_best, "launches": len(iso),
+                              "note": "median of single launches, each after a 256 MB L2-flush write and with its own "
+                                      "event pair (launch latency included): one gen_step by itself, nothing to overlap with"},
+        "interleaved": {"value": world * N / (step_us_inter * 1e-6), "unit": UNIT, "pair_us": p_us, "foreign_us": f_us,
+                        "step_us": step_us_inter, "frac": N * bmin / (step_us_inter * 1e-6) / 1e9 / peak,
+                        "repetitions": len(p_reps),
+                        "note": "one environment; a foreign kernel (24 MB fill, the policy stand-in) between two steps, "
+                                "so launches cannot chain; step_us = pair - foreign alone"},
+        "step_plus_features": {"turn_us": sf_us, "features_us": of_us, "step_us": sf_us - of_us,
+                               "value": world * N / (sf_us * 1e-6), "unit": UNIT, "dtype": "bf16 feature tensor (R37)",
+                               "note": "gen_step + gen_features every turn (38 channels x 2 players materialised)"},
         "e2e": {"value": world * N * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": N * P * 4,
-                "d2h_bytes_per_step": N * P + N, "api": "gen_step_host (pinned host actions read in place, reward + done written to pinned host arrays, stream synchronised every step)",
+                "d2h_bytes_per_step": N * P + N,
+                "best": world * N * K / min(e2e_reps), "repetitions": len(e2e_reps),
+                "api": "gen_step_host: pinned host actions read in place, reward + done written to pinned host arrays, "
+                       "stream synchronised every step; the observation planes stay on the device BY DESIGN (a GPU-resident "
+                       "learner reads them there: 94 MB per step would not fit the bus) and are not part of the returned result",
                 "done_checksum": checksum},
-        "same_env": {"value": world * N * K / (same_ms * 1e-3), "unit": UNIT, "us_per_launch": 1e3 * same_ms / K,
-                     "note": "one environment stepped K times back to back (true game-by-game dependency between "
-                             "launches; working set partly L2-resident: not a roofline figure)"},
-        "rollout": {"value": world * N * 32 * n_roll / (roll_ms * 1e-3), "unit": UNIT, "K": 32, "launches": n_roll,
-                    "obs": "digest every turn, planes of the last turn", "bound": "alu"},
+        "same_env": dict(same_env, note="one environment stepped K times back to back (true game-by-game dependency "
+                                        "between launches; working set partly L2-resident: not a roofline figure)"),
+        "rollout": {"value": roll_value, "unit": UNIT, "K": 32, "launches": n_roll, "repetitions": len(roll_reps),
+                    "obs": "digest every turn, planes of the last turn",
+                    "roofline": {"bound": "alu", "inst_per_env_step": ROLLOUT_INST_PER_ENV_STEP,
+                                 "inst_source": ROLLOUT_INST_SOURCE,
+                                 "achieved": roll_value / world * ROLLOUT_INST_PER_ENV_STEP, "peak": ISSUE_PEAK,
+                                 "unit": "warp-inst/s", "frac": roll_value / world * ROLLOUT_INST_PER_ENV_STEP / ISSUE_PEAK}},
     }
+    if large:
+        NL = 262144
+        l_ach = NL * bmin / (large["us_per_launch"] * 1e-6) / 1e9
+        tr = NCU_DRAM_BYTES_PER_LAUNCH_LARGE.get(NL)
+        line["roofline_large"] = {"bound": "hbm", "achieved": l_ach, "peak": peak, "unit": "GB/s", "frac": l_ach / peak,
+                                  "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
+                                  "traffic_over_algorithmic": tr[0] / (NL * bmin) if tr else None,
+                                  "value": large["value"], "best": large["best"], "units_per_launch": NL,
+                                  "avg_launch_us": large["us_per_launch"], "repetitions": large["repetitions"],
+                                  "launches_per_repetition": large["launches_per_repetition"],
+                                  "kernel": kname + " (gen_step), 2 replicas of 262,144 games in rotation"}
     if not args.no_cpu_baseline:
-        sample, steps = 256, 400
+        # config 2's first 1,024 games; 500 turns instead of 2,000 so that the leg stays near 20 s of CPU
+        sample, steps = 1024, 500
         v, _ = oracle_throughput(dict(cfg, game_id_base=0), sample, steps, 5)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                "sample": f"first {sample} global game ids x {steps} turns of {WORKLOAD}, single thread"}
+                                "sample": f"first {sample} global game ids x {steps} turns of {WORKLOAD}, single thread "
+                                          "(SURVEY 8(d) names 2,000 turns: bounded to about 20 s of CPU work)"}
+        c1, t1 = workloads.config("c1_8x8")
+        v1, _ = oracle_throughput(c1, c1["n_games"], t1, 0)
+        line["cpu_baseline_config1"] = {"value": v1, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                        "sample": "config 1 in full: 64 games x 300 turns, 8x8, single thread"}
         try:
             va, cores = oracle_throughput_all_cores(dict(cfg), 64, 300)
             line["cpu_baseline_all_cores"] = {"value": va, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -536,6 +683,7 @@ def main():
     ap.add_argument("--games", type=int, default=0, help="override games per GPU (default: config 2's 16,384)")
     ap.add_argument("--replicas", type=int, default=0, help="replicas in the round-robin (default: enough for 640 MB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-large", action="store_true", help="skip the N = 262,144 leg (roofline_large)")
     ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
     ap.add_argument("--rows", default="", help="with --sweep: only the rows whose workload name contains this")
     ap.add_argument("--workload", default="", help="with --features: workload name (default c2_24x24)")

@@ -23,6 +23,8 @@
  *                     closed form, tiny boards by hand (tests/test_oracle_mapgen.py)
  *   feature tensor  : (R35) hand-worked example W12 (tests/golden/features_worked_example.txt), channel identities,
  *                     closed form, an independent memory log (test_oracle_features.py); bfloat16 (R37): torch's conversion
+ *   history windows : (R39) closed form C1 through a ring wrap with 1, 2 (free-for-all) and 2 (2v2) enemies,
+ *                     and an independent per-turn log on sampled play with auto-reset (test_oracle_properties.py)
  *   sampler         : brute force "valid set == set of board-changing actions"
  * Parity unpinned BY THE PAPER (fixed by decree in DESIGN.md, the paper prints no
  * value that decides them): R6 move order, R11 rounding of the transferred half,
@@ -791,5 +793,37 @@ int32_t orc_features_bf16(const orc_config *cfg, const orc_buffers *b, const orc
     if (rc != 0) return rc;
     const size_t n = (size_t)cfg->n_games * (size_t)cfg->n_players * FEAT_C * (size_t)plane_stride(cfg);
     for (size_t i = 0; i < n; ++i) feat16[i] = bf16_rne(scratch[i]);
+    return 0;
+}
+
+/* ===================================================================== NEXT-2: the two temporal tokens' windows
+ * PAPER.md P:L141 "Two additional non-spatial tokens carry global temporal statistics ...: a 512-step sliding window
+ * of the opponent's total army count and a matching window of their total land count" (also P:L312).  Reading R39
+ * (DESIGN.md): for game g and agent p, win[g][p][0][i] is the enemies' summed army total and win[g][p][1][i] their
+ * summed land count at turn t - 511 + i of the CURRENT episode (t = turn[g]; i = 511 is the turn the scoreboard
+ * stands at now, i = 0 the oldest step of the window), and 0 for the steps before the episode's first turn.
+ * "The opponent" is every player off p's team (R38).  The values are read from the ring of R34 (slot turn mod 512). */
+int32_t orc_history_windows(const orc_config *cfg, const orc_buffers *b, int32_t *win)
+{
+    const int P = cfg->n_players;
+    if (!b->score_hist) return -1;
+    for (int g = 0; g < cfg->n_games; ++g) {
+        const int t = b->turn[g];
+        for (int p = 0; p < P; ++p) {
+            int32_t *army_w = win + (((size_t)g * P + p) * 2 + 0) * HIST_LEN;
+            int32_t *land_w = win + (((size_t)g * P + p) * 2 + 1) * HIST_LEN;
+            for (int i = 0; i < HIST_LEN; ++i) {
+                const int tt = t - (HIST_LEN - 1) + i;            /* the turn this entry of the window shows */
+                int32_t army = 0, land = 0;
+                if (tt >= 0) {
+                    const int32_t *slot = b->score_hist + ((size_t)g * HIST_LEN + (size_t)(tt % HIST_LEN)) * 2 * P;
+                    for (int q = 0; q < P; ++q)
+                        if (team_of(cfg, q) != team_of(cfg, p)) { land += slot[2 * q]; army += slot[2 * q + 1]; }
+                }
+                army_w[i] = army;
+                land_w[i] = land;
+            }
+        }
+    }
     return 0;
 }

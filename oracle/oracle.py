@@ -79,6 +79,7 @@ def lib():
                                      C.c_int32]
         _lib.orc_observe.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers)]
         _lib.orc_features.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers), C.POINTER(OrcFeatState), C.c_void_p]
+        _lib.orc_history_windows.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers), C.c_void_p]
         _lib.orc_features_bf16.argtypes = [C.POINTER(OrcConfig), C.POINTER(OrcBuffers), C.POINTER(OrcFeatState),
                                            C.c_void_p, C.c_void_p]
     return _lib
@@ -195,6 +196,14 @@ class Oracle:
         if rc != 0:
             raise ValueError("orc_features failed")
         return self.feat16 if bf16 else self.feat
+
+    def history_windows(self):
+        """NEXT-2 (R39): int32 [N][P][2][512] -- the enemies' army (0) and land (1) totals over the last 512
+        turns of the current episode, oldest first, 0 before the episode's first turn."""
+        win = np.zeros((self.N, self.P, 2, 512), dtype=np.int32)
+        if lib().orc_history_windows(C.byref(self.cfg), C.byref(self.bufs), win.ctypes.data) != 0:
+            raise ValueError("orc_history_windows failed")
+        return win
 
     def set_policy(self, pass_thr=None, half_thr=None, bias_thr=None):
         for k, v in (("pass_thr", pass_thr), ("half_thr", half_thr), ("bias_thr", bias_thr)):

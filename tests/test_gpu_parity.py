@@ -1211,3 +1211,62 @@ def test_random_configurations_fuzz(gpu, oracle_mod):
                 compare(env, o, fields=fields, digest=dg, where=where + f" t={t}")
         done_eps += int(o.episodes_done.sum())
     assert done_eps > 0
+
+
+# ------------------------------------------------------------------------------- sanitizer target
+def test_sanitizer_coverage_run(gpu, oracle_mod):
+    """One short run over every kernel of the library, small enough for compute-sanitizer:
+        compute-sanitizer --tool {memcheck,racecheck,synccheck,initcheck} \\
+            python -m pytest tests/test_gpu_parity.py -q -k sanitizer_coverage_run
+    (summaries under profiles/).  Config 1 (8x8) and a 24x24 batch with a ragged last CTA: gen_reset, chained
+    gen_step launches (k_step: tickets, TMA row loads, 32-bit reductions on int16 pairs), gen_step with explicit
+    actions, gen_rollout(8) with the digest, gen_observe, gen_sample, reset and auto-reset with the official
+    generator, gen_features in both instantiations (fp32 1v1, bfloat16; the multi-player kernel).  It is a parity
+    test in its own right: everything is compared with the oracle."""
+    import torch
+    for name, N, over in (("c1_8x8", 21, dict(auto_reset=1, max_turns=12)),
+                          ("c2_24x24", 21, dict(max_turns=14)),
+                          ("official_23x23", 13, dict(max_turns=9))):
+        cfg, _ = workloads.config(name, n_games=N, **over)
+        env = gpu.GeneralsEnv(cfg, digest=False)
+        o = oracle_mod.Oracle(cfg)
+        env.reset()
+        o.reset()
+        compare_features(env, o, where=f"{name} reset")
+        for t in range(3):                                     # three chained launches, nothing in between
+            env.step()
+            o.step()
+        compare(env, o, digest=False, where=f"{name} chained steps")
+        for t in range(16):
+            env.step()
+            o.step()
+            compare_features(env, o, where=f"{name} step {t}")
+        a = o.sample()
+        assert np.array_equal(env.sample().cpu().numpy(), a)
+        env.step(torch.from_numpy(a).to(env.device))
+        o.step(a)
+        env.observe()
+        compare(env, o, digest=False, where=f"{name} explicit actions + observe")
+        assert env.last_launch_register_resident is False      # gen_observe is the staged kernel
+        env.close()
+    cfg, _ = workloads.config("c2_24x24", n_games=19, max_turns=11)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    env.rollout(8, gpu.OBS_DIGEST)
+    o.rollout(8, oracle_mod.OBS_DIGEST)
+    env.step()
+    o.step()
+    compare(env, o, where="rollout(8) + staged step with digest")
+    bf = env.features(bf16=True)
+    torch.cuda.synchronize()
+    assert bf.dtype == torch.bfloat16 and bool(torch.isfinite(bf.float()).all())
+    cfg, _ = workloads.config("c5a_2v2", n_games=6, height=12, width=12, n_cities=3, spawn_dmin=4, max_turns=10)
+    env, o = make_pair(gpu, oracle_mod, cfg)
+    env.reset()
+    o.reset()
+    for t in range(12):
+        env.step()
+        o.step()
+        compare_features(env, o, where=f"2v2 step {t}")
+    compare(env, o, where="2v2")

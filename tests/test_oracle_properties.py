@@ -666,3 +666,63 @@ def test_R34_history_is_the_scoreboard_of_every_turn(oracle_mod):
                     assert np.array_equal(o.score_hist[g, t % 512, 0::2], land)
                     assert np.array_equal(o.score_hist[g, t % 512, 1::2], army)
     assert int(o.episodes_done.sum()) > 5 and int(o.wins.sum()) > 0
+
+
+def test_R39_history_windows_closed_form_wrap_and_enemy_sums(oracle_mod):
+    """R39 ("a 512-step sliding window of the opponent's total army count and a matching window of their
+    total land count"): under all-pass play every player's army total is 1 + t // 2 + t // 50 at turn t (closed form
+    C1) and the land stays 1, so entry i of agent p's windows must read (#enemies) x that closed form at turn
+    t - 511 + i, and 0 before turn 0 -- before the ring wraps (t = 300), exactly when it fills (t = 511) and after it
+    has wrapped (t = 700); with two players, with three (free-for-all: two enemies) and with 2v2 teams."""
+    for P, team, enemies in ((2, 1, 1), (3, 1, 2), (4, 2, 2)):
+        cfg, _ = workloads.config("c1_8x8", n_games=2, n_players=P, team_size=team, spawn_dmin=3)
+        o = oracle_mod.Oracle(cfg)
+        o.reset()
+        passes = np.zeros((2, P), dtype=np.int32)
+        for t in range(1, 701):
+            o.step(passes)
+            if t in (300, 511, 700):
+                win = o.history_windows()
+                assert win.shape == (2, P, 2, 512)
+                for i in range(512):
+                    tt = t - 511 + i
+                    army = enemies * (1 + tt // 2 + tt // 50) if tt >= 0 else 0
+                    land = enemies if tt >= 0 else 0
+                    assert (win[:, :, 0, i] == army).all() and (win[:, :, 1, i] == land).all(), (P, t, i)
+
+
+def test_R39_history_windows_follow_an_independent_log(oracle_mod):
+    """On sampled play with captures and auto-reset the windows must equal a Python log of the scoreboard kept by the
+    test turn by turn (cleared when the episode changes): oldest first, the newest entry is the current scoreboard,
+    zeros before the episode's first turn -- per agent, summed over the players off its team (2v2: R38)."""
+    cfg, _ = workloads.config("c5a_2v2", n_games=6, height=10, width=10, spawn_dmin=3, n_cities=3, max_turns=60,
+                              pass_thr=0)
+    o = oracle_mod.Oracle(cfg)
+    o.reset()
+    P = 4
+    log = [dict() for _ in range(6)]
+    ep = o.episode.copy()
+
+    def note():
+        for g in range(6):
+            if o.episode[g] != ep[g]:
+                log[g].clear()
+                ep[g] = o.episode[g]
+            log[g][int(o.turn[g])] = (o.land[g].copy(), o.army_total[g].copy())
+
+    note()
+    for step in range(150):
+        o.step()
+        note()
+        if step % 7 == 0 or step > 140:
+            win = o.history_windows()
+            for g in range(6):
+                t = int(o.turn[g])
+                for p in range(P):
+                    enemy = [q for q in range(P) if q // 2 != p // 2]
+                    for i in range(512):
+                        tt = t - 511 + i
+                        want_a = sum(int(log[g][tt][1][q]) for q in enemy) if tt >= 0 else 0
+                        want_l = sum(int(log[g][tt][0][q]) for q in enemy) if tt >= 0 else 0
+                        assert win[g, p, 0, i] == want_a and win[g, p, 1, i] == want_l, (step, g, p, i)
+    assert int(o.episodes_done.sum()) > 3
