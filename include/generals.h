@@ -227,9 +227,28 @@ int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, vo
  * actions through their device alias and one small kernel writes reward + done into the host arrays -- no
  * copy-engine transfers.  Pageable buffers go through cudaMemcpyAsync (actions via bufs->actions_out, which must
  * then be non-NULL; it must be non-NULL whenever h_actions is given).  Whether a buffer is pinned is looked up when
- * the pointer passed differs from the previous call's; do not unregister a buffer between calls and keep passing it. */
+ * a pointer is passed for the first time (the handle remembers the last eight); after unregistering or freeing a
+ * buffer call gen_forget_host_buffers. */
 int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
                   uint8_t *h_done, void *cuda_stream);
+
+/* The same without the synchronisation: enqueues the step (and the transfer of reward + done) and returns.  The
+ * results of the call issued `lag` calls before the latest one are in their host arrays once gen_host_wait(env, lag)
+ * has returned (lag 0 = the latest call; at most 4 calls may be in flight, lag <= 3).  An RL loop waits one step
+ * late -- issue step t with one pair of host slots, then wait for step t - 1 and read the other pair -- so that the
+ * GPU always has the next step queued and no launch latency or host wake-up sits between two steps.  Until its wait
+ * has returned a call OWNS its three host arrays: pinned actions are read in place when the kernel runs, so they
+ * must not be rewritten before.  Use pinned memory: with pageable buffers the copies are staged by the runtime and
+ * the call is asynchronous only in name.  The observation planes stay on the device in both variants (a GPU-resident
+ * learner reads them there; 94 MB per step at config 2 is no bus traffic to plan for). */
+int gen_step_host_async(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
+                        uint8_t *h_done, void *cuda_stream);
+int gen_host_wait(gen_env *env, int32_t lag);
+
+/* Forget what gen_step_host[_async] has learnt about the caller's host pointers (pinned or not, and their device
+ * aliases).  Call it after freeing or unregistering a host buffer that was passed before, so that its address, if
+ * the allocator hands it out again, is looked up afresh. */
+int gen_forget_host_buffers(gen_env *env);
 
 /* ---- the 38-channel feature tensor (Appendix A, Table IV; R35) ----
  * What the paper's policy consumes, built from the state the step leaves behind plus a per-episode memory.
@@ -262,6 +281,7 @@ typedef struct gen_feat_sizes {
     int32_t channels;     /* 38 */
     int32_t plane_stride; /* S */
     size_t feat, mem_bits, last_army, last_seen, hist, feat_bf16; /* bytes */
+    size_t hist_windows;  /* bytes of gen_history_windows' output: int32 [N][P][2][512] */
 } gen_feat_sizes;
 
 /* Byte sizes of the gen_feat_buffers members for `cfg`.  Host-only. */
@@ -273,6 +293,18 @@ int gen_query_feat_sizes(const gen_config *cfg, gen_feat_sizes *out);
  * turn / land / army_total (and play_size if given) only; no game state changes.  One kernel launch on cuda_stream.
  * GEN_ERR_NULL / GEN_ERR_ALIGN on a missing / misaligned pointer. */
 int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *feat, void *cuda_stream);
+
+/* The two temporal tokens' windows ("a 512-step sliding window of the opponent's total army count and a
+ * matching window of their total land count, each projected by an MLP into a single token"; reading R39 of
+ * DESIGN.md).  Reads bufs->score_hist (the ring of R34, required) and bufs->turn; writes d_windows, caller-owned
+ * device memory, int32 [N][P][2][512], 16-byte aligned (gen_feat_sizes.hist_windows bytes): for game g and agent p,
+ * [g][p][0][i] is the summed army total and [g][p][1][i] the summed land count of every player off p's team (R38;
+ * with two players: the opponent) at turn t - 511 + i of the CURRENT episode, t = turn[g] -- oldest first, entry 511
+ * is the scoreboard as it stands now -- and 0 for the entries before the episode's first turn (also the leftovers of an
+ * earlier episode in the ring are masked).  The MLP that turns a window into a token is the policy's.  One kernel
+ * launch on cuda_stream, no state changes.  GEN_ERR_NULL when the ring was not given, GEN_ERR_ALIGN on a misaligned
+ * pointer. */
+int gen_history_windows(gen_env *env, const gen_buffers *bufs, int32_t *d_windows, void *cuda_stream);
 
 /* Launch geometry override for tuning: games per CTA in {4, 8, 16, 32} (8 threads per game); 0 restores
  * the default (8).  Results do not depend on it. */

@@ -15,7 +15,8 @@ RULE_TICK_PLAIN_ONLY, RULE_CAPTURE_HALF_FLOOR, RULE_ROTATE_PRIORITY = 1, 2, 4
 
 EXPORTS = ["gen_query_sizes", "gen_init", "gen_set_policy", "gen_set_spawn", "gen_global_step", "gen_set_global_step",
            "gen_reset", "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host",
-           "gen_query_feat_sizes", "gen_features",
+           "gen_step_host_async", "gen_host_wait", "gen_forget_host_buffers",
+           "gen_query_feat_sizes", "gen_features", "gen_history_windows",
            "gen_set_launch", "gen_set_generic", "gen_set_chaining", "gen_last_variant",
            "gen_launch_count", "gen_last_cuda_error", "gen_destroy",
            "gen_error_string", "gen_version"]
@@ -95,7 +96,8 @@ class GenFeatBuffers(C.Structure):
 
 
 class GenFeatSizes(C.Structure):
-    _fields_ = ([("channels", C.c_int32), ("plane_stride", C.c_int32)] + [(n, C.c_size_t) for n, _, _ in FEAT_BUFFERS])
+    _fields_ = ([("channels", C.c_int32), ("plane_stride", C.c_int32)] + [(n, C.c_size_t) for n, _, _ in FEAT_BUFFERS]
+                + [("hist_windows", C.c_size_t)])
 
 
 _lib = None
@@ -126,8 +128,15 @@ def load_library(path=None):
     lib.gen_observe.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p]
     lib.gen_sample.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
     lib.gen_step_host.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.gen_step_host_async.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.gen_host_wait.argtypes = [env_p, C.c_int32]
+    lib.gen_forget_host_buffers.argtypes = [env_p]
+    for name in ("gen_step_host_async", "gen_host_wait", "gen_forget_host_buffers"):
+        getattr(lib, name).restype = C.c_int
     lib.gen_query_feat_sizes.argtypes = [C.POINTER(GenConfig), C.POINTER(GenFeatSizes)]
     lib.gen_features.argtypes = [env_p, C.POINTER(GenBuffers), C.POINTER(GenFeatBuffers), C.c_void_p]
+    lib.gen_history_windows.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
+    lib.gen_history_windows.restype = C.c_int
     lib.gen_set_launch.argtypes = [env_p, C.c_int32]
     lib.gen_set_generic.argtypes = [env_p, C.c_int32, C.c_int32]
     lib.gen_set_chaining.argtypes = [env_p, C.c_int32]
@@ -337,6 +346,17 @@ class GeneralsEnv:
         self._check(self.lib.gen_features(self._env, C.byref(self.bufs), C.byref(self.feat_bufs), self._stream(stream)))
         return self.feat
 
+    def history_windows(self, out=None, stream=None):
+        """NEXT-2 (R39): int32 CUDA tensor [N][P][2][512] -- the enemies' army (0) and land (1) totals over the
+        last 512 turns of the current episode, oldest first, 0 before its first turn.  Needs history=True."""
+        if out is None:
+            if not hasattr(self, "_windows"):
+                self._windows = self.torch.zeros((self.N, self.P, 2, 512), dtype=self.torch.int32, device=self.device)
+            out = self._windows
+        self._check(self.lib.gen_history_windows(self._env, C.byref(self.bufs), C.c_void_p(out.data_ptr() if out.numel() else 16),
+                                                 self._stream(stream)))
+        return out
+
     def step_host(self, h_actions=None, h_reward=None, h_done=None, stream=None):
         """End to end through host buffers (pinned CPU tensors); synchronises the stream."""
         ptr = lambda t: None if t is None else C.c_void_p(t.data_ptr())   # noqa: E731
@@ -344,6 +364,22 @@ class GeneralsEnv:
             assert t is None or (not t.is_cuda and t.is_contiguous())
         self._check(self.lib.gen_step_host(self._env, C.byref(self.bufs), ptr(h_actions), ptr(h_reward),
                                            ptr(h_done), self._stream(stream)))
+
+    def step_host_async(self, h_actions=None, h_reward=None, h_done=None, stream=None):
+        """gen_step_host without the synchronisation; host_wait(lag) tells when a call's results have landed."""
+        ptr = lambda t: None if t is None else C.c_void_p(t.data_ptr())   # noqa: E731
+        code = self.lib.gen_step_host_async(self._env, self._bufs_ref, ptr(h_actions), ptr(h_reward), ptr(h_done),
+                                            self._stream(stream))
+        if code != 0:
+            self._check(code)
+
+    def host_wait(self, lag=0):
+        code = self.lib.gen_host_wait(self._env, int(lag))
+        if code != 0:
+            self._check(code)
+
+    def forget_host_buffers(self):
+        self._check(self.lib.gen_forget_host_buffers(self._env))
 
     # ------------------------------------------------------------------ helpers
     def field(self, name, slot=0):

@@ -21,8 +21,15 @@ struct gen_env {
     int32_t last_variant;    // index into GEN_VARIANTS of the last launch (-1: none yet)
     const uint32_t *chain_buf;  // non-NULL: the last launch of this handle was a k_step that kept records there
     int32_t no_chain;        // tests: never chain
-    const void *hp_key[3];   // gen_step_host: the host pointers last looked up (actions, reward, done) ...
-    void *hp_dev[3];         // ... and their device aliases (nullptr: pageable memory)
+    // gen_step_host / gen_step_host_async: host pointers looked up so far and their device aliases (nullptr:
+    // pageable memory); a small table, so that double-buffered host slots do not look up again every call
+    const void *hp_key[8];
+    void *hp_dev[8];
+    int32_t hp_used, hp_next;
+    // gen_step_host_async: one event per call in flight (ring), created on first use
+    cudaEvent_t ev[4];
+    int32_t ev_ready;        // events created
+    uint64_t async_calls;    // gen_step_host_async calls so far
 };
 
 namespace {
@@ -420,46 +427,104 @@ int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, vo
     return launch(env, bufs, gen::F_SAMPLE_ONLY | gen::F_SAMPLER, 0, nullptr, d_actions_out, cuda_stream);
 }
 
-int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
-                  uint8_t *h_done, void *cuda_stream) {
-    if (!env || !bufs) return GEN_ERR_NULL;
+static void *host_alias(gen_env *env, const void *h) {
+    if (!h) return nullptr;
+    for (int i = 0; i < env->hp_used; ++i)
+        if (env->hp_key[i] == h) return env->hp_dev[i];
+    const int slot = env->hp_used < 8 ? env->hp_used++ : (env->hp_next++ & 7);
+    env->hp_key[slot] = h;
+    env->hp_dev[slot] = mapped_alias(h);
+    return env->hp_dev[slot];
+}
+
+// the body of gen_step_host / gen_step_host_async: everything but the wait
+static int step_host_enqueue(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
+                             uint8_t *h_done, cudaStream_t s) {
     if (h_actions && !bufs->actions_out) return GEN_ERR_NULL;
-    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    if (int e = check_buffers(bufs, true)) return e;         // before anything is enqueued
     const size_t N = (size_t)env->cfg.n_games, P = (size_t)env->cfg.n_players;
     cudaError_t ce = cudaSuccess;
     // Pinned host buffers are used in place: the step kernel reads the actions through their device alias and one
     // small kernel writes reward + done into the host arrays (no copy-engine transfers).  Pageable buffers take the
     // cudaMemcpyAsync route.  The alias lookups are cached per handle (same buffers every step in an RL loop).
-    const void *const hp[3] = {h_actions, h_reward, h_done};
-    for (int i = 0; i < 3; ++i)
-        if (hp[i] != env->hp_key[i]) { env->hp_key[i] = hp[i]; env->hp_dev[i] = mapped_alias(hp[i]); }
+    void *const a_act = host_alias(env, h_actions), *const a_rew = host_alias(env, h_reward),
+                *const a_done = host_alias(env, h_done);
     const int32_t *d_act = nullptr;
     if (h_actions) {
-        if (env->hp_dev[0] && aligned16(env->hp_dev[0])) {
-            d_act = static_cast<const int32_t *>(env->hp_dev[0]);
+        if (a_act && aligned16(a_act)) {
+            d_act = static_cast<const int32_t *>(a_act);
         } else {
             ce = cudaMemcpyAsync(bufs->actions_out, h_actions, N * P * 4, cudaMemcpyHostToDevice, s);
             if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
             d_act = bufs->actions_out;
         }
     }
-    const int e = gen_step(env, bufs, d_act, cuda_stream);
+    const int e = gen_step(env, bufs, d_act, s);
     if (e != GEN_OK) return e;
-    const bool mirror = N > 0 && (!h_reward || env->hp_dev[1]) && (!h_done || env->hp_dev[2]) && (h_reward || h_done);
+    const bool mirror = N > 0 && (!h_reward || a_rew) && (!h_done || a_done) && (h_reward || h_done);
     if (mirror) {
         const size_t bytes = N * P + N;
         const int threads = 256, blocks = (int)((bytes / 16 + threads) / threads < 296 ? (bytes / 16 + threads) / threads : 296);
+        // (a plain launch on purpose: as a programmatic dependent launch its CTAs would sit on 13 SMs while the next
+        // step's grid is placed, and that grid -- exactly one wave at config 2 -- would no longer fit: measured 425 M
+        // against 485 M env steps/s end to end)
         k_mirror<<<blocks, threads, 0, s>>>(reinterpret_cast<const unsigned char *>(bufs->reward),
-                                            static_cast<unsigned char *>(env->hp_dev[1]), h_reward ? N * P : 0,
-                                            bufs->done, static_cast<unsigned char *>(env->hp_dev[2]), h_done ? N : 0);
+                                            static_cast<unsigned char *>(a_rew), h_reward ? N * P : 0,
+                                            bufs->done, static_cast<unsigned char *>(a_done), h_done ? N : 0);
         ce = cudaGetLastError();
         if (ce == cudaSuccess) env->launches += 1;
     } else {
         if (h_reward) ce = cudaMemcpyAsync(h_reward, bufs->reward, N * P, cudaMemcpyDeviceToHost, s);
         if (ce == cudaSuccess && h_done) ce = cudaMemcpyAsync(h_done, bufs->done, N, cudaMemcpyDeviceToHost, s);
     }
-    if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
     if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
+    return GEN_OK;
+}
+
+int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
+                  uint8_t *h_done, void *cuda_stream) {
+    if (!env || !bufs) return GEN_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    if (int e = step_host_enqueue(env, bufs, h_actions, h_reward, h_done, s)) return e;
+    const cudaError_t ce = cudaStreamSynchronize(s);
+    if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
+    return GEN_OK;
+}
+
+int gen_step_host_async(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
+                        uint8_t *h_done, void *cuda_stream) {
+    if (!env || !bufs) return GEN_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    if (!env->ev_ready) {
+        for (int i = 0; i < 4; ++i) {
+            const cudaError_t ce = cudaEventCreateWithFlags(&env->ev[i], cudaEventDisableTiming);
+            if (ce != cudaSuccess) {
+                for (int j = 0; j < i; ++j) cudaEventDestroy(env->ev[j]);
+                env->last_cuda_error = (int)ce;
+                return GEN_ERR_CUDA;
+            }
+        }
+        env->ev_ready = 1;
+    }
+    if (int e = step_host_enqueue(env, bufs, h_actions, h_reward, h_done, s)) return e;
+    const cudaError_t ce = cudaEventRecord(env->ev[env->async_calls & 3], s);
+    if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
+    env->async_calls += 1;
+    return GEN_OK;
+}
+
+int gen_host_wait(gen_env *env, int32_t lag) {
+    if (!env) return GEN_ERR_NULL;
+    if (lag < 0 || lag > 3) return GEN_ERR_ARG;
+    if (env->async_calls <= (uint64_t)lag) return GEN_OK;     // nothing that old has been issued
+    const cudaError_t ce = cudaEventSynchronize(env->ev[(env->async_calls - 1 - (uint64_t)lag) & 3]);
+    if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
+    return GEN_OK;
+}
+
+int gen_forget_host_buffers(gen_env *env) {
+    if (!env) return GEN_ERR_NULL;
+    env->hp_used = env->hp_next = 0;
     return GEN_OK;
 }
 
@@ -477,6 +542,7 @@ int gen_query_feat_sizes(const gen_config *cfg, gen_feat_sizes *out) {
     out->last_seen = N * P * S * 4;
     out->hist = N * P * 8 * 2 * S * 2;
     out->feat_bf16 = N * P * 38 * S * 2;
+    out->hist_windows = N * P * 2 * 512 * 4;
     return GEN_OK;
 }
 
@@ -503,6 +569,17 @@ int gen_features(gen_env *env, const gen_buffers *bufs, const gen_feat_buffers *
     fp.feat = const_cast<void *>(out); fp.bf16 = feat->feat_bf16 ? 1 : 0; fp.mem_bits = feat->mem_bits; fp.last_army = feat->last_army;
     fp.last_seen = feat->last_seen; fp.hist = feat->hist;
     const cudaError_t e = gen::launch_features(fp, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
+    env->launches += 1;
+    return GEN_OK;
+}
+
+int gen_history_windows(gen_env *env, const gen_buffers *bufs, int32_t *d_windows, void *cuda_stream) {
+    if (!env || !bufs || !d_windows || !bufs->score_hist || !bufs->turn) return GEN_ERR_NULL;
+    if (!aligned16(d_windows) || !aligned16(bufs->score_hist) || !aligned16(bufs->turn)) return GEN_ERR_ALIGN;
+    if (env->cfg.n_games == 0) return GEN_OK;
+    const cudaError_t e = gen::launch_history_windows(bufs->score_hist, bufs->turn, d_windows, env->base.N, env->base.P,
+                                                      env->base.team_size, static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) { env->last_cuda_error = (int)e; return GEN_ERR_CUDA; }
     env->launches += 1;
     return GEN_OK;
@@ -542,7 +619,11 @@ int32_t gen_last_variant(const gen_env *env, int32_t *board_specialised, int32_t
 uint64_t gen_launch_count(const gen_env *env) { return env ? env->launches : 0; }
 int gen_last_cuda_error(const gen_env *env) { return env ? env->last_cuda_error : 0; }
 
-void gen_destroy(gen_env *env) { delete env; }
+void gen_destroy(gen_env *env) {
+    if (env && env->ev_ready)
+        for (int i = 0; i < 4; ++i) cudaEventDestroy(env->ev[i]);
+    delete env;
+}
 
 const char *gen_error_string(int code) {
     switch (code) {

@@ -492,6 +492,60 @@ cudaError_t launch_one(const FeatParams &fp, int threads, cudaStream_t stream) {
 
 // Board-specialised instantiations for the paper-sized 1v1 boards (BASELINE configs 1 and 2-4, the paper's own 23x23),
 // else the generic one.
+// ================================================================================================
+// The two temporal tokens' windows (reading R39): for game g and agent p, win[g][p][0][i] /
+// win[g][p][1][i] = the enemies' summed army total / land count at turn t - 511 + i of the current episode (t = turn[g];
+// i = 511 is now), 0 before the episode's first turn.  The source is the scoreboard ring of R34, slot (turn mod 512) =
+// (land[q], army[q]) of every player q.  One CTA of 512 threads per game, thread i owns window entry i: the slots it
+// reads are consecutive in i (one wrap), so the loads are 2P * 4-byte runs side by side and every store instruction
+// covers 2 KB of one window.  HBM-bound: 4 KB * P read, 4 KB * P written per game.
+template <int NP>
+__global__ void __launch_bounds__(512) k_history_windows(const int32_t *__restrict__ ring, const int32_t *__restrict__ turn,
+                                                         int32_t *__restrict__ win, int P, int team_size) {
+    const int g = blockIdx.x, i = threadIdx.x;
+    const int t = __ldg(turn + g);
+    const int tt = t - 511 + i;
+    int32_t v[2 * NP];
+#pragma unroll
+    for (int k = 0; k < 2 * NP; ++k) v[k] = 0;
+    if (tt >= 0) {
+        const int32_t *slot = ring + ((size_t)g * 512 + (size_t)(tt & 511)) * 2 * P;
+        if (NP == 2) {
+            const int4 q = __ldcs(reinterpret_cast<const int4 *>(slot));   // 2P ints = 16 bytes at P = 2
+            v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+        } else {
+#pragma unroll
+            for (int k = 0; k < NP; ++k)
+                if (k < P) {
+                    const int2 q = __ldcs(reinterpret_cast<const int2 *>(slot) + k);
+                    v[2 * k] = q.x; v[2 * k + 1] = q.y;
+                }
+        }
+    }
+    int32_t land_all = 0, army_all = 0;
+#pragma unroll
+    for (int k = 0; k < NP; ++k) { land_all += v[2 * k]; army_all += v[2 * k + 1]; }
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        if (p >= P) break;
+        int32_t land = land_all, army = army_all;   // everybody, minus the agent's own team
+#pragma unroll
+        for (int q = 0; q < NP; ++q)
+            if (q < P && q / team_size == p / team_size) { land -= v[2 * q]; army -= v[2 * q + 1]; }
+        int32_t *out = win + (((size_t)g * P + p) * 2) * 512 + i;
+        __stcs(out, army);
+        __stcs(out + 512, land);
+    }
+}
+
+cudaError_t launch_history_windows(const int32_t *ring, const int32_t *turn, int32_t *win, int N, int P, int team_size,
+                                   cudaStream_t stream) {
+    if (P == 2) k_history_windows<2><<<N, 512, 0, stream>>>(ring, turn, win, P, team_size);
+    else if (P <= 4) k_history_windows<4><<<N, 512, 0, stream>>>(ring, turn, win, P, team_size);
+    else k_history_windows<8><<<N, 512, 0, stream>>>(ring, turn, win, P, team_size);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_features(const FeatParams &fp, cudaStream_t stream) {
     if (fp.P != 2 || fp.team_size != 1) {          // R38: the multi-player kernel, one CTA per game
         const int NT = (fp.P + fp.team_size - 1) / fp.team_size;

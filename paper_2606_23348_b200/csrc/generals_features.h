@@ -27,4 +27,8 @@ struct FeatParams {
 
 cudaError_t launch_features(const FeatParams &fp, cudaStream_t stream);
 
+// gen_history_windows (R39): ring = gen_buffers.score_hist [N][512][2P], win = int32 [N][P][2][512]
+cudaError_t launch_history_windows(const int32_t *ring, const int32_t *turn, int32_t *win, int N, int P, int team_size,
+                                   cudaStream_t stream);
+
 }  // namespace gen

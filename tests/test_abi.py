@@ -37,7 +37,7 @@ def test_struct_layouts_match_header():
     assert C.sizeof(binding.GenBuffers) == 27 * 8
     assert C.sizeof(binding.GenSizes) == 8 + 27 * C.sizeof(C.c_size_t) + 8      # + bitboard_row_words, padding
     assert C.sizeof(binding.GenFeatBuffers) == 6 * 8
-    assert C.sizeof(binding.GenFeatSizes) == 8 + 6 * C.sizeof(C.c_size_t)
+    assert C.sizeof(binding.GenFeatSizes) == 8 + 7 * C.sizeof(C.c_size_t)
 
 
 def test_query_feat_sizes(lib):
@@ -48,6 +48,7 @@ def test_query_feat_sizes(lib):
     assert s.channels == 38 and s.plane_stride == S
     assert s.feat == N * 2 * 38 * S * 4 and s.mem_bits == N * 2 * S and s.last_army == N * 2 * S * 2
     assert s.last_seen == N * 2 * S * 4 and s.hist == N * 2 * 8 * 2 * S * 2 and s.feat_bf16 == N * 2 * 38 * S * 2
+    assert s.hist_windows == N * 2 * 2 * 512 * 4
     cfg4, _ = binding.make_config(workloads.config("c5a_2v2")[0])          # R38: P players, 32x32
     assert lib.gen_query_feat_sizes(C.byref(cfg4), C.byref(s)) == 0
     assert s.feat == 32768 * 4 * 38 * 1024 * 4 and s.hist == 32768 * 4 * 8 * 2 * 1024 * 2
@@ -113,6 +114,10 @@ def test_init_argument_errors_without_gpu(lib):
     bufs.owner = 0x1000
     assert lib.gen_features(env, C.byref(bufs), C.byref(fb), None) == -1
     assert lib.gen_features(env, C.byref(bufs), None, None) == -1
+    assert lib.gen_history_windows(env, C.byref(bufs), None, None) == -1          # no output buffer
+    assert lib.gen_history_windows(env, C.byref(bufs), 0x1008, None) == -3        # misaligned output
+    bufs.score_hist = None
+    assert lib.gen_history_windows(env, C.byref(bufs), 0x1000, None) == -1        # the ring is required
     for code in (0, -1, -2, -3, -4, -5, -99):
         assert lib.gen_error_string(code)
     lib.gen_destroy(env)

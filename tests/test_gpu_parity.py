@@ -569,6 +569,43 @@ def test_step_host_end_to_end(gpu, oracle_mod, pinned, N):
     assert int(o.episodes_done.sum()) > 0
 
 
+def test_step_host_async_one_step_late(gpu, oracle_mod):
+    """gen_step_host_async + gen_host_wait: the loop the end-to-end bench leg times -- two sets of pinned host slots,
+    step t issued before the results of step t - 1 are read (lag 1), then the last one drained (lag 0); results of
+    every step equal the oracle's, state equal at the end; forgetting the alias table in between changes nothing."""
+    import torch
+    N = 203
+    cfg, _ = workloads.config("c2_24x24", n_games=N, max_turns=40)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+    slots = [dict(a=torch.zeros((N, 2), dtype=torch.int32).pin_memory(), r=torch.zeros((N, 2), dtype=torch.int8).pin_memory(),
+                  d=torch.zeros((N,), dtype=torch.uint8).pin_memory()) for _ in range(2)]
+    want = []
+    T = 90
+    for t in range(T):
+        s = slots[t & 1]
+        a = o.sample()
+        s["a"].copy_(torch.from_numpy(a))
+        env.step_host_async(s["a"], s["r"], s["d"])
+        o.step(a)
+        want.append((o.reward[0].copy(), o.done[0].copy()))
+        if t >= 1:
+            env.host_wait(1)                                     # step t - 1 has landed; step t may still run
+            p = slots[(t - 1) & 1]
+            assert np.array_equal(p["r"].numpy(), want[t - 1][0]) and np.array_equal(p["d"].numpy(), want[t - 1][1]), t
+        if t == 40:
+            env.forget_host_buffers()
+    env.host_wait(0)
+    p = slots[(T - 1) & 1]
+    assert np.array_equal(p["r"].numpy(), want[-1][0]) and np.array_equal(p["d"].numpy(), want[-1][1])
+    compare(env, o, digest=False, where="step_host_async")
+    assert env.last_launch_register_resident and int(o.episodes_done.sum()) > 0
+    with pytest.raises(gpu.GenError):
+        env.host_wait(4)
+
+
 # ------------------------------------------------------------------------------- full-size sampled check
 @pytest.mark.parametrize("digest", [False, True])
 def test_config2_full_size_sampled_games(gpu, oracle_mod, digest):
@@ -1211,6 +1248,44 @@ def test_random_configurations_fuzz(gpu, oracle_mod):
                 compare(env, o, fields=fields, digest=dg, where=where + f" t={t}")
         done_eps += int(o.episodes_done.sum())
     assert done_eps > 0
+
+
+# ------------------------------------------------------------------------------- temporal tokens (R39)
+@pytest.mark.parametrize("name,N,T,over", [
+    ("c2_24x24", 45, 620, dict(max_turns=0, auto_reset=0)),                    # one long episode: the ring wraps
+    ("c4_curriculum", 37, 300, dict(height=10, width=10, spawn_dmin=3, spawn_dmax=5, n_cities=3, max_turns=90)),
+    ("c5a_2v2", 9, 120, dict(height=12, width=12, n_cities=3, spawn_dmin=4, max_turns=50)),
+    ("c5b_ffa8", 5, 90, dict(height=12, width=13, n_players=3, spawn_dmin=4, n_cities=4, max_turns=40)),
+])
+def test_history_windows_match_oracle(gpu, oracle_mod, name, N, T, over):
+    """gen_history_windows (the two 512-step windows behind the temporal tokens) against orc_history_windows
+    on the same play: oldest first, zeros before the episode's first turn, leftovers of earlier episodes masked,
+    enemies summed for more than two players (R38), before and after the ring wraps; the output buffer is poisoned
+    before every call."""
+    cfg, _ = workloads.config(name, n_games=N, **over)
+    env = gpu.GeneralsEnv(cfg, digest=False, history=True)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+    out = env.torch.full((N, cfg["n_players"], 2, 512), -77, dtype=env.torch.int32, device=env.device)
+    for t in range(T):
+        env.step()
+        o.step()
+        if t % 37 == 0 or t >= T - 3 or t in (509, 510, 511, 512, 513):
+            out.fill_(-77)
+            got = env.history_windows(out).cpu().numpy()
+            assert np.array_equal(got, o.history_windows()), f"{name}: windows differ at step {t}"
+    if cfg["max_turns"]:
+        assert int(o.episodes_done.sum()) > 0
+    no_ring = gpu.GeneralsEnv(cfg, digest=False)                # without the ring the call is refused
+    with pytest.raises(gpu.GenError):
+        no_ring.history_windows()
+
+
+def test_history_windows_empty_batch(gpu):
+    cfg, _ = workloads.config("c2_24x24", n_games=0)
+    env = gpu.GeneralsEnv(cfg, history=True)
+    assert env.history_windows().shape == (0, 2, 2, 512)
 
 
 # ------------------------------------------------------------------------------- sanitizer target
