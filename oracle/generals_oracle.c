@@ -621,7 +621,9 @@ int32_t orc_step(const orc_config *cfg, const orc_buffers *b, const int32_t *act
     for (int g = 0; g < cfg->n_games; ++g) {
         int frozen = !cfg->auto_reset && b->done[g] != 0;
         for (int p = 0; p < P; ++p) {
-            a[p] = actions ? actions[g * P + p] : (frozen ? 0 : sample_action(cfg, b, g, p, global_step));
+            /* R31: a frozen game applies nothing, whatever the caller passed; actions_out reports the action
+             * actually applied (include/generals.h), i.e. 0 = pass */
+            a[p] = frozen ? 0 : (actions ? actions[g * P + p] : sample_action(cfg, b, g, p, global_step));
             if (actions_out) actions_out[g * P + p] = a[p];
         }
         step_game(cfg, b, g, a, (size_t)g);
@@ -657,9 +659,22 @@ int32_t orc_rollout(const orc_config *cfg, const orc_buffers *b, int32_t K, uint
 }
 
 /* observation + scoreboard of a hand-built state (tests) */
+/* The entry point for states written by the caller (hand-built boards).  R40: in every state the rules
+ * produce, the GENERAL cells are exactly the cells general_cell[p] of their owners -- both generators place them so,
+ * and a captured general becomes a CITY (R11).  PAPER.md speaks of "unclaimed castles/generals" once (Table IV ch. 3,
+ * P:L361) and gives no rule for an unclaimed general; a GENERAL cell that is nobody's recorded general is therefore
+ * turned into a CITY here (it is a structure that nobody's elimination hangs on), so that step_game never meets one. */
 int32_t orc_observe(const orc_config *cfg, const orc_buffers *b)
 {
-    for (int g = 0; g < cfg->n_games; ++g) { scoreboard(cfg, b, g); observe(cfg, b, g, (size_t)g); }
+    const int P = cfg->n_players, HW = cfg->height * cfg->width, S = plane_stride(cfg);
+    for (int g = 0; g < cfg->n_games; ++g) {
+        int8_t *owner = b->owner + (size_t)g * S, *terrain = b->terrain + (size_t)g * S;
+        for (int c = 0; c < HW; ++c)
+            if (terrain[c] == T_GENERAL && (owner[c] < 0 || owner[c] >= P || b->general_cell[g * P + owner[c]] != c))
+                terrain[c] = T_CITY;
+        scoreboard(cfg, b, g);
+        observe(cfg, b, g, (size_t)g);
+    }
     return 0;
 }
 

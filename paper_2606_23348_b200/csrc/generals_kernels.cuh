@@ -778,6 +778,23 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     } else {
         mbar_wait(bar, 0);
     }
+    if ((flags & F_OBSERVE_ONLY) && gvalid) {
+        // R40: gen_observe takes a state written by the caller.  In every state the rules produce, the GENERAL cells
+        // are exactly the cells general_cell[p] of their owners (both generators place them so; a captured general
+        // becomes a CITY, R11).  A GENERAL cell that is nobody's recorded general -- an "unclaimed general", a second
+        // one -- is turned into a CITY here, so that no rule ever meets one (the two step kernels tell a general by
+        // the terrain and by general_cell respectively; on well-formed states these agree).
+        int8_t *Tr = s_terr + (size_t)sub * S;
+        const int8_t *O = s_owner + (size_t)sub * S;
+        bool fixed = false;
+        for (int c = ol; c < HW; c += LPG)
+            if (Tr[c] == T_GENERAL) {
+                const int o = O[c];
+                if (o < 0 || o >= P || B.general_cell[(size_t)g * P + o] != c) { Tr[c] = (int8_t)T_CITY; fixed = true; }
+            }
+        if (fixed) atomicOr(&s_game[sub].flags, (uint32_t)GF_TERRAIN_DIRTY);
+    }
+    __syncwarp();
     if (gvalid) build_game(sub);
     __syncwarp();
     if (gvalid) {

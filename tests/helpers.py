@@ -33,7 +33,7 @@ def hand_board(oracle_mod, H, W, P, cells, turn=1, team_size=1, **cfg):
     for (r, c), (t, ow, a) in cells.items():
         i = r * W + c
         o.terrain[0, i], o.owner[0, i], o.army[0, i] = t, ow, a
-        if t == oracle_mod.T_GENERAL:
+        if t == oracle_mod.T_GENERAL and ow >= 0 and o.general_cell[0, ow] < 0:   # the first one listed is the general
             o.general_cell[0, ow] = i
             alive |= 1 << ow
     o.alive[0] = alive

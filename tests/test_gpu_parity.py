@@ -445,6 +445,33 @@ def test_hand_cases_on_gpu(gpu, oracle_mod):
     assert int(env.field("sat_events")[0]) == 1
 
 
+def test_W13_unclaimed_general_on_gpu(gpu, oracle_mod):
+    """R40: gen_observe turns a GENERAL cell that is nobody's recorded general into a CITY (the raw planes are written
+    to the device un-normalised); afterwards both step kernels play W13 like the oracle."""
+    import torch
+    from helpers import hand_board
+    cells = {(0, 0): (GN, 0, 5), (2, 2): (GN, 1, 3), (0, 1): (GN, -1, 2), (2, 0): (GN, 1, 1), (1, 0): (PL, 0, 6)}
+    seq = [[act(0, 0, 3, RIGHT), PASS], [act(1, 0, 3, DOWN), PASS]]
+    for bitboards in (True, False):
+        o = hand_board(oracle_mod, 3, 3, 2, cells, turn=0)
+        env = gpu.GeneralsEnv(dict(n_games=1, height=3, width=3, n_players=2, team_size=1), digest=False, bitboards=bitboards)
+        put_board(env, o)
+        raw = env.tensors["terrain"].clone()
+        raw[0, 1] = GN
+        raw[0, 6] = GN
+        env.tensors["terrain"].copy_(raw)
+        env.observe()
+        compare(env, o, digest=False, where="W13 observe")
+        assert env.field("terrain")[0, 1] == CT and env.field("terrain")[0, 6] == CT
+        for a in seq:
+            a = np.asarray(a, dtype=np.int32).reshape(1, 2)
+            o.step(a)
+            env.step(torch.from_numpy(a).to(env.device))
+            compare(env, o, digest=False, where="W13 step")
+        assert env.last_launch_register_resident == bitboards
+        assert int(env.field("alive")[0]) == 0b11 and env.field("land")[0].tolist() == [4, 1]
+
+
 def test_saturating_growth_on_gpu(gpu, oracle_mod):
     cells = {(0, 0): (GN, 0, 32766), (2, 2): (GN, 1, 1), (1, 1): (CT, 0, 32767), (0, 1): (PL, 0, 32767)}
     seq = [[PASS, PASS]] * 4
@@ -502,6 +529,22 @@ def test_frozen_games_and_empty_batch(gpu, oracle_mod):
     env.rollout(5)
     o.rollout(5)
     compare(env, o, where="frozen rollout")
+    # explicit actions on frozen games (R31): nothing is applied and actions_out reports 0, on both step kernels
+    import torch
+    rng = np.random.default_rng(11)
+    for staged in (False, True):
+        e2 = gpu.GeneralsEnv(cfg, digest=staged)
+        o2 = oracle_mod.Oracle(cfg)
+        e2.reset()
+        o2.reset()
+        for t in range(16):
+            a = workloads.random_actions(rng, 30, 2, 8, 8) if t % 2 else o2.sample()
+            e2.step(torch.from_numpy(a).to(e2.device))
+            want = o2.step(a, want_actions=True)
+            compare(e2, o2, digest=staged, where=f"frozen explicit {t}")
+            assert np.array_equal(e2.field("actions_out"), want), t
+        assert (e2.field("done") == 2).all() and (e2.field("actions_out") == 0).all()
+        assert e2.last_launch_register_resident == (not staged)
     empty = gpu.GeneralsEnv(dict(cfg, n_games=0))
     empty.reset()
     empty.step()
@@ -812,7 +855,7 @@ def test_features_match_oracle_every_turn(gpu, oracle_mod, name, N, T, over):
 def test_features_staged_kernel_and_errors(gpu, oracle_mod):
     """gen_features reads only the state planes and scalars, so it does not matter which kernel stepped the game
     (here the staged one: no bitboard cache), nor whether k_features was compiled for the board (here: not).
-    Multi-player handles are refused."""
+    Multi-player handles are served since R38 (test_multi_player_features_*); an empty batch launches nothing."""
     cfg, _ = workloads.config("c2_24x24", n_games=11, max_turns=64, spawn_dmin=4)
     env = gpu.GeneralsEnv(cfg, bitboards=False)
     env.set_generic(True, True)                              # the generic k_features instantiation on a 24x24 board

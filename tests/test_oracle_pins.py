@@ -298,3 +298,23 @@ def test_invalid_and_out_of_range_actions_are_passes(oracle_mod):
     # a legal move next to them still works
     o.step([[act(1, 1, 3, DOWN), PASS]])
     assert cell(o, 2, 1)[1] == 0
+
+
+def test_W13_unclaimed_or_second_general_is_a_castle(oracle_mod):
+    """R40: the rules never produce a GENERAL cell that is not the recorded general of its owner; a
+    hand-written state that holds one -- an owner-less general ("unclaimed castles/generals", Table IV ch. 3, is the
+    paper's only word on it, with no rule attached), or a second GENERAL cell of a player -- is normalised by the
+    observe entry point: the cell becomes a CITY.  Taking it is then castle arithmetic by hand: 5 - 1 = 4 sent onto
+    2 defenders leaves 2 and the cell changes hands; nobody is eliminated, no land moves, the game goes on; taking
+    the second 'general' of player 1 (a castle now) eliminates nobody either."""
+    cells = {(0, 0): (GN, 0, 5), (2, 2): (GN, 1, 3), (0, 1): (GN, -1, 2), (2, 0): (GN, 1, 1), (1, 0): (PL, 0, 6)}
+    o = hand_board(oracle_mod, 3, 3, 2, cells, turn=0)
+    assert cell(o, 0, 1) == (CT, -1, 2) and cell(o, 2, 0) == (CT, 1, 1)          # normalised
+    assert cell(o, 0, 0)[0] == GN and cell(o, 2, 2)[0] == GN
+    assert o.general_cell[0].tolist() == [0, 8] and int(o.alive[0]) == 0b11
+    o.step([[act(0, 0, 3, RIGHT), PASS]])
+    assert cell(o, 0, 1) == (CT, 0, 2) and cell(o, 0, 0) == (GN, 0, 1)
+    assert int(o.alive[0]) == 0b11 and int(o.done[0, 0]) == 0 and o.land[0].tolist() == [3, 2]
+    o.step([[act(1, 0, 3, DOWN), PASS]])                                         # 5 onto player 1's castle of 1
+    assert cell(o, 2, 0) == (CT, 0, 5) and int(o.alive[0]) == 0b11 and int(o.done[0, 0]) == 0   # 4 left, +1 (turn 2)
+    assert cell(o, 2, 2) == (GN, 1, 4) and o.land[0].tolist() == [4, 1]
