@@ -153,8 +153,8 @@ def run_reference(args):
 MIN_REGION_MS, MIN_REPS, MAX_REPS = 50.0, 5, 60
 # warp-instructions per env step of the fused rollout kernel (gen_rollout(32, GEN_OBS_DIGEST), 24x24 1v1):
 # smsp__inst_executed.sum / (N * K) of the ncu capture summarised in the file named beside it
-ROLLOUT_INST_PER_ENV_STEP = 720.7
-ROLLOUT_INST_SOURCE = "profiles/r01_rollout_full_summary.txt"
+ROLLOUT_INST_PER_ENV_STEP = 656.2
+ROLLOUT_INST_SOURCE = "profiles/r02_rollout_summary.txt"
 ISSUE_PEAK = 148 * 4 * 1.965e9      # warp-instructions/s: 148 SMs x 4 schedulers x 1 per clock x 1.965 GHz
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_step at N = 262,144 (ncu --set full), by games per launch
 NCU_DRAM_BYTES_PER_LAUNCH_LARGE = {262144: (2354906856, "profiles/r01_step_full_262k_summary.txt")}
@@ -510,6 +510,35 @@ def run_ours(args):
     return 0
 
 
+def run_single_leg(args):
+    """--only rollout | step | step-large: one leg by itself, a handful of launches -- the command the ncu captures under
+    profiles/ are taken with (ncu replays every kernel it profiles ~40 times: a full bench run under it takes long)."""
+    import torch
+    import workloads
+    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    n = {"rollout": 16384, "step": 16384, "step-large": 262144}[args.only]
+    cfg, _ = workloads.config(WORKLOAD, n_games=args.games or n)
+    env = GeneralsEnv(cfg, device=dev, digest=(args.only == "rollout"), actions_out=False)
+    env.reset()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    k = max(4, min(args.steps, 12))
+    for _ in range(3):
+        env.rollout(32, OBS_DIGEST) if args.only == "rollout" else env.step()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(k):
+        env.rollout(32, OBS_DIGEST) if args.only == "rollout" else env.step()
+    e1.record()
+    torch.cuda.synchronize()
+    turns = 32 if args.only == "rollout" else 1
+    print(json.dumps({"leg": args.only, "n_games": cfg["n_games"], "launches": k, "turns_per_launch": turns,
+                      "us_per_launch": 1e3 * e0.elapsed_time(e1) / k,
+                      "env_steps_per_s": cfg["n_games"] * turns * k / (e0.elapsed_time(e1) * 1e-3)}))
+    return 0
+
+
 # ------------------------------------------------------------------------------------------ batch sweep
 def time_steps(torch, envs, K, warm, graph):
     """K gen_step launches back to back, replica t % R at launch t; returns ms.  graph=True replays them as one
@@ -709,6 +738,8 @@ def main():
     ap.add_argument("--replicas", type=int, default=0, help="replicas in the round-robin (default: enough for 640 MB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-large", action="store_true", help="skip the N = 262,144 leg (roofline_large)")
+    ap.add_argument("--only", choices=["rollout", "step", "step-large"], default="",
+                    help="one leg by itself, a few launches (the command of the ncu captures under profiles/)")
     ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
     ap.add_argument("--rows", default="", help="with --sweep: only the rows whose workload name contains this")
     ap.add_argument("--workload", default="", help="with --features: workload name (default c2_24x24)")
@@ -716,6 +747,8 @@ def main():
     ap.add_argument("--features", action="store_true", help="NEXT-1: gen_features alone and with gen_step (one JSON line)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.only:
+        return run_single_leg(args)
     if args.sweep:
         return run_sweep(args)
     if args.features:

@@ -1207,11 +1207,21 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     // A fogged cell packs to 0x400000, a visible one to x | 0x1000000, so
     // pack - 0x400000 = vis ? (x | 0xC00000) : 0 (terrain <= 3 leaves bits 22, 23 clear) and
     // h_p = 0x400000 * sum(key) + sum_c vis & (x | 0xC00000) * key(c).  All 8 lanes of the octet call this.
+    // Instruction diet (this loop was half of the fused rollout's instruction stream): x = army | ob << 16 | 0xC00000
+    // is ONE byte permute per cell (the 0xC0 rides on the ob byte, the top byte is the sign replica of the army's
+    // high byte, which is 0 since army <= 32767); x * key mod 2^64 is accumulated per player as a 64-bit sum of
+    // x * key_lo (one wide multiply-add) and a 32-bit sum of x * key_hi (one multiply-add) of x-or-0 by the player's
+    // fog bit -- no 64-bit product is formed and then added under a predicate twice (inline PTX: the compiler
+    // turns every other spelling back into that).
     auto chain_digest = [&](int lg, bool active) {
         uint64_t h[NP];
 #pragma unroll
         for (int p = 0; p < NP; ++p) h[p] = 0;
         if (active) {
+            uint64_t lo[NP];
+            uint32_t hi[NP];
+#pragma unroll
+            for (int p = 0; p < NP; ++p) { lo[p] = 0; hi[p] = 0; }
             for (int ch = ol; ch < NC8; ch += LPG) {
                 uint32_t vb[NP], any = 0;
 #pragma unroll
@@ -1220,9 +1230,9 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 const uint4 a = *reinterpret_cast<const uint4 *>(s_army + (size_t)lg * S + 8 * ch);
                 const uint2 o = *reinterpret_cast<const uint2 *>(s_owner + (size_t)lg * S + 8 * ch);
                 const uint2 t = *reinterpret_cast<const uint2 *>(s_terr + (size_t)lg * S + 8 * ch);
-                // per byte: (owner + 2) | terrain << 4
-                const uint32_t otx = (((o.x & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu) | (t.x << 4);
-                const uint32_t oty = (((o.y & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu) | (t.y << 4);
+                // per byte: (owner + 2) | terrain << 4 | 0xC0
+                const uint32_t otx = (((o.x & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu) | (t.x << 4) | 0xC0C0C0C0u;
+                const uint32_t oty = (((o.y & 0x0F0F0F0Fu) + 0x02020202u) & 0x0F0F0F0Fu) | (t.y << 4) | 0xC0C0C0C0u;
                 const uint32_t aw[4] = {a.x, a.y, a.z, a.w};
                 // the eight keys of the chunk: four 16-byte loads (cells past the board are never visible)
                 unsigned long long key[8];
@@ -1233,14 +1243,25 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
                 }
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    const uint32_t half = (i & 1) ? (aw[i >> 1] >> 16) : (aw[i >> 1] & 0xFFFFu);
-                    const uint32_t ob = (((i < 4) ? otx : oty) >> (8 * (i & 3))) & 0xFFu;
-                    const uint64_t xk = (uint64_t)(half | (ob << 16) | 0xC00000u) * key[i];
+                    // bytes of x: army low, army high, ob | 0xC0, 0 (sign replica of the army's high byte)
+                    const uint32_t sel = (i & 1) ? (0xB032u | ((4u + (i & 3)) << 8)) : (0x9010u | ((4u + (i & 3)) << 8));
+                    const uint32_t x = prmt(aw[i >> 1], (i < 4) ? otx : oty, sel);
+                    const uint32_t klo = (uint32_t)key[i], khi = (uint32_t)(key[i] >> 32);
 #pragma unroll
                     for (int p = 0; p < NP; ++p)
-                        if (p < P && ((vb[p] >> i) & 1u)) h[p] += xk;
+                        if (p < P)  // four instructions per cell and player: fog bit -> x or 0, two multiply-adds
+                            asm("{\n\t.reg .pred q;\n\t.reg .b32 t, xm;\n\t"
+                                "and.b32 t, %2, %3;\n\t"
+                                "setp.ne.u32 q, t, 0;\n\t"
+                                "selp.b32 xm, %4, 0, q;\n\t"
+                                "mad.wide.u32 %0, xm, %5, %0;\n\t"
+                                "mad.lo.u32 %1, xm, %6, %1;\n\t}"
+                                : "+l"(lo[p]), "+r"(hi[p])
+                                : "r"(vb[p]), "r"(1u << i), "r"(x), "r"(klo), "r"(khi));
                 }
             }
+#pragma unroll
+            for (int p = 0; p < NP; ++p) h[p] = lo[p] + ((uint64_t)hi[p] << 32);
         }
 #pragma unroll
         for (int p = 0; p < NP; ++p) {

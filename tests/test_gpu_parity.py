@@ -1388,3 +1388,103 @@ def test_sanitizer_coverage_run(gpu, oracle_mod):
         o.step()
         compare_features(env, o, where=f"2v2 step {t}")
     compare(env, o, where="2v2")
+
+
+# ------------------------------------------------------------------------------- memory discipline without a sanitizer
+def test_guard_bands_and_poisoned_outputs(gpu, oracle_mod):
+    """compute-sanitizer is closed on this GPU pool (profiles/r02_sanitizer.md), so the checks it would make are made
+    by hand.  (1) memcheck's part: every device buffer of the handle is carved out of a larger allocation filled with
+    0xA5 -- 4 KB of guard band on both sides, also around the feature buffers and the window output -- and the bands
+    must be untouched after resets, chained steps, explicit-action steps, fused rollouts, gen_observe, gen_sample,
+    gen_features and gen_history_windows on every kernel variant a ragged batch reaches.  (2) initcheck's part:
+    every OUTPUT buffer is poisoned before each call, so a cell the kernels fail to write shows up as a mismatch
+    with the oracle.  Boards: 24x24 1v1 (board-specialised kernels), 23x23 official maps, 12x13 with 3 players
+    (generic kernels, stride padding), 32x32 2v2."""
+    import ctypes as C
+    import torch
+    GUARD = 4096
+    OUT = ["reward", "done", "winner", "obs_army", "obs_owner", "obs_terrain", "obs_vis", "actions_out"]
+
+    def fence(env):
+        """Move every tensor of env into the middle of a poisoned allocation; returns the guard checkers."""
+        bands = []
+        for name, t in list(env.tensors.items()):
+            nbytes = t.numel() * t.element_size()
+            raw = torch.full((nbytes + 2 * GUARD,), 0xA5, dtype=torch.uint8, device=env.device)
+            mid = raw[GUARD:GUARD + nbytes]
+            mid.copy_(t.view(torch.uint8).reshape(-1))
+            view = mid.view(t.dtype).reshape(t.shape)
+            assert view.data_ptr() % 16 == 0
+            env.tensors[name] = view
+            setattr(env, name, view)
+            setattr(env.bufs, name, view.data_ptr())
+            bands.append((name, raw, nbytes))
+        return bands
+
+    def check(bands, where):
+        torch.cuda.synchronize()
+        for name, raw, nbytes in bands:
+            assert bool((raw[:GUARD] == 0xA5).all()) and bool((raw[GUARD + nbytes:] == 0xA5).all()), \
+                f"{where}: write outside {name}"
+
+    def poison(env):
+        for name in OUT:
+            if name in env.tensors:
+                env.tensors[name].view(torch.uint8).fill_(0x5A)
+
+    cases = [("c2_24x24", 37, dict(max_turns=25), True), ("official_23x23", 21, dict(max_turns=20), True),
+             ("c5b_ffa8", 11, dict(height=12, width=13, n_players=3, spawn_dmin=4, n_cities=4, max_turns=30), True),
+             ("c5a_2v2", 7, dict(max_turns=20), False)]
+    for name, N, over, digest in cases:
+        cfg, _ = workloads.config(name, n_games=N, **over)
+        for step_kernel in (True, False):
+            use_digest = digest and not step_kernel
+            env = gpu.GeneralsEnv(cfg, digest=use_digest, history=True, bitboards=step_kernel)
+            if step_kernel:
+                env.set_generic(False, -1)
+            o = oracle_mod.Oracle(cfg)
+            bands = fence(env)
+            poison(env)
+            env.reset()
+            o.reset()
+            compare(env, o, digest=False, where=f"{name} reset")
+            for t in range(30):
+                poison(env)
+                if t % 5 == 4:
+                    a = o.sample()
+                    env.step(torch.from_numpy(a).to(env.device))
+                    o.step(a)
+                else:
+                    env.step()
+                    o.step()
+                compare(env, o, digest=False, where=f"{name} step {t}")
+            assert env.last_launch_register_resident == step_kernel
+            poison(env)
+            env.rollout(7, gpu.OBS_DIGEST if use_digest else gpu.OBS_NONE)
+            o.rollout(7, oracle_mod.OBS_DIGEST if use_digest else oracle_mod.OBS_NONE)
+            assert np.array_equal(env.sample().cpu().numpy(), o.sample())
+            poison(env)
+            env.observe()
+            compare(env, o, fields=STATE_FIELDS + OUT_FIELDS[3:], digest=False, where=f"{name} rollout + observe")
+            # feature tensor and windows, their buffers fenced too
+            env.features()
+            fb = []
+            for k, t in list(env.feat_tensors.items()):
+                nbytes = t.numel() * t.element_size()
+                raw = torch.full((nbytes + 2 * GUARD,), 0xA5, dtype=torch.uint8, device=env.device)
+                mid = raw[GUARD:GUARD + nbytes]
+                mid.copy_(t.view(torch.uint8).reshape(-1))
+                view = mid.view(t.dtype).reshape(t.shape)
+                env.feat_tensors[k] = view
+                setattr(env.feat_bufs, k, view.data_ptr())
+                fb.append((k, raw, nbytes))
+            env.feat = env.feat_tensors["feat"]
+            env.feat.fill_(float("nan"))
+            f = env.features()
+            torch.cuda.synchronize()
+            assert bool(torch.isfinite(f).all())
+            wraw = torch.full((N * cfg["n_players"] * 2 * 512 * 4 + 2 * GUARD,), 0xA5, dtype=torch.uint8, device=env.device)
+            win = wraw[GUARD:-GUARD].view(torch.int32).reshape(N, cfg["n_players"], 2, 512)
+            assert np.array_equal(env.history_windows(win).cpu().numpy(), o.history_windows())
+            check(bands + fb + [("windows", wraw, wraw.numel() - 2 * GUARD)], f"{name} step_kernel={step_kernel}")
+            env.close()
