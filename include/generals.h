@@ -124,7 +124,16 @@ typedef struct gen_buffers {
     int8_t *play_size;       /* state [N][2]  playable rows, columns of the current map, may be NULL: written by the
                                 generators (H, W unless map_mode 1 with play_min, R36); gen_features reads it for Table
                                 IV's "known padded border" (0 = not recorded = the full board) */
+    uint32_t *stack_cache;   /* state [N][P+1]  largest owned stack per player + validity stamp, may be NULL (see below) */
 } gen_buffers;
+
+/* `stack_cache` serves the biased policy (gen_policy.bias_thr, R25: "70 % of moves from the largest owned stack"):
+ * the per-step kernel's observation pass holds every army value in registers anyway, so it leaves each player's
+ * largest owned stack of the state it emits -- ((army + 1) << 10 | (1023 - cell)), ties to the lowest cell, 0 = owns
+ * nothing -- in [g][p] and the global step at which that state will be sampled in [g][P]; the next gen_step's
+ * sampler takes it from there instead of scanning the army plane.  Derived state like `bitboards`: a stamp that does
+ * not match (after gen_reset, gen_rollout, a staged-kernel step, gen_set_global_step) sends the sampler back to the
+ * scan, so it is never stale.  Allocate it zeroed.  Results do not depend on it. */
 
 /* `step_epoch` lets consecutive gen_step launches of one handle overlap.  Without it a launch starts working only
  * when the whole previous grid in the stream has completed (griddepcontrol.wait); the batch then moves through the
@@ -170,7 +179,7 @@ typedef struct gen_sizes {
     size_t army, owner, terrain, turn, episode, alive, general_cell, land, army_total;
     size_t reward, done, winner, obs_army, obs_owner, obs_terrain, obs_vis;
     size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out, bitboards, obs_packed, score_hist;
-    size_t step_epoch, play_size;
+    size_t step_epoch, play_size, stack_cache;
     int32_t bitboard_row_words; /* BW */
 } gen_sizes;
 

@@ -67,6 +67,7 @@ BUFFERS = [
     ("score_hist", "int32", lambda N, P, S, K: (N, 512, 2 * P)),
     ("step_epoch", "int32", lambda N, P, S, K: (2, (N + 3) // 4)),                      # bits of uint32
     ("play_size", "int8", lambda N, P, S, K: (N, 2)),
+    ("stack_cache", "int32", lambda N, P, S, K: (N, P + 1)),                             # bits of uint32
 ]
 
 
@@ -186,7 +187,7 @@ class GeneralsEnv:
     """
 
     def __init__(self, cfg, device="cuda:0", k_slots=1, digest=True, actions_out=True, bitboards=True,
-                 packed=False, history=False, chain=True):
+                 packed=False, history=False, chain=True, stack_cache=True):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -206,7 +207,7 @@ class GeneralsEnv:
         self.tensors = {}
         for name, dt, shape in BUFFERS:
             if ((name == "obs_digest" and not digest) or (name == "actions_out" and not actions_out)
-                    or (name == "bitboards" and not bitboards) or (name == "obs_packed" and not packed) or (name == "score_hist" and not history) or (name == "step_epoch" and not chain)
+                    or (name == "bitboards" and not bitboards) or (name == "obs_packed" and not packed) or (name == "score_hist" and not history) or (name == "step_epoch" and not chain) or (name == "stack_cache" and not stack_cache)
                     or (packed and name in ("obs_owner", "obs_terrain", "obs_vis"))):
                 setattr(self.bufs, name, None)
                 continue

@@ -85,6 +85,7 @@ void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
     s->score_hist = N * 512 * 2 * P * 4;
     s->step_epoch = (N + 3) / 4 * 8;
     s->play_size = N * 2;
+    s->stack_cache = N * (P + 1) * 4;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -110,6 +111,7 @@ int check_buffers(const gen_buffers *b, bool need_obs) {
     if (b->score_hist && !aligned16(b->score_hist)) return GEN_ERR_ALIGN;
     if (b->step_epoch && !aligned16(b->step_epoch)) return GEN_ERR_ALIGN;
     if (b->play_size && !aligned16(b->play_size)) return GEN_ERR_ALIGN;
+    if (b->stack_cache && !aligned16(b->stack_cache)) return GEN_ERR_ALIGN;
     return GEN_OK;
 }
 
@@ -170,6 +172,10 @@ const gen::Variant kVariants[gen::N_VARIANTS] = {
 const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, bool step_ok) {
     const int kind = (step_ok ? 1 : 0) + (kp.map_mode == 1 ? 2 : 0);
     const gen::Variant *generic = nullptr, *exact = nullptr;
+    // k_step: ff = 1 is the build whose observation pass also finds each player's largest stack (stack_cache) for
+    // the biased policy; where the board has no such build the plain one serves (its sampler scans the army plane)
+    const bool want_stack = (kind & 1) && kp.bias_thr != 0 && (kp.flags & gen::F_SAMPLER) && kp.b.stack_cache != nullptr;
+    for (int pass = want_stack ? 0 : 1; pass < 2 && !exact; ++pass)
     for (const gen::Variant &v : kVariants) {
         if (v.kind != kind) continue;
         if (v.h == 0) {
@@ -179,6 +185,7 @@ const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, boo
         if (env->force_generic || v.np != kp.P || v.h != kp.H || v.w != kp.W) continue;
         if (v.np == 2 && kp.team_size > 1) continue;
         if ((kind & 1) == 0 && v.ff != (kp.flags & ~gen::F_SAMPLER)) continue;
+        if ((kind & 1) == 1 && (v.ff != 0) != (pass == 0)) continue;
         if (!exact) { exact = &v; continue; }
         // the same kernel under several register budgets (resident CTAs per SM): 14 if only that holds the whole
         // batch resident in one wave, 12 for smaller batches and while the launches of a multi-wave batch still chain

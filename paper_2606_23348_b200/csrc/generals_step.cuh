@@ -44,6 +44,7 @@ struct StepGame {  // per-game scalars in shared memory
     uint32_t alive, done, episode, flags, sat;
     int32_t rew_bits;
     int32_t tot[8], land[8], act[8], gcell[8];
+    uint32_t best[8], best_ok;  // BIAS: largest owned stack per player from gen_buffers.stack_cache, and whether it is current
 };
 
 enum : uint32_t {
@@ -57,10 +58,13 @@ enum : uint32_t {
 // ================================================================================================
 // NP = bound of the player loops; CH x CW > 0: board size fixed at compile time and P == NP; MAXT / MINB:
 // launch bounds (threads per CTA, resident CTAs per SM the register allocation must allow).
-template <int NP, int CH, int CW, int MAXT, int MINB, bool OFFICIAL>
+// BIAS: the build for the biased policy (R25): the observation pass also finds each player's largest owned stack and
+// leaves it in gen_buffers.stack_cache for the next turn's sampler (which then does not scan the army plane).
+template <int NP, int CH, int CW, int MAXT, int MINB, bool OFFICIAL, bool BIAS>
 __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KParams kp) {
     constexpr bool FIXED = CH > 0;
     constexpr int LPP = LPG / NP;
+    static_assert(!BIAS || NP < LPG, "lane P of the octet carries the stamp of gen_buffers.stack_cache");
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x;
     const uint32_t lane = tid & 31u;
@@ -171,6 +175,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         if (ol == 0) { gs.turn = v_turn; gs.episode = v_ep; }
         if (ol == 1) { gs.alive = v_alive; gs.done = v_done; gs.winner = v_win; }
         if (ol == 2) { gs.flags = 0; gs.sat = 0; gs.rew_bits = 0; }
+        if constexpr (BIAS) {
+            const uint32_t v_st = B.stack_cache ? __ldcg(B.stack_cache + (size_t)g * (P + 1) + min(ol, P)) : 0u;
+            if (ol < P) gs.best[ol] = v_st;
+            if (ol == P) gs.best_ok = (B.stack_cache && v_st == kp.global_step0) ? 1u : 0u;
+        }
     }
     __syncthreads();  // the only CTA barrier: tables and the mbarrier init are visible
     if (nwg <= 0) return;
@@ -231,7 +240,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
             // owned cell (four independent 16-byte loads per word), compares in registers, the player's lanes reduce.
             const int16_t *Ag = B.army + (size_t)(wg0 + lg) * S;
             uint32_t best = 0;
-            for (int j = js; j < je; ++j) {
+            const bool cached = BIAS && s_game[lg].best_ok != 0;  // left by the previous turn's observation pass
+            if (cached) best = s_game[lg].best[p];
+            for (int j = cached ? je : js; j < je; ++j) {
                 const uint32_t m = own[j] & s_inb[j];
                 uint4 v[4];
 #pragma unroll
@@ -676,6 +687,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         const bool packed = B.obs_packed != nullptr;
         const unsigned char *sv = reinterpret_cast<const unsigned char *>(vrow(0, lg)) + ol;
         const int nit = (NC8 - ol + LPG - 1) / LPG;
+        uint32_t bb[NP];  // BIAS: largest owned stack per player among this lane's chunks
+#pragma unroll
+        for (int p = 0; p < NP; ++p) bb[p] = 0;
         for (int i0 = 0; i0 < nit; i0 += EB) {
             // ---- pass A: army
             uint4 a[EB];
@@ -695,6 +709,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
                     xa.x = a[k].x & prmt(s0, 0u, 0x9988u); xa.y = a[k].y & prmt(s0, 0u, 0xBBAAu);
                     xa.z = a[k].z & prmt(s1, 0u, 0x9988u); xa.w = a[k].w & prmt(s1, 0u, 0xBBAAu);
                     __stcs(reinterpret_cast<uint4 *>(oa + 2 * (size_t)p * (size_t)S + 128 * i), xa);
+                    if constexpr (BIAS) {  // (army + 1) << 10 | (1023 - cell): max = largest stack, ties to the lowest cell
+                        const uint32_t ob = row8(p, lg)[ol + LPG * i];
+                        if (ob) {
+                            const uint32_t aa[4] = {a[k].x, a[k].y, a[k].z, a[k].w};
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) {
+                                const uint32_t army = (aa[e >> 1] >> (16 * (e & 1))) & 0xFFFFu;
+                                const uint32_t key = ((army + 1u) << 10) | (uint32_t)(1023 - (8 * (ol + LPG * i) + e));
+                                if ((ob >> e) & 1u) bb[p] = max(bb[p], key);
+                            }
+                        }
+                    }
                 }
             }
             // ---- pass B: owner, terrain, visibility -- three byte planes, or one packed byte (R33)
@@ -743,6 +769,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
                     __stcs(reinterpret_cast<uint2 *>(ot + po + 64 * i), xt);
                     __stcs(reinterpret_cast<uint2 *>(ov + po + 64 * i), xv);
                 }
+            }
+        }
+        if constexpr (BIAS) {
+            if (B.stack_cache) {
+                uint32_t mine = kp.global_step0 + 1u;  // lane P: the step at which this state will be sampled
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+#pragma unroll
+                    for (int o = LPG / 2; o >= 1; o >>= 1) bb[p] = max(bb[p], __shfl_xor_sync(gmask, bb[p], o));
+                    if (ol == p) mine = bb[p];
+                }
+                if (ol <= P) B.stack_cache[(size_t)(wg0 + lg) * (P + 1) + ol] = mine;
             }
         }
     };

@@ -25,13 +25,13 @@ template <typename S> struct KernelOf<S, 0> {
     static constexpr auto fn = k_generals<S::NP, S::H, S::W, S::FF, false>;
 };
 template <typename S> struct KernelOf<S, 1> {
-    static constexpr auto fn = k_step<S::NP, S::H, S::W, S::MAXT, S::MINB, false>;
+    static constexpr auto fn = k_step<S::NP, S::H, S::W, S::MAXT, S::MINB, false, (S::FF != 0)>;
 };
 template <typename S> struct KernelOf<S, 2> {   // kinds 2 / 3: the same kernels with the official generator (R36)
     static constexpr auto fn = k_generals<S::NP, S::H, S::W, S::FF, true>;
 };
 template <typename S> struct KernelOf<S, 3> {
-    static constexpr auto fn = k_step<S::NP, S::H, S::W, S::MAXT, S::MINB, true>;
+    static constexpr auto fn = k_step<S::NP, S::H, S::W, S::MAXT, S::MINB, true, false>;
 };
 
 #define GEN_CAT_(a, b) a##b

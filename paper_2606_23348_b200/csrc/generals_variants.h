@@ -35,8 +35,13 @@ constexpr uint32_t FF_ROLL_DIGEST = F_OBS_PLANES | F_DIGEST;     // gen_rollout(
     X(14, 3, 2, 23, 23, 0, 64, 10)               \
     X(15, 2, 2, 0, 0, F_RUNTIME, 256, 1)         \
     X(16, 3, 2, 0, 0, 0, 256, 2)                 \
-    X(17, 1, 2, 24, 24, 0, 64, 12)
-constexpr int N_VARIANTS = 18;
+    X(17, 1, 2, 24, 24, 0, 64, 12)               \
+    X(18, 1, 2, 24, 24, 1, 64, 14)               \
+    X(19, 1, 2, 24, 24, 1, 64, 12)               \
+    X(20, 1, 2, 24, 24, 1, 64, 10)
+constexpr int N_VARIANTS = 21;
+// Variants 18-20: variants 7 / 17 / 11 for the biased policy (R25; BASELINE config 4): flags = 1 compiles the
+// observation pass that also finds each player's largest owned stack and leaves it in gen_buffers.stack_cache.
 // Kinds 2 / 3 are kinds 0 / 1 compiled with the official map generator (R36; gen_config.map_mode = 1, 1v1 only): the
 // generator is a template flag, not a runtime branch, so that the kernels of BASELINE's configs are exactly what they
 // were without it.  Variants 13 and 14: the paper's own board ("up to 23x23"; workload official_23x23) under

@@ -194,6 +194,57 @@ def test_kernels_interleave_coherently(gpu, oracle_mod):
     assert int(o.episodes_done.sum()) > 0
 
 
+def test_stack_cache_of_the_biased_policy_is_never_stale(gpu, oracle_mod):
+    """gen_buffers.stack_cache (the largest owned stack the observation pass leaves for the next turn's biased
+    sampler, R25): the actions drawn must equal the oracle's through everything that invalidates the cache -- resets,
+    fused rollouts, staged-kernel steps, explicit-action steps, gen_set_global_step -- and with the cache poisoned by
+    hand; a handle without the buffer (the sampler scans the army plane) must agree too."""
+    import torch
+    cfg, _ = workloads.config("c4_curriculum", n_games=77, max_turns=60)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    bare = gpu.GeneralsEnv(cfg, digest=False, stack_cache=False)
+    o = oracle_mod.Oracle(cfg)
+    for e in (env, bare):
+        e.reset()
+    o.reset()
+
+    def steps(n, where):
+        for t in range(n):
+            acts = o.step(want_actions=True)
+            for e in (env, bare):
+                e.step()
+                assert np.array_equal(e.field("actions_out"), acts), f"{where} step {t}"
+        compare(env, o, digest=False, where=where)
+        compare(bare, o, digest=False, where=where + " (no cache)")
+
+    steps(70, "plain")
+    assert int(o.episodes_done.sum()) > 0                       # auto-resets regenerate boards under the cache
+    assert env.last_launch_specialised and env.last_launch_register_resident
+    assert int((env.tensors["stack_cache"][:, 2] == env.global_step).sum()) == 77      # every stamp is current
+    for e in (env, bare):
+        e.rollout(5, gpu.OBS_NONE)
+    o.rollout(5, oracle_mod.OBS_NONE)
+    steps(7, "after a rollout")
+    env.set_generic(False, True)                               # one staged-kernel step: the cache goes stale
+    acts = o.step(want_actions=True)
+    env.step()
+    bare.step()
+    env.set_generic(False, False)
+    steps(9, "after a staged step")
+    a = o.sample()
+    for e in (env, bare):
+        e.step(torch.from_numpy(a).to(e.device))
+    o.step(a)
+    steps(9, "after explicit actions")
+    env.tensors["stack_cache"][:, :2] = 0x7FFFFFF                # wrong stacks under a CURRENT stamp would be used ...
+    env.tensors["stack_cache"][:, 2] = 0                         # ... so the stamp is made stale with them
+    steps(9, "poisoned cache, stale stamp")
+    for e in (env, bare):
+        e.reset()
+    o.reset()
+    steps(30, "after reset")
+
+
 def test_specialised_rollout_kernel_matches_oracle(gpu, oracle_mod):
     cfg, _ = workloads.config("c2_24x24", n_games=70, max_turns=90)
     env, o = make_pair(gpu, oracle_mod, cfg)
