@@ -157,7 +157,7 @@ ROLLOUT_INST_PER_ENV_STEP = 656.2
 ROLLOUT_INST_SOURCE = "profiles/r02_rollout_summary.txt"
 ISSUE_PEAK = 148 * 4 * 1.965e9      # warp-instructions/s: 148 SMs x 4 schedulers x 1 per clock x 1.965 GHz
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_step at N = 262,144 (ncu --set full), by games per launch
-NCU_DRAM_BYTES_PER_LAUNCH_LARGE = {262144: (2354906856, "profiles/r01_step_full_262k_summary.txt")}
+NCU_DRAM_BYTES_PER_LAUNCH_LARGE = {262144: (2303562752, "profiles/r02_step_full_262k_summary.txt")}
 
 
 def run_ours(args):
@@ -533,9 +533,39 @@ def run_single_leg(args):
     e1.record()
     torch.cuda.synchronize()
     turns = 32 if args.only == "rollout" else 1
-    print(json.dumps({"leg": args.only, "n_games": cfg["n_games"], "launches": k, "turns_per_launch": turns,
-                      "us_per_launch": 1e3 * e0.elapsed_time(e1) / k,
-                      "env_steps_per_s": cfg["n_games"] * turns * k / (e0.elapsed_time(e1) * 1e-3)}))
+    out = {"leg": args.only, "n_games": cfg["n_games"], "launches": k, "turns_per_launch": turns,
+           "us_per_launch": 1e3 * e0.elapsed_time(e1) / k,
+           "env_steps_per_s": cfg["n_games"] * turns * k / (e0.elapsed_time(e1) * 1e-3)}
+    # Development builds (GEN_NVCC_FLAGS=-DGEN_TRACE python -m paper_2606_23348_b200.build --force) keep a per-warp
+    # timeline of the per-step kernel (%globaltimer at every phase boundary): one lone launch after an L2 flush and
+    # one behind a foreign kernel, summarised as mean / max time since the first warp started, in microseconds.
+    variant = env.lib.gen_last_variant(env._env, None, None)
+    reader = getattr(env.lib, f"gen_debug_trace_{variant}", None) if args.only == "step" else None
+    if reader is not None:
+        import ctypes
+        import numpy as np
+        names = ["start", "scalars", "rows", "sampler", "moves", "growth", "end_of_turn", "fog", "emit", "store"]
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        foreign = torch.empty(24 << 20, dtype=torch.uint8, device=dev)
+        warps = min(8192, (cfg["n_games"] + 3) // 4)
+        out["timeline_us"] = {}
+        for tag, pre in (("lone_after_l2_flush", lambda: flush.fill_(1)), ("behind_foreign_kernel", lambda: foreign.fill_(3))):
+            for _ in range(3):
+                pre()
+                torch.cuda.synchronize()
+                env.step()
+                torch.cuda.synchronize()
+            buf = np.zeros(warps * 16, dtype=np.uint64)
+            reader(buf.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(warps * 16))
+            t = buf.reshape(warps, 16).astype(np.int64)
+            t0 = t[:, 0].min()
+            done = (t[:, 9] - t0) / 1e3
+            out["timeline_us"][tag] = {
+                "phase_end_mean_max": {n: [round(float((t[:, i].mean() - t0) / 1e3), 1), round(float((t[:, i].max() - t0) / 1e3), 1)]
+                                       for i, n in enumerate(names)},
+                "warps_finished_by_us": {str(b): int((done <= b).sum()) for b in (16, 20, 24, 28, 32, 36, 40)},
+                "warps": warps}
+    print(json.dumps(out))
     return 0
 
 

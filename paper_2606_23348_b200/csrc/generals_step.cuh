@@ -45,6 +45,7 @@ struct StepGame {  // per-game scalars in shared memory
     int32_t rew_bits;
     int32_t tot[8], land[8], act[8], gcell[8];
     uint32_t best[8], best_ok;  // BIAS: largest owned stack per player from gen_buffers.stack_cache, and whether it is current
+    uint32_t rdirty[2];         // cache rows own[0..P-1], army >= 2: bit r * (BW / 8) + s = 32-byte sector s of row r changed
 };
 
 enum : uint32_t {
@@ -53,6 +54,7 @@ enum : uint32_t {
     SG_GROW_EVEN = 1u << 2,  // owned structures +1 this turn
     SG_GROW_TICK = 1u << 3,  // all owned cells +1 this turn
     SG_STATIC_DIRTY = 1u << 4,  // structure / mountain rows changed (regenerated): write them back too
+    SG_ROWS_DIRTY = 1u << 5,    // own / army >= 2 rows changed wholesale (land transfer, 50-turn tick): write them all back
 };
 
 // ================================================================================================
@@ -110,6 +112,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     auto set_bit = [&](uint32_t *r, int c, bool on) {
         const uint32_t bit = 1u << (c & 31);
         if (on) r[c >> 5] |= bit; else r[c >> 5] &= ~bit;
+    };
+    // The dynamic cache rows (own[p], army >= 2) go back to HBM by 32-byte sector, and only the sectors a turn
+    // changed: a move flips a handful of bits.  mark_row: word j of row m of game gs changed.
+    auto mark_row = [&](StepGame &gs, int m, int j) {
+        const int sct = m * (BW >> 3) + (j >> 3);
+        gs.rdirty[sct >> 5] |= 1u << (sct & 31);
+    };
+    auto set_bit_row = [&](StepGame &gs, int lg, int m, int c, bool on) {  // set_bit on row m, recording a change
+        uint32_t *r = row(m, lg);
+        const uint32_t bit = 1u << (c & 31), old = r[c >> 5], now = on ? (old | bit) : (old & ~bit);
+        if (now != old) { r[c >> 5] = now; mark_row(gs, m, c >> 5); }
     };
 
     // ================================================================ prologue
@@ -174,7 +187,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         if (ol < P) { gs.tot[ol] = v_tot; gs.land[ol] = v_land; gs.gcell[ol] = v_gc; }
         if (ol == 0) { gs.turn = v_turn; gs.episode = v_ep; }
         if (ol == 1) { gs.alive = v_alive; gs.done = v_done; gs.winner = v_win; }
-        if (ol == 2) { gs.flags = 0; gs.sat = 0; gs.rew_bits = 0; }
+        if (ol == 2) { gs.flags = 0; gs.sat = 0; gs.rew_bits = 0; gs.rdirty[0] = 0; gs.rdirty[1] = 0; }
         if constexpr (BIAS) {
             const uint32_t v_st = B.stack_cache ? __ldcg(B.stack_cache + (size_t)g * (P + 1) + min(ol, P)) : 0u;
             if (ol < P) gs.best[ol] = v_st;
@@ -384,16 +397,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
             }
             A[cell] = (int16_t)nsrc;
             A[dst] = (int16_t)ndst;
-            set_bit(a2row, cell, nsrc >= 2);
-            set_bit(a2row, dst, ndst >= 2);
+            set_bit_row(gs, lg, R_A2, cell, nsrc >= 2);
+            set_bit_row(gs, lg, R_A2, dst, ndst >= 2);
             if (nown != t) {
                 O[dst] = (int8_t)nown;
-                set_bit(row(nown, lg), dst, true);
+                set_bit_row(gs, lg, nown, dst, true);
                 gs.land[nown] += 1;
-                if (t >= 0) { set_bit(row(t, lg), dst, false); gs.land[t] -= 1; }
+                if (t >= 0) { set_bit_row(gs, lg, t, dst, false); gs.land[t] -= 1; }
             }
             if (captured) {  // a4: land transfer (R11); the general becomes a city
                 const int q = t;
+                gs.flags |= SG_ROWS_DIRTY;
                 Tr[dst] = (int8_t)T_CITY;
                 gs.alive &= ~(1u << q);
                 gs.gcell[q] = -1;
@@ -526,7 +540,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
                 }
                 if (inc) atomicAdd(&gs.tot[p], inc);
             }
-            if (changed) row(R_A2, lg)[j] = a2w;
+            if (changed) {
+                row(R_A2, lg)[j] = a2w;
+                const int sct = R_A2 * (BW >> 3) + (j >> 3);
+                atomicOr(&gs.rdirty[sct >> 5], 1u << (sct & 31));
+            }
         }
     };
 
@@ -673,7 +691,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     // terrain, 8 + 8 bytes.  Every chunk is masked once per player with that player's fog byte and leaves
     // as one 16-byte and three 8-byte streaming stores.
     auto emit_planes = [&](int lg) {
-        constexpr int EB = FIXED ? ((cS / 8 + LPG - 1) / LPG < 9 ? (cS / 8 + LPG - 1) / LPG : 9) : 4;  // chunks per batch
+#ifndef GEN_EB
+#define GEN_EB 9
+#endif
+        constexpr int EB = FIXED ? ((cS / 8 + LPG - 1) / LPG < GEN_EB ? (cS / 8 + LPG - 1) / LPG : GEN_EB) : 4;  // chunks per batch
         const size_t gbase = (size_t)(wg0 + lg) * (size_t)S;
         const size_t obase = gbase * (size_t)P;
         const unsigned char *__restrict__ ga = reinterpret_cast<const unsigned char *>(B.army + gbase) + 16 * ol;
@@ -836,8 +857,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         const int nrows = (gs.flags & SG_STATIC_DIRTY) ? P + 3 : P + 1;  // own[p] + army >= 2 (+ structure, mountain)
         const uint4 *src = reinterpret_cast<const uint4 *>(row(0, sub));
         uint4 *dst = reinterpret_cast<uint4 *>(B.bitboards + (size_t)g * (size_t)(P + 3) * (size_t)BW);
-        if (!frozen)
-            for (int u = ol; u < nrows * BW / 4; u += LPG) dst[u] = src[u];
+        if (!frozen) {
+            const bool all = (gs.flags & (SG_STATIC_DIRTY | SG_ROWS_DIRTY | SG_GROW_TICK)) != 0;  // the tick rewrites army >= 2
+            for (int u = ol; u < nrows * BW / 4; u += LPG)   // 16-byte unit u lies in sector u >> 1 (rows are BW / 8 sectors)
+                if (all || ((gs.rdirty[u >> 6] >> ((u >> 1) & 31)) & 1u)) dst[u] = src[u];
+        }
         if (ol < P) {
             B.land[(size_t)g * P + ol] = gs.land[ol];
             B.army_total[(size_t)g * P + ol] = gs.tot[ol];
