@@ -339,7 +339,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
             if (q < P && bit_of(row(q, lg), c)) t = q;
         return t;
     };
-    auto play_moves = [&](int lg) {
+    // Movers i0 .. i1 - 1 of the turn's order; the call that reaches the last mover also advances the turn counter.
+    auto play_moves = [&](int lg, int i0, int i1) {
         StepGame &gs = s_game[lg];
         const int gg = wg0 + lg;
         int16_t *A = B.army + (size_t)gg * S;
@@ -347,7 +348,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         uint32_t *a2row = row(R_A2, lg);
         const uint32_t *mtn = row(R_MTN, lg);
         const int first = (kp.rule_flags & GEN_RULE_ROTATE_PRIORITY) ? (gs.turn % P) : 0;
-        for (int i = 0; i < P; ++i) {
+        for (int i = i0; i < i1; ++i) {
             int p = first + i;
             if (p >= P) p -= P;
             const int a = gs.act[p];
@@ -440,6 +441,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
                 gs.land[q] = 0;
             }
         }
+        if (i1 < P) return;
         // a6: turn counter; growth itself is applied by the next parallel pass (R1, R2, R3)
         const int turn = gs.turn + 1;
         gs.turn = turn;
@@ -824,9 +826,21 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     }
     __syncwarp();
     GEN_TRACE_MARK(2);  // sampler
-    if (gvalid && ol == 0) {
+    if constexpr (NP > 2) {
+        // One mover per divergent region.  The moves run on one lane per game while the other 28 lanes wait at the
+        // region's convergence barrier; when that wait is long -- eight movers, two dependent L2 round trips each --
+        // the waiting lanes were observed (ncu, k_step<8,32,32>: 16 active threads per instruction from here to the end
+        // of the kernel, every store instruction issued twice and its sectors written in two parts) to be let go and
+        // never to rejoin the moving lanes: __syncwarp() makes them wait for each other but does not merge them.
+        // Short regions reconverge.
+        for (int i = 0; i < P; ++i) {
+            if (gvalid && ol == 0 && !frozen) play_moves(sub, i, i + 1);
+            __syncwarp();
+        }
+        if (gvalid && ol == 0 && frozen) s_game[sub].flags |= SG_FROZEN;
+    } else if (gvalid && ol == 0) {
         if (frozen) s_game[sub].flags |= SG_FROZEN;
-        else play_moves(sub);
+        else play_moves(sub, 0, P);
     }
     __syncwarp();
     GEN_TRACE_MARK(3);  // moves
