@@ -187,11 +187,13 @@ const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, boo
         if ((kind & 1) == 0 && v.ff != (kp.flags & ~gen::F_SAMPLER)) continue;
         if ((kind & 1) == 1 && (v.ff != 0) != (pass == 0)) continue;
         if (!exact) { exact = &v; continue; }
-        // the same kernel under several register budgets (resident CTAs per SM): 14 if only that holds the whole
-        // batch resident in one wave, 12 for smaller batches and while the launches of a multi-wave batch still chain
-        // (launch()), else 10; the closest budget on offer wins, the roomier one on a tie
+        // the same kernel under several register budgets (resident CTAs per SM): 12 for batches below one wave of it,
+        // 14 up to the size where launches stop chaining (launch()) -- only that holds config 2's batch resident in
+        // one wave --, else 10; the closest budget on offer wins, the roomier one on a tie
         const long ctas = (kp.N + 2 * gen::GW - 1) / (2 * gen::GW);
-        const int want = ctas <= 12 * kSMs ? 12 : ctas <= 14 * kSMs ? 14 : ctas <= 8 * 14 * kSMs ? 12 : 10;
+        // (round 2, rotation of replicas, 72- against 80-register build: equal at 24,576 and 32,768 games, 97.2 against
+        // 98.5 us at 65,536, 194.3 against 197.0 us at 131,072 -- so 14 wherever the launches still chain)
+        const int want = ctas <= 12 * kSMs ? 12 : ctas <= 8 * 14 * kSMs ? 14 : 10;
         const int dv = v.min_ctas > want ? v.min_ctas - want : want - v.min_ctas;
         const int de = exact->min_ctas > want ? exact->min_ctas - want : want - exact->min_ctas;
         if (dv < de || (dv == de && v.min_ctas < exact->min_ctas)) exact = &v;
