@@ -131,8 +131,8 @@ def run_reference(args):
         return 0
     import workloads
     cfg, _ = workloads.config(WORKLOAD)
-    sample = 256
-    steps = min(args.steps, 400)
+    sample = 1024                      # config 2's first 1,024 games
+    steps = min(args.steps, 500)
     value, dt = oracle_throughput(cfg, sample, steps, min(args.warmup, 20))
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
