@@ -459,8 +459,8 @@ def run_ours(args):
                 "d2h_bytes_per_step": N * P + N,
                 "best": world * N * K / min(async_reps), "repetitions": len(async_reps),
                 "api": "gen_step_host_async + gen_host_wait(1): pinned host actions read in place, reward + done written "
-                       "to two alternating sets of pinned host arrays, the host reads the results of step t - 1 after "
-                       "issuing step t (no synchronisation per step); the observation planes stay on the device BY "
+                       "by the step kernel into two alternating sets of pinned host arrays, the host reads the results of "
+                       "step t - 1 after issuing step t (no synchronisation per step, no second kernel); the observation planes stay on the device BY "
                        "DESIGN (a GPU-resident learner reads them there: 94 MB per step is no bus traffic to plan for) "
                        "and are not part of the returned result",
                 "synchronised_every_step": {"value": world * N * K / e2e_s, "best": world * N * K / min(e2e_reps),

@@ -233,8 +233,11 @@ int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, vo
 /* End-to-end convenience: HOST actions in (int32 [N][P], may be NULL = sampler), HOST results out
  * (reward int8 [N][P], done uint8 [N]; either may be NULL); runs gen_step on cuda_stream and synchronises that stream
  * before returning.  Pinned (page-locked or registered) host buffers are used in place: the step kernel reads the
- * actions through their device alias and one small kernel writes reward + done into the host arrays -- no
- * copy-engine transfers.  Pageable buffers go through cudaMemcpyAsync (actions via bufs->actions_out, which must
+ * actions through their device alias and writes every game's reward + done to the host arrays as it writes them to
+ * the device buffers (posted writes through the mapped aliases; a second small kernel does it where the staged kernel
+ * serves the step) -- no copy-engine transfers.  h_actions must have been written by the HOST: a step whose actions
+ * sit in pinned host memory chains behind the previous step like one without actions (nothing on the device produced
+ * them).  Pageable buffers go through cudaMemcpyAsync (actions via bufs->actions_out, which must
  * then be non-NULL; it must be non-NULL whenever h_actions is given).  Whether a buffer is pinned is looked up when
  * a pointer is passed for the first time (the handle remembers the last eight); after unregistering or freeing a
  * buffer call gen_forget_host_buffers. */

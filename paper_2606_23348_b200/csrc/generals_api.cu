@@ -30,6 +30,12 @@ struct gen_env {
     cudaEvent_t ev[4];
     int32_t ev_ready;        // events created
     uint64_t async_calls;    // gen_step_host_async calls so far
+    // set by step_host_enqueue around its gen_step call: where k_step also writes reward / done (NULL: nowhere), and
+    // whether the actions it passes were written by the HOST (pinned memory read in place: nothing on the device
+    // produced them, so the launch may chain)
+    int8_t *mirror_reward;
+    uint8_t *mirror_done;
+    int32_t mirror_armed, mirror_done_in_kernel, actions_from_host;
 };
 
 namespace {
@@ -253,10 +259,16 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     // (measured on config 2's boards: chained launches sustain 290 / 490 / 620-660 M env steps/s at 2,048 / 4,096 /
     // 8,192-131,072 games against 118 / 227 / 420-653 M with the grid-wide wait; beyond ~8 waves the waves of one
     // launch mix the phases by themselves and the record's release costs 1-2 %, so those launches keep no records)
+    kp.mirror_reward = nullptr; kp.mirror_done = nullptr;
+    env->mirror_done_in_kernel = 0;
+    if ((v->kind & 1) && env->mirror_armed) {
+        kp.mirror_reward = env->mirror_reward; kp.mirror_done = env->mirror_done;
+        env->mirror_done_in_kernel = 1;
+    }
     kp.count = ((v->kind & 1) && bufs->step_epoch && !env->no_chain && grid <= 8 * 14 * (int)kSMs) ? 1 : 0;
     // A chained launch skips the grid-wide wait, so it may consume nothing a foreign kernel produced: with explicit
     // actions (written by whatever ran before this call) the launch always waits for its stream predecessor.
-    kp.chain = (kp.count && env->chain_buf == bufs->step_epoch && !actions) ? 1 : 0;
+    kp.chain = (kp.count && env->chain_buf == bufs->step_epoch && (!actions || env->actions_from_host)) ? 1 : 0;
     cudaError_t e = v->launch(kp, grid, 32 * kp.WPC, kp.smem_bytes, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) { env->last_cuda_error = (int)e; env->chain_buf = nullptr; return GEN_ERR_CUDA; }
     env->chain_buf = kp.count ? bufs->step_epoch : nullptr;
@@ -468,10 +480,18 @@ static int step_host_enqueue(gen_env *env, const gen_buffers *bufs, const int32_
             d_act = bufs->actions_out;
         }
     }
-    const int e = gen_step(env, bufs, d_act, s);
-    if (e != GEN_OK) return e;
     const bool mirror = N > 0 && (!h_reward || a_rew) && (!h_done || a_done) && (h_reward || h_done);
-    if (mirror) {
+    env->mirror_armed = mirror ? 1 : 0;
+    env->mirror_reward = h_reward ? static_cast<int8_t *>(a_rew) : nullptr;
+    env->mirror_done = h_done ? static_cast<uint8_t *>(a_done) : nullptr;
+    env->actions_from_host = (d_act && d_act == static_cast<const int32_t *>(a_act)) ? 1 : 0;
+    const int e = gen_step(env, bufs, d_act, s);
+    env->mirror_armed = 0;
+    env->actions_from_host = 0;
+    if (e != GEN_OK) return e;
+    if (mirror && env->mirror_done_in_kernel) {
+        // the step kernel has written reward + done to the host arrays as well: nothing to launch
+    } else if (mirror) {
         const size_t bytes = N * P + N;
         const int threads = 256, blocks = (int)((bytes / 16 + threads) / threads < 296 ? (bytes / 16 + threads) / threads : 296);
         // (a plain launch on purpose: as a programmatic dependent launch its CTAs would sit on 13 SMs while the next

@@ -96,6 +96,10 @@ struct KParams {
     gen_buffers b;
     const int32_t *actions;
     int32_t *sample_out;
+    // gen_step_host[_async] on k_step: every game's reward [P] and done are also written to these (device aliases of
+    // pinned host arrays [N][P] / [N]; either may be NULL) by the lane that writes them to the device buffers
+    int8_t *mirror_reward;
+    uint8_t *mirror_done;
     uint32_t notcol0[32], notcolL[32], inb[32];  // column / in-bounds masks of bitboard word j
 };
 

@@ -562,6 +562,16 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         }
         B.done[gg] = (uint8_t)done;
         B.winner[gg] = (int8_t)winner;
+        // gen_step_host[_async] with pinned result arrays: the same values straight to the host (posted writes through
+        // the mapped aliases; the four games of a warp are adjacent, so a warp sends 4 * P + 4 contiguous bytes) --
+        // no second kernel behind the step
+        if (kp.mirror_reward) {
+            int8_t *hr = kp.mirror_reward + (size_t)gg * P;
+            if (P == 2) *reinterpret_cast<uint16_t *>(hr) = (uint16_t)(((uint32_t)(uint8_t)(((rew_bits >> 0) & 3) - 1)) |
+                                                                        ((uint32_t)(uint8_t)(((rew_bits >> 2) & 3) - 1) << 8));
+            else for (int p = 0; p < P; ++p) hr[p] = (int8_t)(((rew_bits >> (2 * p)) & 3) - 1);
+        }
+        if (kp.mirror_done) kp.mirror_done[gg] = (uint8_t)done;
     };
     auto finish_turn = [&](int lg) {
         StepGame &gs = s_game[lg];
