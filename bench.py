@@ -301,7 +301,34 @@ def run_ours(args):
     pair(Wm)
     f_reps, p_reps = timed(only_foreign, K), timed(pair, K)
     f_us, p_us = 1e3 * statistics.median(f_reps) / K, 1e3 * statistics.median(p_reps) / K
-    del foreign
+    # the same with TWO environments on two streams (the usual schedule of a learner with two env batches: the policy
+    # works on one while the other steps): each stream alternates its foreign kernel and its step
+    side = [torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)]
+    foreign2 = torch.empty(24 << 20, dtype=torch.uint8, device=dev)
+    two_envs, two_bufs = [envs[0], envs[1]], [foreign, foreign2]
+
+    def on_two_streams(body):
+        def run(k):
+            cur = torch.cuda.current_stream(dev)
+            for st in side:
+                st.wait_stream(cur)
+            for _ in range(k):
+                for i in range(2):
+                    with torch.cuda.stream(side[i]):
+                        body(i)
+            for st in side:
+                cur.wait_stream(st)
+        return run
+
+    def two_pair(i):
+        two_bufs[i].fill_(3)
+        two_envs[i].step(stream=side[i])
+
+    on_two_streams(two_pair)(Wm)
+    f2_reps = timed(on_two_streams(lambda i: two_bufs[i].fill_(3)), K)
+    p2_reps = timed(on_two_streams(two_pair), K)
+    f2_us, p2_us = 1e3 * statistics.median(f2_reps) / (2 * K), 1e3 * statistics.median(p2_reps) / (2 * K)
+    del foreign, foreign2, two_bufs
 
     # ---- gen_step + gen_features (bfloat16 feature tensor, R37) every turn: the featuriser between two steps
     fenv = envs[1]
@@ -452,6 +479,15 @@ def run_ours(args):
                         "repetitions": len(p_reps),
                         "note": "one environment; a foreign kernel (24 MB fill, the policy stand-in) between two steps, "
                                 "so launches cannot chain; step_us = pair - foreign alone"},
+        "interleaved_two_batches": {"loop_value": world * N / (p2_us * 1e-6), "loop_value_one_batch": world * N / (p_us * 1e-6),
+                                    "unit": UNIT, "pair_us": p2_us, "foreign_us": f2_us, "step_us": p2_us - f2_us,
+                                    "repetitions": len(p2_reps),
+                                    "note": "two environments on two streams, each alternating a foreign kernel (24 MB fill) "
+                                            "and its step -- the schedule of a learner with two env batches: one batch's store "
+                                            "phase runs under the other's foreign kernel and rules.  loop_value = env steps/s of "
+                                            "the whole loop, foreign kernels included (one batch on one stream beside it); "
+                                            "pair_us = time per (foreign + step) pair; step_us = pair - foreign alone attributes "
+                                            "ALL of the overlap to the step and is not a roofline figure"},
         "step_plus_features": {"turn_us": sf_us, "features_us": of_us, "step_us": sf_us - of_us,
                                "value": world * N / (sf_us * 1e-6), "unit": UNIT, "dtype": "bf16 feature tensor (R37)",
                                "note": "gen_step + gen_features every turn (38 channels x 2 players materialised)"},
