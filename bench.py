@@ -555,8 +555,10 @@ def run_single_leg(args):
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     n = {"rollout": 16384, "step": 16384, "step-large": 262144}[args.only]
-    cfg, _ = workloads.config(WORKLOAD, n_games=args.games or n)
+    cfg, _ = workloads.config(args.workload or WORKLOAD, n_games=args.games or n)
     env = GeneralsEnv(cfg, device=dev, digest=(args.only == "rollout"), actions_out=False)
+    if args.force_step:
+        env.set_generic(False, -1)      # the register-resident kernel also where the staged one is the default (P > 4)
     env.reset()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     k = max(4, min(args.steps, 12))
@@ -804,11 +806,12 @@ def main():
     ap.add_argument("--replicas", type=int, default=0, help="replicas in the round-robin (default: enough for 640 MB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-large", action="store_true", help="skip the N = 262,144 leg (roofline_large)")
+    ap.add_argument("--force-step", action="store_true", help="with --only step: k_step also for more than 4 players")
     ap.add_argument("--only", choices=["rollout", "step", "step-large"], default="",
                     help="one leg by itself, a few launches (the command of the ncu captures under profiles/)")
     ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
     ap.add_argument("--rows", default="", help="with --sweep: only the rows whose workload name contains this")
-    ap.add_argument("--workload", default="", help="with --features: workload name (default c2_24x24)")
+    ap.add_argument("--workload", default="", help="with --features / --only: workload name (default c2_24x24)")
     ap.add_argument("--bf16", action="store_true", help="with --features: the bfloat16 feature tensor (R37)")
     ap.add_argument("--features", action="store_true", help="NEXT-1: gen_features alone and with gen_step (one JSON line)")
     args = ap.parse_args()
