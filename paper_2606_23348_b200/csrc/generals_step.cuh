@@ -117,7 +117,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     // changed: a move flips a handful of bits.  mark_row: word j of row m of game gs changed.
     auto mark_row = [&](StepGame &gs, int m, int j) {
         const int sct = m * (BW >> 3) + (j >> 3);
-        gs.rdirty[sct >> 5] |= 1u << (sct & 31);
+        if (FIXED && (NP + 1) * (((cNW + 7) / 8 * 8) >> 3) <= 32) gs.rdirty[0] |= 1u << sct;   // one word holds them all
+        else gs.rdirty[sct >> 5] |= 1u << (sct & 31);
     };
     auto set_bit_row = [&](StepGame &gs, int lg, int m, int c, bool on) {  // set_bit on row m, recording a change
         uint32_t *r = row(m, lg);
@@ -213,9 +214,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
     // As in the staged kernel: the LPP lanes (pl, 0..LPP-1) of the octet serve player pl and split the NW
     // words; the valid list is ordered (direction, cell).  The four "target is free" masks are formed on
     // the fly from the mountain row (sliding window of three words).
-    auto freew = [&](const uint32_t *mtn, int j) -> uint32_t {
-        return ((unsigned)j < (unsigned)NW) ? (~mtn[j] & s_inb[j]) : 0u;
-    };
+    // No bounds test (it compiled to a divergent branch: 6 % of the kernel's instructions at 12 active threads): j runs
+    // from -1 to NW, where s_inb[j] = 0 (guard words at both ends of the table; words past the board are 0 anyway) and
+    // mtn[j] is some word of the warp's own shared memory.
+    auto freew = [&](const uint32_t *mtn, int j) -> uint32_t { return ~mtn[j] & s_inb[j]; };
     auto sample = [&](int lg, uint32_t gstep) -> int {
         const int p = min(pl, P - 1);
         const uint32_t gid = kp.gid_base + (uint32_t)(wg0 + lg);
