@@ -199,7 +199,9 @@ const gen::Variant *pick_variant(const gen_env *env, const gen::KParams &kp, boo
         const long ctas = (kp.N + 2 * gen::GW - 1) / (2 * gen::GW);
         // (round 2, rotation of replicas, 72- against 80-register build: equal at 24,576 and 32,768 games, 97.2 against
         // 98.5 us at 65,536, 194.3 against 197.0 us at 131,072 -- so 14 wherever the launches still chain)
-        const int want = ctas <= 12 * kSMs ? 12 : ctas <= 8 * 14 * kSMs ? 14 : 10;
+        // (beyond that size: four planes 391 us at 10 against 406 us at 14 CTAs per SM for 262,144 games; the packed
+        // observation, with 40 % fewer bytes to store per step, 325 us at 10 against 305 us at 14)
+        const int want = ctas <= 12 * kSMs ? 12 : (ctas <= 8 * 14 * kSMs || kp.b.obs_packed) ? 14 : 10;
         const int dv = v.min_ctas > want ? v.min_ctas - want : want - v.min_ctas;
         const int de = exact->min_ctas > want ? exact->min_ctas - want : want - exact->min_ctas;
         if (dv < de || (dv == de && v.min_ctas < exact->min_ctas)) exact = &v;
