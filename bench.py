@@ -164,7 +164,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     import workloads
-    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, replicas
+    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, OBS_EVERY_STEP, replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -364,6 +364,22 @@ def run_ours(args):
     roll_reps = timed(roll, n_roll)
     roll_value = world * N * 32 * n_roll / (statistics.median(roll_reps) * 1e-3)
     del renv
+    # ---- fused rollout with the planes of EVERY turn written (K = 8 slots): the same output as eight gen_step
+    # launches with the built-in sampler, the state read once per launch
+    KE = 8
+    eenv = GeneralsEnv(replicas.weak_replica_config(cfg, rank), device=dev, k_slots=KE, digest=False, actions_out=False)
+    eenv.reset()
+    eenv.rollout(KE, OBS_EVERY_STEP)
+    n_every = max(2, K // KE)
+
+    def roll_every(k):
+        for _ in range(k):
+            eenv.rollout(KE, OBS_EVERY_STEP)
+
+    every_reps = timed(roll_every, n_every)
+    every_value = world * N * KE * n_every / (statistics.median(every_reps) * 1e-3)
+    every_bytes = bmin - 4 * H * W * (KE - 1) / KE
+    del eenv
 
     # ---- end-to-end leg: host actions in (pinned), gen_step_host, host reward + done out, every step
     env.reset()
@@ -428,6 +444,19 @@ def run_ours(args):
         l_reps = timed(lrot, KL)
         large = summary(l_reps, KL, NL)
         del lenvs
+        torch.cuda.empty_cache()
+        leenv = GeneralsEnv(replicas.weak_replica_config(dict(cfg, n_games=NL), rank), device=dev, k_slots=KE, digest=False,
+                            actions_out=False)
+        leenv.reset()
+        leenv.rollout(KE, OBS_EVERY_STEP)
+
+        def lroll_every(k):
+            for _ in range(k):
+                leenv.rollout(KE, OBS_EVERY_STEP)
+
+        le_reps = timed(lroll_every, 4)
+        large["rollout_every_step"] = world * NL * KE * 4 / (statistics.median(le_reps) * 1e-3)
+        del leenv
         torch.cuda.empty_cache()
 
     # The timed regions above last tens of milliseconds each, nvidia-smi samples every 100 ms: the sampler has seen the
@@ -510,6 +539,13 @@ def run_ours(args):
                                  "inst_source": ROLLOUT_INST_SOURCE,
                                  "achieved": roll_value / world * ROLLOUT_INST_PER_ENV_STEP, "peak": ISSUE_PEAK,
                                  "unit": "warp-inst/s", "frac": roll_value / world * ROLLOUT_INST_PER_ENV_STEP / ISSUE_PEAK}},
+        "rollout_every_step": {"value": every_value, "unit": UNIT, "K": KE, "launches": n_every, "repetitions": len(every_reps),
+                               "obs": "four planes x 2 players of EVERY turn, K-strided slots (what K gen_step launches with "
+                                      "the built-in sampler write)",
+                               "roofline": {"bound": "hbm", "algorithmic_bytes_per_env_step": every_bytes,
+                                            "achieved": every_value / world * every_bytes / 1e9, "peak": peak, "unit": "GB/s",
+                                            "frac": every_value / world * every_bytes / 1e9 / peak,
+                                            "kernel": "gen::k_generals<2, 24, 24, F_OBS_PLANES | F_OBS_EVERY> (gen_rollout)"}},
     }
     if large:
         NL = 262144
@@ -521,7 +557,10 @@ def run_ours(args):
                                   "value": large["value"], "best": large["best"], "units_per_launch": NL,
                                   "avg_launch_us": large["us_per_launch"], "repetitions": large["repetitions"],
                                   "launches_per_repetition": large["launches_per_repetition"],
-                                  "kernel": kname + " (gen_step), 2 replicas of 262,144 games in rotation"}
+                                  "kernel": kname + " (gen_step), 2 replicas of 262,144 games in rotation",
+                                  "rollout_every_step": {"value": large["rollout_every_step"], "unit": UNIT, "K": KE,
+                                                         "frac": large["rollout_every_step"] / world * every_bytes / 1e9 / peak,
+                                                         "note": "gen_rollout(8, GEN_OBS_EVERY_STEP) at the same batch size"}}
     if not args.no_cpu_baseline:
         # config 2's first 1,024 games; 500 turns instead of 2,000 so that the leg stays near 20 s of CPU
         sample, steps = 1024, 500
