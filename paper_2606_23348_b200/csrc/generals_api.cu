@@ -166,6 +166,7 @@ constexpr long kSMs = 148;  // B200
 using gen::F_RUNTIME;
 using gen::F_OBS_PLANES;
 using gen::F_OBS_EVERY;
+using gen::F_RESET;
 using gen::FF_ROLL_DIGEST;
 const gen::Variant kVariants[gen::N_VARIANTS] = {
 #define GEN_ROW(id, kind, np, h, w, ff, maxt, minb) {kind, np, h, w, ff, maxt, minb, gen::launch_variant_##id},
