@@ -42,8 +42,10 @@ constexpr uint32_t FF_ROLL_DIGEST = F_OBS_PLANES | F_DIGEST;     // gen_rollout(
     X(21, 0, 8, 32, 32, F_OBS_PLANES, 256, 1)    \
     X(22, 0, 2, 24, 24, F_OBS_PLANES | F_OBS_EVERY, 256, 1)  \
     X(23, 0, 2, 24, 24, F_RESET | F_OBS_PLANES, 256, 1)      \
-    X(24, 2, 2, 23, 23, F_RESET | F_OBS_PLANES, 256, 1)
-constexpr int N_VARIANTS = 25;
+    X(24, 2, 2, 23, 23, F_RESET | F_OBS_PLANES, 256, 1)      \
+    X(25, 0, 4, 32, 32, F_RESET | F_OBS_PLANES, 256, 1)      \
+    X(26, 0, 8, 32, 32, F_RESET | F_OBS_PLANES, 256, 1)
+constexpr int N_VARIANTS = 27;
 // Variant 21: gen_step of the 8-player free-for-all on 32x32 (BASELINE config 5b) on the staged kernel compiled for
 // that board and mode (more than 4 players stay on the staged kernel, generals_api.cu): 83 -> 101 M env steps/s at
 // 32,768 games (57 -> 69.5 % of the HBM copy peak).  The same for 2v2 (4, 32, 32) was tried and is slower than
@@ -52,6 +54,7 @@ constexpr int N_VARIANTS = 25;
 // steps/s at 16,384 games, 811 -> 944-947 M at 262,144 (the generic kernel served this call before).
 // Variant 23: gen_reset on 24x24 1v1 (synthetic generator + first observation): 108 -> 92 us for 16,384 boards,
 // 196 -> 222 M maps/s at 262,144.  Variant 24: the same for the official generator on 23x23 (118 -> 132 M maps/s).
+// Variants 25 / 26: gen_reset of config 5's boards (2v2: 691 -> 538 us, FFA-8: 1,516 -> 1,250 us for 32,768 boards).
 // Variants 18-20: variants 7 / 17 / 11 for the biased policy (R25; BASELINE config 4): flags = 1 compiles the
 // observation pass that also finds each player's largest owned stack and leaves it in gen_buffers.stack_cache.
 // Kinds 2 / 3 are kinds 0 / 1 compiled with the official map generator (R36; gen_config.map_mode = 1, 1v1 only): the
