@@ -663,6 +663,43 @@ def test_step_host_end_to_end(gpu, oracle_mod, pinned, N):
     assert int(o.episodes_done.sum()) > 0
 
 
+def test_actions_produced_on_the_device_between_chained_steps(gpu, oracle_mod):
+    """a chained gen_step skips the grid-wide wait, so it must never be chained when it consumes actions
+    another kernel produced.  Here a foreign kernel (a torch elementwise op) writes the actions into ONE reused
+    buffer right before every explicit-action step, sampler steps (which do chain) run in between, nothing
+    synchronises the stream: a step that started before its producer had finished would read the previous turn's
+    actions and diverge from the oracle."""
+    import torch
+    N, T = 2048, 36
+    cfg, _ = workloads.config("c2_24x24", n_games=N, max_turns=30)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+    explicit = [t % 3 != 2 for t in range(T)]
+    stream = []                                               # the oracle plays first: its sampled actions are the inputs
+    for t in range(T):
+        if explicit[t]:
+            a = o.sample()
+            stream.append(a)
+            o.step(a)
+        else:
+            stream.append(None)
+            o.step()
+    dev_all = torch.from_numpy(np.stack([a if a is not None else np.zeros((N, 2), np.int32) for a in stream])).to(env.device)
+    acts = torch.zeros((N, 2), dtype=torch.int32, device=env.device)
+    zero = torch.zeros((N, 2), dtype=torch.int32, device=env.device)
+    torch.cuda.synchronize()
+    for t in range(T):
+        if explicit[t]:
+            torch.add(dev_all[t], zero, out=acts)             # the producer: same buffer every time
+            env.step(acts)
+        else:
+            env.step()                                        # built-in sampler: these launches chain
+    compare(env, o, digest=False, where="device-produced actions between chained steps")
+    assert env.last_launch_register_resident and int(o.episodes_done.sum()) > 0
+
+
 def test_step_host_async_one_step_late(gpu, oracle_mod):
     """gen_step_host_async + gen_host_wait: the loop the end-to-end bench leg times -- two sets of pinned host slots,
     step t issued before the results of step t - 1 are read (lag 1), then the last one drained (lag 0); results of
