@@ -663,6 +663,44 @@ def test_step_host_end_to_end(gpu, oracle_mod, pinned, N):
     assert int(o.episodes_done.sum()) > 0
 
 
+def test_checkpoint_and_resume(gpu, oracle_mod):
+    """SURVEY section 5 (checkpoint / resume): the handle holds no game state -- everything lives in the caller's
+    tensors plus the global step -- so cloning the STATE tensors and gen_global_step is a checkpoint.  A fresh handle
+    that is given the cloned state (derived caches rebuilt by gen_observe, nothing else copied) must continue bit for
+    bit like the original and like the oracle, through auto-resets, on the per-step kernel and through a fused
+    rollout."""
+    cfg, _ = workloads.config("c4_curriculum", n_games=150, max_turns=45)
+    env = gpu.GeneralsEnv(cfg, digest=False, history=True)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+    for _ in range(60):
+        env.step()
+        o.step()
+    state = ["army", "owner", "terrain", "turn", "episode", "alive", "general_cell", "done", "winner", "episodes_done",
+             "wins", "truncations", "sat_events", "play_size", "score_hist"]
+    ckpt = {k: env.tensors[k].clone() for k in state}
+    step0 = env.global_step
+    twin = gpu.GeneralsEnv(cfg, digest=False, history=True)    # nothing but the checkpoint goes in
+    for k in state:
+        twin.tensors[k].copy_(ckpt[k])
+    twin.global_step = step0
+    twin.observe()                                              # scoreboard, bitboard cache and observation from the planes
+    for t in range(70):
+        env.step()
+        twin.step()
+        o.step()
+        if t % 10 == 9:
+            compare(env, o, digest=False, where=f"original, step {t}")
+            compare(twin, o, digest=False, where=f"resumed, step {t}")
+    assert np.array_equal(twin.field("score_hist"), env.field("score_hist"))
+    for e in (env, twin):
+        e.rollout(9, gpu.OBS_NONE)
+    o.rollout(9, oracle_mod.OBS_NONE)
+    compare(twin, o, fields=STATE_FIELDS, digest=False, where="resumed, after a rollout")
+    assert twin.last_launch_register_resident is False and int(o.episodes_done.sum()) > 100
+
+
 def test_actions_produced_on_the_device_between_chained_steps(gpu, oracle_mod):
     """a chained gen_step skips the grid-wide wait, so it must never be chained when it consumes actions
     another kernel produced.  Here a foreign kernel (a torch elementwise op) writes the actions into ONE reused
