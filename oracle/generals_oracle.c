@@ -83,6 +83,9 @@ typedef struct {
     uint8_t *obs_packed;      /* [N][P][S] or NULL: owner, terrain and visibility in one byte (R33) */
     int32_t *score_hist;      /* [N][512][2P] or NULL: ring of the public scoreboard per turn (R34) */
     int8_t *play_size;        /* [N][2] or NULL: playable rows, columns of the current map (R36; R35 padded border) */
+    uint32_t *invalid_actions; /* [N] or NULL: diagnostic: actions since reset that were no pass and were not
+                                  applied -- index out of range, not the mover's cell, army < 2, target a mountain or off
+                                  the board, also when an earlier mover of the same turn made them so (R7) */
 } orc_buffers;
 
 /* ------------------------------------------------------------------ Philox
@@ -520,7 +523,12 @@ static void step_game(const orc_config *cfg, const orc_buffers *b, int g, const 
     int first = (cfg->rule_flags & RULE_ROTATE_PRIORITY) ? b->turn[g] % P : 0;
     for (int i = 0; i < P; ++i) {
         int p = (first + i) % P, src, dst, half;
-        if (!decode(cfg, army, owner, terrain, p, actions[p], &src, &dst, &half)) continue;
+        if (!decode(cfg, army, owner, terrain, p, actions[p], &src, &dst, &half)) {
+            const int32_t a = actions[p];
+            const int is_pass = a >= 0 && a < 9 * HW && a % 9 == 0;          /* R22: k = 0 */
+            if (!is_pass && b->invalid_actions) b->invalid_actions[g] += 1;   /* an invalid action is a pass (R5, R10) */
+            continue;
+        }
         int m = half ? army[src] / 2 : army[src] - 1;     /* R4 */
         army[src] = (int16_t)(army[src] - m);
         int t = owner[dst], d = army[dst];
@@ -591,6 +599,7 @@ int32_t orc_reset(const orc_config *cfg, const orc_buffers *b)
         scoreboard(cfg, b, g);
         b->done[g] = 0; b->winner[g] = -1;
         b->episodes_done[g] = 0; b->truncations[g] = 0; b->sat_events[g] = 0;
+        if (b->invalid_actions) b->invalid_actions[g] = 0;
         for (int p = 0; p < P; ++p) { b->reward[g * P + p] = 0; b->wins[g * P + p] = 0; }
         record_history(cfg, b, g);
         observe(cfg, b, g, (size_t)g);

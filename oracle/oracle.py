@@ -45,7 +45,7 @@ _BUF_FIELDS = [
     ("obs_army", np.int16), ("obs_owner", np.int8), ("obs_terrain", np.int8), ("obs_vis", np.uint8),
     ("episodes_done", np.uint32), ("wins", np.uint32), ("truncations", np.uint32),
     ("sat_events", np.uint32), ("obs_digest", np.uint64), ("obs_packed", np.uint8),
-    ("score_hist", np.int32), ("play_size", np.int8),
+    ("score_hist", np.int32), ("play_size", np.int8), ("invalid_actions", np.uint32),
 ]
 
 
@@ -133,7 +133,7 @@ class Oracle:
             "obs_army": (Kb, N, P, S), "obs_owner": (Kb, N, P, S), "obs_terrain": (Kb, N, P, S),
             "obs_vis": (Kb, N, P, S), "episodes_done": (N,), "wins": (N, P), "truncations": (N,),
             "sat_events": (N,), "obs_digest": (N,), "obs_packed": (Kb, N, P, S),
-            "score_hist": (N, 512, 2 * P), "play_size": (N, 2),
+            "score_hist": (N, 512, 2 * P), "play_size": (N, 2), "invalid_actions": (N,),
         }
         self.bufs = OrcBuffers()
         for name, dt in _BUF_FIELDS:

@@ -318,3 +318,35 @@ def test_W13_unclaimed_or_second_general_is_a_castle(oracle_mod):
     o.step([[act(1, 0, 3, DOWN), PASS]])                                         # 5 onto player 1's castle of 1
     assert cell(o, 2, 0) == (CT, 0, 5) and int(o.alive[0]) == 0b11 and int(o.done[0, 0]) == 0   # 4 left, +1 (turn 2)
     assert cell(o, 2, 2) == (GN, 1, 4) and o.land[0].tolist() == [4, 1]
+
+
+def test_invalid_actions_counter_by_hand(oracle_mod):
+    """"Invalid game actions are not errors -- they are passes; a device counter invalid_actions is
+    diagnostic only."  Every kind of rejected non-pass action counts once, passes and applied moves never: worked out
+    by hand on a 3x3 board (player 0: general (0,0) with 5 and a plain cell (1,0) with 1; player 1: general (2,2)
+    with 3 and (1,2) with 4; a mountain at (0,1))."""
+    MT = oracle_mod.T_MOUNTAIN
+    cells = {(0, 0): (GN, 0, 5), (1, 0): (PL, 0, 1), (2, 2): (GN, 1, 3), (1, 2): (PL, 1, 4), (0, 1): (MT, -1, 0)}
+    steps = [
+        ([PASS, PASS], 0),                                            # cell 0, k 0
+        ([4 * 9, 7 * 9], 0),                                          # k = 0 on other cells: still a pass (R22)
+        ([-1, 9 * 9], 2),                                             # both out of range
+        ([act(0, 0, 3, RIGHT), act(1, 2, 3, RIGHT)], 2),              # into the mountain; off the board
+        ([act(1, 0, 3, RIGHT), act(0, 0, 3, DOWN)], 2),               # army 1 < 2; not player 1's cell
+        ([act(0, 0, 3, UP), act(1, 1, 3, LEFT)], 2),                  # off the board; a neutral cell
+        ([act(0, 0, 3, DOWN), act(1, 2, 3, LEFT)], 0),                # both applied
+        ([PASS, act(1, 2, 3, LEFT)], 1),                              # (1,2) was emptied to 1 by the move before
+    ]
+    o = hand_board(oracle_mod, 3, 3, 2, cells, turn=1)
+    total = 0
+    for actions, bad in steps:
+        o.step([actions])
+        total += bad
+        assert int(o.invalid_actions[0]) == total, (actions, int(o.invalid_actions[0]), total)
+    # an action made invalid by an EARLIER mover of the same turn (R7): player 0 takes (1,1) first with 4 > 3,
+    # player 1's move out of (1,1) is then not from its own cell any more
+    o = hand_board(oracle_mod, 3, 3, 2, {(0, 0): (GN, 0, 1), (2, 2): (GN, 1, 1), (1, 0): (PL, 0, 5), (1, 1): (PL, 1, 3)}, turn=1)
+    o.step([[act(1, 0, 3, RIGHT), act(1, 1, 3, UP)]])
+    assert cell(o, 1, 1) == (PL, 0, 1) and int(o.invalid_actions[0]) == 1
+    o.reset()
+    assert int(o.invalid_actions[0]) == 0
