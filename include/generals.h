@@ -125,6 +125,10 @@ typedef struct gen_buffers {
                                 generators (H, W unless map_mode 1 with play_min, R36); gen_features reads it for Table
                                 IV's "known padded border" (0 = not recorded = the full board) */
     uint32_t *stack_cache;   /* state [N][P+1]  largest owned stack per player + validity stamp, may be NULL (see below) */
+    uint32_t *invalid_actions; /* accum [N]  diagnostic, may be NULL: actions since gen_reset that were no pass (R22: k != 0
+                                or an index outside [0, 9 H W)) and were not applied -- not the mover's cell, army < 2,
+                                target a mountain or off the board, also when an earlier mover of the same turn made
+                                them so (R7).  Invalid actions are not errors: they are passes (R5, R10) */
 } gen_buffers;
 
 /* `stack_cache` serves the biased policy (gen_policy.bias_thr, R25: "70 % of moves from the largest owned stack"):
@@ -179,7 +183,7 @@ typedef struct gen_sizes {
     size_t army, owner, terrain, turn, episode, alive, general_cell, land, army_total;
     size_t reward, done, winner, obs_army, obs_owner, obs_terrain, obs_vis;
     size_t episodes_done, wins, truncations, sat_events, obs_digest, actions_out, bitboards, obs_packed, score_hist;
-    size_t step_epoch, play_size, stack_cache;
+    size_t step_epoch, play_size, stack_cache, invalid_actions;
     int32_t bitboard_row_words; /* BW */
 } gen_sizes;
 

@@ -68,6 +68,7 @@ BUFFERS = [
     ("step_epoch", "int32", lambda N, P, S, K: (2, (N + 3) // 4)),                      # bits of uint32
     ("play_size", "int8", lambda N, P, S, K: (N, 2)),
     ("stack_cache", "int32", lambda N, P, S, K: (N, P + 1)),                             # bits of uint32
+    ("invalid_actions", "int32", lambda N, P, S, K: (N,)),                               # bits of uint32
 ]
 
 
@@ -391,7 +392,7 @@ class GeneralsEnv:
                     "obs_packed"):
             t = t[slot]
         a = t.cpu().numpy()
-        if name in ("episode", "episodes_done", "wins", "truncations", "sat_events"):
+        if name in ("episode", "episodes_done", "wins", "truncations", "sat_events", "invalid_actions"):
             a = a.view(np.uint32)
         elif name == "obs_digest":
             a = a.view(np.uint64)

@@ -92,6 +92,7 @@ void fill_sizes(const gen_config *c, int32_t K, gen_sizes *s) {
     s->step_epoch = (N + 3) / 4 * 8;
     s->play_size = N * 2;
     s->stack_cache = N * (P + 1) * 4;
+    s->invalid_actions = N * 4;
 }
 
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -118,6 +119,7 @@ int check_buffers(const gen_buffers *b, bool need_obs) {
     if (b->step_epoch && !aligned16(b->step_epoch)) return GEN_ERR_ALIGN;
     if (b->play_size && !aligned16(b->play_size)) return GEN_ERR_ALIGN;
     if (b->stack_cache && !aligned16(b->stack_cache)) return GEN_ERR_ALIGN;
+    if (b->invalid_actions && !aligned16(b->invalid_actions)) return GEN_ERR_ALIGN;
     return GEN_OK;
 }
 

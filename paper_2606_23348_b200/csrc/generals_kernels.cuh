@@ -775,6 +775,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             gs.dirtyO = 0; gs.dirtyA[0] = 0; gs.dirtyA[1] = 0; gs.rew_bits = 0;
             B.episode[g] = gs.episode;
             B.episodes_done[g] = 0; B.truncations[g] = 0; B.sat_events[g] = 0;
+            if (B.invalid_actions) B.invalid_actions[g] = 0;
             for (int p = 0; p < P; ++p) B.wins[(size_t)g * P + p] = 0;
         }
         __syncwarp();
@@ -909,11 +910,13 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
         const int gg = wg0 + lg;
         const int first = (kp.rule_flags & GEN_RULE_ROTATE_PRIORITY) ? (gs.turn % P) : 0;
         uint32_t dA0 = 0, dA1 = 0, dO = 0, gflags = 0;
+        int bad = 0;  // non-pass actions that are not applied (diagnostic counter invalid_actions)
         for (int i = 0; i < P; ++i) {
             int p = first + i;
             if (p >= P) p -= P;
             const int a = gs.act[p];
-            if (a <= 0 || a >= 9 * HW) continue;
+            if (a == 0) continue;
+            if (a < 0 || a >= 9 * HW) { ++bad; continue; }
             const int cell = (int)(((uint32_t)a * 7282u) >> 16);  // a / 9 for a < 9 * 1024
             const int kk = a - 9 * cell;
             if (kk == 0) continue;
@@ -925,9 +928,9 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             else if (dir == 1) { dst = cell + W; ok = r < H - 1; }
             else if (dir == 2) { dst = cell - 1; ok = col > 0; }
             else { dst = cell + 1; ok = col < W - 1; }
-            if (!ok) continue;
+            if (!ok) { ++bad; continue; }
             const int asrc = A[cell];
-            if (O[cell] != p || asrc < 2 || Tr[dst] == T_MOUNTAIN) continue;
+            if (O[cell] != p || asrc < 2 || Tr[dst] == T_MOUNTAIN) { ++bad; continue; }
             const int m = half ? (asrc >> 1) : (asrc - 1);  // R4
             const int nsrc = asrc - m;
             const int t = O[dst], d = A[dst];
@@ -989,6 +992,7 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
             }
         }
         // a6: turn counter; growth itself is applied by the next parallel pass (R1, R2, R3)
+        if (bad && B.invalid_actions) B.invalid_actions[gg] += (uint32_t)bad;
         const int turn = gs.turn + 1;
         gs.turn = turn;
         if ((turn & 1) == 0) gflags |= GF_GROW_EVEN;

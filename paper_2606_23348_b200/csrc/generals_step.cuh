@@ -350,11 +350,13 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         uint32_t *a2row = row(R_A2, lg);
         const uint32_t *mtn = row(R_MTN, lg);
         const int first = (kp.rule_flags & GEN_RULE_ROTATE_PRIORITY) ? (gs.turn % P) : 0;
+        int bad = 0;  // non-pass actions that are not applied (diagnostic counter invalid_actions)
         for (int i = i0; i < i1; ++i) {
             int p = first + i;
             if (p >= P) p -= P;
             const int a = gs.act[p];
-            if (a <= 0 || a >= 9 * HW) continue;
+            if (a == 0) continue;
+            if (a < 0 || a >= 9 * HW) { ++bad; continue; }
             const int cell = (int)(((uint32_t)a * 7282u) >> 16);  // a / 9 for a < 9 * 1024
             const int kk = a - 9 * cell;
             if (kk == 0) continue;
@@ -366,9 +368,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
             else if (dir == 1) { dst = cell + W; ok = r < H - 1; }
             else if (dir == 2) { dst = cell - 1; ok = col > 0; }
             else { dst = cell + 1; ok = col < W - 1; }
-            if (!ok) continue;
+            if (!ok) { ++bad; continue; }
             // R5, R10: own the source, army >= 2 (the row is exact), target no mountain
-            if (!bit_of(row(p, lg), cell) || !bit_of(a2row, cell) || bit_of(mtn, dst)) continue;
+            if (!bit_of(row(p, lg), cell) || !bit_of(a2row, cell) || bit_of(mtn, dst)) { ++bad; continue; }
             const int asrc = __ldcg(A + cell), d = __ldcg(A + dst);
             const int m = half ? (asrc >> 1) : (asrc - 1);  // R4
             const int nsrc = asrc - m;
@@ -443,6 +445,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
                 gs.land[q] = 0;
             }
         }
+        if (bad && B.invalid_actions) B.invalid_actions[gg] += (uint32_t)bad;
         if (i1 < P) return;
         // a6: turn counter; growth itself is applied by the next parallel pass (R1, R2, R3)
         const int turn = gs.turn + 1;

@@ -2,7 +2,7 @@
 import numpy as np
 
 STATE_FIELDS = ["army", "owner", "terrain", "turn", "episode", "alive", "general_cell", "land",
-                "army_total", "episodes_done", "wins", "truncations", "sat_events", "play_size"]
+                "army_total", "episodes_done", "wins", "truncations", "sat_events", "play_size", "invalid_actions"]
 OUT_FIELDS = ["reward", "done", "winner", "obs_army", "obs_owner", "obs_terrain", "obs_vis"]
 
 UP, DOWN, LEFT, RIGHT = 0, 1, 2, 3

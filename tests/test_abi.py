@@ -34,8 +34,8 @@ def binding_err(name):
 
 def test_struct_layouts_match_header():
     assert C.sizeof(binding.GenConfig) == 13 * 4 + 3 * 4 + 8 + 4 * 4
-    assert C.sizeof(binding.GenBuffers) == 28 * 8
-    assert C.sizeof(binding.GenSizes) == 8 + 28 * C.sizeof(C.c_size_t) + 8      # + bitboard_row_words, padding
+    assert C.sizeof(binding.GenBuffers) == 29 * 8
+    assert C.sizeof(binding.GenSizes) == 8 + 29 * C.sizeof(C.c_size_t) + 8      # + bitboard_row_words, padding
     assert C.sizeof(binding.GenFeatBuffers) == 6 * 8
     assert C.sizeof(binding.GenFeatSizes) == 8 + 7 * C.sizeof(C.c_size_t)
 

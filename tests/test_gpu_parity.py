@@ -678,7 +678,7 @@ def test_checkpoint_and_resume(gpu, oracle_mod):
         env.step()
         o.step()
     state = ["army", "owner", "terrain", "turn", "episode", "alive", "general_cell", "done", "winner", "episodes_done",
-             "wins", "truncations", "sat_events", "play_size", "score_hist"]
+             "wins", "truncations", "sat_events", "invalid_actions", "play_size", "score_hist"]
     ckpt = {k: env.tensors[k].clone() for k in state}
     step0 = env.global_step
     twin = gpu.GeneralsEnv(cfg, digest=False, history=True)    # nothing but the checkpoint goes in
