@@ -709,7 +709,7 @@ def run_sweep(args):
         out = {"workload": name, "reset_us": 1e3 * reset_ms, "maps_per_s": N / (reset_ms * 1e-3), "obs_format": "army + packed byte (R33)" if packed else "4 planes", "n_games": N, "n_players": P, "board": f"{H}x{W}", "replicas_in_rotation": R,
                "steps": K, "algorithmic_bytes_per_env_step": bmin}
         for graph in (False, True):
-            ms = time_steps(torch, envs, K, max(args.warmup, R), graph)
+            ms = statistics.median(time_steps(torch, envs, K, max(args.warmup, R), graph) for _ in range(5))
             key = "step_graph" if graph else "step"
             out[key] = {"env_steps_per_s": N * K / (ms * 1e-3), "us_per_launch": 1e3 * ms / K,
                         "hbm_frac": N * bmin / (ms / K * 1e-3) / 1e9 / peak}
