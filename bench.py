@@ -600,7 +600,7 @@ def run_single_leg(args):
         env.set_generic(False, -1)      # the register-resident kernel also where the staged one is the default (P > 4)
     env.reset()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    k = max(4, min(args.steps, 12))
+    k = max(4, min(args.steps, 400))
     for _ in range(3):
         env.rollout(32, OBS_DIGEST) if args.only == "rollout" else env.step()
     torch.cuda.synchronize()

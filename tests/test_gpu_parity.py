@@ -738,19 +738,26 @@ def test_actions_produced_on_the_device_between_chained_steps(gpu, oracle_mod):
     assert env.last_launch_register_resident and int(o.episodes_done.sum()) > 0
 
 
-def test_step_host_async_one_step_late(gpu, oracle_mod):
+@pytest.mark.parametrize("name,N,over", [
+    ("c2_24x24", 203, dict(max_turns=40)),
+    ("c5a_2v2", 37, dict(height=12, width=12, n_cities=3, spawn_dmin=4, max_turns=30)),     # P = 4: byte-wise reward writes
+    ("c5b_ffa8", 21, dict(height=12, width=13, n_players=3, spawn_dmin=4, n_cities=4, max_turns=30)),
+])
+def test_step_host_async_one_step_late(gpu, oracle_mod, name, N, over):
     """gen_step_host_async + gen_host_wait: the loop the end-to-end bench leg times -- two sets of pinned host slots,
     step t issued before the results of step t - 1 are read (lag 1), then the last one drained (lag 0); results of
-    every step equal the oracle's, state equal at the end; forgetting the alias table in between changes nothing."""
+    every step equal the oracle's, state equal at the end; forgetting the alias table in between changes nothing.
+    The step kernel writes reward + done to the host arrays itself (2, 3 and 4 players: the reward row is written
+    as one halfword or byte by byte)."""
     import torch
-    N = 203
-    cfg, _ = workloads.config("c2_24x24", n_games=N, max_turns=40)
+    cfg, _ = workloads.config(name, n_games=N, **over)
+    P = cfg["n_players"]
     env = gpu.GeneralsEnv(cfg, digest=False)
     o = oracle_mod.Oracle(cfg)
     env.reset()
     o.reset()
-    slots = [dict(a=torch.zeros((N, 2), dtype=torch.int32).pin_memory(), r=torch.zeros((N, 2), dtype=torch.int8).pin_memory(),
-                  d=torch.zeros((N,), dtype=torch.uint8).pin_memory()) for _ in range(2)]
+    slots = [dict(a=torch.zeros((N, P), dtype=torch.int32).pin_memory(), r=torch.full((N, P), 99, dtype=torch.int8).pin_memory(),
+                  d=torch.full((N,), 99, dtype=torch.uint8).pin_memory()) for _ in range(2)]
     want = []
     T = 90
     for t in range(T):
@@ -771,6 +778,12 @@ def test_step_host_async_one_step_late(gpu, oracle_mod):
     assert np.array_equal(p["r"].numpy(), want[-1][0]) and np.array_equal(p["d"].numpy(), want[-1][1])
     compare(env, o, digest=False, where="step_host_async")
     assert env.last_launch_register_resident and int(o.episodes_done.sum()) > 0
+    n_before = env.launch_count
+    env.step_host_async(None, slots[0]["r"], slots[0]["d"])       # sampler + host results: still one launch (no mirror kernel)
+    env.host_wait(0)
+    o.step()
+    assert env.launch_count == n_before + 1
+    assert np.array_equal(slots[0]["r"].numpy(), o.reward[0]) and np.array_equal(slots[0]["d"].numpy(), o.done[0])
     with pytest.raises(gpu.GenError):
         env.host_wait(4)
 
