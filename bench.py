@@ -153,7 +153,7 @@ def run_reference(args):
 MIN_REGION_MS, MIN_REPS, MAX_REPS = 50.0, 5, 60
 # warp-instructions per env step of the fused rollout kernel (gen_rollout(32, GEN_OBS_DIGEST), 24x24 1v1):
 # smsp__inst_executed.sum / (N * K) of the ncu capture summarised in the file named beside it
-ROLLOUT_INST_PER_ENV_STEP = 550.9
+ROLLOUT_INST_PER_ENV_STEP = 659.4
 ROLLOUT_INST_SOURCE = "profiles/r02_rollout_summary.txt"
 ISSUE_PEAK = 148 * 4 * 1.965e9      # warp-instructions/s: 148 SMs x 4 schedulers x 1 per clock x 1.965 GHz
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_step at N = 262,144 (ncu --set full), by games per launch

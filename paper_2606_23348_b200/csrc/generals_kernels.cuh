@@ -76,7 +76,6 @@ struct GameS {
     unsigned long long digest;
     int32_t tot[8], land[8], act[8];
     int32_t rew_bits, pad_;
-    uint8_t vlist[128];  // digest: the 8-cell chunks some player sees this turn, compacted (chunk indices)
 };
 
 struct KParams {
@@ -1222,40 +1221,20 @@ __global__ void __launch_bounds__(256) k_generals(const __grid_constant__ KParam
     // x * key_lo (one wide multiply-add) and a 32-bit sum of x * key_hi (one multiply-add) of x-or-0 by the player's
     // fog bit -- no 64-bit product is formed and then added under a predicate twice (inline PTX: the compiler
     // turns every other spelling back into that).
-    // The chunks are compacted first: with the fog over two thirds of the board, a lane that walks its nine chunks in
-    // step with the other 31 runs the (converged) loop body in almost every iteration for the few lanes that have
-    // something to add; with the visible chunks of a game dealt out densely to its octet the body runs about half as
-    // often.  Pass 1 (every lane of the warp, also for games that do not take part): one ballot per group of eight
-    // chunks, ranks by popcount, chunk indices into gs.vlist.
     auto chain_digest = [&](int lg, bool active) {
         uint64_t h[NP];
 #pragma unroll
         for (int p = 0; p < NP; ++p) h[p] = 0;
-        uint8_t *vl = s_game[lg].vlist;
-        int nvis = 0;
-        for (int c0 = 0; c0 < NC8; c0 += LPG) {
-            const int ch = c0 + ol;
-            uint32_t any = 0;
-            if (active && ch < NC8) {
-#pragma unroll
-                for (int p = 0; p < NP; ++p)
-                    if (p < P) any |= mrow8(R_VIS + p, lg)[ch];
-            }
-            const uint32_t mine = (__ballot_sync(FULL, any != 0) >> (LPG * lg)) & ((1u << LPG) - 1u);
-            if (any) vl[nvis + __popc(mine & ((1u << ol) - 1u))] = (uint8_t)ch;
-            nvis += __popc(mine);
-        }
-        __syncwarp();
         if (active) {
             uint64_t lo[NP];
             uint32_t hi[NP];
 #pragma unroll
             for (int p = 0; p < NP; ++p) { lo[p] = 0; hi[p] = 0; }
-            for (int k = ol; k < nvis; k += LPG) {
-                const int ch = vl[k];
-                uint32_t vb[NP];
+            for (int ch = ol; ch < NC8; ch += LPG) {
+                uint32_t vb[NP], any = 0;
 #pragma unroll
-                for (int p = 0; p < NP; ++p) vb[p] = (p < P) ? mrow8(R_VIS + p, lg)[ch] : 0u;
+                for (int p = 0; p < NP; ++p) { vb[p] = (p < P) ? mrow8(R_VIS + p, lg)[ch] : 0u; any |= vb[p]; }
+                if (any == 0) continue;
                 const uint4 a = *reinterpret_cast<const uint4 *>(s_army + (size_t)lg * S + 8 * ch);
                 const uint2 o = *reinterpret_cast<const uint2 *>(s_owner + (size_t)lg * S + 8 * ch);
                 const uint2 t = *reinterpret_cast<const uint2 *>(s_terr + (size_t)lg * S + 8 * ch);
