@@ -39,7 +39,8 @@ enum {
     GEN_ERR_CONFIG = -2,  /* H/W/P/team_size out of range, lo > hi, infeasible counts */
     GEN_ERR_ALIGN = -3,   /* a device pointer is not 16-byte aligned */
     GEN_ERR_ARG = -4,     /* K <= 0, unknown flag, missing buffer for the requested mode */
-    GEN_ERR_CUDA = -5     /* launch / runtime error (cudaGetLastError captured; see gen_last_cuda_error) */
+    GEN_ERR_CUDA = -5,    /* launch / runtime error (cudaGetLastError captured; see gen_last_cuda_error) */
+    GEN_ERR_SIZE = -6     /* gen_step_noalloc: the batch needs more than GEN_NOALLOC_SCRATCH_BYTES of built-in scratch */
 };
 
 /* rule_flags: alternative readings of the paper, honoured by both sides (R2, R11, R6) */
@@ -219,6 +220,39 @@ int gen_reset(gen_env *env, const gen_buffers *bufs, uint32_t flags, void *cuda_
  * winner, the four observation planes per player, actions_out / obs_digest if given.
  * global_step += 1. */
 int gen_step(gen_env *env, const gen_buffers *bufs, const int32_t *d_actions, void *cuda_stream);
+
+/* gen_step for callers that cannot allocate device memory.
+ *
+ * The fast path of gen_step (the register-resident kernel) wants `bufs->bitboards`: working memory that is neither
+ * input nor result, which a caller normally allocates once.  Not every caller can.  If your code runs as an operator
+ * inside another system's executor (a custom call of a compiled graph, a runtime plug-in) you are given operands and
+ * results and no workspace, and you must not call the CUDA allocator yourself; if the learner took all of HBM at
+ * start-up, a later cudaMalloc fails; and in an actor loop that must not stall, cudaMalloc / cudaFree are off the
+ * table because they synchronise the whole device.  This call is for those cases: it plays one turn exactly like
+ * gen_step (same arguments, same outputs, same global_step += 1, bit-identical results) and takes the cache from a
+ * fixed array inside the library instead -- GEN_NOALLOC_SCRATCH_BYTES of device memory that every GPU holds from the
+ * moment the library is loaded on it until the process ends.  It calls no cudaMalloc, no cudaFree and no library
+ * routine that allocates.
+ *   - You still pass every input and output in `bufs`.  `bufs->bitboards`, `step_epoch` and `stack_cache` are ignored
+ *     (leave them NULL); `bufs->obs_digest` must be NULL and n_players <= 4 (GEN_ERR_ARG otherwise: those steps run
+ *     the staged kernel, which needs no cache -- plain gen_step with bitboards = NULL already allocates nothing).
+ *   - Limit: n_games * (n_players + 3) * bitboard_row_words * 4 bytes must fit the array, i.e. 17,476 games of 24x24
+ *     1v1, 6,553 of 32x32 2v2.  A larger batch is refused with GEN_ERR_SIZE before anything is launched; split it
+ *     into several handles (game_id_base) and call them one after the other on one stream.
+ *   - The array is shared by every handle and every call in the process and keeps whatever the last call left in it.
+ *     That is harmless by construction: each call first rewrites, from your planes, every word the step will read
+ *     (one extra small kernel, about 4 bytes read per cell), so nothing has to be cleared and nothing stale is ever
+ *     used.  But two calls that run on the GPU AT THE SAME TIME (different streams, different threads, different
+ *     handles) write the same array and corrupt each other: keep all gen_step_noalloc calls of a process on one
+ *     stream, or order them with events.
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ *     current -- so call it with the device you will run on selected).  Make that first call during start-up, before
+ *     any stream capture begins.  Later calls on the device only read the remembered address.
+ *   - Launches are never chained (each waits for its stream predecessor) and the build pass costs extra traffic, so
+ *     callers who CAN allocate should keep using gen_step with their own buffers: this is the slower of the two.
+ * Errors as gen_step, plus GEN_ERR_SIZE and GEN_ERR_ARG above; GEN_ERR_CUDA if the address look-up or a launch fails. */
+#define GEN_NOALLOC_SCRATCH_BYTES (8u << 20)
+int gen_step_noalloc(gen_env *env, const gen_buffers *bufs, const int32_t *d_actions, void *cuda_stream);
 
 /* a13: K sampled turns in ONE launch, the board resident in shared memory throughout (R28).
  * flags: one of GEN_OBS_DIGEST / GEN_OBS_EVERY_STEP / GEN_OBS_NONE.  EVERY_STEP needs buffers sized

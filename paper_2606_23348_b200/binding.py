@@ -12,9 +12,11 @@ LIB_PATH = os.path.join(HERE, "libgenerals.so")
 OBS_DIGEST, OBS_EVERY_STEP, OBS_NONE = 0, 1, 2
 GEN_KEEP_EPISODE = 1
 RULE_TICK_PLAIN_ONLY, RULE_CAPTURE_HALF_FLOOR, RULE_ROTATE_PRIORITY = 1, 2, 4
+GEN_ERR_SIZE = -6
+NOALLOC_SCRATCH_BYTES = 8 << 20     # GEN_NOALLOC_SCRATCH_BYTES: the array behind gen_step_noalloc
 
 EXPORTS = ["gen_query_sizes", "gen_init", "gen_set_policy", "gen_set_spawn", "gen_global_step", "gen_set_global_step",
-           "gen_reset", "gen_step", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host",
+           "gen_reset", "gen_step", "gen_step_noalloc", "gen_rollout", "gen_observe", "gen_sample", "gen_step_host",
            "gen_step_host_async", "gen_host_wait", "gen_forget_host_buffers",
            "gen_query_feat_sizes", "gen_features", "gen_history_windows",
            "gen_set_launch", "gen_set_generic", "gen_set_chaining", "gen_last_variant",
@@ -126,6 +128,8 @@ def load_library(path=None):
     lib.gen_set_global_step.argtypes = [env_p, C.c_uint32]
     lib.gen_reset.argtypes = [env_p, C.POINTER(GenBuffers), C.c_uint32, C.c_void_p]
     lib.gen_step.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
+    lib.gen_step_noalloc.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
+    lib.gen_step_noalloc.restype = C.c_int
     lib.gen_rollout.argtypes = [env_p, C.POINTER(GenBuffers), C.c_int32, C.c_uint32, C.c_void_p]
     lib.gen_observe.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p]
     lib.gen_sample.argtypes = [env_p, C.POINTER(GenBuffers), C.c_void_p, C.c_void_p]
@@ -312,6 +316,17 @@ class GeneralsEnv:
         code = self.lib.gen_step(self._env, self._bufs_ref, ptr, self._stream(stream))
         if code != 0:
             self._check(code)
+
+    def step_noalloc(self, actions=None, stream=None):
+        """gen_step_noalloc: step() for callers that cannot allocate device memory -- the bitboard cache comes from a
+        fixed 8 MiB array inside the library (see include/generals.h for who needs this, the size limit and the rule
+        that such calls must not overlap on the GPU).  Build the env with bitboards=False, digest=False."""
+        ptr = None
+        if actions is not None:
+            assert actions.is_cuda and actions.dtype == self.torch.int32 and actions.is_contiguous()
+            assert actions.numel() == self.N * self.P
+            ptr = C.c_void_p(actions.data_ptr())
+        self._check(self.lib.gen_step_noalloc(self._env, self._bufs_ref, ptr, self._stream(stream)))
 
     def rollout(self, K, obs_mode=OBS_DIGEST, stream=None):
         if obs_mode == OBS_EVERY_STEP and K > self.K:

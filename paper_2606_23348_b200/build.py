@@ -19,7 +19,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgenerals.so")
 DEPS = [os.path.join(CSRC, f) for f in ("generals_api.cu", "generals_variant.cu", "generals_variants.h",
                                         "generals_kernels.cuh", "generals_step.cuh", "generals_features.cu",
-                                        "generals_features.h")] + [os.path.join(ROOT, "include", "generals.h")]
+                                        "generals_features.h", "generals_noalloc.cu")] + [os.path.join(ROOT, "include", "generals.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 
@@ -46,6 +46,7 @@ def build(force=False, verbose=False):
         base += ["-Xptxas", "-v"]
     jobs = [(base + ["-c", os.path.join(CSRC, "generals_api.cu"), "-o", os.path.join(OBJ, "api.o")])]
     jobs.append(base + ["-c", os.path.join(CSRC, "generals_features.cu"), "-o", os.path.join(OBJ, "features.o")])
+    jobs.append(base + ["-c", os.path.join(CSRC, "generals_noalloc.cu"), "-o", os.path.join(OBJ, "noalloc.o")])
     for i in range(n_variants()):
         jobs.append(base + [f"-DGEN_VARIANT_ID={i}", "-c", os.path.join(CSRC, "generals_variant.cu"),
                             "-o", os.path.join(OBJ, f"variant{i}.o")])

@@ -321,6 +321,12 @@ uint64_t host_mix64(uint64_t z) {  // splitmix64 finaliser: the digest keys of R
 
 }  // namespace
 
+namespace gen {
+// for generals_noalloc.cu, to which gen_env is an opaque type: the handle's configuration and its launch counter
+const gen_config *env_config(const gen_env *env) { return &env->cfg; }
+void env_count_launch(gen_env *env) { env->launches += 1; }
+}  // namespace gen
+
 extern "C" {
 
 int gen_query_sizes(const gen_config *cfg, int32_t k_slots, gen_sizes *out) {
@@ -668,6 +674,7 @@ const char *gen_error_string(int code) {
         case GEN_ERR_ALIGN: return "device pointer not 16-byte aligned";
         case GEN_ERR_ARG: return "invalid argument";
         case GEN_ERR_CUDA: return "CUDA runtime error (see gen_last_cuda_error)";
+        case GEN_ERR_SIZE: return "batch too large for the built-in scratch of gen_step_noalloc (GEN_NOALLOC_SCRATCH_BYTES)";
         default: return "unknown error code";
     }
 }

@@ -29,7 +29,8 @@ def test_exports_every_declared_symbol(lib):
 
 
 def binding_err(name):
-    return {"GEN_ERR_NULL": -1, "GEN_ERR_CONFIG": -2, "GEN_ERR_ALIGN": -3, "GEN_ERR_ARG": -4, "GEN_ERR_CUDA": -5}[name]
+    return {"GEN_ERR_NULL": -1, "GEN_ERR_CONFIG": -2, "GEN_ERR_ALIGN": -3, "GEN_ERR_ARG": -4, "GEN_ERR_CUDA": -5,
+            "GEN_ERR_SIZE": -6}[name]
 
 
 def test_struct_layouts_match_header():
@@ -118,8 +119,42 @@ def test_init_argument_errors_without_gpu(lib):
     assert lib.gen_history_windows(env, C.byref(bufs), 0x1008, None) == -3        # misaligned output
     bufs.score_hist = None
     assert lib.gen_history_windows(env, C.byref(bufs), 0x1000, None) == -1        # the ring is required
-    for code in (0, -1, -2, -3, -4, -5, -99):
+    for code in (0, -1, -2, -3, -4, -5, -6, -99):
         assert lib.gen_error_string(code)
+    lib.gen_destroy(env)
+
+
+def test_step_noalloc_argument_errors_without_gpu(lib):
+    """gen_step_noalloc refuses what it cannot serve before it touches the device: missing pointers, a batch beyond
+    its built-in 8 MiB scratch array (GEN_ERR_SIZE), a digest buffer or more than four players (GEN_ERR_ARG)."""
+    assert binding.NOALLOC_SCRATCH_BYTES == 8 << 20
+    header = open(os.path.join(ROOT, "include", "generals.h")).read()
+    assert "#define GEN_NOALLOC_SCRATCH_BYTES (8u << 20)" in header and "GEN_ERR_SIZE = -6" in header
+    bufs = binding.GenBuffers()                                       # all NULL
+    for over, want in ((dict(n_games=17476), "GEN_ERR_NULL"),         # fits; the planes are missing
+                       (dict(n_games=17477), "GEN_ERR_SIZE"),
+                       (dict(n_games=1 << 20), "GEN_ERR_SIZE")):
+        cfg, _ = binding.make_config(workloads.config("c2_24x24", **over)[0])
+        env = C.c_void_p()
+        assert lib.gen_init(C.byref(cfg), C.byref(env)) == 0
+        assert lib.gen_step_noalloc(env, C.byref(bufs), None, None) == binding_err(want)
+        assert lib.gen_step_noalloc(env, None, None, None) == binding_err("GEN_ERR_NULL")
+        assert lib.gen_global_step(env) == 0 and lib.gen_launch_count(env) == 0
+        lib.gen_destroy(env)
+    assert lib.gen_step_noalloc(None, C.byref(bufs), None, None) == binding_err("GEN_ERR_NULL")
+    cfg, _ = binding.make_config(workloads.config("c5b_ffa8", n_games=8)[0])
+    env = C.c_void_p()
+    assert lib.gen_init(C.byref(cfg), C.byref(env)) == 0
+    assert lib.gen_step_noalloc(env, C.byref(bufs), None, None) == binding_err("GEN_ERR_ARG")     # 8 players
+    lib.gen_destroy(env)
+    cfg, _ = binding.make_config(workloads.config("c1_8x8")[0])
+    assert lib.gen_init(C.byref(cfg), C.byref(env)) == 0
+    bufs.obs_digest = 0x1000
+    assert lib.gen_step_noalloc(env, C.byref(bufs), None, None) == binding_err("GEN_ERR_ARG")     # digest buffer
+    bufs.obs_digest = None
+    bufs.army, bufs.owner, bufs.terrain = 0x1000, 0x1008, 0x1000
+    assert lib.gen_step_noalloc(env, C.byref(bufs), None, None) == binding_err("GEN_ERR_ALIGN")
+    assert b"GEN_NOALLOC_SCRATCH_BYTES" in lib.gen_error_string(-6)
     lib.gen_destroy(env)
 
 
