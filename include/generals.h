@@ -136,9 +136,11 @@ typedef struct gen_buffers {
  * the per-step kernel's observation pass holds every army value in registers anyway, so it leaves each player's
  * largest owned stack of the state it emits -- ((army + 1) << 10 | (1023 - cell)), ties to the lowest cell, 0 = owns
  * nothing -- in [g][p] and the global step at which that state will be sampled in [g][P]; the next gen_step's
- * sampler takes it from there instead of scanning the army plane.  Derived state like `bitboards`: a stamp that does
- * not match (after gen_reset, gen_rollout, a staged-kernel step, gen_set_global_step) sends the sampler back to the
- * scan, so it is never stale.  Allocate it zeroed.  Results do not depend on it. */
+ * sampler takes it from there instead of scanning the army plane.  Derived state like `bitboards`: the sampler reads
+ * it only when the handle's previous launch was such a step on this buffer, one global step ago (the handle keeps
+ * track; the stamp is a second, per-game check) -- after gen_reset, gen_rollout, gen_observe, a staged-kernel step, a
+ * step with explicit actions or gen_set_global_step, and on a fresh handle, it goes back to the scan -- so it is never
+ * stale.  Allocate it zeroed.  Results do not depend on it. */
 
 /* `step_epoch` lets consecutive gen_step launches of one handle overlap.  Without it a launch starts working only
  * when the whole previous grid in the stream has completed (griddepcontrol.wait); the batch then moves through the
@@ -277,14 +279,16 @@ int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, vo
  * sit in pinned host memory chains behind the previous step like one without actions (nothing on the device produced
  * them).  Pageable buffers go through cudaMemcpyAsync (actions via bufs->actions_out, which must
  * then be non-NULL; it must be non-NULL whenever h_actions is given).  Whether a buffer is pinned is looked up when
- * a pointer is passed for the first time (the handle remembers the last eight); after unregistering or freeing a
- * buffer call gen_forget_host_buffers. */
+ * a pinned pointer is passed for the first time (the handle remembers the last eight action arrays and the last eight
+ * result arrays; pageable pointers are looked up every call); after unregistering or freeing a pinned buffer call
+ * gen_forget_host_buffers. */
 int gen_step_host(gen_env *env, const gen_buffers *bufs, const int32_t *h_actions, int8_t *h_reward,
                   uint8_t *h_done, void *cuda_stream);
 
 /* The same without the synchronisation: enqueues the step (and the transfer of reward + done) and returns.  The
  * results of the call issued `lag` calls before the latest one are in their host arrays once gen_host_wait(env, lag)
- * has returned (lag 0 = the latest call; at most 4 calls may be in flight, lag <= 3).  An RL loop waits one step
+ * has returned (lag 0 = the latest call; at most 4 calls may be in flight, lag <= 3: a fifth call first waits, inside
+ * gen_step_host_async, for the oldest one nobody has waited for).  An RL loop waits one step
  * late -- issue step t with one pair of host slots, then wait for step t - 1 and read the other pair -- so that the
  * GPU always has the next step queued and no launch latency or host wake-up sits between two steps.  Until its wait
  * has returned a call OWNS its three host arrays: pinned actions are read in place when the kernel runs, so they

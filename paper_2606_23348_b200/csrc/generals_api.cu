@@ -21,15 +21,24 @@ struct gen_env {
     int32_t last_variant;    // index into GEN_VARIANTS of the last launch (-1: none yet)
     const uint32_t *chain_buf;  // non-NULL: the last launch of this handle was a k_step that kept records there
     int32_t no_chain;        // tests: never chain
+    // non-NULL: the last launch of this handle was a BIAS k_step that left every player's largest stack there, for the
+    // state that will be sampled at global step stack_step.  Any other launch, gen_set_global_step or a failed launch
+    // clears it: the device-side stamp alone can match again after gen_reset or gen_set_global_step.
+    const uint32_t *stack_buf;
+    uint32_t stack_step;
     // gen_step_host / gen_step_host_async: host pointers looked up so far and their device aliases (nullptr:
     // pageable memory); a small table, so that double-buffered host slots do not look up again every call
-    const void *hp_key[8];
-    void *hp_dev[8];
-    int32_t hp_used, hp_next;
+    // Two tables of eight: [0] action arrays (a caller may pass a new one every step), [1] result arrays -- so that a
+    // stream of action pointers never evicts the reward / done entries.  Only pinned buffers are remembered: a
+    // pageable one is looked up again each call (it may have been registered since).
+    const void *hp_key[2][8];
+    void *hp_dev[2][8];
+    int32_t hp_used[2], hp_next[2];
     // gen_step_host_async: one event per call in flight (ring), created on first use
     cudaEvent_t ev[4];
     int32_t ev_ready;        // events created
     uint64_t async_calls;    // gen_step_host_async calls so far
+    uint64_t async_waited;   // the first async_waited of them are known to have completed (gen_host_wait)
     // set by step_host_enqueue around its gen_step call: where k_step also writes reward / done (NULL: nowhere), and
     // whether the actions it passes were written by the HOST (pinned memory read in place: nothing on the device
     // produced them, so the launch may chain)
@@ -275,9 +284,19 @@ int launch(gen_env *env, const gen_buffers *bufs, uint32_t flags, int32_t K, con
     // A chained launch skips the grid-wide wait, so it may consume nothing a foreign kernel produced: with explicit
     // actions (written by whatever ran before this call) the launch always waits for its stream predecessor.
     kp.chain = (kp.count && env->chain_buf == bufs->step_epoch && (!actions || env->actions_from_host)) ? 1 : 0;
+    // gen_buffers.stack_cache is trusted only when the previous launch of this handle was the BIAS build of k_step on
+    // the same buffer, one global step ago (like chain_buf: validity is the host's knowledge, the stamp a second check)
+    const bool bias_build = (v->kind & 1) && v->ff != 0;
+    kp.stack_ok = (bias_build && env->stack_buf && env->stack_buf == bufs->stack_cache &&
+                   env->stack_step == env->global_step) ? 1 : 0;
     cudaError_t e = v->launch(kp, grid, 32 * kp.WPC, kp.smem_bytes, static_cast<cudaStream_t>(stream));
-    if (e != cudaSuccess) { env->last_cuda_error = (int)e; env->chain_buf = nullptr; return GEN_ERR_CUDA; }
+    if (e != cudaSuccess) {
+        env->last_cuda_error = (int)e; env->chain_buf = nullptr; env->stack_buf = nullptr;
+        return GEN_ERR_CUDA;
+    }
     env->chain_buf = kp.count ? bufs->step_epoch : nullptr;
+    env->stack_buf = bias_build ? bufs->stack_cache : nullptr;
+    env->stack_step = env->global_step + 1u;
     env->launches += 1;
     env->last_variant = (int32_t)(v - kVariants);
     return GEN_OK;
@@ -405,6 +424,7 @@ uint32_t gen_global_step(const gen_env *env) { return env ? env->global_step : 0
 int gen_set_global_step(gen_env *env, uint32_t step) {
     if (!env) return GEN_ERR_NULL;
     env->global_step = step;
+    env->stack_buf = nullptr;
     return GEN_OK;
 }
 
@@ -460,14 +480,16 @@ int gen_sample(gen_env *env, const gen_buffers *bufs, int32_t *d_actions_out, vo
     return launch(env, bufs, gen::F_SAMPLE_ONLY | gen::F_SAMPLER, 0, nullptr, d_actions_out, cuda_stream);
 }
 
-static void *host_alias(gen_env *env, const void *h) {
+static void *host_alias(gen_env *env, const void *h, int table) {
     if (!h) return nullptr;
-    for (int i = 0; i < env->hp_used; ++i)
-        if (env->hp_key[i] == h) return env->hp_dev[i];
-    const int slot = env->hp_used < 8 ? env->hp_used++ : (env->hp_next++ & 7);
-    env->hp_key[slot] = h;
-    env->hp_dev[slot] = mapped_alias(h);
-    return env->hp_dev[slot];
+    for (int i = 0; i < env->hp_used[table]; ++i)
+        if (env->hp_key[table][i] == h) return env->hp_dev[table][i];
+    void *dev = mapped_alias(h);
+    if (!dev) return nullptr;                                  // pageable: not remembered
+    const int slot = env->hp_used[table] < 8 ? env->hp_used[table]++ : (env->hp_next[table]++ & 7);
+    env->hp_key[table][slot] = h;
+    env->hp_dev[table][slot] = dev;
+    return dev;
 }
 
 // the body of gen_step_host / gen_step_host_async: everything but the wait
@@ -480,8 +502,8 @@ static int step_host_enqueue(gen_env *env, const gen_buffers *bufs, const int32_
     // Pinned host buffers are used in place: the step kernel reads the actions through their device alias and one
     // small kernel writes reward + done into the host arrays (no copy-engine transfers).  Pageable buffers take the
     // cudaMemcpyAsync route.  The alias lookups are cached per handle (same buffers every step in an RL loop).
-    void *const a_act = host_alias(env, h_actions), *const a_rew = host_alias(env, h_reward),
-                *const a_done = host_alias(env, h_done);
+    void *const a_act = host_alias(env, h_actions, 0), *const a_rew = host_alias(env, h_reward, 1),
+                *const a_done = host_alias(env, h_done, 1);
     const int32_t *d_act = nullptr;
     if (h_actions) {
         if (a_act && aligned16(a_act)) {
@@ -493,7 +515,10 @@ static int step_host_enqueue(gen_env *env, const gen_buffers *bufs, const int32_
         }
     }
     const bool mirror = N > 0 && (!h_reward || a_rew) && (!h_done || a_done) && (h_reward || h_done);
-    env->mirror_armed = mirror ? 1 : 0;
+    // the step kernel writes a two-player reward row as one 16-bit store: a pinned array at an odd address (a slice of
+    // a byte buffer) is served by k_mirror below, which copies byte by byte when it has to
+    const bool rew_ok = !h_reward || P != 2 || (reinterpret_cast<uintptr_t>(a_rew) & 1u) == 0;
+    env->mirror_armed = (mirror && rew_ok) ? 1 : 0;
     env->mirror_reward = h_reward ? static_cast<int8_t *>(a_rew) : nullptr;
     env->mirror_done = h_done ? static_cast<uint8_t *>(a_done) : nullptr;
     env->actions_from_host = (d_act && d_act == static_cast<const int32_t *>(a_act)) ? 1 : 0;
@@ -547,10 +572,22 @@ int gen_step_host_async(gen_env *env, const gen_buffers *bufs, const int32_t *h_
         }
         env->ev_ready = 1;
     }
-    if (int e = step_host_enqueue(env, bufs, h_actions, h_reward, h_done, s)) return e;
+    // at most four calls in flight: the event this call records is the one of the call issued four calls ago -- if
+    // nobody has waited for that one yet, wait for it here instead of losing track of it
+    if (env->async_calls - env->async_waited >= 4) {
+        const cudaError_t we = cudaEventSynchronize(env->ev[env->async_calls & 3]);
+        if (we != cudaSuccess) { env->last_cuda_error = (int)we; return GEN_ERR_CUDA; }
+        env->async_waited = env->async_calls - 3;
+    }
+    const uint32_t step_before = env->global_step;
+    const int e = step_host_enqueue(env, bufs, h_actions, h_reward, h_done, s);
+    if (e != GEN_OK && env->global_step == step_before) return e;   // nothing was launched
+    // also when a transfer behind the launched step failed: the step counts as a call, so that gen_host_wait(0) waits
+    // for it and not for its predecessor
     const cudaError_t ce = cudaEventRecord(env->ev[env->async_calls & 3], s);
-    if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
     env->async_calls += 1;
+    if (e != GEN_OK) return e;
+    if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
     return GEN_OK;
 }
 
@@ -558,14 +595,17 @@ int gen_host_wait(gen_env *env, int32_t lag) {
     if (!env) return GEN_ERR_NULL;
     if (lag < 0 || lag > 3) return GEN_ERR_ARG;
     if (env->async_calls <= (uint64_t)lag) return GEN_OK;     // nothing that old has been issued
-    const cudaError_t ce = cudaEventSynchronize(env->ev[(env->async_calls - 1 - (uint64_t)lag) & 3]);
+    const uint64_t call = env->async_calls - 1 - (uint64_t)lag;
+    if (call < env->async_waited) return GEN_OK;               // already known to have completed
+    const cudaError_t ce = cudaEventSynchronize(env->ev[call & 3]);
     if (ce != cudaSuccess) { env->last_cuda_error = (int)ce; return GEN_ERR_CUDA; }
+    env->async_waited = call + 1;                              // stream order: everything before it has completed too
     return GEN_OK;
 }
 
 int gen_forget_host_buffers(gen_env *env) {
     if (!env) return GEN_ERR_NULL;
-    env->hp_used = env->hp_next = 0;
+    env->hp_used[0] = env->hp_used[1] = env->hp_next[0] = env->hp_next[1] = 0;
     return GEN_OK;
 }
 

@@ -90,6 +90,7 @@ struct KParams {
     int32_t K, WPC;  // turns per launch; warps per CTA
     int32_t count;   // k_step: take a ticket per group of 4 games in gen_buffers.step_epoch and record completion
     int32_t chain;   // k_step: wait per warp for the earlier tickets of its group instead of for the previous grid
+    int32_t stack_ok;  // k_step (BIAS): gen_buffers.stack_cache was written by this handle's previous launch for this step
     // shared memory: [tables | digest keys | warp 0 | warp 1 | ...]; w_* are offsets inside a warp's slice
     uint32_t off_key, off_warp0, warp_bytes, w_owner, w_terr, w_mask, w_game, w_bar, w_scratch, smem_bytes;
     unsigned long long key_sum;  // sum of the digest keys of cells 0..HW-1

@@ -190,9 +190,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_step(const __grid_constant__ KPa
         if (ol == 1) { gs.alive = v_alive; gs.done = v_done; gs.winner = v_win; }
         if (ol == 2) { gs.flags = 0; gs.sat = 0; gs.rew_bits = 0; gs.rdirty[0] = 0; gs.rdirty[1] = 0; }
         if constexpr (BIAS) {
-            const uint32_t v_st = B.stack_cache ? __ldcg(B.stack_cache + (size_t)g * (P + 1) + min(ol, P)) : 0u;
+            const bool use = B.stack_cache && kp.stack_ok;  // the host vouches for the cache (generals_api.cu: launch)
+            const uint32_t v_st = use ? __ldcg(B.stack_cache + (size_t)g * (P + 1) + min(ol, P)) : 0u;
             if (ol < P) gs.best[ol] = v_st;
-            if (ol == P) gs.best_ok = (B.stack_cache && v_st == kp.global_step0) ? 1u : 0u;
+            if (ol == P) gs.best_ok = (use && v_st == kp.global_step0) ? 1u : 0u;
         }
     }
     __syncthreads();  // the only CTA barrier: tables and the mbarrier init are visible

@@ -245,6 +245,66 @@ def test_stack_cache_of_the_biased_policy_is_never_stale(gpu, oracle_mod):
     steps(30, "after reset")
 
 
+def test_stack_cache_validity_is_the_handles_knowledge(gpu, oracle_mod):
+    """the stamp in gen_buffers.stack_cache can match by accident -- gen_reset puts global_step back to 0,
+    explicit-action steps and gen_observe write no stamp, a zeroed cache reads "step 0, owns nothing".  The handle now
+    vouches for the cache (previous launch = a BIAS step on this buffer, one step ago); three orders that used to
+    sample from a stale cache must give the oracle's actions."""
+    import torch
+    cfg, _ = workloads.config("c4_curriculum", n_games=77, max_turns=0, auto_reset=0)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+
+    def sampled(n, where):
+        for t in range(n):
+            acts = o.step(want_actions=True)
+            env.step()
+            assert np.array_equal(env.field("actions_out"), acts), f"{where} step {t}"
+        compare(env, o, digest=False, where=where)
+
+    # 1. k sampler steps leave stamp k; reset; k explicit steps (no stamp written); the sampler at step k
+    k = 12
+    sampled(k, "before the reset")
+    env.reset()
+    o.reset()
+    passes = np.zeros((77, 2), dtype=np.int32)
+    for t in range(k):
+        env.step(torch.from_numpy(passes).to(env.device))
+        o.step(passes)
+    assert int((env.tensors["stack_cache"][:, 2] == env.global_step).sum()) == 77      # every stale stamp matches
+    sampled(6, "reset, explicit steps, sampler")
+    # 2. a BIAS step, then the caller rewrites the planes and calls gen_observe (R40)
+    gc = np.asarray(o.general_cell)
+    for g in range(77):
+        for p in range(2):
+            if gc[g, p] >= 0:
+                o.army[g, gc[g, p]] += 500 + 10 * p
+    env.tensors["army"].copy_(torch.from_numpy(np.asarray(o.army).copy()).to(env.device))
+    env.observe()
+    o.observe()
+    sampled(6, "edited planes + gen_observe")
+    # 3. a fresh handle, zeroed cache, global step 0, a state written by the caller
+    env3 = gpu.GeneralsEnv(cfg, digest=False)
+    o3 = oracle_mod.Oracle(cfg)
+    env3.reset()
+    o3.reset()
+    for f in ("army", "owner", "terrain", "turn", "alive", "general_cell"):
+        np.asarray(getattr(o3, f))[...] = np.asarray(getattr(o, f))
+    o3.observe()
+    env3.tensors["stack_cache"].zero_()
+    put_board(env3, o3)
+    env3.global_step = 0
+    assert o3.global_step == 0
+    for t in range(4):
+        acts = o3.step(want_actions=True)
+        env3.step()
+        assert np.array_equal(env3.field("actions_out"), acts), f"zeroed cache at step 0: step {t}"
+    assert env3.last_launch_register_resident and env3.last_launch_specialised
+    compare(env3, o3, digest=False, where="zeroed cache at step 0")
+
+
 def test_specialised_rollout_kernel_matches_oracle(gpu, oracle_mod):
     cfg, _ = workloads.config("c2_24x24", n_games=70, max_turns=90)
     env, o = make_pair(gpu, oracle_mod, cfg)
@@ -660,6 +720,69 @@ def test_step_host_end_to_end(gpu, oracle_mod, pinned, N):
     o.step()
     assert np.array_equal(h_d.numpy(), o.done[0])
     compare(env, o, where="step_host")
+    assert int(o.episodes_done.sum()) > 0
+
+
+def test_step_host_with_an_odd_reward_pointer(gpu, oracle_mod):
+    """a pinned int8 result array that starts at an odd address (a slice of a byte buffer).  The step
+    kernel's own host write of a two-player reward row is one 16-bit store; such an array must take the byte-wise
+    mirror kernel instead of faulting."""
+    import torch
+    N = 203
+    cfg, _ = workloads.config("c2_24x24", n_games=N, max_turns=25)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+    raw = torch.zeros(2 * N + 1, dtype=torch.int8).pin_memory()
+    h_r = raw[1:]
+    assert h_r.data_ptr() % 2 == 1 and h_r.is_contiguous()
+    h_d = torch.zeros((N,), dtype=torch.uint8).pin_memory()
+    for t in range(40):
+        before = env.launch_count
+        if t % 2:
+            env.step_host(None, h_r, h_d)
+        else:
+            env.step_host_async(None, h_r, h_d)
+            env.host_wait(0)
+        o.step()
+        assert env.launch_count == before + 2                     # the step and the mirror kernel
+        assert np.array_equal(h_r.numpy().reshape(N, 2), o.reward[0]) and np.array_equal(h_d.numpy(), o.done[0])
+    assert env.last_launch_register_resident and int(o.episodes_done.sum()) > 0
+    compare(env, o, digest=False, where="odd reward pointer")
+
+
+def test_step_host_async_more_than_four_calls_and_many_action_arrays(gpu, oracle_mod):
+    """(a) "at most 4 calls in flight" is now kept by the library -- six calls issued with no wait in
+    between (six sets of host slots), then one wait: every call's results are in its own slots; (b) a new pinned
+    actions array every step (twelve of them in rotation) next to one fixed pair of result arrays."""
+    import torch
+    N = 203
+    cfg, _ = workloads.config("c2_24x24", n_games=N, max_turns=30)
+    env = gpu.GeneralsEnv(cfg, digest=False)
+    o = oracle_mod.Oracle(cfg)
+    env.reset()
+    o.reset()
+    slots = [dict(r=torch.full((N, 2), 99, dtype=torch.int8).pin_memory(),
+                  d=torch.full((N,), 99, dtype=torch.uint8).pin_memory()) for _ in range(6)]
+    for rnd in range(6):
+        want = []
+        for s in slots:
+            env.step_host_async(None, s["r"], s["d"])            # no wait: the fifth and sixth call wait inside
+            o.step()
+            want.append((o.reward[0].copy(), o.done[0].copy()))
+        env.host_wait(0)
+        for i, s in enumerate(slots):
+            assert np.array_equal(s["r"].numpy(), want[i][0]) and np.array_equal(s["d"].numpy(), want[i][1]), (rnd, i)
+    many = [torch.zeros((N, 2), dtype=torch.int32).pin_memory() for _ in range(12)]
+    h_r, h_d = slots[0]["r"], slots[0]["d"]
+    for t in range(36):
+        a = o.sample()
+        many[t % 12].copy_(torch.from_numpy(a))
+        env.step_host(many[t % 12], h_r, h_d)
+        o.step(a)
+        assert np.array_equal(h_r.numpy(), o.reward[0]) and np.array_equal(h_d.numpy(), o.done[0]), t
+    compare(env, o, digest=False, where="async in-flight limit / many action arrays")
     assert int(o.episodes_done.sum()) > 0
 
 
