@@ -269,10 +269,12 @@ def test_stack_cache_validity_is_the_handles_knowledge(gpu, oracle_mod):
     sampled(k, "before the reset")
     env.reset()
     o.reset()
-    passes = np.zeros((77, 2), dtype=np.int32)
-    for t in range(k):
-        env.step(torch.from_numpy(passes).to(env.device))
-        o.step(passes)
+    for t in range(k):                 # the sampler's moves with the split flipped (R22; valid whenever the move is, R5):
+        a = o.sample()                 # the same boards as before the reset now carry different stacks
+        kk = a % 9
+        a = np.where(kk == 0, a, np.where(kk % 2 == 1, a + 1, a - 1)).astype(np.int32)
+        env.step(torch.from_numpy(a).to(env.device))
+        o.step(a)
     assert int((env.tensors["stack_cache"][:, 2] == env.global_step).sum()) == 77      # every stale stamp matches
     sampled(6, "reset, explicit steps, sampler")
     # 2. a BIAS step, then the caller rewrites the planes and calls gen_observe (R40)
@@ -1060,6 +1062,139 @@ def test_full_size_configs_sampled_games(gpu, oracle_mod, name, N, T, roll):
         assert torch.equal(env.tensors["army_total"][:, p].to(torch.int64), (army.to(torch.int64) * mine).sum(1))
         assert bool((env.tensors["obs_vis"][0, :, p, :HW][mine] == 1).all())      # fog: vis contains owned (I5)
     assert int(env.tensors["episodes_done"].sum()) >= 0
+
+
+def _sample_ids(N, extra=23):
+    return sorted(set(list(range(12)) + list(range(N - 12, N)) + list(range(7, N, max(1, N // extra)))))
+
+
+def _gather(env, fields, ids, slot=0):
+    import torch
+    sel = torch.tensor(ids, device=env.device)
+    out = {}
+    for f in fields:
+        t = env.tensors[f]
+        if f in OUT_FIELDS or f in ("obs_packed", "actions_out"):
+            t = t[slot]
+        out[f] = t.index_select(0, sel).cpu().numpy()
+    return out
+
+
+def _same_game(have, want, what):
+    if have.dtype != want.dtype:
+        have = have.view(want.dtype)
+    assert np.array_equal(have, want.reshape(have.shape)), what
+
+
+@pytest.mark.parametrize("leg,N,variant", [
+    ("rollout_digest", 16384, 3), ("rollout_digest", 262144, 3),
+    ("rollout_every", 16384, 22), ("rollout_every", 262144, 22),
+    ("packed", 16384, 7), ("packed", 262144, 7),
+    ("host_async", 16384, 7),
+])
+def test_timed_legs_at_their_own_size_and_mode(gpu, oracle_mod, leg, N, variant):
+    """the kernel build that runs is a function of the batch size and of the output format
+    (pick_variant), so every leg bench.py publishes is checked here at its own size and in its own mode -- the fused
+    32-turn digest rollout, the 8-turn rollout that writes every turn's planes, the packed observation, and the
+    end-to-end loop whose step kernel writes reward / done into pinned host arrays -- on BASELINE config 2 / 3's boards
+    (max_turns shortened so that auto-resets fall inside the run; it is a run-time parameter, the build is the same).
+    The oracle replays a sample of global game ids (first / last / strided: a game depends on its id only)."""
+    import torch
+    cfg, _ = workloads.config("c2_24x24" if N == 16384 else "c3_sweep", n_games=N, max_turns=70)
+    ids = _sample_ids(N, 15)
+    lib = gpu.load_library()
+
+    def oracles(**kw):
+        out = []
+        for gid in ids:
+            o = oracle_mod.Oracle(dict(cfg, n_games=1, game_id_base=gid), **kw)
+            o.reset()
+            out.append(o)
+        return out
+
+    if leg == "rollout_digest":
+        env = gpu.GeneralsEnv(cfg, digest=True, actions_out=False)
+        env.reset()
+        for _ in range(5):
+            env.rollout(32, gpu.OBS_DIGEST)
+        env.torch.cuda.synchronize()
+        fields = STATE_FIELDS + OUT_FIELDS + ["obs_digest"]
+        got = _gather(env, fields, ids)
+        for k, o in enumerate(oracles()):
+            for _ in range(5):
+                o.rollout(32)
+            for f in fields:
+                _same_game(got[f][k], np.asarray(o.field(f))[0], (leg, ids[k], f))
+    elif leg == "rollout_every":
+        K = 8
+        env = gpu.GeneralsEnv(cfg, k_slots=K, digest=False, actions_out=False)
+        env.reset()
+        os_ = oracles(every_step_K=K, digest=False)
+        for it in range(11):
+            env.rollout(K, gpu.OBS_EVERY_STEP)
+            if it not in (0, 8, 10):                       # slots compared for three of the launches, the state at the end
+                for o in os_:
+                    o.rollout(K, oracle_mod.OBS_EVERY_STEP)
+                continue
+            env.torch.cuda.synchronize()
+            got = [_gather(env, OUT_FIELDS, ids, slot=k) for k in range(K)]
+            for j, o in enumerate(os_):
+                o.rollout(K, oracle_mod.OBS_EVERY_STEP)
+                for k in range(K):
+                    for f in OUT_FIELDS:
+                        _same_game(got[k][f][j], np.asarray(getattr(o, f))[k][0], (leg, it, k, ids[j], f))
+        got = _gather(env, STATE_FIELDS, ids)
+        for j, o in enumerate(os_):
+            for f in STATE_FIELDS:
+                _same_game(got[f][j], np.asarray(o.field(f))[0], (leg, ids[j], f))
+    elif leg == "packed":
+        env = gpu.GeneralsEnv(cfg, digest=False, actions_out=False, packed=True)
+        env.reset()
+        T = 150
+        for _ in range(T):
+            env.step()
+        env.torch.cuda.synchronize()
+        got = _gather(env, PACKED_FIELDS, ids)
+        for k, o in enumerate(oracles(digest=False)):
+            for _ in range(T):
+                o.step()
+            for f in PACKED_FIELDS:
+                _same_game(got[f][k], np.asarray(o.field(f))[0], (leg, ids[k], f))
+        assert env.last_launch_register_resident
+    else:                                                  # bench.py's e2e leg: pinned actions, results one step late
+        T = 90
+        env = gpu.GeneralsEnv(cfg, digest=False)
+        env.reset()
+        h_actions = torch.empty((T, N, 2), dtype=torch.int32).pin_memory()
+        for t in range(T):                                 # the action stream: the device sampler's, as in bench.py
+            env.step()
+            h_actions[t].copy_(env.tensors["actions_out"][0], non_blocking=True)
+        env.torch.cuda.synchronize()
+        env.reset()
+        slots = [(torch.full((N, 2), 99, dtype=torch.int8).pin_memory(), torch.full((N,), 99, dtype=torch.uint8).pin_memory())
+                 for _ in range(2)]
+        seen = []                                          # host results of the sampled games, every step
+        for t in range(T):
+            r, d = slots[t & 1]
+            env.step_host_async(h_actions[t], r, d)
+            if t >= 1:
+                env.host_wait(1)
+                pr, pd = slots[(t - 1) & 1]
+                seen.append((pr.numpy()[ids].copy(), pd.numpy()[ids].copy()))
+        env.host_wait(0)
+        pr, pd = slots[(T - 1) & 1]
+        seen.append((pr.numpy()[ids].copy(), pd.numpy()[ids].copy()))
+        assert env.launch_count == 1 + T + 1 + T           # one launch per step: the kernel writes the host arrays itself
+        got = _gather(env, STATE_FIELDS + OUT_FIELDS, ids)
+        for k, o in enumerate(oracles(digest=False)):
+            for t in range(T):
+                acts = o.step(want_actions=True)
+                assert np.array_equal(acts[0], h_actions[t, ids[k]].numpy()), (leg, t, ids[k], "actions")
+                assert np.array_equal(seen[t][0][k], o.reward[0][0]) and seen[t][1][k] == o.done[0][0], (leg, t, ids[k])
+            for f in STATE_FIELDS + OUT_FIELDS:
+                _same_game(got[f][k], np.asarray(o.field(f))[0], (leg, ids[k], f))
+    assert lib.gen_last_variant(env._env, None, None) == variant          # the build bench.py's leg runs
+    assert int(env.tensors["episodes_done"].sum()) > 0
 
 
 # ------------------------------------------------------------------------------- NEXT-1: 38-channel features (R35)
