@@ -149,6 +149,70 @@ def run_reference(args):
     return 0
 
 
+
+# ------------------------------------------------------------------------------------------ parity of the timed legs
+PARITY_STATE = ["army", "owner", "terrain", "turn", "episode", "alive", "general_cell", "land", "army_total",
+                "episodes_done", "wins", "truncations", "sat_events"]
+PARITY_OUT = ["reward", "done", "winner", "obs_army", "obs_owner", "obs_terrain", "obs_vis"]
+
+
+def parity_check(envs, mode="step", K=1, n_ids=8, actions=None, host_results=None):
+    """after a timed leg and OUTSIDE every timed region, the CPU oracle (oracle/, the same test
+    infrastructure the cpu_baseline leg times) replays `n_ids` games of the environments that leg stepped -- first, last
+    and strided ids, split over `envs` -- for all the turns each environment has played since its last reset, through
+    the same call sequence (mode "step": gen_step with the sampler; "rollout": gen_rollout(K, DIGEST); "every":
+    gen_rollout(K, EVERY_STEP), all K slots compared; "actions": gen_step with the explicit action stream `actions`
+    [T][N][P]).  Every state tensor, the scoreboard, reward / done / winner and the four observation planes of those
+    games (plus the chained digest in mode "rollout", plus the host copies `host_results` = (reward, done) of the last
+    step in mode "actions") must be bit-equal.  Returns the JSON object {"games", "turns", "ok", ...}."""
+    import numpy as np
+    import torch
+    from oracle import oracle
+    per_env = max(1, n_ids // len(envs))
+    games, turns, bad = 0, 0, None
+    for env in envs:
+        torch.cuda.synchronize()
+        N, T = env.N, env.global_step
+        ids = sorted({(k * (N - 1)) // max(1, per_env - 1) for k in range(per_env)})
+        sel = torch.tensor(ids, device=env.device)
+        slots = K if mode == "every" else 1
+        fields = PARITY_STATE + PARITY_OUT + (["obs_digest"] if mode == "rollout" else [])
+        got = [{f: (env.tensors[f][k] if f in PARITY_OUT else env.tensors[f]).index_select(0, sel).cpu().numpy()
+                for f in fields if k == 0 or f in PARITY_OUT} for k in range(slots)]
+        for j, g in enumerate(ids):
+            cfg1 = dict(env.cfg_dict, n_games=1, game_id_base=env.cfg_dict.get("game_id_base", 0) + g)
+            o = oracle.Oracle(cfg1, every_step_K=K if mode == "every" else 0, digest=(mode == "rollout"))
+            o.reset()
+            if mode == "step":
+                for _ in range(T):
+                    o.step()
+            elif mode == "actions":
+                for t in range(T):
+                    o.step(actions[t, g].numpy().reshape(1, -1))
+            else:
+                for _ in range(T // K):
+                    o.rollout(K, oracle.OBS_EVERY_STEP if mode == "every" else oracle.OBS_DIGEST)
+            for k in range(slots):
+                for f, have in got[k].items():
+                    want = np.asarray(getattr(o, f))
+                    want = want[k][0] if f in PARITY_OUT else want[0]
+                    if have[j].dtype != want.dtype:
+                        want = want.view(have[j].dtype) if want.ndim else np.asarray(want).astype(have[j].dtype)
+                    if not np.array_equal(have[j], want.reshape(have[j].shape)) and bad is None:
+                        bad = {"game": int(cfg1["game_id_base"]), "field": f, "slot": k}
+            if host_results is not None and bad is None:
+                hr, hd = host_results
+                if not (np.array_equal(hr.numpy()[g], o.reward[0][0]) and int(hd.numpy()[g]) == int(o.done[0][0])):
+                    bad = {"game": int(cfg1["game_id_base"]), "field": "host reward / done"}
+        games += len(ids)
+        turns = max(turns, T)
+    out = {"games": games, "turns": turns, "ok": bad is None, "against": "oracle/ replay of the sampled games, all "
+           "state tensors, scoreboard, reward / done / winner and observation planes bit-equal"}
+    if bad is not None:
+        out["first_mismatch"] = bad
+    return out
+
+
 # ------------------------------------------------------------------------------------------ our arm
 MIN_REGION_MS, MIN_REPS, MAX_REPS = 50.0, 5, 60
 # warp-instructions per env step of the fused rollout kernel (gen_rollout(32, GEN_OBS_DIGEST), 24x24 1v1):
@@ -216,11 +280,16 @@ def run_ours(args):
                 "us_per_launch": 1e3 * med / k, "best_us_per_launch": 1e3 * best / k, "repetitions": len(reps),
                 "launches_per_repetition": k}
 
+    def checked(envs_, **kw):
+        # the oracle is test infrastructure: it runs here only beside the cpu_baseline leg, never inside a timed region
+        return None if args.no_cpu_baseline else parity_check(envs_, **kw)
+
     def make_replicas(cfg_r, n_games, count, actions_out_first=False):
         out = []
         for r in range(count):
             c = replicas.weak_replica_config(dict(cfg_r, n_games=n_games, game_id_base=0), rank * count + r)
             out.append(GeneralsEnv(c, device=dev, digest=False, actions_out=(actions_out_first and r == 0)))
+            out[-1].cfg_dict = c
         return out
 
     # Replicas of the batch, stepped round-robin, so that every launch finds its inputs in HBM and not in
@@ -259,6 +328,7 @@ def run_ours(args):
     launches = (sum(e.launch_count for e in envs) - launches0) // len(reps)
     head = summary(reps, K, N)
     total_ms = statistics.median(reps)
+    head_parity = checked([envs[0], envs[R - 1]])
     specialised, reg_resident = env.last_launch_specialised, env.last_launch_register_resident
 
     # ---- one environment stepped K times back to back (launch t+1 depends on launch t game by game; the 132 MB
@@ -269,6 +339,7 @@ def run_ours(args):
 
     same(Wm)
     same_env = summary(timed(same, K), K, N)
+    same_parity = checked([env])
 
     # ---- isolated launches: a 256 MB L2-flush write before every launch and one event pair per launch (includes
     # the launch latency a back-to-back stream hides); what a loop with other kernels between the steps gets
@@ -301,6 +372,7 @@ def run_ours(args):
     pair(Wm)
     f_reps, p_reps = timed(only_foreign, K), timed(pair, K)
     f_us, p_us = 1e3 * statistics.median(f_reps) / K, 1e3 * statistics.median(p_reps) / K
+    inter_parity = checked([env])                            # covers the isolated launches before it as well
     # the same with TWO environments on two streams (the usual schedule of a learner with two env batches: the policy
     # works on one while the other steps): each stream alternates its foreign kernel and its step
     side = [torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)]
@@ -328,6 +400,7 @@ def run_ours(args):
     f2_reps = timed(on_two_streams(lambda i: two_bufs[i].fill_(3)), K)
     p2_reps = timed(on_two_streams(two_pair), K)
     f2_us, p2_us = 1e3 * statistics.median(f2_reps) / (2 * K), 1e3 * statistics.median(p2_reps) / (2 * K)
+    two_parity = checked(two_envs)
     del foreign, foreign2, two_bufs
 
     # ---- gen_step + gen_features (bfloat16 feature tensor, R37) every turn: the featuriser between two steps
@@ -353,6 +426,7 @@ def run_ours(args):
 
     # ---- fused rollout leg (K_r = 32 turns per launch, observation digest chained every turn)
     renv = GeneralsEnv(replicas.weak_replica_config(cfg, rank), device=dev, digest=True, actions_out=False)
+    renv.cfg_dict = replicas.weak_replica_config(cfg, rank)
     renv.reset()
     renv.rollout(32, OBS_DIGEST)
     n_roll = max(2, K // 32)
@@ -363,11 +437,14 @@ def run_ours(args):
 
     roll_reps = timed(roll, n_roll)
     roll_value = world * N * 32 * n_roll / (statistics.median(roll_reps) * 1e-3)
+    roll_parity = checked([renv], mode="rollout", K=32)
+    roll_variant = renv.lib.gen_last_variant(renv._env, None, None)
     del renv
     # ---- fused rollout with the planes of EVERY turn written (K = 8 slots): the same output as eight gen_step
     # launches with the built-in sampler, the state read once per launch
     KE = 8
     eenv = GeneralsEnv(replicas.weak_replica_config(cfg, rank), device=dev, k_slots=KE, digest=False, actions_out=False)
+    eenv.cfg_dict = replicas.weak_replica_config(cfg, rank)
     eenv.reset()
     eenv.rollout(KE, OBS_EVERY_STEP)
     n_every = max(2, K // KE)
@@ -379,6 +456,8 @@ def run_ours(args):
     every_reps = timed(roll_every, n_every)
     every_value = world * N * KE * n_every / (statistics.median(every_reps) * 1e-3)
     every_bytes = bmin - 4 * H * W * (KE - 1) / KE
+    every_parity = checked([eenv], mode="every", K=KE)
+    every_variant = eenv.lib.gen_last_variant(eenv._env, None, None)
     del eenv
 
     # ---- end-to-end leg: host actions in (pinned), gen_step_host, host reward + done out, every step
@@ -399,12 +478,11 @@ def run_ours(args):
         torch.cuda.synchronize()
         e2e_reps.append(max_over_ranks(time.perf_counter() - t0))
     e2e_s = statistics.median(e2e_reps)
-    checksum = int(h_done.sum())
     # the same loop without a synchronisation per step: gen_step_host_async, two sets of pinned result slots, the
     # results of step t - 1 read (gen_host_wait(1)) after step t has been issued
     slots = [(torch.zeros((N, P), dtype=torch.int8).pin_memory(), torch.zeros((N,), dtype=torch.uint8).pin_memory())
              for _ in range(2)]
-    async_reps, async_sum = [], 0
+    async_reps, async_sum = [], 0                            # async_sum: the host really reads a result every step
     for _ in range(MIN_REPS):
         env.reset()
         for t in range(Wm):
@@ -421,6 +499,8 @@ def run_ours(args):
         async_sum += int(slots[(Wm + K - 1) & 1][1][0])
         async_reps.append(max_over_ranks(time.perf_counter() - t0))
     async_s = statistics.median(async_reps)
+    e2e_parity = checked([env], mode="actions", actions=h_actions, host_results=slots[(Wm + K - 1) & 1])
+    e2e_variant = env.lib.gen_last_variant(env._env, None, None)
 
     # ---- large batch ("quote the fraction from N >= 262,144"): the same kernel where one launch is
     # 22 waves and the batch (2.1 GB of state + observations per replica) is far larger than L2
@@ -443,10 +523,12 @@ def run_ours(args):
         KL = max(8, min(K, 20))
         l_reps = timed(lrot, KL)
         large = summary(l_reps, KL, NL)
+        large["parity_checked"] = checked(lenvs)
         del lenvs
         torch.cuda.empty_cache()
         leenv = GeneralsEnv(replicas.weak_replica_config(dict(cfg, n_games=NL), rank), device=dev, k_slots=KE, digest=False,
                             actions_out=False)
+        leenv.cfg_dict = replicas.weak_replica_config(dict(cfg, n_games=NL), rank)
         leenv.reset()
         leenv.rollout(KE, OBS_EVERY_STEP)
 
@@ -456,6 +538,7 @@ def run_ours(args):
 
         le_reps = timed(lroll_every, 4)
         large["rollout_every_step"] = world * NL * KE * 4 / (statistics.median(le_reps) * 1e-3)
+        large["rollout_every_parity"] = checked([leenv], mode="every", K=KE)
         del leenv
         torch.cuda.empty_cache()
 
@@ -489,6 +572,7 @@ def run_ours(args):
                              "best repetition in value_best",
                    "parallelism": f"replicas x{world}, disjoint game-id ranges, no collective"},
         "value_best": head["best"], "repetitions": len(reps),
+        "parity_checked": head_parity,
         "clocks": clock_info,
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
@@ -507,7 +591,8 @@ def run_ours(args):
                         "step_us": step_us_inter, "frac": N * bmin / (step_us_inter * 1e-6) / 1e9 / peak,
                         "repetitions": len(p_reps),
                         "note": "one environment; a foreign kernel (24 MB fill, the policy stand-in) between two steps, "
-                                "so launches cannot chain; step_us = pair - foreign alone"},
+                                "so launches cannot chain; step_us = pair - foreign alone",
+                        "parity_checked": inter_parity},
         "interleaved_two_batches": {"loop_value": world * N / (p2_us * 1e-6), "loop_value_one_batch": world * N / (p_us * 1e-6),
                                     "unit": UNIT, "pair_us": p2_us, "foreign_us": f2_us, "step_us": p2_us - f2_us,
                                     "repetitions": len(p2_reps),
@@ -516,7 +601,8 @@ def run_ours(args):
                                             "phase runs under the other's foreign kernel and rules.  loop_value = env steps/s of "
                                             "the whole loop, foreign kernels included (one batch on one stream beside it); "
                                             "pair_us = time per (foreign + step) pair; step_us = pair - foreign alone attributes "
-                                            "ALL of the overlap to the step and is not a roofline figure"},
+                                            "ALL of the overlap to the step and is not a roofline figure",
+                                    "parity_checked": two_parity},
         "step_plus_features": {"turn_us": sf_us, "features_us": of_us, "step_us": sf_us - of_us,
                                "value": world * N / (sf_us * 1e-6), "unit": UNIT, "dtype": "bf16 feature tensor (R37)",
                                "note": "gen_step + gen_features every turn (38 channels x 2 players materialised)"},
@@ -530,16 +616,18 @@ def run_ours(args):
                        "and are not part of the returned result",
                 "synchronised_every_step": {"value": world * N * K / e2e_s, "best": world * N * K / min(e2e_reps),
                                             "api": "gen_step_host (cudaStreamSynchronize per step)"},
-                "done_checksum": checksum + async_sum},
-        "same_env": dict(same_env, note="one environment stepped K times back to back (true game-by-game dependency "
+                "parity_checked": e2e_parity, "kernel_variant": e2e_variant},
+        "same_env": dict(same_env, parity_checked=same_parity, note="one environment stepped K times back to back (true game-by-game dependency "
                                         "between launches; working set partly L2-resident: not a roofline figure)"),
         "rollout": {"value": roll_value, "unit": UNIT, "K": 32, "launches": n_roll, "repetitions": len(roll_reps),
                     "obs": "digest every turn, planes of the last turn",
+                    "parity_checked": roll_parity, "kernel_variant": roll_variant,
                     "roofline": {"bound": "alu", "inst_per_env_step": ROLLOUT_INST_PER_ENV_STEP,
                                  "inst_source": ROLLOUT_INST_SOURCE,
                                  "achieved": roll_value / world * ROLLOUT_INST_PER_ENV_STEP, "peak": ISSUE_PEAK,
                                  "unit": "warp-inst/s", "frac": roll_value / world * ROLLOUT_INST_PER_ENV_STEP / ISSUE_PEAK}},
         "rollout_every_step": {"value": every_value, "unit": UNIT, "K": KE, "launches": n_every, "repetitions": len(every_reps),
+                               "parity_checked": every_parity, "kernel_variant": every_variant,
                                "obs": "four planes x 2 players of EVERY turn, K-strided slots (what K gen_step launches with "
                                       "the built-in sampler write)",
                                "roofline": {"bound": "hbm", "algorithmic_bytes_per_env_step": every_bytes,
@@ -555,11 +643,13 @@ def run_ours(args):
                                   "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
                                   "traffic_over_algorithmic": tr[0] / (NL * bmin) if tr else None,
                                   "value": large["value"], "best": large["best"], "units_per_launch": NL,
+                                  "parity_checked": large["parity_checked"],
                                   "avg_launch_us": large["us_per_launch"], "repetitions": large["repetitions"],
                                   "launches_per_repetition": large["launches_per_repetition"],
                                   "kernel": kname + " (gen_step), 2 replicas of 262,144 games in rotation",
                                   "rollout_every_step": {"value": large["rollout_every_step"], "unit": UNIT, "K": KE,
                                                          "frac": large["rollout_every_step"] / world * every_bytes / 1e9 / peak,
+                                                         "parity_checked": large["rollout_every_parity"],
                                                          "note": "gen_rollout(8, GEN_OBS_EVERY_STEP) at the same batch size"}}
     if not args.no_cpu_baseline:
         # config 2's first 1,024 games; 500 turns instead of 2,000 so that the leg stays near 20 s of CPU
