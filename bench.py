@@ -215,20 +215,28 @@ def parity_check(envs, mode="step", K=1, n_ids=8, actions=None, host_results=Non
 
 # ------------------------------------------------------------------------------------------ our arm
 MIN_REGION_MS, MIN_REPS, MAX_REPS = 50.0, 5, 60
+PHASE_STRIDE = 160                  # turns between the starting phases of consecutive replicas of the headline rotation
 # warp-instructions per env step of the fused rollout kernel (gen_rollout(32, GEN_OBS_DIGEST), 24x24 1v1):
 # smsp__inst_executed.sum / (N * K) of the ncu capture summarised in the file named beside it
 ROLLOUT_INST_PER_ENV_STEP = 659.4
 ROLLOUT_INST_SOURCE = "profiles/r02_rollout_summary.txt"
+# the method's own work per env step as SURVEY 8(d) estimates it ("3-4 x 10^2 warp-instructions" at 24x24 1v1: fog test +
+# selects + mix per visible cell and player, growth, sampler, moves); the kernel executes more than that (index
+# arithmetic, staging, reductions), so frac_algorithmic < frac says how much of the issued work is overhead
+ROLLOUT_ALGORITHMIC_INST_PER_ENV_STEP = 350.0
 ISSUE_PEAK = 148 * 4 * 1.965e9      # warp-instructions/s: 148 SMs x 4 schedulers x 1 per clock x 1.965 GHz
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of k_step at N = 262,144 (ncu --set full), by games per launch
 NCU_DRAM_BYTES_PER_LAUNCH_LARGE = {262144: (2303562752, "profiles/r02_step_full_262k_summary.txt")}
+# the same for the headline rotation (six replicas of 16,384 games, caches left alone between launches: mean of 36
+# consecutive launches, ncu --cache-control none)
+NCU_DRAM_BYTES_PER_LAUNCH = {16384: (144697216, "profiles/r03_rotation_dram.md")}
 
 
 def run_ours(args):
     import torch
     import torch.distributed as dist
     import workloads
-    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, OBS_EVERY_STEP, replicas
+    from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST, OBS_EVERY_STEP, OBS_NONE, replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -311,10 +319,17 @@ def run_ours(args):
         clocks.start()                                       # sampling spans warm-up and every timed leg below
 
     # ---- headline: K gen_step launches back to back, replica t % R at step t
-    for e in envs:
+    # Phase mix: an episode of config 2 runs 1,000 turns and the board fills up on the way, so replica
+    # r is first played forward to turn r * PHASE_STRIDE with one state-only fused rollout (untimed); the timed launches
+    # then sample early, middle and late game and, on the last replica, the truncation + auto-reset at turn 1,000.
+    for r, e in enumerate(envs):
         e.reset()
+        if r and not args.no_phase_mix:
+            e.rollout(r * PHASE_STRIDE, OBS_NONE)
     for t in range(max(Wm, 2 * R)):                          # every replica stepped at least twice before timing
         envs[t % R].step()
+    torch.cuda.synchronize()
+    turns_before = [e.global_step for e in envs]
     counter = [0]
 
     def rotate(k):
@@ -329,6 +344,7 @@ def run_ours(args):
     head = summary(reps, K, N)
     total_ms = statistics.median(reps)
     head_parity = checked([envs[0], envs[R - 1]])
+    turns_timed = [f"{a}-{e.global_step}" for a, e in zip(turns_before, envs)]
     specialised, reg_resident = env.last_launch_specialised, env.last_launch_register_resident
 
     # ---- one environment stepped K times back to back (launch t+1 depends on launch t game by game; the 132 MB
@@ -567,6 +583,8 @@ def run_ours(args):
                          f"{N * bmin / 1e6:.0f} MB of algorithmic traffic between two steps of one replica; L2 is "
                          "126 MB); K launches back to back, one CUDA event pair around them",
                    "replicas_in_rotation": R,
+                   "turns_timed": "turns of the episode each replica played inside the timed repetitions (replica r "
+                                  f"pre-rolled to turn r x {PHASE_STRIDE}; max_turns 1000): " + ", ".join(turns_timed),
                    "timing": f"value = median of {len(reps)} repetitions of exactly {K} launches (one event pair each, "
                              f"barrier + synchronize on both sides; repeated until >= {MIN_REGION_MS:.0f} ms in total); "
                              "best repetition in value_best",
@@ -576,9 +594,10 @@ def run_ours(args):
         "clocks": clock_info,
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None,
-                     "traffic_note": "not captured per run; one serialised cold launch under ncu leaves part of its stores "
-                                     "in L2 and undercounts -- the usable traffic ratio is roofline_large's",
+                     "traffic": (NCU_DRAM_BYTES_PER_LAUNCH.get(N) or (None, None))[0],
+                     "traffic_source": (NCU_DRAM_BYTES_PER_LAUNCH.get(N) or (None, None))[1],
+                     "traffic_over_algorithmic": (NCU_DRAM_BYTES_PER_LAUNCH[N][0] / (N * bmin)
+                                                  if N in NCU_DRAM_BYTES_PER_LAUNCH else None),
                      "kernel": kname + " (gen_step)", "peak_source": peak_src,
                      "algorithmic_bytes_per_env_step": bmin, "units_per_launch": N,
                      "avg_launch_us": 1e3 * launch_ms, "best_launch_us": head["best_us_per_launch"],
@@ -625,7 +644,10 @@ def run_ours(args):
                     "roofline": {"bound": "alu", "inst_per_env_step": ROLLOUT_INST_PER_ENV_STEP,
                                  "inst_source": ROLLOUT_INST_SOURCE,
                                  "achieved": roll_value / world * ROLLOUT_INST_PER_ENV_STEP, "peak": ISSUE_PEAK,
-                                 "unit": "warp-inst/s", "frac": roll_value / world * ROLLOUT_INST_PER_ENV_STEP / ISSUE_PEAK}},
+                                 "unit": "warp-inst/s", "frac": roll_value / world * ROLLOUT_INST_PER_ENV_STEP / ISSUE_PEAK,
+                                 "algorithmic_inst_per_env_step": ROLLOUT_ALGORITHMIC_INST_PER_ENV_STEP,
+                                 "algorithmic_source": "SURVEY.md 8(d) estimate (3-4e2 warp-instructions per env step)",
+                                 "frac_algorithmic": roll_value / world * ROLLOUT_ALGORITHMIC_INST_PER_ENV_STEP / ISSUE_PEAK}},
         "rollout_every_step": {"value": every_value, "unit": UNIT, "K": KE, "launches": n_every, "repetitions": len(every_reps),
                                "parity_checked": every_parity, "kernel_variant": every_variant,
                                "obs": "four planes x 2 players of EVERY turn, K-strided slots (what K gen_step launches with "
@@ -669,6 +691,8 @@ def run_ours(args):
                                                         f"300 turns of {WORKLOAD} each, disjoint global game ids"}
         except Exception as exc:                                   # a baseline, never a reason to lose the line
             line["cpu_baseline_all_cores"] = {"value": None, "error": repr(exc)}
+    for k in ("same_env", "interleaved_two_batches", "interleaved", "roofline_isolated"):
+        line[k] = line.pop(k)             # last in the line: a log that keeps only the tail of stdout keeps these
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -683,8 +707,37 @@ def run_single_leg(args):
     from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
-    n = {"rollout": 16384, "step": 16384, "step-large": 262144}[args.only]
+    n = {"rollout": 16384, "step": 16384, "step-large": 262144, "rotation": 16384}[args.only]
     cfg, _ = workloads.config(args.workload or WORKLOAD, n_games=args.games or n)
+    if args.only == "rotation":
+        # the headline leg by itself: R replicas of the batch (640 MB of algorithmic traffic between two steps of one
+        # replica), pre-rolled to different phases of the episode, stepped round-robin -- the command of the
+        # dram__bytes capture behind roofline.traffic (ncu --cache-control none: the caches carry over from launch to
+        # launch as they do in the timed run)
+        from paper_2606_23348_b200 import OBS_NONE
+        N = cfg["n_games"]
+        bmin = algorithmic_bytes_per_env_step(cfg["height"], cfg["width"], cfg["n_players"])
+        R = args.replicas or max(2, -(-(640 << 20) // (N * bmin)))
+        envs = [GeneralsEnv(dict(cfg, game_id_base=r * N), device=dev, digest=False, actions_out=False) for r in range(R)]
+        for r, e in enumerate(envs):
+            e.reset()
+            if r and not args.no_phase_mix:
+                e.rollout(r * PHASE_STRIDE, OBS_NONE)
+        for t in range(2 * R):
+            envs[t % R].step()
+        k = max(2 * R, min(args.steps, 400))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for t in range(k):
+            envs[t % R].step()
+        e1.record()
+        torch.cuda.synchronize()
+        print(json.dumps({"leg": "rotation", "n_games": N, "replicas": R, "launches": k, "warmup_launches": 2 * R,
+                          "us_per_launch": 1e3 * e0.elapsed_time(e1) / k,
+                          "env_steps_per_s": N * k / (e0.elapsed_time(e1) * 1e-3),
+                          "kernel_variant": envs[0].lib.gen_last_variant(envs[0]._env, None, None)}))
+        return 0
     env = GeneralsEnv(cfg, device=dev, digest=(args.only == "rollout"), actions_out=False)
     if args.force_step:
         env.set_generic(False, -1)      # the register-resident kernel also where the staged one is the default (P > 4)
@@ -935,8 +988,9 @@ def main():
     ap.add_argument("--replicas", type=int, default=0, help="replicas in the round-robin (default: enough for 640 MB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-large", action="store_true", help="skip the N = 262,144 leg (roofline_large)")
+    ap.add_argument("--no-phase-mix", action="store_true", help="headline rotation: every replica starts at turn 0")
     ap.add_argument("--force-step", action="store_true", help="with --only step: k_step also for more than 4 players")
-    ap.add_argument("--only", choices=["rollout", "step", "step-large"], default="",
+    ap.add_argument("--only", choices=["rollout", "step", "step-large", "rotation"], default="",
                     help="one leg by itself, a few launches (the command of the ncu captures under profiles/)")
     ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
     ap.add_argument("--rows", default="", help="with --sweep: only the rows whose workload name contains this")
