@@ -707,7 +707,7 @@ def run_single_leg(args):
     from paper_2606_23348_b200 import GeneralsEnv, OBS_DIGEST
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
-    n = {"rollout": 16384, "step": 16384, "step-large": 262144, "rotation": 16384}[args.only]
+    n = {"rollout": 16384, "step": 16384, "step-large": 262144, "rotation": 16384, "noalloc": 16384}[args.only]
     cfg, _ = workloads.config(args.workload or WORKLOAD, n_games=args.games or n)
     if args.only == "rotation":
         # the headline leg by itself: R replicas of the batch (640 MB of algorithmic traffic between two steps of one
@@ -737,6 +737,31 @@ def run_single_leg(args):
                           "us_per_launch": 1e3 * e0.elapsed_time(e1) / k,
                           "env_steps_per_s": N * k / (e0.elapsed_time(e1) * 1e-3),
                           "kernel_variant": envs[0].lib.gen_last_variant(envs[0]._env, None, None)}))
+        return 0
+    if args.only == "noalloc":
+        # gen_step_noalloc (bitboard cache in the library's fixed device array, rebuilt per call, never chained) beside
+        # gen_step with a caller-allocated cache on the same boards: what the convenience costs
+        out = {"leg": "noalloc", "n_games": cfg["n_games"]}
+        k = max(4, min(args.steps, 400))
+        for name, kw in (("gen_step", {}), ("gen_step_noalloc", dict(bitboards=False, chain=False, stack_cache=False))):
+            env = GeneralsEnv(cfg, device=dev, digest=False, actions_out=False, **kw)
+            call = env.step_noalloc if kw else env.step
+            env.reset()
+            for _ in range(10):
+                call()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            l0 = env.launch_count
+            e0.record()
+            for _ in range(k):
+                call()
+            e1.record()
+            torch.cuda.synchronize()
+            out[name] = {"us_per_call": 1e3 * e0.elapsed_time(e1) / k, "kernels_per_call": (env.launch_count - l0) / k,
+                         "env_steps_per_s": cfg["n_games"] * k / (e0.elapsed_time(e1) * 1e-3)}
+            del env
+        out["note"] = "one environment stepped back to back (partly L2-resident: compare the two, not with the headline)"
+        print(json.dumps(out))
         return 0
     env = GeneralsEnv(cfg, device=dev, digest=(args.only == "rollout"), actions_out=False)
     if args.force_step:
@@ -990,7 +1015,7 @@ def main():
     ap.add_argument("--no-large", action="store_true", help="skip the N = 262,144 leg (roofline_large)")
     ap.add_argument("--no-phase-mix", action="store_true", help="headline rotation: every replica starts at turn 0")
     ap.add_argument("--force-step", action="store_true", help="with --only step: k_step also for more than 4 players")
-    ap.add_argument("--only", choices=["rollout", "step", "step-large", "rotation"], default="",
+    ap.add_argument("--only", choices=["rollout", "step", "step-large", "rotation", "noalloc"], default="",
                     help="one leg by itself, a few launches (the command of the ncu captures under profiles/)")
     ap.add_argument("--sweep", action="store_true", help="config-3 batch sweep + configs 4 / 5 rows (one JSON line each)")
     ap.add_argument("--rows", default="", help="with --sweep: only the rows whose workload name contains this")
